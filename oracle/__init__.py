@@ -1,0 +1,136 @@
+"""CPU oracle for gint_vlocal -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes binding of oracle/gint_oracle.c (which holds all the arithmetic and
+cites the paper).  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package; it imports nothing
+from the product package except nothing at all -- inputs arrive as numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(_build.build())
+        c_dp = ctypes.POINTER(ctypes.c_double)
+        c_ip = ctypes.POINTER(ctypes.c_int)
+        c_i32p = ctypes.POINTER(ctypes.c_int32)
+        c_i64p = ctypes.POINTER(ctypes.c_int64)
+        lib.orc_phi.restype = ctypes.c_int
+        lib.orc_phi.argtypes = [ctypes.c_int, c_dp, c_dp, c_ip, c_ip, c_ip, c_dp, ctypes.c_int, ctypes.c_int, c_dp, c_dp]
+        lib.orc_enumerate_blocks.restype = ctypes.c_int64
+        lib.orc_enumerate_blocks.argtypes = [c_dp, ctypes.c_int, c_dp, c_dp, ctypes.c_int64, c_i32p, c_i32p, c_i32p]
+        lib.orc_vlocal.restype = ctypes.c_int
+        lib.orc_vlocal.argtypes = [c_dp, c_ip, ctypes.c_int, c_dp, c_dp, c_ip, c_ip, c_ip, c_dp, ctypes.c_int, c_ip,
+                                   c_dp, c_dp, ctypes.c_int64, c_i32p, c_i32p, c_i32p, c_i64p, c_dp, ctypes.c_int]
+        _lib = lib
+    return _lib
+
+
+def _p(a, ct):
+    return a.ctypes.data_as(ctypes.POINTER(ct))
+
+
+class _SpeciesPack:
+    """Flatten a list of species (objects with rcut, dr, l, table) for the C side."""
+
+    def __init__(self, species: Sequence):
+        self.n = len(species)
+        self.rcut = np.array([float(s.rcut) for s in species], dtype=np.float64)
+        self.dr = np.array([float(s.dr) for s in species], dtype=np.float64)
+        self.ntab = np.array([int(np.asarray(s.table).shape[1]) for s in species], dtype=np.intc)
+        self.nrad = np.array([int(np.asarray(s.l).shape[0]) for s in species], dtype=np.intc)
+        self.l = np.ascontiguousarray(np.concatenate([np.asarray(s.l, dtype=np.intc) for s in species]), dtype=np.intc)
+        self.table = np.ascontiguousarray(np.concatenate([np.asarray(s.table, dtype=np.float64).ravel() for s in species]))
+        self.norb = np.array([int(np.sum(2 * np.asarray(s.l) + 1)) for s in species], dtype=np.int64)
+
+    def args(self):
+        return (self.n, _p(self.rcut, ctypes.c_double), _p(self.dr, ctypes.c_double), _p(self.ntab, ctypes.c_int),
+                _p(self.nrad, ctypes.c_int), _p(self.l, ctypes.c_int), _p(self.table, ctypes.c_double))
+
+
+def phi(species: Sequence, which: int, d: np.ndarray) -> np.ndarray:
+    """Orbital values phi_mu(d) of species `which` at displacements d[npts][3] (Eq. 1)."""
+    lib = _load()
+    sp = _SpeciesPack(species)
+    d = np.ascontiguousarray(np.asarray(d, dtype=np.float64).reshape(-1, 3))
+    out = np.empty((d.shape[0], int(sp.norb[which])), dtype=np.float64)
+    rc = lib.orc_phi(*sp.args(), int(which), int(d.shape[0]), _p(d, ctypes.c_double), _p(out, ctypes.c_double))
+    if rc < 0:
+        raise RuntimeError("orc_phi failed: %d" % rc)
+    return out
+
+
+def enumerate_blocks(lattice, species, atom_species, atom_pos) -> Tuple[np.ndarray, np.ndarray, np.ndarray, np.ndarray]:
+    """All (I,J,R) with overlapping cutoff spheres, sorted by (I,J,R1,R2,R3).
+    Returns (iat, jat, R[nblk][3], offset[nblk+1]) with offset the prefix sum of n_I*n_J."""
+    lib = _load()
+    lattice = np.ascontiguousarray(lattice, dtype=np.float64)
+    pos = np.ascontiguousarray(atom_pos, dtype=np.float64)
+    asp = np.asarray(atom_species)
+    rc_atom = np.ascontiguousarray([float(species[s].rcut) for s in asp], dtype=np.float64)
+    natom = pos.shape[0]
+    dummy = np.zeros(3, dtype=np.int32)
+    n = lib.orc_enumerate_blocks(_p(lattice, ctypes.c_double), natom, _p(pos, ctypes.c_double),
+                                 _p(rc_atom, ctypes.c_double), 0, _p(dummy, ctypes.c_int32),
+                                 _p(dummy, ctypes.c_int32), _p(dummy, ctypes.c_int32))
+    if n < 0:
+        raise RuntimeError("orc_enumerate_blocks failed")
+    bi = np.empty(max(n, 1), dtype=np.int32)
+    bj = np.empty(max(n, 1), dtype=np.int32)
+    bR = np.empty((max(n, 1), 3), dtype=np.int32)
+    lib.orc_enumerate_blocks(_p(lattice, ctypes.c_double), natom, _p(pos, ctypes.c_double),
+                             _p(rc_atom, ctypes.c_double), n, _p(bi, ctypes.c_int32), _p(bj, ctypes.c_int32),
+                             _p(bR, ctypes.c_int32))
+    bi, bj, bR = bi[:n], bj[:n], bR[:n]
+    norb = np.array([int(np.sum(2 * np.asarray(species[s].l) + 1)) for s in asp], dtype=np.int64)
+    off = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(norb[bi] * norb[bj], out=off[1:])
+    return bi, bj, bR, off
+
+
+def vlocal(lattice, ngrid, species, atom_species, atom_pos, V, blocks=None, nthreads: int = 0,
+           return_threads: bool = False):
+    """H blocks of Eq. 45 for `blocks` = (iat, jat, R) (default: all, sorted).
+    Returns (H_flat, (iat, jat, R, offset)); H_flat holds the listed blocks back to back,
+    each row-major n_I x n_J.  The listed blocks must be grouped by iat."""
+    lib = _load()
+    lattice = np.ascontiguousarray(lattice, dtype=np.float64)
+    ngrid_c = np.ascontiguousarray(ngrid, dtype=np.intc)
+    pos = np.ascontiguousarray(atom_pos, dtype=np.float64)
+    asp = np.ascontiguousarray(atom_species, dtype=np.intc)
+    V = np.ascontiguousarray(V, dtype=np.float64)
+    assert V.shape == tuple(int(x) for x in ngrid_c)
+    sp = _SpeciesPack(species)
+    if blocks is None:
+        bi, bj, bR, off = enumerate_blocks(lattice, species, asp, pos)
+    else:
+        bi = np.ascontiguousarray(blocks[0], dtype=np.int32)
+        bj = np.ascontiguousarray(blocks[1], dtype=np.int32)
+        bR = np.ascontiguousarray(blocks[2], dtype=np.int32).reshape(-1, 3)
+        norb = sp.norb[asp]
+        off = np.zeros(bi.shape[0] + 1, dtype=np.int64)
+        np.cumsum(norb[bi] * norb[bj], out=off[1:])
+    out = np.zeros(int(off[-1]), dtype=np.float64)
+    nb = int(bi.shape[0])
+    if nb:
+        rc = lib.orc_vlocal(_p(lattice, ctypes.c_double), _p(ngrid_c, ctypes.c_int), *sp.args(), int(pos.shape[0]),
+                            _p(asp, ctypes.c_int), _p(pos, ctypes.c_double), _p(V, ctypes.c_double), nb,
+                            _p(bi, ctypes.c_int32), _p(bj, ctypes.c_int32), _p(bR, ctypes.c_int32),
+                            _p(off, ctypes.c_int64), _p(out, ctypes.c_double), int(nthreads))
+        if rc < 0:
+            raise RuntimeError("orc_vlocal failed: %d" % rc)
+    else:
+        rc = 0
+    if return_threads:
+        return out, (bi, bj, bR, off), rc
+    return out, (bi, bj, bR, off)
