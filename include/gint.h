@@ -1,0 +1,147 @@
+/*
+ * gint.h -- C ABI of the B200-native gint_vlocal library (libgint_b200.so).
+ *
+ * The library builds the local-potential Hamiltonian of NAO-based (RT-TD)DFT on
+ * a uniform real-space mesh,
+ *
+ *   H_mu,nu(R) = sum_g phi_mu(r_g - tau_I) V(r_g) phi_nu(r_g - tau_J - R) dV
+ *                                   -- PAPER.md:393-398 (Sec. 3.3.1, Eq. 45)
+ *   phi_mu(r)  = f_{I,l,zeta}(|r|) Y_lm(r/|r|)
+ *                                   -- PAPER.md:66-70 (Sec. 2.1, Eq. 1)
+ *
+ * with R the lattice vector from the cell of mu (atom I) to the cell of nu
+ * (atom J) -- PAPER.md:104-106 -- and the result stored as dense blocks per
+ * (I, J, R).  gint_setup plays the role of the paper's GintInfo initialisation
+ * (mesh -> BigGrid partition -> per-BigGrid atom lists; Fig. 2 at
+ * PAPER.md:368); gint_vlocal is the paper's cal_gint_vl.
+ *
+ * Conventions:
+ *   - Units bohr / Hartree, FP64 only, real V, one spin channel.
+ *   - Mesh point (i,j,k) sits at (i/N1) a1 + (j/N2) a2 + (k/N3) a3; dV = |det A|/(N1 N2 N3).
+ *   - The sum over g runs over all space with V periodic on the mesh.
+ *   - Radial part: 4-point (cubic) Lagrange interpolation of the table on the
+ *     forward stencil k..k+3, k = floor(r/dr); phi = 0 iff r >= rcut.
+ *   - Real Y_lm, l <= 2, no Condon-Shortley phase, with (x,y,z) = r/|r|:
+ *       l=0: 1/(2 sqrt(pi));   l=1: sqrt(3/4pi) * {y, z, x};
+ *       l=2: {1/2 sqrt(15/pi) xy, 1/2 sqrt(15/pi) yz, 1/4 sqrt(5/pi) (3z^2-1),
+ *             1/2 sqrt(15/pi) xz, 1/4 sqrt(15/pi) (x^2-y^2)}.
+ *     For |r| < 1e-12 bohr the l>0 components are 0.
+ *   - Orbital order inside an atom: radial functions in the order given, each
+ *     followed by its 2l+1 m-components in the order above.
+ *   - Block set: every (I,J,R) with |tau_J + R - tau_I| < rcut_I + rcut_J
+ *     (strict), both (I,J,R) and (J,I,-R) stored, sorted lexicographically by
+ *     (I, J, R1, R2, R3); block = row-major n_I x n_J (rows: orbitals of I);
+ *     blocks are packed back to back (offset = prefix sum of n_I*n_J).
+ *   - Atom positions are used as given (never wrapped into the cell); R labels are
+ *     relative to them.
+ *
+ * Pointers are HOST pointers unless the name ends in _dev.  All calls return 0
+ * (GINT_OK) or a negative error code; nothing throws or aborts across this
+ * boundary.  A gint_ctx may be used from one thread at a time.
+ */
+#ifndef GINT_B200_H
+#define GINT_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GINT_OK 0
+#define GINT_EINVAL (-1)       /* null pointer, bad shape, non-positive size, table too short, singular lattice */
+#define GINT_EUNSUPPORTED (-2) /* l > 2, too many orbitals per atom, H too large for 32-bit block offsets */
+#define GINT_ENOMEM (-3)       /* host or device allocation failed */
+#define GINT_ECUDA (-4)        /* CUDA runtime error; text via gint_last_error() */
+#define GINT_ENODEVICE (-5)    /* call needs a device but the context was created host-only (cuda_device < 0) */
+
+typedef struct gint_ctx gint_ctx; /* opaque; owns all host and device metadata */
+
+/* One atomic species: nrad tabulated radial functions f(r), node k at r = k*dr.
+ * Requirements: dr > 0, rcut > 0, ntab*dr >= rcut + 3*dr (the forward stencil may
+ * read three nodes past floor(rcut/dr)); 0 <= l[k] <= 2; sum(2l+1) <= 64.
+ * The arrays are copied during gint_setup and not retained. */
+typedef struct {
+    double rcut;         /* phi == 0 for r >= rcut (bohr)                          */
+    double dr;           /* radial table step (bohr)                               */
+    int32_t ntab;        /* nodes per table                                        */
+    int32_t nrad;        /* number of radial functions                             */
+    const int32_t *l;    /* [nrad] angular momentum of each radial function        */
+    const double *table; /* [nrad][ntab], row-major                                */
+} gint_species;
+
+/* Tuning / sharding options; pass NULL for the defaults. */
+typedef struct {
+    int32_t bcell[3]; /* big-cell edge in mesh points ("BigGrid"); 0 -> 4.  Need not divide N. */
+    int32_t rank;     /* this process' share of the big cells: cells with                                   */
+    int32_t nranks;   /*   (cell index along a1) % nranks == rank are integrated; 0/1 -> all (single GPU)  */
+} gint_options;
+
+/* Build the context: validate, enumerate (I,J,R) blocks, partition the mesh into
+ * big cells, build the per-cell (atom, image) lists and the work queue, upload.
+ *   lattice[9]        rows a1, a2, a3 (Cartesian, bohr); any non-singular cell
+ *   ngrid[3]          N1, N2, N3 > 0
+ *   atom_species[natom], atom_pos[natom][3] (Cartesian)
+ *   cuda_device       >= 0: device ordinal; < 0: host-only context (no CUDA call is
+ *                     made; block table and statistics can be queried, gint_vlocal
+ *                     returns GINT_ENODEVICE)
+ * On failure *out is NULL. */
+int gint_setup(gint_ctx **out, const double *lattice, const int32_t *ngrid, int32_t nspecies,
+               const gint_species *species, int32_t natom, const int32_t *atom_species, const double *atom_pos,
+               int32_t cuda_device, const gint_options *opt);
+
+/* Number of H blocks and length of the H buffer in doubles. */
+int gint_num_blocks(const gint_ctx *ctx, int64_t *nblocks, int64_t *h_len);
+
+/* Block table: iat[nblocks], jat[nblocks], R[nblocks][3], offset[nblocks+1] (in
+ * doubles).  Any output pointer may be NULL. */
+int gint_get_blocks(const gint_ctx *ctx, int32_t *iat, int32_t *jat, int32_t *R, int64_t *offset);
+
+/* H <- Eq. 45 for the potential V.
+ *   V_dev   device pointer, [N1][N2][N3] doubles, third index fastest; read only
+ *   H_dev   device pointer, h_len doubles; OVERWRITTEN (not accumulated into)
+ *   stream  cudaStream_t (as void*), NULL = legacy default stream
+ * Asynchronous: enqueues a memset, the integration kernel and the mirror kernel
+ * on `stream`; no host synchronisation, no allocation, no host<->device copy.
+ * With nranks > 1 H holds this rank's partial sum (sum over ranks = full H).
+ * Kernel faults surface at the caller's next synchronisation. */
+int gint_vlocal(gint_ctx *ctx, const double *V_dev, double *H_dev, void *stream);
+
+/* Convenience end-to-end call with HOST buffers: copies V to the device, runs
+ * gint_vlocal, copies H back, synchronises.  V_host [N1][N2][N3], H_host [h_len]. */
+int gint_vlocal_host(gint_ctx *ctx, const double *V_host, double *H_host);
+
+/* Statistics of the setup (all host-side, valid for host-only contexts too).
+ * stats[0] big cells total        stats[1] non-empty work items
+ * stats[2] (atom image, cell) list entries          stats[3] max orbitals in one work item
+ * stats[4] sum over items of K*n_c^2 (executed MACs, full square, no symmetry)
+ * stats[5] sum over items of n_c^2   stats[6] dynamic shared memory per CTA (bytes)
+ * stats[7] number of kernels launched per gint_vlocal call (memsets not counted)
+ * stats[8] F_pt = sum_g 2 n(g)^2, n(g) = orbitals non-zero at mesh point g (useful flops, no symmetry)
+ * stats[9] F_sym = sum_g n(g) (n(g)+1) (useful flops when H(R)=H(-R)^T is exploited)
+ * stats[10] in-sphere (atom image, point) pairs   stats[11] work items whose point range was split
+ * Returns the number of entries written (<= n). */
+int gint_get_stats(const gint_ctx *ctx, double *stats, int32_t n);
+
+/* Copy out the per-cell lists (host logic tests).  cell_start[ncell+1] indexes
+ * entry_atom[nentry] / entry_R[nentry][3]; cells are numbered (c1*nc2 + c2)*nc3 + c3.
+ * Call with all pointers NULL to get ncell and nentry only. */
+int gint_get_cell_lists(const gint_ctx *ctx, int64_t *ncell, int64_t *nentry, int64_t *cell_start,
+                        int32_t *entry_atom, int32_t *entry_R);
+
+/* Measure the sustained FP64 tensor-core (DMMA.8x8x4) rate of the current device with
+ * a register-resident kernel: the "FP64 tensor peak" of the roofline.  Returns
+ * TFLOP/s in *tflops. */
+int gint_measure_fp64_peak(int32_t cuda_device, double seconds, double *tflops);
+
+int gint_destroy(gint_ctx *ctx);
+
+/* Text for an error code; gint_last_error() returns the detail of the last
+ * failure in this thread (e.g. the CUDA error string). */
+const char *gint_strerror(int code);
+const char *gint_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GINT_B200_H */

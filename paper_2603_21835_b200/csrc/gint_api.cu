@@ -1,0 +1,269 @@
+// gint_api.cu -- extern "C" boundary of libgint_b200.so (declared in include/gint.h).
+#include <cuda_runtime.h>
+
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/gint.h"
+#include "gint_device.hpp"
+#include "gint_plan.hpp"
+
+static_assert(sizeof(gint::Entry) == sizeof(gint::EntryDev), "Entry layout mismatch");
+static_assert(sizeof(gint::WorkItem) == sizeof(gint::WorkItemDev), "WorkItem layout mismatch");
+static_assert(sizeof(gint::MirrorItem) == sizeof(gint::MirrorItemDev), "MirrorItem layout mismatch");
+static_assert(gint::kMaxItemPoints == gint::kMaxItemPointsDev, "K mismatch");
+
+struct gint_ctx {
+    gint::Plan plan;
+    gint::DevicePlan dev{};
+    int device = -1;
+    int nsm = 0;
+    std::vector<void*> allocs;
+    double* V_scratch = nullptr;   // gint_vlocal_host only
+    double* H_scratch = nullptr;
+};
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int fail(int code, const std::string& msg) {
+    g_last_error = msg;
+    return code;
+}
+int fail_cuda(cudaError_t e, const char* where) {
+    g_last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    return GINT_ECUDA;
+}
+
+template <typename T>
+cudaError_t upload(gint_ctx* ctx, const std::vector<T>& host, const T** dev_out) {
+    void* p = nullptr;
+    const size_t bytes = host.size() * sizeof(T);
+    cudaError_t e = cudaMalloc(&p, bytes ? bytes : 16);
+    if (e != cudaSuccess) return e;
+    ctx->allocs.push_back(p);
+    if (bytes) e = cudaMemcpy(p, host.data(), bytes, cudaMemcpyHostToDevice);
+    *dev_out = reinterpret_cast<const T*>(p);
+    return e;
+}
+
+void release(gint_ctx* ctx) {
+    if (ctx->device >= 0) {
+        cudaSetDevice(ctx->device);
+        for (void* p : ctx->allocs) cudaFree(p);
+        if (ctx->V_scratch) cudaFree(ctx->V_scratch);
+        if (ctx->H_scratch) cudaFree(ctx->H_scratch);
+    }
+    delete ctx;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int32_t nspecies,
+               const gint_species* species, int32_t natom, const int32_t* atom_species, const double* atom_pos,
+               int32_t cuda_device, const gint_options* opt) {
+    if (!out) return fail(GINT_EINVAL, "out is null");
+    *out = nullptr;
+    if (!species || nspecies <= 0) return fail(GINT_EINVAL, "no species");
+    gint_ctx* ctx = new (std::nothrow) gint_ctx;
+    if (!ctx) return fail(GINT_ENOMEM, "host allocation failed");
+    try {
+        std::vector<gint::SpeciesHost> sp((size_t)nspecies);
+        for (int s = 0; s < nspecies; s++) {
+            const gint_species& in = species[s];
+            if (!in.l || !in.table || in.nrad <= 0 || in.ntab <= 0 || in.nrad > 64) {
+                delete ctx;
+                return fail(GINT_EINVAL, "bad species descriptor");
+            }
+            sp[s].rcut = in.rcut;
+            sp[s].dr = in.dr;
+            sp[s].ntab = in.ntab;
+            sp[s].nrad = in.nrad;
+            sp[s].l.assign(in.l, in.l + in.nrad);
+            sp[s].table.assign(in.table, in.table + (size_t)in.nrad * in.ntab);
+        }
+        std::string err;
+        const int32_t* bc = opt ? opt->bcell : nullptr;
+        const int rc = gint::build_plan(ctx->plan, lattice, ngrid, nspecies, sp.data(), natom, atom_species, atom_pos,
+                                        bc, opt ? opt->rank : 0, opt ? opt->nranks : 1, err);
+        if (rc != GINT_OK) {
+            delete ctx;
+            return fail(rc, err);
+        }
+    } catch (const std::bad_alloc&) {
+        delete ctx;
+        return fail(GINT_ENOMEM, "host allocation failed");
+    }
+    if (cuda_device < 0) {   // host-only context
+        *out = ctx;
+        return GINT_OK;
+    }
+    cudaError_t e = cudaSetDevice(cuda_device);
+    if (e != cudaSuccess) { delete ctx; return fail_cuda(e, "cudaSetDevice"); }
+    ctx->device = cuda_device;
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, cuda_device);
+    if (e != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaGetDeviceProperties"); }
+    ctx->nsm = prop.multiProcessorCount;
+    if (ctx->plan.smem_bytes > (size_t)prop.sharedMemPerBlockOptin) {
+        release(ctx);
+        return fail(GINT_EUNSUPPORTED, "device offers too little shared memory per block");
+    }
+    gint::Plan& P = ctx->plan;
+    gint::DevicePlan& D = ctx->dev;
+    const gint::Entry* d_entries = nullptr;
+    const gint::WorkItem* d_items = nullptr;
+    const gint::MirrorItem* d_mirror = nullptr;
+#define UP(vec, ptr)                                                   \
+    if ((e = upload(ctx, vec, ptr)) != cudaSuccess) {                  \
+        release(ctx);                                                  \
+        return fail_cuda(e, "upload " #vec);                           \
+    }
+    UP(P.entries, &d_entries)
+    UP(P.items, &d_items)
+    UP(P.mirror, &d_mirror)
+    UP(P.hash_keys, &D.hash_keys)
+    UP(P.hash_vals, &D.hash_vals)
+    UP(P.tab_packed, &D.tab)
+    UP(P.sp_meta, &D.sp_meta)
+    UP(P.sp_real, &D.sp_real)
+#undef UP
+    D.entries = reinterpret_cast<const gint::EntryDev*>(d_entries);
+    D.items = reinterpret_cast<const gint::WorkItemDev*>(d_items);
+    D.mirror = reinterpret_cast<const gint::MirrorItemDev*>(d_mirror);
+    void* ctr = nullptr;
+    if ((e = cudaMalloc(&ctr, 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
+    ctx->allocs.push_back(ctr);
+    D.counter = reinterpret_cast<unsigned int*>(ctr);
+    std::memcpy(D.estep, P.estep, sizeof(D.estep));
+    D.dV = P.dV;
+    for (int d = 0; d < 3; d++) {
+        D.ngrid[d] = P.ngrid[d];
+        D.bcell[d] = P.bcell[d];
+    }
+    D.nitems = (int32_t)P.items.size();
+    D.nmirror = (int32_t)P.mirror.size();
+    D.tab_doubles = (int32_t)P.tab_packed.size();
+    D.max_entries = P.max_entries;
+    D.max_rows_pad = (P.max_rows + 7) & ~7;
+    D.hash_mask = P.hash_mask;
+    if ((e = gint::configure_kernels(D, P.smem_bytes, P.tables_in_smem)) != cudaSuccess) {
+        release(ctx);
+        return fail_cuda(e, "cudaFuncSetAttribute");
+    }
+    *out = ctx;
+    return GINT_OK;
+}
+
+int gint_num_blocks(const gint_ctx* ctx, int64_t* nblocks, int64_t* h_len) {
+    if (!ctx) return fail(GINT_EINVAL, "ctx is null");
+    if (nblocks) *nblocks = (int64_t)ctx->plan.blk_i.size();
+    if (h_len) *h_len = ctx->plan.blk_off.back();
+    return GINT_OK;
+}
+
+int gint_get_blocks(const gint_ctx* ctx, int32_t* iat, int32_t* jat, int32_t* R, int64_t* offset) {
+    if (!ctx) return fail(GINT_EINVAL, "ctx is null");
+    const gint::Plan& P = ctx->plan;
+    const size_t n = P.blk_i.size();
+    if (iat && n) std::memcpy(iat, P.blk_i.data(), n * sizeof(int32_t));
+    if (jat && n) std::memcpy(jat, P.blk_j.data(), n * sizeof(int32_t));
+    if (R && n) std::memcpy(R, P.blk_R.data(), 3 * n * sizeof(int32_t));
+    if (offset) std::memcpy(offset, P.blk_off.data(), (n + 1) * sizeof(int64_t));
+    return GINT_OK;
+}
+
+int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream) {
+    if (!ctx || !V_dev || !H_dev) return fail(GINT_EINVAL, "null argument");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    cudaError_t e = gint::launch_vlocal(ctx->dev, ctx->plan.smem_bytes, ctx->plan.tables_in_smem, ctx->nsm,
+                                        (size_t)ctx->plan.blk_off.back(), V_dev, H_dev,
+                                        reinterpret_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "gint_vlocal launch");
+    return GINT_OK;
+}
+
+int gint_vlocal_host(gint_ctx* ctx, const double* V_host, double* H_host) {
+    if (!ctx || !V_host || !H_host) return fail(GINT_EINVAL, "null argument");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaSetDevice");
+    const size_t nV = (size_t)ctx->plan.ngrid[0] * ctx->plan.ngrid[1] * ctx->plan.ngrid[2];
+    const size_t nH = (size_t)ctx->plan.blk_off.back();
+    if (!ctx->V_scratch && (e = cudaMalloc(&ctx->V_scratch, nV * sizeof(double))) != cudaSuccess)
+        return fail_cuda(e, "cudaMalloc V");
+    if (!ctx->H_scratch && (e = cudaMalloc(&ctx->H_scratch, (nH ? nH : 1) * sizeof(double))) != cudaSuccess)
+        return fail_cuda(e, "cudaMalloc H");
+    if ((e = cudaMemcpyAsync(ctx->V_scratch, V_host, nV * sizeof(double), cudaMemcpyHostToDevice, 0)) != cudaSuccess)
+        return fail_cuda(e, "H2D V");
+    const int rc = gint_vlocal(ctx, ctx->V_scratch, ctx->H_scratch, nullptr);
+    if (rc != GINT_OK) return rc;
+    if ((e = cudaMemcpyAsync(H_host, ctx->H_scratch, nH * sizeof(double), cudaMemcpyDeviceToHost, 0)) != cudaSuccess)
+        return fail_cuda(e, "D2H H");
+    if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return fail_cuda(e, "synchronize");
+    return GINT_OK;
+}
+
+int gint_get_stats(const gint_ctx* ctx, double* stats, int32_t n) {
+    if (!ctx || !stats) return fail(GINT_EINVAL, "null argument");
+    const int m = n < 12 ? n : 12;
+    for (int i = 0; i < m; i++) stats[i] = ctx->plan.stats[i];
+    return m;
+}
+
+int gint_get_cell_lists(const gint_ctx* ctx, int64_t* ncell, int64_t* nentry, int64_t* cell_start,
+                        int32_t* entry_atom, int32_t* entry_R) {
+    if (!ctx) return fail(GINT_EINVAL, "ctx is null");
+    const gint::Plan& P = ctx->plan;
+    if (ncell) *ncell = (int64_t)P.cell_start.size() - 1;
+    if (nentry) *nentry = (int64_t)P.entries.size();
+    if (cell_start) std::memcpy(cell_start, P.cell_start.data(), P.cell_start.size() * sizeof(int64_t));
+    for (size_t i = 0; i < P.entries.size(); i++) {
+        if (entry_atom) entry_atom[i] = P.entries[i].atom;
+        if (entry_R) {
+            const int rp = P.entries[i].Rpack;
+            entry_R[3 * i] = ((rp >> 16) & 0xFF) - 128;
+            entry_R[3 * i + 1] = ((rp >> 8) & 0xFF) - 128;
+            entry_R[3 * i + 2] = (rp & 0xFF) - 128;
+        }
+    }
+    return GINT_OK;
+}
+
+int gint_measure_fp64_peak(int32_t cuda_device, double seconds, double* tflops) {
+    if (!tflops || cuda_device < 0) return fail(GINT_EINVAL, "bad argument");
+    cudaError_t e = cudaSetDevice(cuda_device);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaSetDevice");
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, cuda_device)) != cudaSuccess) return fail_cuda(e, "cudaGetDeviceProperties");
+    if ((e = gint::measure_dmma_peak(seconds, prop.multiProcessorCount, tflops)) != cudaSuccess)
+        return fail_cuda(e, "dmma peak kernel");
+    return GINT_OK;
+}
+
+int gint_destroy(gint_ctx* ctx) {
+    if (!ctx) return GINT_OK;
+    release(ctx);
+    return GINT_OK;
+}
+
+const char* gint_strerror(int code) {
+    switch (code) {
+        case GINT_OK: return "ok";
+        case GINT_EINVAL: return "invalid argument";
+        case GINT_EUNSUPPORTED: return "unsupported input";
+        case GINT_ENOMEM: return "out of memory";
+        case GINT_ECUDA: return "CUDA error";
+        case GINT_ENODEVICE: return "context has no device";
+        default: return "unknown error";
+    }
+}
+
+const char* gint_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"
