@@ -111,6 +111,14 @@ int gint_vlocal(gint_ctx *ctx, const double *V_dev, double *H_dev, void *stream)
  * gint_vlocal, copies H back, synchronises.  V_host [N1][N2][N3], H_host [h_len]. */
 int gint_vlocal_host(gint_ctx *ctx, const double *V_host, double *H_host);
 
+/* Per-kernel timing on the launch stream.  After gint_set_profiling(ctx, 1) every
+ * gint_vlocal call records CUDA events around its integration kernel and its mirror
+ * kernel on `stream`; gint_get_kernel_ms synchronises on the last call's events and
+ * returns their durations in milliseconds (ms[0] integration, ms[1] mirror, ms[2] whole
+ * call incl. the memsets).  Used by bench.py for the roofline's per-launch duration. */
+int gint_set_profiling(gint_ctx *ctx, int32_t on);
+int gint_get_kernel_ms(gint_ctx *ctx, double *ms /* [3] */);
+
 /* Statistics of the setup (all host-side, valid for host-only contexts too).
  * stats[0] big cells total        stats[1] non-empty work items
  * stats[2] (atom image, cell) list entries          stats[3] max orbitals in one work item

@@ -239,11 +239,12 @@ static inline int64_t pmod(int64_t a, int64_t n)
  * double of block b in out; block is row-major n_I x n_J.
  * nthreads <= 0: OpenMP default.  Returns threads used, or <0 on error.      */
 int orc_vlocal(const double *lattice, const int *ngrid, int nspecies, const double *sp_rcut, const double *sp_dr,
-               const int *sp_ntab, const int *sp_nrad, const int *sp_l, const double *sp_table, int natom,
+               const int *sp_ntab, const int *sp_nrad, const int *sp_l, const double *sp_table, int natom_unused,
                const int *atom_species, const double *pos, const double *V, int64_t nblk, const int32_t *bi,
                const int32_t *bj, const int32_t *bR, const int64_t *out_off, double *out, int nthreads)
 {
     orc_species sp[16];
+    (void)natom_unused;
     if (nspecies > 16) return -1;
     unpack_species(nspecies, sp_rcut, sp_dr, sp_ntab, sp_nrad, sp_l, sp_table, sp);
     for (int s = 0; s < nspecies; s++)

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgint_b200.so")
 GINT_OK, GINT_EINVAL, GINT_EUNSUPPORTED, GINT_ENOMEM, GINT_ECUDA, GINT_ENODEVICE = 0, -1, -2, -3, -4, -5
 
 EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
-            "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
+            "gint_set_profiling", "gint_get_kernel_ms", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "sum_K_n2", "sum_n2", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "split_cells")
@@ -59,6 +59,10 @@ def _load() -> ctypes.CDLL:
     lib.gint_vlocal_host.argtypes = [vp, P(dbl), P(dbl)]
     lib.gint_get_stats.restype = ctypes.c_int
     lib.gint_get_stats.argtypes = [vp, P(dbl), i32]
+    lib.gint_set_profiling.restype = ctypes.c_int
+    lib.gint_set_profiling.argtypes = [vp, i32]
+    lib.gint_get_kernel_ms.restype = ctypes.c_int
+    lib.gint_get_kernel_ms.argtypes = [vp, P(dbl)]
     lib.gint_get_cell_lists.restype = ctypes.c_int
     lib.gint_get_cell_lists.argtypes = [vp, P(i64), P(i64), P(i64), P(i32), P(i32)]
     lib.gint_measure_fp64_peak.restype = ctypes.c_int
@@ -114,6 +118,15 @@ class GintContext:
         s = np.zeros(12, dtype=np.float64)
         n = _check(_lib.gint_get_stats(self._h, _ptr(s, ctypes.c_double), 12), "gint_get_stats")
         return {STAT_NAMES[i]: float(s[i]) for i in range(n)}
+
+    def gint_set_profiling(self, on: bool = True):
+        _check(_lib.gint_set_profiling(self._h, 1 if on else 0), "gint_set_profiling")
+
+    def gint_get_kernel_ms(self):
+        """(integration kernel ms, mirror kernel ms, whole call ms) of the last gint_vlocal call."""
+        ms = np.zeros(3, dtype=np.float64)
+        _check(_lib.gint_get_kernel_ms(self._h, _ptr(ms, ctypes.c_double)), "gint_get_kernel_ms")
+        return float(ms[0]), float(ms[1]), float(ms[2])
 
     def gint_get_cell_lists(self):
         nc, ne = ctypes.c_int64(), ctypes.c_int64()

@@ -21,6 +21,9 @@ struct gint_ctx {
     int device = -1;
     int nsm = 0;
     std::vector<void*> allocs;
+    bool profiling = false;
+    bool have_events = false;
+    cudaEvent_t ev[4];
     double* V_scratch = nullptr;   // gint_vlocal_host only
     double* H_scratch = nullptr;
 };
@@ -54,6 +57,8 @@ void release(gint_ctx* ctx) {
     if (ctx->device >= 0) {
         cudaSetDevice(ctx->device);
         for (void* p : ctx->allocs) cudaFree(p);
+        if (ctx->have_events)
+            for (int i = 0; i < 4; i++) cudaEventDestroy(ctx->ev[i]);
         if (ctx->V_scratch) cudaFree(ctx->V_scratch);
         if (ctx->H_scratch) cudaFree(ctx->H_scratch);
     }
@@ -183,7 +188,7 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
     cudaError_t e = gint::launch_vlocal(ctx->dev, ctx->plan.smem_bytes, ctx->plan.tables_in_smem, ctx->nsm,
                                         (size_t)ctx->plan.blk_off.back(), V_dev, H_dev,
-                                        reinterpret_cast<cudaStream_t>(stream));
+                                        reinterpret_cast<cudaStream_t>(stream), ctx->profiling ? ctx->ev : nullptr);
     if (e != cudaSuccess) return fail_cuda(e, "gint_vlocal launch");
     return GINT_OK;
 }
@@ -206,6 +211,36 @@ int gint_vlocal_host(gint_ctx* ctx, const double* V_host, double* H_host) {
     if ((e = cudaMemcpyAsync(H_host, ctx->H_scratch, nH * sizeof(double), cudaMemcpyDeviceToHost, 0)) != cudaSuccess)
         return fail_cuda(e, "D2H H");
     if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return fail_cuda(e, "synchronize");
+    return GINT_OK;
+}
+
+int gint_set_profiling(gint_ctx* ctx, int32_t on) {
+    if (!ctx) return fail(GINT_EINVAL, "ctx is null");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    if (on && !ctx->have_events) {
+        cudaSetDevice(ctx->device);
+        for (int i = 0; i < 4; i++) {
+            cudaError_t e = cudaEventCreate(&ctx->ev[i]);
+            if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
+        }
+        ctx->have_events = true;
+    }
+    ctx->profiling = on != 0;
+    return GINT_OK;
+}
+
+int gint_get_kernel_ms(gint_ctx* ctx, double* ms) {
+    if (!ctx || !ms) return fail(GINT_EINVAL, "null argument");
+    if (!ctx->profiling || !ctx->have_events) return fail(GINT_EINVAL, "profiling is off");
+    cudaError_t e = cudaEventSynchronize(ctx->ev[3]);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
+    float a = 0, b = 0, c = 0;
+    cudaEventElapsedTime(&a, ctx->ev[1], ctx->ev[2]);
+    cudaEventElapsedTime(&b, ctx->ev[2], ctx->ev[3]);
+    cudaEventElapsedTime(&c, ctx->ev[0], ctx->ev[3]);
+    ms[0] = a;
+    ms[1] = b;
+    ms[2] = c;
     return GINT_OK;
 }
 

@@ -48,8 +48,9 @@ struct DevicePlan {
 };
 
 cudaError_t configure_kernels(const DevicePlan& P, size_t smem_bytes, bool tab_smem);
+// ev: nullptr, or 4 events recorded at call start / before main / after main / after mirror
 cudaError_t launch_vlocal(const DevicePlan& P, size_t smem_bytes, bool tab_smem, int nsm, size_t h_len,
-                          const double* V, double* H, cudaStream_t stream);
+                          const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev);
 cudaError_t measure_dmma_peak(double seconds, int nsm, double* tflops);
 
 }  // namespace gint

@@ -350,11 +350,13 @@ cudaError_t configure_kernels(const DevicePlan& P, size_t smem_bytes, bool tab_s
 }
 
 cudaError_t launch_vlocal(const DevicePlan& P, size_t smem_bytes, bool tab_smem, int nsm, size_t h_len,
-                          const double* V, double* H, cudaStream_t stream) {
+                          const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev) {
+    if (ev) cudaEventRecord(ev[0], stream);
     cudaError_t e = cudaMemsetAsync(H, 0, h_len * sizeof(double), stream);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int), stream);
     if (e != cudaSuccess) return e;
+    if (ev) cudaEventRecord(ev[1], stream);
     if (P.nitems > 0) {
         const int grid = P.nitems < nsm ? P.nitems : nsm;
         if (tab_smem)
@@ -364,11 +366,13 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t smem_bytes, bool tab_smem,
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
+    if (ev) cudaEventRecord(ev[2], stream);
     if (P.nmirror > 0) {
         const int wpb = 256 / 32;
         gint_mirror_kernel<<<(P.nmirror + wpb - 1) / wpb, 256, 0, stream>>>(P.mirror, P.nmirror, H);
         e = cudaGetLastError();
     }
+    if (ev) cudaEventRecord(ev[3], stream);
     return e;
 }
 

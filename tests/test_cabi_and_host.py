@@ -1,0 +1,167 @@
+"""CPU-side tests: the C-ABI library loads and exports every symbol of include/gint.h;
+host logic of gint_setup (block table, big-cell lists, error codes) checked without a GPU."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2603_21835_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2603_21835_b200 import binding
+    hdr = open(os.path.join(ROOT, "include", "gint.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(gint_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.EXPORTED), declared ^ set(binding.EXPORTED)
+    lib = ctypes.CDLL(binding.LIB_PATH)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_product_does_not_import_oracle():
+    """The product path shares no code with the oracle and never calls it."""
+    pkg = os.path.join(ROOT, "paper_2603_21835_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cpp", ".hpp", ".h")):
+                txt = open(os.path.join(dp, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "gint_oracle" not in txt and "libgint_oracle" not in txt and "oracle/" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2603_21835_b200 import" not in txt and "libgint_b200" not in txt, f
+
+
+@pytest.fixture(scope="module")
+def host_ctx_cfg1(cfg1):
+    from paper_2603_21835_b200 import gint_setup
+    w = cfg1
+    return gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1)
+
+
+def test_block_table_matches_oracle_enumeration(cfg1, host_ctx_cfg1):
+    import oracle
+    bi, bj, bR, off = oracle.enumerate_blocks(cfg1.lattice, cfg1.species, cfg1.atom_species, cfg1.atom_pos)
+    i2, j2, R2, o2 = host_ctx_cfg1.gint_get_blocks()
+    assert np.array_equal(bi, i2) and np.array_equal(bj, j2) and np.array_equal(bR, R2) and np.array_equal(off, o2)
+    assert host_ctx_cfg1.nblocks == 376 and host_ctx_cfg1.h_len == 6016
+
+
+def test_host_only_context_refuses_device_calls(cfg1, host_ctx_cfg1):
+    from paper_2603_21835_b200 import binding
+    with pytest.raises(binding.GintError) as e:
+        host_ctx_cfg1.gint_vlocal_host(cfg1.V)
+    assert e.value.code == binding.GINT_ENODEVICE
+
+
+def brute_cell_lists(w, bcell):
+    """Independent (numpy) construction of the per-cell (atom, image) lists: an image is
+    listed iff one of the cell's mesh points lies strictly inside its cutoff sphere."""
+    n = np.array(w.ngrid)
+    nc = -(-n // np.array(bcell))
+    idx = np.stack(np.meshgrid(*[np.arange(x) for x in n], indexing="ij"), axis=-1).reshape(-1, 3)
+    pts = (idx / n) @ w.lattice
+    cell = ((idx[:, 0] // bcell[0]) * nc[1] + idx[:, 1] // bcell[1]) * nc[2] + idx[:, 2] // bcell[2]
+    out = set()
+    counts = np.zeros(len(idx), dtype=np.int64)
+    for I in range(w.natom):
+        sp = w.species[w.atom_species[I]]
+        for a in range(-3, 4):
+            for b in range(-3, 4):
+                for c in range(-3, 4):
+                    d = pts - w.atom_pos[I] - np.array([a, b, c]) @ w.lattice
+                    inside = np.einsum("ij,ij->i", d, d) < sp.rcut ** 2
+                    counts += inside * sp.norb
+                    for cc in np.unique(cell[inside]):
+                        out.add((int(cc), I, a, b, c))
+    return out, counts
+
+
+@pytest.mark.parametrize("bcell", [(4, 4, 4), (3, 2, 4)])
+def test_cell_lists_exact_and_sorted(bcell):
+    from paper_2603_21835_b200 import gint_setup
+    w = wl.tiny(seed=7)
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1, bcell=bcell)
+    start, atom, R = ctx.gint_get_cell_lists()
+    got = set()
+    for c in range(len(start) - 1):
+        keys = [(int(atom[i]), int(R[i, 0]), int(R[i, 1]), int(R[i, 2])) for i in range(start[c], start[c + 1])]
+        assert keys == sorted(keys)             # canonical order inside a cell
+        got |= {(c,) + k for k in keys}
+    want, counts = brute_cell_lists(w, bcell)
+    assert got == want
+    st = ctx.gint_get_stats()
+    assert st["F_pt"] == pytest.approx(float(np.sum(2.0 * counts * counts)), rel=1e-14)
+    assert st["F_sym"] == pytest.approx(float(np.sum(counts * (counts + 1.0))), rel=1e-14)
+    assert st["entries"] == len(want)
+
+
+def test_survey_sizes_cfg1_cfg2(cfg1, host_ctx_cfg1):
+    """cfg1 F_pt = 6.95e7, F_sym = 3.60e7, in-sphere pairs 3.12e5."""
+    st = host_ctx_cfg1.gint_get_stats()
+    assert st["F_pt"] == pytest.approx(6.95e7, rel=5e-3)
+    assert st["F_sym"] == pytest.approx(3.60e7, rel=5e-3)
+    assert st["insphere_pairs"] == pytest.approx(3.12e5, rel=5e-3)
+
+
+def test_rank_sharding_partitions_the_cells():
+    from paper_2603_21835_b200 import gint_setup
+    w = wl.tiny(seed=7)
+    full = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1)
+    sf, af, Rf = full.gint_get_cell_lists()
+    tot = 0
+    seen = np.zeros(len(sf) - 1, dtype=int)
+    for r in range(3):
+        part = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1, rank=r, nranks=3)
+        s, a, R = part.gint_get_cell_lists()
+        tot += len(a)
+        seen += (np.diff(s) > 0)
+        assert part.nblocks == full.nblocks      # same H layout on every rank
+    assert tot == len(af) and np.all(seen == (np.diff(sf) > 0))
+    assert full.gint_get_stats()["F_pt"] == pytest.approx(sum(
+        gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1, rank=r, nranks=3)
+        .gint_get_stats()["F_pt"] for r in range(3)))
+
+
+def test_error_codes():
+    from paper_2603_21835_b200 import binding, gint_setup
+    w = wl.tiny(seed=7)
+
+    def setup(**kw):
+        a = dict(lattice=w.lattice, ngrid=w.ngrid, species=w.species, atom_species=w.atom_species,
+                 atom_pos=w.atom_pos, cuda_device=-1)
+        a.update(kw)
+        return gint_setup(**a)
+    with pytest.raises(binding.GintError) as e:
+        setup(lattice=np.array([[1.0, 0, 0], [2.0, 0, 0], [0, 0, 1.0]]))
+    assert e.value.code == binding.GINT_EINVAL
+    with pytest.raises(binding.GintError) as e:
+        setup(ngrid=[4, 0, 4])
+    assert e.value.code == binding.GINT_EINVAL
+    with pytest.raises(binding.GintError) as e:
+        setup(atom_species=np.array([0, 5, 0]))
+    assert e.value.code == binding.GINT_EINVAL
+    sp = w.species[0]
+    short = wl.Species("short", sp.rcut, sp.dr, sp.l, sp.table[:, : int(sp.rcut / sp.dr) + 1].copy())
+    with pytest.raises(binding.GintError) as e:
+        setup(species=[short])
+    assert e.value.code == binding.GINT_EINVAL
+    f_shell = wl.Species("f", sp.rcut, sp.dr, np.array([3], dtype=np.int32), sp.table[:1].copy())
+    with pytest.raises(binding.GintError) as e:
+        setup(species=[f_shell])
+    assert e.value.code == binding.GINT_EUNSUPPORTED
+    with pytest.raises(binding.GintError) as e:
+        setup(bcell=(8, 4, 4))
+    assert e.value.code == binding.GINT_EUNSUPPORTED
+    pos = w.atom_pos.copy()
+    pos[0, 0] = np.nan
+    with pytest.raises(binding.GintError) as e:
+        setup(atom_pos=pos)
+    assert e.value.code == binding.GINT_EINVAL
+    assert binding._strerror(binding.GINT_ECUDA) == "CUDA error"
