@@ -10,10 +10,6 @@
 #include "gint_device.hpp"
 #include "gint_plan.hpp"
 
-static_assert(sizeof(gint::Entry) == sizeof(gint::EntryDev), "Entry layout mismatch");
-static_assert(sizeof(gint::WorkItem) == sizeof(gint::WorkItemDev), "WorkItem layout mismatch");
-static_assert(sizeof(gint::MirrorItem) == sizeof(gint::MirrorItemDev), "MirrorItem layout mismatch");
-static_assert(gint::kMaxItemPoints == gint::kMaxItemPointsDev, "K mismatch");
 
 struct gint_ctx {
     gint::Plan plan;
@@ -121,43 +117,37 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     }
     gint::Plan& P = ctx->plan;
     gint::DevicePlan& D = ctx->dev;
-    const gint::Entry* d_entries = nullptr;
-    const gint::WorkItem* d_items = nullptr;
-    const gint::MirrorItem* d_mirror = nullptr;
 #define UP(vec, ptr)                                                   \
     if ((e = upload(ctx, vec, ptr)) != cudaSuccess) {                  \
         release(ctx);                                                  \
         return fail_cuda(e, "upload " #vec);                           \
     }
-    UP(P.entries, &d_entries)
-    UP(P.items, &d_items)
-    UP(P.mirror, &d_mirror)
-    UP(P.hash_keys, &D.hash_keys)
-    UP(P.hash_vals, &D.hash_vals)
+    UP(P.items, &D.items)
+    UP(P.regions, &D.regions)
+    UP(P.entries, &D.entries)
+    UP(P.tasks, &D.tasks)
+    UP(P.gmask, &D.gmask)
+    UP(P.rowinfo, &D.rowinfo)
+    UP(P.pair, &D.pair)
+    UP(P.slot_xyz, &D.slot_xyz)
+    UP(P.mirror, &D.mirror)
     UP(P.tab_packed, &D.tab)
     UP(P.sp_meta, &D.sp_meta)
     UP(P.sp_real, &D.sp_real)
 #undef UP
-    D.entries = reinterpret_cast<const gint::EntryDev*>(d_entries);
-    D.items = reinterpret_cast<const gint::WorkItemDev*>(d_items);
-    D.mirror = reinterpret_cast<const gint::MirrorItemDev*>(d_mirror);
     void* ctr = nullptr;
     if ((e = cudaMalloc(&ctr, 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
     std::memcpy(D.estep, P.estep, sizeof(D.estep));
     D.dV = P.dV;
-    for (int d = 0; d < 3; d++) {
-        D.ngrid[d] = P.ngrid[d];
-        D.bcell[d] = P.bcell[d];
-    }
+    for (int d = 0; d < 3; d++) D.ngrid[d] = P.ngrid[d];
+    D.nks_pad = P.nks_pad;
+    D.nslice = P.nslice;
     D.nitems = (int32_t)P.items.size();
     D.nmirror = (int32_t)P.mirror.size();
     D.tab_doubles = (int32_t)P.tab_packed.size();
-    D.max_entries = P.max_entries;
-    D.max_rows_pad = (P.max_rows + 7) & ~7;
-    D.hash_mask = P.hash_mask;
-    if ((e = gint::configure_kernels(D, P.smem_bytes, P.tables_in_smem)) != cudaSuccess) {
+    if ((e = gint::configure_kernels(P.smem_bytes, P.tables_in_smem)) != cudaSuccess) {
         release(ctx);
         return fail_cuda(e, "cudaFuncSetAttribute");
     }
@@ -256,17 +246,10 @@ int gint_get_cell_lists(const gint_ctx* ctx, int64_t* ncell, int64_t* nentry, in
     if (!ctx) return fail(GINT_EINVAL, "ctx is null");
     const gint::Plan& P = ctx->plan;
     if (ncell) *ncell = (int64_t)P.cell_start.size() - 1;
-    if (nentry) *nentry = (int64_t)P.entries.size();
+    if (nentry) *nentry = (int64_t)P.cell_atom.size();
     if (cell_start) std::memcpy(cell_start, P.cell_start.data(), P.cell_start.size() * sizeof(int64_t));
-    for (size_t i = 0; i < P.entries.size(); i++) {
-        if (entry_atom) entry_atom[i] = P.entries[i].atom;
-        if (entry_R) {
-            const int rp = P.entries[i].Rpack;
-            entry_R[3 * i] = ((rp >> 16) & 0xFF) - 128;
-            entry_R[3 * i + 1] = ((rp >> 8) & 0xFF) - 128;
-            entry_R[3 * i + 2] = (rp & 0xFF) - 128;
-        }
-    }
+    if (entry_atom && !P.cell_atom.empty()) std::memcpy(entry_atom, P.cell_atom.data(), P.cell_atom.size() * sizeof(int32_t));
+    if (entry_R && !P.cell_R.empty()) std::memcpy(entry_R, P.cell_R.data(), P.cell_R.size() * sizeof(int32_t));
     return GINT_OK;
 }
 

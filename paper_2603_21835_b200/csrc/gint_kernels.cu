@@ -2,20 +2,23 @@
 //
 //   H_mu,nu(R) = sum_g phi_mu(r_g - tau_I) V(r_g) phi_nu(r_g - tau_J - R) dV   (Eq. 45)
 //
-// One persistent CTA per SM pulls work items (big cell x point range) from a
-// global queue.  Per item (the paper's "BigGrid" batch):
-//   A. stage V*dV of the cell's points, the row map and the (entry,entry)->H-offset
-//      table in shared memory;
-//   B. evaluate phi for every listed (atom image, point) into a dense shared-memory
-//      tile  phi[row = orbital][col = point]  (Eq. 1: 4-point Lagrange radial table x
-//      real Y_lm) -- each phi value is computed exactly once per call;
-//   C. contract  C = phi diag(V dV) phi^T  on the FP64 tensor cores
-//      (mma.sync.m8n8k4.f64 -> DMMA.8x8x4; tcgen05 has no FP64 kind), upper
-//      triangle only, skipping (8-row fragment, 4-point k-step) pairs that hold no
-//      in-sphere point, and add the fragments into the canonical H blocks with
-//      red.global.add.f64.
-// A second kernel writes every non-canonical block as the transpose of its
-// partner, H(J,I,-R) = H(I,J,R)^T, and symmetrises the (I,I,0) blocks.
+// Output-stationary design.  One persistent CTA per SM (16 warps) pulls work items
+// from a global queue.  A work item is a set of up to 16 32x32 tiles (one per warp) of
+// the upper triangle of one region's  C = phi diag(V dV) phi^T  (the paper's per-BigGrid
+// dense contraction).  Each warp keeps its tile in registers (4 x 4
+// DMMA fragments) while the CTA streams the region's mesh points through shared memory
+// in slices of 32 points (8 k-steps of the FP64 tensor-core shape m8n8k4):
+//   * evaluate: phi of the orbitals the item needs on the slice's points (Eq. 1: 4-point
+//     Lagrange radial table x real Y_lm) into a double-buffered tile
+//     phi[row = orbital][col = point], and w = V dV of the points;
+//   * contract: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has no FP64 kind), A and
+//     B operands read from the same tile, B scaled by w as it is loaded; (fragment,
+//     k-step) pairs that hold no in-sphere point are skipped via host-built activity
+//     bytes.
+// After the last slice the warp adds its tile into the canonical H blocks with
+// red.global.add.f64 (once per item, not once per BigGrid).  A second kernel writes
+// every non-canonical block as the transpose of its partner, H(J,I,-R) = H(I,J,R)^T,
+// and symmetrises the (I,I,0) blocks.
 #include <cuda_runtime.h>
 
 #include <cstdint>
@@ -28,49 +31,101 @@ namespace {
 
 constexpr int kThreads = 512;
 constexpr int kWarps = kThreads / 32;
-constexpr int kTileFrags = 4;   // warp tile = 4 x 4 fragments of 8 x 8
+constexpr int kLD = kPhiLD;
+constexpr int kBufDoubles = kMaxSlots * kGroupRows * kLD;
+static_assert(kWarps == kTilesPerItem, "one tile per warp");
 
 __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
 }
-
-__device__ __forceinline__ uint32_t align16u(uint32_t x) { return (x + 15u) & ~15u; }
-
-__device__ __forceinline__ uint64_t hash_mix(uint64_t k) {
-    k ^= k >> 33; k *= 0xff51afd7ed558ccdULL; k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ULL; k ^= k >> 33;
-    return k;
+// warp-uniform condition: the instruction is predicated off as a whole
+__device__ __forceinline__ void dmma8x8x4_if(double& c0, double& c1, double a, double b, uint32_t cond) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
+        "@p mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n\t}"
+        : "+d"(c0), "+d"(c1)
+        : "d"(a), "d"(b), "r"(cond));
 }
 
-__device__ __forceinline__ uint32_t block_lookup(const DevicePlan& P, int I, int J, int r1, int r2, int r3) {
-    const uint64_t key = (((uint64_t)(uint32_t)I << 44) | ((uint64_t)(uint32_t)J << 24) |
-                          ((uint64_t)(uint32_t)(r1 + 128) << 16) | ((uint64_t)(uint32_t)(r2 + 128) << 8) |
-                          (uint64_t)(uint32_t)(r3 + 128)) + 1;
-    uint32_t h = (uint32_t)hash_mix(key) & P.hash_mask;
-    while (true) {
-        const uint64_t k = __ldg(P.hash_keys + h);
-        if (k == key) return __ldg(P.hash_vals + h);
-        if (k == 0) return kNoBlockDev;
-        h = (h + 1) & P.hash_mask;
+// phi of one entry on the 32 points of a slice (lane = point), Eq. 1.
+__device__ __forceinline__ void eval_task(const DevicePlan& P, const double* __restrict__ tab, const Entry* __restrict__ en,
+                                          const EvalTask tk, int slice, int lane, const double* __restrict__ s_off,
+                                          double* __restrict__ buf) {
+    double* p0 = tk.slot[0] >= 0 ? buf + (tk.slot[0] * kGroupRows) * kLD + lane : nullptr;
+    double* p1 = tk.slot[1] >= 0 ? buf + (tk.slot[1] * kGroupRows) * kLD + lane : nullptr;
+    double* p2 = tk.slot[2] >= 0 ? buf + (tk.slot[2] * kGroupRows) * kLD + lane : nullptr;
+    const int rr = tk.row0 & 31;
+    auto put = [&](int mu, double v) {
+        const int R = rr + mu;
+        double* p = (R < 32) ? p0 : ((R < 64) ? p1 : p2);
+        if (p) p[(R & 31) * kLD] = v;
+    };
+    const int norb = en->norb;
+    const uint32_t kbyte = (en->kmask[(slice * kSliceKsteps) >> 5] >> ((slice * kSliceKsteps) & 31)) & 0xFFu;
+    const int sp = (en->Rpack >> 24) & 0x7F;
+    const double rc2 = __ldg(P.sp_real + 2 * sp);
+    const int p = slice * kSlicePts + lane;
+    const double dx = en->rel[0] + s_off[p];
+    const double dy = en->rel[1] + s_off[kMaxRegionPoints + p];
+    const double dz = en->rel[2] + s_off[2 * kMaxRegionPoints + p];
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const bool inside = (kbyte != 0u) && (r2 < rc2);
+    if (__ballot_sync(0xffffffffu, inside) == 0u) {
+        for (int mu = 0; mu < norb; mu++) put(mu, 0.0);
+        return;
     }
-}
-
-struct EInfo {   // per entry, in shared memory
-    int32_t row0, norb, atom, Rpack;
-};
-
-// k-step mask of an entry restricted to the item's point range: bit s <=> any of
-// the 4 points p0+4s .. p0+4s+3 lies inside the entry's sphere.
-__device__ __forceinline__ uint32_t kstep_mask(uint32_t mlo, uint32_t mhi, int p0, int npts) {
-    uint64_t m = (((uint64_t)mhi << 32) | mlo) >> p0;
-    if (npts < 64) m &= (1ull << npts) - 1ull;
-    m |= m >> 1;
-    m |= m >> 2;             // bit 4s now holds the OR of bits 4s..4s+3
-    uint32_t out = 0;
-#pragma unroll
-    for (int s = 0; s < 16; s++) out |= (uint32_t)((m >> (4 * s)) & 1ull) << s;
-    return out;
+    const int32_t* meta = P.sp_meta + 12 * sp;
+    const int tab_off = __ldg(meta + 0), ntab = __ldg(meta + 1), nrad = __ldg(meta + 2);
+    const double inv_dr = __ldg(P.sp_real + 2 * sp + 1);
+    double x = 0.0, y = 0.0, z = 0.0, r = 0.0, lnz = 0.0;   // lnz: 1 if l>0 components survive
+    if (r2 >= 1e-24) {
+        const double rinv = rsqrt(r2);
+        r = r2 * rinv;
+        x = dx * rinv;
+        y = dy * rinv;
+        z = dz * rinv;
+        lnz = 1.0;
+    }
+    const double s = r * inv_dr;
+    int k = (int)s;
+    k = min(k, ntab - 4);
+    const double t = s - (double)k;
+    const double t1 = 1.0 - t, t2 = 2.0 - t, t3 = 3.0 - t;
+    const double in = inside ? 1.0 : 0.0;
+    const double L0 = in * (t1 * t2 * t3 * (1.0 / 6.0));
+    const double L1 = in * (t * t2 * t3 * 0.5);
+    const double L2 = in * (-t * t1 * t3 * 0.5);
+    const double L3 = in * (t * t1 * t2 * (1.0 / 6.0));
+    const double* Tk = tab + tab_off + (inside ? k : 0) * nrad;
+    // real Y_lm, l <= 2 (no Condon-Shortley phase; order fixed in include/gint.h)
+    const double Y00 = 0.28209479177387814;
+    const double c1 = 0.48860251190291992 * lnz;
+    const double c2a = 1.0925484305920792, c2b = 0.31539156525252005 * lnz, c2c = 0.54627421529603959;
+    int mu = 0;
+    for (int f = 0; f < nrad; f++) {
+        const double fv = Tk[f] * L0 + Tk[nrad + f] * L1 + Tk[2 * nrad + f] * L2 + Tk[3 * nrad + f] * L3;
+        const int l = __ldg(meta + 4 + f);
+        if (l == 0) {
+            put(mu, fv * Y00);
+            mu += 1;
+        } else if (l == 1) {
+            const double g1 = fv * c1;
+            put(mu, g1 * y);
+            put(mu + 1, g1 * z);
+            put(mu + 2, g1 * x);
+            mu += 3;
+        } else {
+            const double ga = fv * c2a;
+            put(mu, ga * (x * y));
+            put(mu + 1, ga * (y * z));
+            put(mu + 2, (fv * c2b) * (3.0 * z * z - 1.0));
+            put(mu + 3, ga * (x * z));
+            put(mu + 4, (fv * c2c) * (x * x - y * y));
+            mu += 5;
+        }
+    }
 }
 
 }  // namespace
@@ -78,255 +133,179 @@ __device__ __forceinline__ uint32_t kstep_mask(uint32_t mlo, uint32_t mhi, int p
 template <bool TAB_SMEM>
 __global__ void __launch_bounds__(kThreads, 1)
 gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__ V, double* __restrict__ H) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-
-    // ---- shared memory carve-up (mirrors fixed_smem_bytes() in gint_plan.cpp) ----
-    uint32_t off = 0;
-    double* s_tab = reinterpret_cast<double*>(smem_raw);
-    off += TAB_SMEM ? align16u((uint32_t)P.tab_doubles * 8u) : 0u;
-    double* s_w = reinterpret_cast<double*>(smem_raw + off);
-    off += kMaxItemPointsDev * 8;
-    int* s_misc = reinterpret_cast<int*>(smem_raw + off);   // [0] item index, [1] tile counter
-    off += 64;
-    EInfo* s_einfo = reinterpret_cast<EInfo*>(smem_raw + off);
-    off += align16u((uint32_t)P.max_entries * 16u);
-    uint16_t* s_rowinfo = reinterpret_cast<uint16_t*>(smem_raw + off);
-    off += align16u((uint32_t)P.max_rows_pad * 2u);
-    uint32_t* s_fragmask = reinterpret_cast<uint32_t*>(smem_raw + off);
-    off += align16u((uint32_t)(P.max_rows_pad / 8) * 4u);
-    uint32_t* s_pair = reinterpret_cast<uint32_t*>(smem_raw + off);
-    off += align16u((uint32_t)(P.max_entries * P.max_entries) * 4u);
-    double* s_phi = reinterpret_cast<double*>(smem_raw + off);
+    const SmemLayout L = smem_layout(TAB_SMEM ? (size_t)P.tab_doubles * sizeof(double) : 0);
+    double* s_tab = reinterpret_cast<double*>(smem_raw + L.tab);
+    double* s_off = reinterpret_cast<double*>(smem_raw + L.off);      // [3][512] Cartesian offset of a point slot
+    double* s_w = reinterpret_cast<double*>(smem_raw + L.w);          // [2][32]  V dV of the slice's points
+    uint8_t* s_gmask = smem_raw + L.gmask;                            // [slot][k-step] fragment activity nibbles
+    EvalTask* s_tasks = reinterpret_cast<EvalTask*>(smem_raw + L.tasks);
+    WorkItem* s_item = reinterpret_cast<WorkItem*>(smem_raw + L.item);
+    Region* s_region = reinterpret_cast<Region*>(smem_raw + L.item + sizeof(WorkItem));
+    int* s_misc = reinterpret_cast<int*>(smem_raw + L.misc);
+    double* s_phi = reinterpret_cast<double*>(smem_raw + L.phi);      // [2][slot*32 + row][kLD]
 
     if (TAB_SMEM) {
         for (int i = tid; i < P.tab_doubles; i += kThreads) s_tab[i] = __ldg(P.tab + i);
     }
     const double* tab = TAB_SMEM ? s_tab : P.tab;
-
-    const int by = P.bcell[1], bz = P.bcell[2];
-    const int byz = by * bz;
+    for (int p = tid; p < P.nslice * kSlicePts; p += kThreads) {
+        const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
+        for (int k = 0; k < 3; k++)
+            s_off[k * kMaxRegionPoints + p] = c.x * P.estep[k] + c.y * P.estep[3 + k] + c.z * P.estep[6 + k];
+    }
+    const int frow = lane >> 2, fk = lane & 3;
 
     while (true) {
         if (tid == 0) s_misc[0] = (int)atomicAdd(P.counter, 1u);
-        __syncthreads();   // also: every warp has left phase C of the previous item
+        __syncthreads();   // also: every warp has finished the previous item (flush reads s_item / s_region)
         const int item = s_misc[0];
         if (item >= P.nitems) break;
-        const WorkItemDev wi = P.items[item];
-        const int m = wi.nentry, nrow = wi.nrow, nrow_pad = (nrow + 7) & ~7, npts = wi.npts, p0 = wi.p0;
-        const int LD = npts + 4;
-        const EntryDev* ent = P.entries + wi.entry0;
-
-        // ---------------- phase A: staging ----------------------------------------
-        if (tid == 0) s_misc[1] = 0;
-        for (int e = tid; e < m; e += kThreads) {
-            EInfo ei;
-            ei.row0 = ent[e].row0;
-            ei.norb = ent[e].norb;
-            ei.atom = ent[e].atom;
-            ei.Rpack = ent[e].Rpack;
-            s_einfo[e] = ei;
-            for (int mu = 0; mu < ei.norb; mu++) s_rowinfo[ei.row0 + mu] = (uint16_t)((e << 6) | mu);
-        }
-        for (int r = nrow + tid; r < nrow_pad; r += kThreads) s_rowinfo[r] = 0xFFFFu;
-        for (int c = tid; c < kMaxItemPointsDev; c += kThreads) {
-            double wv = 0.0;
-            if (c < npts) {
-                const int p = p0 + c;
-                const int ix = p / byz, iy = (p - ix * byz) / bz, iz = p - ix * byz - iy * bz;
-                const int g1 = wi.origin[0] + ix, g2 = wi.origin[1] + iy, g3 = wi.origin[2] + iz;
-                if (ix < P.bcell[0] && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
-                    wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
-            }
-            s_w[c] = wv;
-        }
-        for (int f = tid; f < nrow_pad / 8; f += kThreads) {
-            uint32_t msk = 0;
-            for (int e = 0; e < m; e++) {
-                const int r0 = ent[e].row0, r1 = r0 + ent[e].norb;
-                if (r0 < 8 * f + 8 && r1 > 8 * f) msk |= kstep_mask(ent[e].mask_lo, ent[e].mask_hi, p0, npts);
-            }
-            s_fragmask[f] = msk;
-        }
-        for (int idx = tid; idx < m * m; idx += kThreads) {
-            const int ea = idx / m, eb = idx - ea * m;
-            if (ea > eb) continue;
-            const int Ra = ent[ea].Rpack, Rb = ent[eb].Rpack;
-            s_pair[idx] = block_lookup(P, ent[ea].atom, ent[eb].atom, ((Rb >> 16) & 0xFF) - ((Ra >> 16) & 0xFF),
-                                       ((Rb >> 8) & 0xFF) - ((Ra >> 8) & 0xFF), (Rb & 0xFF) - (Ra & 0xFF));
-        }
-        for (int idx = tid; idx < (nrow_pad - nrow) * LD; idx += kThreads) s_phi[nrow * LD + idx] = 0.0;
-
-        // ---------------- phase B: phi tile (Eq. 1) ----------------------------------
+        // ---------------- stage the item ---------------------------------------------------------
+        if (tid < (int)(sizeof(WorkItem) / 4))
+            reinterpret_cast<uint32_t*>(s_item)[tid] = __ldg(reinterpret_cast<const uint32_t*>(P.items + item) + tid);
+        __syncthreads();
+        const int ntask = s_item->ntask, ntile = s_item->ntile, nslot = s_item->nslot;
+        const uint32_t slice_mask = s_item->slice_mask;
+        const Region* greg = P.regions + s_item->region;
+        if (tid < (int)(sizeof(Region) / 4))
+            reinterpret_cast<uint32_t*>(s_region)[tid] = __ldg(reinterpret_cast<const uint32_t*>(greg) + tid);
+        for (int i = tid; i < ntask * (int)(sizeof(EvalTask) / 4); i += kThreads)
+            reinterpret_cast<uint32_t*>(s_tasks)[i] = __ldg(reinterpret_cast<const uint32_t*>(P.tasks + s_item->task0) + i);
         {
-            const int ngroups = (npts + 31) >> 5;
-            for (int task = warp; task < m * ngroups; task += kWarps) {
-                const int e = task / ngroups, g = task - e * ngroups;
-                const EntryDev en = ent[e];
-                const int col = 32 * g + lane;
-                const int p = p0 + col;
-                const bool colvalid = col < npts;
-                const uint32_t mword = (p < 32) ? en.mask_lo : en.mask_hi;
-                const bool inside = colvalid && ((mword >> (p & 31)) & 1u);
-                double* dst = s_phi + en.row0 * LD + col;
-                if (__ballot_sync(0xffffffffu, inside) == 0u) {
-                    if (colvalid)
-                        for (int mu = 0; mu < en.norb; mu++) dst[mu * LD] = 0.0;
-                    continue;
-                }
-                const int sp = (en.Rpack >> 24) & 0x7F;
-                const int32_t* meta = P.sp_meta + 12 * sp;
-                const int tab_off = __ldg(meta + 0), ntab = __ldg(meta + 1), nrad = __ldg(meta + 2);
-                const double inv_dr = __ldg(P.sp_real + 2 * sp + 1);
-                const int ix = p / byz, iy = (p - ix * byz) / bz, iz = p - ix * byz - iy * bz;
-                const double dx = en.rel[0] + ix * P.estep[0] + iy * P.estep[3] + iz * P.estep[6];
-                const double dy = en.rel[1] + ix * P.estep[1] + iy * P.estep[4] + iz * P.estep[7];
-                const double dz = en.rel[2] + ix * P.estep[2] + iy * P.estep[5] + iz * P.estep[8];
-                const double r2 = dx * dx + dy * dy + dz * dz;
-                double x = 0.0, y = 0.0, z = 0.0, r = 0.0, lnz = 0.0;   // lnz: 1 if l>0 components survive
-                if (r2 >= 1e-24) {
-                    const double rinv = rsqrt(r2);
-                    r = r2 * rinv;
-                    x = dx * rinv;
-                    y = dy * rinv;
-                    z = dz * rinv;
-                    lnz = 1.0;
-                }
-                const double s = r * inv_dr;
-                int k = (int)s;
-                k = min(k, ntab - 4);
-                const double t = s - (double)k;
-                const double t1 = 1.0 - t, t2 = 2.0 - t, t3 = 3.0 - t;
-                const double in = inside ? 1.0 : 0.0;
-                const double L0 = in * (t1 * t2 * t3 * (1.0 / 6.0));
-                const double L1 = in * (t * t2 * t3 * 0.5);
-                const double L2 = in * (-t * t1 * t3 * 0.5);
-                const double L3 = in * (t * t1 * t2 * (1.0 / 6.0));
-                const double* Tk = tab + tab_off + (inside ? k : 0) * nrad;
-                // real Y_lm, l <= 2 (no Condon-Shortley phase; order fixed in include/gint.h)
-                const double Y00 = 0.28209479177387814;
-                const double c1 = 0.48860251190291992 * lnz;
-                const double c2a = 1.0925484305920792, c2b = 0.31539156525252005 * lnz, c2c = 0.54627421529603959;
-                double* o = dst;
-                for (int f = 0; f < nrad; f++) {
-                    const double fv = Tk[f] * L0 + Tk[nrad + f] * L1 + Tk[2 * nrad + f] * L2 + Tk[3 * nrad + f] * L3;
-                    const int l = __ldg(meta + 4 + f);
-                    if (l == 0) {
-                        if (colvalid) o[0] = fv * Y00;
-                        o += LD;
-                    } else if (l == 1) {
-                        const double g1 = fv * c1;
-                        if (colvalid) {
-                            o[0] = g1 * y;
-                            o[LD] = g1 * z;
-                            o[2 * LD] = g1 * x;
-                        }
-                        o += 3 * LD;
-                    } else {
-                        const double ga = fv * c2a;
-                        if (colvalid) {
-                            o[0] = ga * (x * y);
-                            o[LD] = ga * (y * z);
-                            o[2 * LD] = (fv * c2b) * (3.0 * z * z - 1.0);
-                            o[3 * LD] = ga * (x * z);
-                            o[4 * LD] = (fv * c2c) * (x * x - y * y);
-                        }
-                        o += 5 * LD;
-                    }
-                }
+            const int wpr = P.nks_pad >> 2;   // 32-bit words per group row of activity bytes
+            const int gmask_off = __ldg(&greg->gmask_off);
+            for (int i = tid; i < nslot * wpr; i += kThreads) {
+                const int slot = i / wpr, wd = i - slot * wpr;
+                reinterpret_cast<uint32_t*>(s_gmask + slot * kMaxKsteps)[wd] =
+                    __ldg(reinterpret_cast<const uint32_t*>(P.gmask + gmask_off + (int)s_item->slot_group[slot] * P.nks_pad) + wd);
             }
         }
         __syncthreads();
+        const int ox = s_region->origin[0], oy = s_region->origin[1], oz = s_region->origin[2];
 
-        // ---------------- phase C: C = phi diag(w) phi^T, upper triangle ----------------
-        {
-            const int NF = nrow_pad >> 3;
-            const int NT = (NF + kTileFrags - 1) / kTileFrags;
-            const int ntiles = NT * (NT + 1) / 2;
-            const int nk = npts >> 2;
-            const int frow = lane >> 2, fk = lane & 3;
-            while (true) {
-                int t = 0;
-                if (lane == 0) t = atomicAdd(&s_misc[1], 1);
-                t = __shfl_sync(0xffffffffu, t, 0);
-                if (t >= ntiles) break;
-                // tile index -> (ti <= tj), column-major over the upper triangle, large tj first
-                t = ntiles - 1 - t;
-                int tj = (int)((sqrtf(8.0f * (float)t + 1.0f) - 1.0f) * 0.5f);
-                while ((tj + 1) * (tj + 2) / 2 <= t) tj++;
-                while (tj * (tj + 1) / 2 > t) tj--;
-                const int ti = t - tj * (tj + 1) / 2;
-                const int fi0 = kTileFrags * ti, fj0 = kTileFrags * tj;
-                uint32_t rmask[kTileFrags], cmask[kTileFrags];
+        auto evaluate = [&](int slice, int b) {
+            double* buf = s_phi + b * kBufDoubles;
+            if (warp == kWarps - 1) {   // w = V dV of the slice's points (0 outside the mesh)
+                const int p = slice * kSlicePts + lane;
+                const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
+                const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
+                double wv = 0.0;
+                if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
+                    wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
+                s_w[b * kSlicePts + lane] = wv;
+            }
+            for (int t = warp; t < ntask; t += kWarps) {
+                const EvalTask tk = s_tasks[t];
+                eval_task(P, tab, P.entries + tk.entry, tk, slice, lane, s_off, buf);
+            }
+        };
+
+        double acc[4][4][2];
 #pragma unroll
-                for (int i = 0; i < kTileFrags; i++) {
-                    rmask[i] = (fi0 + i < NF) ? s_fragmask[fi0 + i] : 0u;
-                    cmask[i] = (fj0 + i < NF) ? s_fragmask[fj0 + i] : 0u;
-                }
-                double acc[kTileFrags][kTileFrags][2];
+        for (int i = 0; i < 4; i++)
 #pragma unroll
-                for (int i = 0; i < kTileFrags; i++)
+            for (int j = 0; j < 4; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+        const bool has_tile = warp < ntile;
+        const int sa = has_tile ? s_item->tiles[warp][0] : 0, sb = has_tile ? s_item->tiles[warp][1] : 0;
+        const uint32_t tile_mask = (sa == sb) ? 0x8CEFu : 0xFFFFu;   // diagonal tile: fragments i <= j only
+
+        // ---------------- stream the slices ------------------------------------------------------
+        uint32_t todo = slice_mask;
+        int cur = __ffs(todo) - 1;
+        todo &= todo - 1;
+        int b = 0;
+        evaluate(cur, 0);
+        __syncthreads();
+        while (true) {
+            const int next = todo ? __ffs(todo) - 1 : -1;
+            todo &= todo - 1;
+            if (next >= 0) evaluate(next, b ^ 1);
+            if (has_tile) {
+                const double* bufp = s_phi + b * kBufDoubles;
+                const double* pa = bufp + (sa * kGroupRows + frow) * kLD + fk;
+                const double* pb = bufp + (sb * kGroupRows + frow) * kLD + fk;
+                const double* pw = s_w + b * kSlicePts + fk;
+                const uint2 ra8 = *reinterpret_cast<const uint2*>(s_gmask + sa * kMaxKsteps + cur * kSliceKsteps);
+                const uint2 ca8 = *reinterpret_cast<const uint2*>(s_gmask + sb * kMaxKsteps + cur * kSliceKsteps);
+#pragma unroll 1
+                for (int ks = 0; ks < kSliceKsteps; ks++) {
+                    const uint32_t rw = (ks < 4) ? ra8.x : ra8.y, cw = (ks < 4) ? ca8.x : ca8.y;
+                    const uint32_t ra = (rw >> (8 * (ks & 3))) & 0xFu, ca = (cw >> (8 * (ks & 3))) & 0xFu;
+                    // pair mask: bit 4i+j <=> row fragment i and column fragment j both active
+                    const uint32_t spread = (ra & 1u) | ((ra & 2u) << 3) | ((ra & 4u) << 6) | ((ra & 8u) << 9);
+                    const uint32_t pm = (ca * spread) & tile_mask;
+                    if (pm == 0u) continue;
+                    const double wv = pw[4 * ks];
+                    double a[4], bb[4];
 #pragma unroll
-                    for (int j = 0; j < kTileFrags; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
-                const double* pa = s_phi + (8 * fi0 + frow) * LD + fk;
-                const double* pb = s_phi + (8 * fj0 + frow) * LD + fk;
-                for (int s = 0; s < nk; s++) {
-                    uint32_t ra = 0, ca = 0;
-#pragma unroll
-                    for (int i = 0; i < kTileFrags; i++) {
-                        ra |= ((rmask[i] >> s) & 1u) << i;
-                        ca |= ((cmask[i] >> s) & 1u) << i;
+                    for (int i = 0; i < 4; i++) {
+                        a[i] = pa[(8 * i) * kLD + 4 * ks];
+                        bb[i] = wv * pb[(8 * i) * kLD + 4 * ks];
                     }
-                    if (ra == 0u || ca == 0u) continue;
-                    const double wv = s_w[4 * s + fk];
-                    double a[kTileFrags], b[kTileFrags];
+                    if (pm == 0xFFFFu) {
 #pragma unroll
-                    for (int i = 0; i < kTileFrags; i++) {
-                        a[i] = ((ra >> i) & 1u) ? pa[(8 * i) * LD + 4 * s] : 0.0;
-                        b[i] = ((ca >> i) & 1u) ? wv * pb[(8 * i) * LD + 4 * s] : 0.0;
+                        for (int i = 0; i < 4; i++)
+#pragma unroll
+                            for (int j = 0; j < 4; j++) dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i], bb[j]);
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 4; i++)
+#pragma unroll
+                            for (int j = 0; j < 4; j++)
+                                dmma8x8x4_if(acc[i][j][0], acc[i][j][1], a[i], bb[j], pm & (1u << (4 * i + j)));
                     }
-#pragma unroll
-                    for (int i = 0; i < kTileFrags; i++)
-#pragma unroll
-                        for (int j = 0; j < kTileFrags; j++)
-                            if (((ra >> i) & 1u) && ((ca >> j) & 1u) && (fi0 + i <= fj0 + j))
-                                dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i], b[j]);
                 }
-                // ---- flush: add the fragments into the canonical H blocks ----
+            }
+            __syncthreads();
+            if (next < 0) break;
+            cur = next;
+            b ^= 1;
+        }
+
+        // ---------------- flush: add the tile into the canonical H blocks ---------------------------
+        if (has_tile) {
+            const int ga = s_item->slot_group[sa], gb = s_item->slot_group[sb];
+            const uint32_t* rinfo = P.rowinfo + s_region->rowinfo_off;
+            const uint32_t* pair = P.pair + s_region->pair_off;
+            const int m = s_region->nentry;
 #pragma unroll
-                for (int i = 0; i < kTileFrags; i++) {
-                    if (rmask[i] == 0u) continue;
-                    const int r = 8 * (fi0 + i) + frow;
-                    const uint32_t ri = s_rowinfo[r];
-                    if (ri == 0xFFFFu) continue;
-                    const int ea = ri >> 6, mu = ri & 63;
+            for (int i = 0; i < 4; i++) {
+                const int row = ga * kGroupRows + 8 * i + frow;
+                const uint32_t ri = __ldg(rinfo + row);
+                if (ri == kNoBlock) continue;
+                const int ea = ri & 0xFFF, mu = (ri >> 12) & 0xFF, nI = ri >> 20;
 #pragma unroll
-                    for (int j = 0; j < kTileFrags; j++) {
-                        if ((rmask[i] & cmask[j]) == 0u || (fi0 + i > fj0 + j)) continue;
+                for (int j = 0; j < 4; j++) {
+                    if (sa == sb && i > j) continue;
 #pragma unroll
-                        for (int h = 0; h < 2; h++) {
-                            const int c = 8 * (fj0 + j) + 2 * fk + h;
-                            const uint32_t ci = s_rowinfo[c];
-                            if (ci == 0xFFFFu || r > c) continue;
-                            const int eb = ci >> 6, nu = ci & 63;
-                            const uint32_t base = s_pair[ea * m + eb];
-                            if (base == kNoBlockDev) continue;
-                            atomicAdd(H + (size_t)base + (size_t)(mu * s_einfo[eb].norb + nu), acc[i][j][h]);
-                        }
+                    for (int h = 0; h < 2; h++) {
+                        const double v = acc[i][j][h];
+                        if (v == 0.0) continue;
+                        const int col = gb * kGroupRows + 8 * j + 2 * fk + h;
+                        if (row > col) continue;
+                        const uint32_t ci = __ldg(rinfo + col);
+                        if (ci == kNoBlock) continue;
+                        const int eb = ci & 0xFFF, nu = (ci >> 12) & 0xFF, nJ = ci >> 20;
+                        const uint32_t pr = __ldg(pair + ea * m + eb);
+                        if (pr == kNoBlock) continue;
+                        const uint32_t idx = (pr & kPairTransposed) ? (uint32_t)(nu * nI + mu) : (uint32_t)(mu * nJ + nu);
+                        atomicAdd(H + (size_t)(pr & ~kPairTransposed) + idx, v);
                     }
                 }
             }
         }
-        // loop-top __syncthreads separates phase C from the next item's staging
+        // loop-top __syncthreads separates the flush from the next item's staging
     }
 }
 
 // H(J,I,-R) = H(I,J,R)^T for every non-canonical block; lower <- upper for (I,I,0).
-__global__ void __launch_bounds__(256) gint_mirror_kernel(const MirrorItemDev* __restrict__ items, int nitems,
+__global__ void __launch_bounds__(256) gint_mirror_kernel(const MirrorItem* __restrict__ items, int nitems,
                                                           double* __restrict__ H) {
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (w >= nitems) return;
-    const MirrorItemDev it = items[w];
+    const MirrorItem it = items[w];
     const int n = it.nI * it.nJ;
     if (it.src == it.dst) {
         for (int idx = lane; idx < n; idx += 32) {
@@ -342,8 +321,7 @@ __global__ void __launch_bounds__(256) gint_mirror_kernel(const MirrorItemDev* _
 }
 
 // ---- launchers -----------------------------------------------------------------------
-cudaError_t configure_kernels(const DevicePlan& P, size_t smem_bytes, bool tab_smem) {
-    (void)P;
+cudaError_t configure_kernels(size_t smem_bytes, bool tab_smem) {
     if (tab_smem)
         return cudaFuncSetAttribute(gint_vlocal_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     return cudaFuncSetAttribute(gint_vlocal_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);

@@ -2,6 +2,7 @@
 #include "gint_plan.hpp"
 
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstring>
 #include <numeric>
@@ -38,24 +39,6 @@ inline int64_t floordiv(int64_t a, int64_t b) {
 inline size_t align16(size_t x) { return (x + 15) & ~size_t(15); }
 
 }  // namespace
-
-// Must mirror the carve-up in gint_kernels.cu (SmemLayout).
-static size_t fixed_smem_bytes(int max_entries, int max_rows_pad, size_t table_bytes) {
-    size_t b = 0;
-    b += align16(table_bytes);
-    b += kMaxItemPoints * sizeof(double);                    // w[p] = V dV
-    b += 64;                                                 // counters
-    b += align16((size_t)max_entries * 16);                  // entry info (row0, norb, atom, Rpack)
-    b += align16((size_t)max_rows_pad * sizeof(uint16_t));   // row -> (entry, mu)
-    b += align16((size_t)max_rows_pad / 8 * sizeof(uint32_t));   // per fragment-row k-step masks
-    b += align16((size_t)max_entries * max_entries * sizeof(uint32_t));   // pair -> H offset
-    return b;
-}
-
-size_t item_smem_bytes(int nrow, int npts, int nentry, size_t table_bytes) {
-    const int nrow_pad = (nrow + 7) & ~7;
-    return fixed_smem_bytes(nentry, nrow_pad, table_bytes) + (size_t)nrow_pad * (npts + 4) * sizeof(double);
-}
 
 int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecies, const SpeciesHost* species,
                int natom, const int32_t* atom_species, const double* atom_pos, const int32_t bcell[3], int rank,
@@ -104,16 +87,22 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         for (int c = 0; c < 3; c++)
             if (!std::isfinite(atom_pos[3 * a + c])) { err = "atom position not finite"; return GINT_EINVAL; }
     }
-    int B = 1;
+    int64_t bprod = 1;
     for (int d = 0; d < 3; d++) {
         P.ngrid[d] = ngrid[d];
-        P.bcell[d] = (bcell && bcell[d] > 0) ? bcell[d] : 4;
-        if (P.bcell[d] > ngrid[d]) P.bcell[d] = ngrid[d];
-        P.ncell[d] = (ngrid[d] + P.bcell[d] - 1) / P.bcell[d];
-        B *= P.bcell[d];
+        int b = (bcell && bcell[d] > 0) ? bcell[d] : 0;
+        bprod *= (b > 0 ? b : 1);
+        if (b == 0) {   // default: the largest of 8, 6, 4 that divides N (8 with a ragged last region otherwise)
+            b = 8;
+            for (int c : {8, 6, 4})
+                if (ngrid[d] % c == 0) { b = c; break; }
+        }
+        if (b > ngrid[d]) b = ngrid[d];
+        P.bcell[d] = b;
+        P.ncell[d] = (ngrid[d] + b - 1) / b;
         for (int c = 0; c < 3; c++) P.estep[3 * d + c] = lattice[3 * d + c] / (double)ngrid[d];
     }
-    if (B > 64) { err = "big cell larger than 64 mesh points"; return GINT_EUNSUPPORTED; }
+    if (bprod > kMaxRegionPoints || (int64_t)P.bcell[0] * P.bcell[1] * P.bcell[2] > kMaxRegionPoints) { err = "region (bcell) larger than 512 mesh points"; return GINT_EUNSUPPORTED; }
     P.dV = vol / ((double)ngrid[0] * (double)ngrid[1] * (double)ngrid[2]);
 
     double inv[9];
@@ -219,16 +208,44 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     }
     const size_t table_bytes_all = P.tab_packed.size() * sizeof(double);
     P.tables_in_smem = table_bytes_all <= 64 * 1024;
-    const size_t table_bytes = P.tables_in_smem ? table_bytes_all : 0;
 
-    // ---- per-cell (atom image) lists --------------------------------------------
+    // smem: the radial tables go to shared memory when the phi double buffer leaves room for them
+    if (P.tables_in_smem && smem_layout(table_bytes_all).total > kSmemLimit) P.tables_in_smem = false;
+    const size_t table_bytes = P.tables_in_smem ? table_bytes_all : 0;
+    P.smem_bytes = smem_layout(table_bytes).total;
+    if (P.smem_bytes > kSmemLimit) { err = "internal: shared-memory layout exceeds 227 KB"; return GINT_EUNSUPPORTED; }
+
+    // ---- point order inside a region: k-steps of 4 points, slices of 8 k-steps -----------------
     const int bx = P.bcell[0], by = P.bcell[1], bz = P.bcell[2];
+    P.npts = bx * by * bz;
+    {
+        std::vector<std::array<uint8_t, 4>> order;
+        if (bx % 2 == 0 && by % 2 == 0) {   // compact 2 x 2 x 1 k-steps (fewer partially covered k-steps)
+            for (int x = 0; x < bx; x += 2)
+                for (int y = 0; y < by; y += 2)
+                    for (int z = 0; z < bz; z++)
+                        for (int q = 0; q < 4; q++) order.push_back({(uint8_t)(x + (q >> 1)), (uint8_t)(y + (q & 1)), (uint8_t)z, 1});
+        } else {
+            for (int x = 0; x < bx; x++)
+                for (int y = 0; y < by; y++)
+                    for (int z = 0; z < bz; z++) order.push_back({(uint8_t)x, (uint8_t)y, (uint8_t)z, 1});
+        }
+        P.nks = (P.npts + kKstepPts - 1) / kKstepPts;
+        P.nslice = (P.nks + kSliceKsteps - 1) / kSliceKsteps;
+        P.nks_pad = P.nslice * kSliceKsteps;
+        while ((int)order.size() < P.nks_pad * kKstepPts) order.push_back({0, 0, 0, 0});
+        P.slot_xyz.resize(order.size() * 4);
+        for (size_t i = 0; i < order.size(); i++)
+            for (int c = 0; c < 4; c++) P.slot_xyz[4 * i + c] = order[i][c];
+    }
+    const int nslot_pts = P.nks_pad * kKstepPts;
+
+    // ---- (region, atom image) entries -------------------------------------------------------------
     const int64_t ncells = (int64_t)P.ncell[0] * P.ncell[1] * P.ncell[2];
     const double* e1 = P.estep;
     const double* e2 = P.estep + 3;
     const double* e3 = P.estep + 6;
-    // bounding-sphere radius of a full cell about its centre point
-    double cell_rad = 0;
+    double cell_rad = 0;   // bounding-sphere radius of a full region about its centre
     for (int s1 = -1; s1 <= 1; s1 += 2)
         for (int s2 = -1; s2 <= 1; s2 += 2) {
             double v[3];
@@ -236,9 +253,9 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 v[c] = 0.5 * ((bx - 1) * e1[c] + s1 * (by - 1) * e2[c] + s2 * (bz - 1) * e3[c]);
             cell_rad = std::max(cell_rad, std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
         }
-    struct Tmp { int64_t cell; Entry e; };
+    struct Tmp { int64_t cell; int npop; Entry e; };
     std::vector<Tmp> tmp;
-    tmp.reserve((size_t)natom * 2048);
+    tmp.reserve((size_t)natom * 256);
     std::vector<int32_t> npoint_orb((size_t)ngrid[0] * ngrid[1] * ngrid[2], 0);
     double n_insphere = 0;
     for (int I = 0; I < natom; I++) {
@@ -252,7 +269,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             nlo[d] = (int64_t)std::floor((f - rc * blen[d]) * ngrid[d]) - 1;
             nhi[d] = (int64_t)std::ceil((f + rc * blen[d]) * ngrid[d]) + 1;
         }
-        // walk unwrapped (image q, cell c) pairs covering [nlo, nhi] in each dimension
+        // walk unwrapped (image q, region c) pairs covering [nlo, nhi] in each dimension
         std::vector<std::pair<int, int>> rng[3];   // (q, c)
         for (int d = 0; d < 3; d++) {
             const int64_t N = ngrid[d];
@@ -269,118 +286,279 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                     const int c[3] = {qc1.second, qc2.second, qc3.second};
                     if (std::abs(q[0]) > 127 || std::abs(q[1]) > 127 || std::abs(q[2]) > 127) { err = "image index beyond +-127"; return GINT_EUNSUPPORTED; }
                     Entry e;
+                    std::memset(&e, 0, sizeof(e));
                     const int o[3] = {c[0] * bx, c[1] * by, c[2] * bz};
                     for (int k = 0; k < 3; k++) {
                         const double origin = o[0] * e1[k] + o[1] * e2[k] + o[2] * e3[k];
                         const double centre = tau[k] - (q[0] * lattice[k] + q[1] * lattice[3 + k] + q[2] * lattice[6 + k]);
                         e.rel[k] = origin - centre;
                     }
-                    // quick reject with the bounding sphere of the (full) cell
+                    // quick reject with the bounding sphere of the (full) region
                     double cc[3];
                     for (int k = 0; k < 3; k++)
                         cc[k] = e.rel[k] + 0.5 * ((bx - 1) * e1[k] + (by - 1) * e2[k] + (bz - 1) * e3[k]);
                     const double dcen = std::sqrt(cc[0] * cc[0] + cc[1] * cc[1] + cc[2] * cc[2]);
                     if (dcen >= rc + cell_rad + 1e-9) continue;
-                    uint64_t mask = 0;
-                    for (int ix = 0; ix < bx; ix++) {
-                        if (o[0] + ix >= ngrid[0]) break;
-                        for (int iy = 0; iy < by; iy++) {
-                            if (o[1] + iy >= ngrid[1]) break;
-                            for (int iz = 0; iz < bz; iz++) {
-                                if (o[2] + iz >= ngrid[2]) break;
-                                const double dx = e.rel[0] + ix * e1[0] + iy * e2[0] + iz * e3[0];
-                                const double dy = e.rel[1] + ix * e1[1] + iy * e2[1] + iz * e3[1];
-                                const double dz = e.rel[2] + ix * e1[2] + iy * e2[2] + iz * e3[2];
-                                if (dx * dx + dy * dy + dz * dz < rc2) {
-                                    mask |= 1ull << ((ix * by + iy) * bz + iz);
-                                    npoint_orb[((size_t)(o[0] + ix) * ngrid[1] + (o[1] + iy)) * ngrid[2] + (o[2] + iz)] += norb;
-                                }
-                            }
+                    int npin = 0;
+                    for (int s = 0; s < nslot_pts; s++) {
+                        const uint8_t* xyz = &P.slot_xyz[4 * (size_t)s];
+                        if (!xyz[3]) continue;
+                        const int ix = xyz[0], iy = xyz[1], iz = xyz[2];
+                        if (o[0] + ix >= ngrid[0] || o[1] + iy >= ngrid[1] || o[2] + iz >= ngrid[2]) continue;
+                        const double dx = e.rel[0] + ix * e1[0] + iy * e2[0] + iz * e3[0];
+                        const double dy = e.rel[1] + ix * e1[1] + iy * e2[1] + iz * e3[1];
+                        const double dz = e.rel[2] + ix * e1[2] + iy * e2[2] + iz * e3[2];
+                        if (dx * dx + dy * dy + dz * dz < rc2) {
+                            const int ks = s / kKstepPts;
+                            e.kmask[ks >> 5] |= 1u << (ks & 31);
+                            npin++;
+                            npoint_orb[((size_t)(o[0] + ix) * ngrid[1] + (o[1] + iy)) * ngrid[2] + (o[2] + iz)] += norb;
                         }
                     }
-                    if (!mask) continue;
-                    n_insphere += (double)__builtin_popcountll(mask);
+                    if (!npin) continue;
+                    n_insphere += (double)npin;
                     e.atom = I;
                     e.Rpack = ((-q[0] + 128) << 16) | ((-q[1] + 128) << 8) | (-q[2] + 128) | (sp_id << 24);
-                    e.mask_lo = (uint32_t)mask;
-                    e.mask_hi = (uint32_t)(mask >> 32);
-                    e.row0 = 0;
                     e.norb = norb;
-                    tmp.push_back({((int64_t)c[0] * P.ncell[1] + c[1]) * P.ncell[2] + c[2], e});
+                    int npop = 0;
+                    for (int k = 0; k < 4; k++) npop += __builtin_popcount(e.kmask[k]);
+                    tmp.push_back({((int64_t)c[0] * P.ncell[1] + c[1]) * P.ncell[2] + c[2], npop, e});
                 }
         }
     }
-    // sort by (cell, atom, R1, R2, R3): inside a cell a<b in list order implies block (I_a,I_b,R_b-R_a) canonical
     auto rkey = [](const Entry& e) { return (uint32_t)(e.Rpack & 0xFFFFFF); };
+    // query lists: per region sorted by (atom, R)
+    {
+        std::vector<size_t> idx(tmp.size());
+        std::iota(idx.begin(), idx.end(), size_t(0));
+        std::sort(idx.begin(), idx.end(), [&](size_t a, size_t b) {
+            if (tmp[a].cell != tmp[b].cell) return tmp[a].cell < tmp[b].cell;
+            if (tmp[a].e.atom != tmp[b].e.atom) return tmp[a].e.atom < tmp[b].e.atom;
+            return rkey(tmp[a].e) < rkey(tmp[b].e);
+        });
+        P.cell_start.assign((size_t)ncells + 1, 0);
+        for (auto& t : tmp) P.cell_start[(size_t)t.cell + 1]++;
+        for (int64_t c = 0; c < ncells; c++) P.cell_start[(size_t)c + 1] += P.cell_start[(size_t)c];
+        P.cell_atom.resize(tmp.size());
+        P.cell_R.resize(3 * tmp.size());
+        for (size_t i = 0; i < idx.size(); i++) {
+            const Entry& e = tmp[idx[i]].e;
+            P.cell_atom[i] = e.atom;
+            P.cell_R[3 * i] = ((e.Rpack >> 16) & 0xFF) - 128;
+            P.cell_R[3 * i + 1] = ((e.Rpack >> 8) & 0xFF) - 128;
+            P.cell_R[3 * i + 2] = (e.Rpack & 0xFF) - 128;
+        }
+    }
+    // kernel order: per region densest entries first (most active k-steps), then (atom, R)
     std::sort(tmp.begin(), tmp.end(), [&](const Tmp& a, const Tmp& b) {
         if (a.cell != b.cell) return a.cell < b.cell;
+        if (a.npop != b.npop) return a.npop > b.npop;
         if (a.e.atom != b.e.atom) return a.e.atom < b.e.atom;
         return rkey(a.e) < rkey(b.e);
     });
-    P.cell_start.assign((size_t)ncells + 1, 0);
-    for (auto& t : tmp) P.cell_start[(size_t)t.cell + 1]++;
-    for (int64_t c = 0; c < ncells; c++) P.cell_start[(size_t)c + 1] += P.cell_start[(size_t)c];
     P.entries.resize(tmp.size());
     for (size_t i = 0; i < tmp.size(); i++) P.entries[i] = tmp[i].e;
+
+    // ---- per region: rows, fragment / group activity, row info, pair table, tiles, work items -----
+    struct ItemCost { double cost; };
+    std::vector<double> item_cost;
+    double exec_dmma = 0, flush_elems = 0, phi_tasks = 0, max_rows = 0;
+    const int nks_pad = P.nks_pad, nslice = P.nslice;
+    size_t pos = 0;
+    while (pos < tmp.size()) {
+        size_t end = pos;
+        while (end < tmp.size() && tmp[end].cell == tmp[pos].cell) end++;
+        const int64_t c = tmp[pos].cell;
+        const int m = (int)(end - pos);
+        if (m > 4095) { err = "more than 4095 atom images touch one region"; return GINT_EUNSUPPORTED; }
+        Region R;
+        const int c3 = (int)(c % P.ncell[2]), c2 = (int)((c / P.ncell[2]) % P.ncell[1]), c1 = (int)(c / ((int64_t)P.ncell[1] * P.ncell[2]));
+        R.origin[0] = c1 * bx;
+        R.origin[1] = c2 * by;
+        R.origin[2] = c3 * bz;
+        int rows = 0;
+        for (int i = 0; i < m; i++) {
+            P.entries[pos + i].row0 = rows;
+            rows += P.entries[pos + i].norb;
+        }
+        const int nfrag = (rows + 7) / 8, ngroup = (nfrag + 3) / 4;
+        if (ngroup > kMaxGroups) { err = "too many orbitals listed for one region; use a smaller bcell"; return GINT_EUNSUPPORTED; }
+        max_rows = std::max(max_rows, (double)rows);
+        R.nrow = rows;
+        R.nentry = m;
+        R.gmask_off = (int32_t)P.gmask.size();
+        R.rowinfo_off = (int32_t)P.rowinfo.size();
+        R.pair_off = (int32_t)P.pair.size();
+        if (P.gmask.size() + (size_t)ngroup * nks_pad > 0x7FFFFFFFu || P.pair.size() + (size_t)m * m > 0x7FFFFFFFu) {
+            err = "plan tables exceed 2^31 entries";
+            return GINT_EUNSUPPORTED;
+        }
+        // fragment activity: OR of the k-step masks of the entries that own rows of the fragment
+        std::vector<std::array<uint32_t, 4>> fmask((size_t)ngroup * 4, std::array<uint32_t, 4>{0, 0, 0, 0});
+        P.rowinfo.resize(P.rowinfo.size() + (size_t)ngroup * kGroupRows, kNoBlock);
+        for (int i = 0; i < m; i++) {
+            const Entry& e = P.entries[pos + i];
+            for (int mu = 0; mu < e.norb; mu++) P.rowinfo[(size_t)R.rowinfo_off + e.row0 + mu] = pack_rowinfo(i, mu, e.norb);
+            for (int f = e.row0 / 8; f <= (e.row0 + e.norb - 1) / 8; f++)
+                for (int k = 0; k < 4; k++) fmask[(size_t)f][k] |= e.kmask[k];
+        }
+        P.gmask.resize(P.gmask.size() + (size_t)ngroup * nks_pad, 0);
+        uint8_t* gm = &P.gmask[(size_t)R.gmask_off];
+        for (int g = 0; g < ngroup; g++)
+            for (int ks = 0; ks < nks_pad; ks++) {
+                uint8_t b = 0;
+                for (int i = 0; i < 4; i++) b |= (uint8_t)(((fmask[(size_t)4 * g + i][ks >> 5] >> (ks & 31)) & 1u) << i);
+                gm[(size_t)g * nks_pad + ks] = b;
+            }
+        // pair table: (row entry a <= column entry b) -> canonical block offset (+ transposed flag)
+        P.pair.resize(P.pair.size() + (size_t)m * m, kNoBlock);
+        for (int a = 0; a < m; a++)
+            for (int b = a; b < m; b++) {
+                const Entry& ea = P.entries[pos + a];
+                const Entry& eb = P.entries[pos + b];
+                const int r1 = ((eb.Rpack >> 16) & 0xFF) - ((ea.Rpack >> 16) & 0xFF);
+                const int r2 = ((eb.Rpack >> 8) & 0xFF) - ((ea.Rpack >> 8) & 0xFF);
+                const int r3 = (eb.Rpack & 0xFF) - (ea.Rpack & 0xFF);
+                const bool zeroR = (r1 == 0 && r2 == 0 && r3 == 0);
+                const bool posR = (r1 > 0) || (r1 == 0 && (r2 > 0 || (r2 == 0 && r3 > 0)));
+                const bool canonical = (ea.atom < eb.atom) || (ea.atom == eb.atom && (zeroR || posR));
+                uint32_t off = canonical ? lookup(ea.atom, eb.atom, r1, r2, r3) : lookup(eb.atom, ea.atom, -r1, -r2, -r3);
+                if (off != kNoBlock && !canonical) off |= kPairTransposed;
+                P.pair[(size_t)R.pair_off + (size_t)a * m + b] = off;
+            }
+        // tiles (group gi <= gj) and their cost per slice
+        auto tile_slice_cost = [&](int gi, int gj, int s) {
+            int n = 0;
+            for (int ks = s * kSliceKsteps; ks < (s + 1) * kSliceKsteps; ks++) {
+                const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
+                if (gi != gj) n += __builtin_popcount(ra) * __builtin_popcount(ca);
+                else
+                    for (int i = 0; i < 4; i++)
+                        if ((ra >> i) & 1u) n += __builtin_popcount(ca >> i);
+            }
+            return n;
+        };
+        struct Proto { std::vector<std::pair<int, int>> tiles; std::vector<int> groups; };
+        auto add_group = [](std::vector<int>& v, int g) { if (std::find(v.begin(), v.end(), g) == v.end()) v.push_back(g); };
+        std::vector<std::vector<double>> tcost((size_t)ngroup, std::vector<double>((size_t)ngroup, 0.0));
+        for (int gi = 0; gi < ngroup; gi++)
+            for (int gj = gi; gj < ngroup; gj++) {
+                int n = 0;
+                for (int s = 0; s < nslice; s++) n += tile_slice_cost(gi, gj, s);
+                tcost[(size_t)gi][(size_t)gj] = n;
+            }
+        std::vector<Proto> protos;
+        const int chunk = 5;   // 5 groups -> a clique of 15 tiles
+        const int nchunk = (ngroup + chunk - 1) / chunk;
+        for (int k = 0; k < nchunk; k++) {
+            const int k0 = k * chunk, k1 = std::min(ngroup, k0 + chunk);
+            Proto p;
+            for (int gi = k0; gi < k1; gi++)
+                for (int gj = gi; gj < k1; gj++)
+                    if (tcost[(size_t)gi][(size_t)gj] > 0) { p.tiles.push_back({gi, gj}); add_group(p.groups, gi); add_group(p.groups, gj); }
+            if (!p.tiles.empty()) protos.push_back(p);
+            for (int l = k + 1; l < nchunk; l++) {
+                const int l0 = l * chunk, l1 = std::min(ngroup, l0 + chunk);
+                const int width = std::max(1, std::min(kTilesPerItem / (k1 - k0), kMaxSlots - (k1 - k0)));
+                for (int cj = l0; cj < l1; cj += width) {
+                    Proto r;
+                    for (int gi = k0; gi < k1; gi++)
+                        for (int gj = cj; gj < std::min(l1, cj + width); gj++)
+                            if (tcost[(size_t)gi][(size_t)gj] > 0) { r.tiles.push_back({gi, gj}); add_group(r.groups, gi); add_group(r.groups, gj); }
+                    if (!r.tiles.empty()) protos.push_back(r);
+                }
+            }
+        }
+        // greedy merge of small proto-items (fewer phi evaluations, fewer items)
+        for (bool merged = true; merged;) {
+            merged = false;
+            int best_a = -1, best_b = -1, best_union = 1 << 30;
+            for (size_t a = 0; a < protos.size(); a++)
+                for (size_t b = a + 1; b < protos.size(); b++) {
+                    if (protos[a].tiles.size() + protos[b].tiles.size() > (size_t)kTilesPerItem) continue;
+                    std::vector<int> u = protos[a].groups;
+                    for (int g : protos[b].groups) add_group(u, g);
+                    if ((int)u.size() > kMaxSlots) continue;
+                    const int growth = (int)u.size() - (int)std::max(protos[a].groups.size(), protos[b].groups.size());
+                    if (growth < best_union) { best_union = growth; best_a = (int)a; best_b = (int)b; }
+                }
+            if (best_a >= 0) {
+                for (auto& t : protos[(size_t)best_b].tiles) protos[(size_t)best_a].tiles.push_back(t);
+                for (int g : protos[(size_t)best_b].groups) add_group(protos[(size_t)best_a].groups, g);
+                protos.erase(protos.begin() + best_b);
+                merged = true;
+            }
+        }
+        const int region_index = (int)P.regions.size();
+        for (Proto& p : protos) {
+            std::sort(p.groups.begin(), p.groups.end());
+            WorkItem w;
+            std::memset(&w, 0, sizeof(w));
+            w.region = region_index;
+            w.nslot = (int32_t)p.groups.size();
+            for (size_t s = 0; s < p.groups.size(); s++) w.slot_group[s] = (uint8_t)p.groups[s];
+            auto slot_of = [&](int g) { return (int)(std::find(p.groups.begin(), p.groups.end(), g) - p.groups.begin()); };
+            // heaviest tiles first: warp w takes tile w
+            std::sort(p.tiles.begin(), p.tiles.end(), [&](const std::pair<int, int>& a, const std::pair<int, int>& b) {
+                return tcost[(size_t)a.first][(size_t)a.second] > tcost[(size_t)b.first][(size_t)b.second];
+            });
+            w.ntile = (int16_t)p.tiles.size();
+            double cost = 0;
+            for (size_t t = 0; t < p.tiles.size(); t++) {
+                w.tiles[t][0] = (uint8_t)slot_of(p.tiles[t].first);
+                w.tiles[t][1] = (uint8_t)slot_of(p.tiles[t].second);
+                cost += tcost[(size_t)p.tiles[t].first][(size_t)p.tiles[t].second];
+                for (int s = 0; s < nslice; s++)
+                    if (tile_slice_cost(p.tiles[t].first, p.tiles[t].second, s) > 0) w.slice_mask |= 1u << s;
+            }
+            exec_dmma += cost;
+            flush_elems += 1024.0 * (double)p.tiles.size();
+            // evaluation tasks: entries owning rows in the item's groups
+            w.task0 = (int32_t)P.tasks.size();
+            int ntask = 0;
+            for (int i = 0; i < m; i++) {
+                const Entry& e = P.entries[pos + i];
+                const int g0 = e.row0 >> 5, g1 = (e.row0 + e.norb - 1) >> 5;
+                EvalTask t;
+                std::memset(&t, 0, sizeof(t));
+                t.entry = (int32_t)(pos + i);
+                t.row0 = (int16_t)e.row0;
+                bool any = false;
+                for (int k = 0; k < 3; k++) {
+                    t.slot[k] = -1;
+                    const int g = g0 + k;
+                    if (g > g1) continue;
+                    const int s = slot_of(g);
+                    if (s < (int)p.groups.size()) { t.slot[k] = (int8_t)s; any = true; }
+                }
+                if (!any) continue;
+                P.tasks.push_back(t);
+                ntask++;
+                for (int s = 0; s < nslice; s++)
+                    if (((w.slice_mask >> s) & 1u) && ((e.kmask[(s * kSliceKsteps) >> 5] >> ((s * kSliceKsteps) & 31)) & 0xFFu)) {
+                        phi_tasks += 1;
+                        cost += 12.0;   // one (entry, slice) phi evaluation ~ 12 DMMA issue times of FP64 pipe
+                    }
+            }
+            if (ntask > kMaxTasksPerItem) { err = "internal: too many evaluation tasks in one work item"; return GINT_EUNSUPPORTED; }
+            w.ntask = (int16_t)ntask;
+            P.items.push_back(w);
+            item_cost.push_back(cost);
+        }
+        P.regions.push_back(R);
+        pos = end;
+    }
     tmp.clear();
     tmp.shrink_to_fit();
-
-    // ---- work items ----------------------------------------------------------------
-    P.max_entries = 0;
-    P.max_rows = 0;
-    for (int64_t c = 0; c < ncells; c++) {
-        const int64_t s = P.cell_start[(size_t)c], t = P.cell_start[(size_t)c + 1];
-        int rows = 0;
-        for (int64_t i = s; i < t; i++) {
-            P.entries[(size_t)i].row0 = rows;
-            rows += P.entries[(size_t)i].norb;
-        }
-        if (t - s > kMaxEntriesPerItem) { err = "more than 255 atom images touch one big cell"; return GINT_EUNSUPPORTED; }
-        P.max_entries = std::max(P.max_entries, (int)(t - s));
-        P.max_rows = std::max(P.max_rows, rows);
+    // longest-processing-time-first order for the dynamic queue
+    {
+        std::vector<size_t> idx(P.items.size());
+        std::iota(idx.begin(), idx.end(), size_t(0));
+        std::stable_sort(idx.begin(), idx.end(), [&](size_t a, size_t b) { return item_cost[a] > item_cost[b]; });
+        std::vector<WorkItem> sorted(P.items.size());
+        for (size_t i = 0; i < idx.size(); i++) sorted[i] = P.items[idx[i]];
+        P.items.swap(sorted);
     }
-    const int max_rows_pad = (P.max_rows + 7) & ~7;
-    const size_t fixed = fixed_smem_bytes(P.max_entries, max_rows_pad, table_bytes);
-    const int Bpad = (B + 3) & ~3;
-    double sum_knn = 0, sum_nn = 0, nsplit = 0;
-    for (int64_t c = 0; c < ncells; c++) {
-        const int64_t s = P.cell_start[(size_t)c], t = P.cell_start[(size_t)c + 1];
-        if (s == t) continue;
-        const Entry& last = P.entries[(size_t)t - 1];
-        const int rows = last.row0 + last.norb;
-        const int rows_pad = (rows + 7) & ~7;
-        int K = std::min(Bpad, kMaxItemPoints);
-        while (K > 4 && fixed + (size_t)rows_pad * (K + 4) * sizeof(double) > kSmemLimit) K = ((K / 2) + 3) & ~3;
-        if (fixed + (size_t)rows_pad * (K + 4) * sizeof(double) > kSmemLimit) { err = "big cell does not fit in shared memory"; return GINT_EUNSUPPORTED; }
-        const int c3 = (int)(c % P.ncell[2]), c2 = (int)((c / P.ncell[2]) % P.ncell[1]), c1 = (int)(c / ((int64_t)P.ncell[1] * P.ncell[2]));
-        if (K < Bpad) nsplit += 1;
-        for (int p0 = 0; p0 < Bpad; p0 += K) {
-            WorkItem w;
-            w.entry0 = (int32_t)s;
-            w.nentry = (int32_t)(t - s);
-            w.nrow = rows;
-            w.p0 = p0;
-            w.npts = std::min(K, Bpad - p0);
-            w.origin[0] = c1 * bx;
-            w.origin[1] = c2 * by;
-            w.origin[2] = c3 * bz;
-            // skip sub-ranges no sphere reaches
-            uint64_t any = 0;
-            for (int64_t i = s; i < t; i++) any |= ((uint64_t)P.entries[(size_t)i].mask_hi << 32) | P.entries[(size_t)i].mask_lo;
-            const uint64_t range = (w.npts >= 64 ? ~0ull : ((1ull << w.npts) - 1)) << p0;
-            if (!(any & range)) continue;
-            P.items.push_back(w);
-            sum_knn += (double)w.npts * rows * rows;
-            sum_nn += (double)rows * rows;
-        }
-    }
-    std::stable_sort(P.items.begin(), P.items.end(), [](const WorkItem& a, const WorkItem& b) {
-        return (int64_t)a.npts * a.nrow * a.nrow > (int64_t)b.npts * b.nrow * b.nrow;
-    });
-    P.smem_bytes = 0;
-    for (const WorkItem& w : P.items)
-        P.smem_bytes = std::max(P.smem_bytes, fixed + (size_t)((w.nrow + 7) & ~7) * (w.npts + 4) * sizeof(double));
-    if (P.items.empty()) P.smem_bytes = fixed;
 
     double fpt = 0, fsym = 0;
     for (int32_t n : npoint_orb) {
@@ -390,15 +568,15 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[0] = (double)ncells;
     P.stats[1] = (double)P.items.size();
     P.stats[2] = (double)P.entries.size();
-    P.stats[3] = (double)P.max_rows;
-    P.stats[4] = sum_knn;
-    P.stats[5] = sum_nn;
+    P.stats[3] = max_rows;
+    P.stats[4] = 512.0 * exec_dmma;
+    P.stats[5] = flush_elems;
     P.stats[6] = (double)P.smem_bytes;
     P.stats[7] = 2;
     P.stats[8] = fpt;
     P.stats[9] = fsym;
     P.stats[10] = n_insphere;
-    P.stats[11] = nsplit;
+    P.stats[11] = phi_tasks * kSlicePts;
     return GINT_OK;
 }
 

@@ -157,7 +157,7 @@ def test_error_codes():
         setup(species=[f_shell])
     assert e.value.code == binding.GINT_EUNSUPPORTED
     with pytest.raises(binding.GintError) as e:
-        setup(bcell=(8, 4, 4))
+        setup(bcell=(16, 8, 8))
     assert e.value.code == binding.GINT_EUNSUPPORTED
     pos = w.atom_pos.copy()
     pos[0, 0] = np.nan
