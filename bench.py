@@ -270,7 +270,7 @@ def main():
         "kernel": "gint_vlocal_kernel", "kernel_ms": main_ms, "mirror_kernel_ms": mirror_ms,
         "kernel_share_of_step": main_ms / ms_per_step,
         "flops_per_launch": F_rank, "flops_accounting": "F_sym = sum_g n(g)(n(g)+1) (symmetry exploited); F_pt = %.4e" % F_pt,
-        "executed_flops_upper_bound": st["sum_K_n2"],
+        "executed_tensor_flops": st["executed_flops"],
         "peak_source": "live DMMA.8x8x4 register-resident microbenchmark (gint_measure_fp64_peak) %.2f; "
                        "rule (MEASURED_PEAKS bf16 %s x 40/2250) %.2f; larger one used" % (peak_live, peaks_src, peak_rule),
         "hbm_algorithmic_bytes": hbm_bytes,

@@ -120,15 +120,18 @@ int gint_set_profiling(gint_ctx *ctx, int32_t on);
 int gint_get_kernel_ms(gint_ctx *ctx, double *ms /* [3] */);
 
 /* Statistics of the setup (all host-side, valid for host-only contexts too).
- * stats[0] big cells total        stats[1] non-empty work items
- * stats[2] (atom image, cell) list entries          stats[3] max orbitals in one work item
- * stats[4] sum over items of K*n_c^2 (executed MACs, full square, no symmetry)
- * stats[5] sum over items of n_c^2   stats[6] dynamic shared memory per CTA (bytes)
+ * stats[0] big cells (regions) total, empty ones included      stats[1] work items
+ * stats[2] (atom image, region) list entries                   stats[3] max orbitals listed for one region
+ * stats[4] executed tensor flops (512 per DMMA.8x8x4 the kernel will issue)
+ * stats[5] accumulator elements flushed (upper bound on red.global.add.f64 per call)
+ * stats[6] dynamic shared memory per CTA (bytes)
  * stats[7] number of kernels launched per gint_vlocal call (memsets not counted)
  * stats[8] F_pt = sum_g 2 n(g)^2, n(g) = orbitals non-zero at mesh point g (useful flops, no symmetry)
  * stats[9] F_sym = sum_g n(g) (n(g)+1) (useful flops when H(R)=H(-R)^T is exploited)
- * stats[10] in-sphere (atom image, point) pairs   stats[11] work items whose point range was split
- * Returns the number of entries written (<= n). */
+ * stats[10] in-sphere (atom image, point) pairs   stats[11] (atom image, point) pairs evaluated per call
+ * stats[12] psi scratch buffer (bytes, device)    stats[13] psi bytes streamed back from L2 per call
+ * stats[14] shared-memory ring stages             stats[15] non-empty regions
+ * Returns the number of entries written (<= n, at most 16). */
 int gint_get_stats(const gint_ctx *ctx, double *stats, int32_t n);
 
 /* Copy out the per-cell lists (host logic tests).  cell_start[ncell+1] indexes

@@ -21,8 +21,9 @@ GINT_OK, GINT_EINVAL, GINT_EUNSUPPORTED, GINT_ENOMEM, GINT_ECUDA, GINT_ENODEVICE
 EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
             "gint_set_profiling", "gint_get_kernel_ms", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
 
-STAT_NAMES = ("cells", "items", "entries", "max_rows", "sum_K_n2", "sum_n2", "smem_bytes", "kernels_per_call",
-              "F_pt", "F_sym", "insphere_pairs", "split_cells")
+STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
+              "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
+              "regions")
 
 
 class GintError(RuntimeError):
@@ -115,8 +116,8 @@ class GintContext:
         return iat[:n], jat[:n], R[:n], off
 
     def gint_get_stats(self) -> dict:
-        s = np.zeros(12, dtype=np.float64)
-        n = _check(_lib.gint_get_stats(self._h, _ptr(s, ctypes.c_double), 12), "gint_get_stats")
+        s = np.zeros(16, dtype=np.float64)
+        n = _check(_lib.gint_get_stats(self._h, _ptr(s, ctypes.c_double), 16), "gint_get_stats")
         return {STAT_NAMES[i]: float(s[i]) for i in range(n)}
 
     def gint_set_profiling(self, on: bool = True):

@@ -125,7 +125,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     UP(P.items, &D.items)
     UP(P.regions, &D.regions)
     UP(P.entries, &D.entries)
-    UP(P.tasks, &D.tasks)
+    UP(P.etasks, &D.etasks)
     UP(P.gmask, &D.gmask)
     UP(P.rowinfo, &D.rowinfo)
     UP(P.pair, &D.pair)
@@ -135,15 +135,26 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     UP(P.sp_meta, &D.sp_meta)
     UP(P.sp_real, &D.sp_real)
 #undef UP
-    void* ctr = nullptr;
-    if ((e = cudaMalloc(&ctr, 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
+    void* ctr = nullptr;   // queue head + one share counter per region
+    if ((e = cudaMalloc(&ctr, sizeof(unsigned int) * (P.regions.size() + 1) + 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counters"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
+    D.ready = D.counter + 1;
+    // psi scratch: zero-filled once; rows and slices that no evaluation task writes stay zero for good
+    void* psi = nullptr;
+    const size_t psi_bytes = (size_t)P.psi_chunks * gint::kChunkBytes;
+    if ((e = cudaMalloc(&psi, psi_bytes ? psi_bytes : 16)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc psi scratch"); }
+    ctx->allocs.push_back(psi);
+    if (psi_bytes && (e = cudaMemset(psi, 0, psi_bytes)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMemset psi scratch"); }
+    D.psi = reinterpret_cast<double*>(psi);
     std::memcpy(D.estep, P.estep, sizeof(D.estep));
     D.dV = P.dV;
     for (int d = 0; d < 3; d++) D.ngrid[d] = P.ngrid[d];
     D.nks_pad = P.nks_pad;
     D.nslice = P.nslice;
+    D.nstage = P.nstage;
+    D.nregions = (int32_t)P.regions.size();
+    D.nring = P.nring;
     D.nitems = (int32_t)P.items.size();
     D.nmirror = (int32_t)P.mirror.size();
     D.tab_doubles = (int32_t)P.tab_packed.size();
@@ -236,7 +247,7 @@ int gint_get_kernel_ms(gint_ctx* ctx, double* ms) {
 
 int gint_get_stats(const gint_ctx* ctx, double* stats, int32_t n) {
     if (!ctx || !stats) return fail(GINT_EINVAL, "null argument");
-    const int m = n < 12 ? n : 12;
+    const int m = n < 16 ? n : 16;
     for (int i = 0; i < m; i++) stats[i] = ctx->plan.stats[i];
     return m;
 }

@@ -1,5 +1,5 @@
 // gint_device.hpp -- kernel parameter block and launchers shared by gint_api.cu and gint_kernels.cu.
-// The plan structures (Entry, Region, WorkItem, EvalTask, MirrorItem, SmemLayout) are plain
+// The plan structures (Entry, Region, WorkItem, ItemDesc, MirrorItem, SmemLayout) are plain
 // C++ and come from gint_plan.hpp; the device reads them exactly as the host wrote them.
 #pragma once
 #include <cuda_runtime.h>
@@ -16,22 +16,25 @@ struct DevicePlan {
     const WorkItem* items;
     const Region* regions;
     const Entry* entries;
-    const EvalTask* tasks;
+    const uint32_t* etasks;   // evaluation tasks: entry within region | slice << 16
     const uint8_t* gmask;
     const uint32_t* rowinfo;
     const uint32_t* pair;
     const uint8_t* slot_xyz;  // [nslice*32][4]
-    const double* tab;        // packed radial tables, per species [ntab][nrad]
-    const int32_t* sp_meta;   // per species 12 ints: tab_offset, ntab, nrad, norb, l[8]
+    const double* tab;        // packed radial tables, per species [ntab+4][nradp]
+    const int32_t* sp_meta;   // per species 12 ints: tab_offset, ntab, nradp, norb, l[8]
     const double* sp_real;    // per species: rcut^2, 1/dr
     const MirrorItem* mirror;
+    double* psi;              // scratch: psi_chunks x 512 doubles, zero-filled once at setup
     unsigned int* counter;    // work-queue head, reset before every launch
+    unsigned int* ready;      // per region: evaluation shares published, reset before every launch
     double estep[9];          // mesh step vectors a_d / N_d (rows)
     double dV;
     int32_t ngrid[3];
-    int32_t nks_pad, nslice;
-    int32_t nitems, nmirror;
+    int32_t nks_pad, nslice, nstage;
+    int32_t nitems, nmirror, nregions;
     int32_t tab_doubles;
+    int32_t nring;
 };
 
 cudaError_t configure_kernels(size_t smem_bytes, bool tab_smem);

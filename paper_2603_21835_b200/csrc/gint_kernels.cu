@@ -2,23 +2,28 @@
 //
 //   H_mu,nu(R) = sum_g phi_mu(r_g - tau_I) V(r_g) phi_nu(r_g - tau_J - R) dV   (Eq. 45)
 //
-// Output-stationary design.  One persistent CTA per SM (16 warps) pulls work items
-// from a global queue.  A work item is a set of up to 16 32x32 tiles (one per warp) of
-// the upper triangle of one region's  C = phi diag(V dV) phi^T  (the paper's per-BigGrid
-// dense contraction).  Each warp keeps its tile in registers (4 x 4
-// DMMA fragments) while the CTA streams the region's mesh points through shared memory
-// in slices of 32 points (8 k-steps of the FP64 tensor-core shape m8n8k4):
-//   * evaluate: phi of the orbitals the item needs on the slice's points (Eq. 1: 4-point
-//     Lagrange radial table x real Y_lm) into a double-buffered tile
-//     phi[row = orbital][col = point], and w = V dV of the points;
-//   * contract: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has no FP64 kind), A and
-//     B operands read from the same tile, B scaled by w as it is loaded; (fragment,
-//     k-step) pairs that hold no in-sphere point are skipped via host-built activity
-//     bytes.
-// After the last slice the warp adds its tile into the canonical H blocks with
-// red.global.add.f64 (once per item, not once per BigGrid).  A second kernel writes
-// every non-canonical block as the transpose of its partner, H(J,I,-R) = H(I,J,R)^T,
-// and symmetrises the (I,I,0) blocks.
+// Output-stationary design.  One persistent CTA per SM pulls work items from a global
+// queue.  A work item is a set of up to 15 32x32 tiles (one per consumer warp) of the
+// upper triangle of one region's  C = psi diag(sign V) psi^T,  psi = phi sqrt(|V dV|)
+// (the paper's per-BigGrid dense contraction, with the V dV weighting
+// of Eq. 45 folded into the operand).  The items of a region sit next to each other in
+// the queue and share its psi through the L2 cache:
+//
+//   phase 1 (evaluate)  the CTA that takes item q of n evaluates share q of the region's
+//       (atom image, 32-point slice) tasks -- Eq. 1: 4-point Lagrange radial table x real
+//       Y_lm, one lane per mesh point -- and stores psi to a global scratch buffer in DMMA
+//       fragment order, then publishes the share (release counter per region).  Phase 1 of
+//       item i+1 runs before phase 2 of item i, so sibling shares are ready when needed.
+//   phase 2 (contract)  a producer warp streams the row groups the item's tiles need back
+//       through a ring of shared-memory stages (16 points each) with cp.async.bulk +
+//       mbarrier; 15 consumer warps keep one 32x32 tile each in registers and issue
+//       mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has no FP64 kind).  (fragment,
+//       k-step) pairs that hold no in-sphere point are skipped by warp-uniform branches on
+//       host-built activity nibbles (a predicated-off DMMA still costs its 16 pipe cycles).
+//   flush   after the last stage the warp adds its tile into the canonical H blocks with
+//       red.global.add.f64 (once per item, not once per BigGrid).
+// A second kernel writes every non-canonical block as the transpose of its partner,
+// H(J,I,-R) = H(I,J,R)^T, and symmetrises the (I,I,0) blocks.
 #include <cuda_runtime.h>
 
 #include <cstdint>
@@ -29,102 +34,130 @@ namespace gint {
 
 namespace {
 
-constexpr int kThreads = 512;
-constexpr int kWarps = kThreads / 32;
-constexpr int kLD = kPhiLD;
-constexpr int kBufDoubles = kMaxSlots * kGroupRows * kLD;
-static_assert(kWarps == kTilesPerItem, "one tile per warp");
+constexpr int kConsumerWarps = kTilesPerItem;          // 15
+constexpr int kConsumerThreads = kConsumerWarps * 32;  // 480
+constexpr int kThreads = kConsumerThreads + 32;        // + 1 producer warp
+constexpr int kStageBytes = kMaxSlots * kChunkBytes;   // 32 KB
 
 __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
 }
-// warp-uniform condition: the instruction is predicated off as a whole
-__device__ __forceinline__ void dmma8x8x4_if(double& c0, double& c1, double a, double b, uint32_t cond) {
+
+// ---- mbarrier / bulk-copy helpers (shared::cta addresses) --------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
-        "@p mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n\t}"
-        : "+d"(c0), "+d"(c1)
-        : "d"(a), "d"(b), "r"(cond));
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void bar_consumers() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory"); }
+
+__device__ __forceinline__ double rsqrt_seed(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
 }
 
-// phi of one entry on the 32 points of a slice (lane = point), Eq. 1.
+// psi = phi sqrt(|V dV|) of one entry on the 32 points of a slice (lane = point), Eq. 1, stored
+// to the region's scratch in fragment order: element (row R, point p of stage s) sits at
+//   chunk(R >> 5, s) + (((R >> 3 & 3) * 2 + kp) * 32 + (R & 7) * 4 + fk) * 2 + kk,
+// p = (2 kp + kk) * 4 + fk, so that one LDS.128 per lane feeds two k-steps of a DMMA operand.
 __device__ __forceinline__ void eval_task(const DevicePlan& P, const double* __restrict__ tab, const Entry* __restrict__ en,
-                                          const EvalTask tk, int slice, int lane, const double* __restrict__ s_off,
-                                          double* __restrict__ buf) {
-    double* p0 = tk.slot[0] >= 0 ? buf + (tk.slot[0] * kGroupRows) * kLD + lane : nullptr;
-    double* p1 = tk.slot[1] >= 0 ? buf + (tk.slot[1] * kGroupRows) * kLD + lane : nullptr;
-    double* p2 = tk.slot[2] >= 0 ? buf + (tk.slot[2] * kGroupRows) * kLD + lane : nullptr;
-    const int rr = tk.row0 & 31;
-    auto put = [&](int mu, double v) {
-        const int R = rr + mu;
-        double* p = (R < 32) ? p0 : ((R < 64) ? p1 : p2);
-        if (p) p[(R & 31) * kLD] = v;
-    };
-    const int norb = en->norb;
-    const uint32_t kbyte = (en->kmask[(slice * kSliceKsteps) >> 5] >> ((slice * kSliceKsteps) & 31)) & 0xFFu;
+                                          int slice, int lane, const double* __restrict__ s_off,
+                                          const double* __restrict__ s_sqrtw, double* __restrict__ psi_region) {
     const int sp = (en->Rpack >> 24) & 0x7F;
-    const double rc2 = __ldg(P.sp_real + 2 * sp);
+    const int32_t* meta = P.sp_meta + 12 * sp;
+    const int tab_off = __ldg(meta + 0), ntab = __ldg(meta + 1), nradp = __ldg(meta + 2);
+    const double rc2 = __ldg(P.sp_real + 2 * sp), inv_dr = __ldg(P.sp_real + 2 * sp + 1);
     const int p = slice * kSlicePts + lane;
     const double dx = en->rel[0] + s_off[p];
     const double dy = en->rel[1] + s_off[kMaxRegionPoints + p];
     const double dz = en->rel[2] + s_off[2 * kMaxRegionPoints + p];
-    const double r2 = dx * dx + dy * dy + dz * dz;
-    const bool inside = (kbyte != 0u) && (r2 < rc2);
-    if (__ballot_sync(0xffffffffu, inside) == 0u) {
-        for (int mu = 0; mu < norb; mu++) put(mu, 0.0);
-        return;
-    }
-    const int32_t* meta = P.sp_meta + 12 * sp;
-    const int tab_off = __ldg(meta + 0), ntab = __ldg(meta + 1), nrad = __ldg(meta + 2);
-    const double inv_dr = __ldg(P.sp_real + 2 * sp + 1);
-    double x = 0.0, y = 0.0, z = 0.0, r = 0.0, lnz = 0.0;   // lnz: 1 if l>0 components survive
+    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    const bool inside = r2 < rc2;
+    double rinv = 0.0, lnz = 0.0;   // lnz: 1 if the l>0 components survive (r >= 1e-12)
     if (r2 >= 1e-24) {
-        const double rinv = rsqrt(r2);
-        r = r2 * rinv;
-        x = dx * rinv;
-        y = dy * rinv;
-        z = dz * rinv;
+        const double y0 = rsqrt_seed(r2);              // relative error ~2^-22
+        const double e = fma(-(r2 * y0), y0, 1.0);     // 1 - r2 y0^2
+        rinv = fma(e * y0, fma(0.375, e, 0.5), y0);    // y0 (1 + e/2 + 3 e^2/8): cubic convergence
         lnz = 1.0;
     }
+    const double r = r2 * rinv;
+    const double x = dx * rinv, y = dy * rinv, z = dz * rinv;
     const double s = r * inv_dr;
-    int k = (int)s;
-    k = min(k, ntab - 4);
+    int k = __double2int_rd(s);
     const double t = s - (double)k;
+    k = inside ? min(k, ntab) : ntab;                  // outside: the four zero nodes after the table
     const double t1 = 1.0 - t, t2 = 2.0 - t, t3 = 3.0 - t;
-    const double in = inside ? 1.0 : 0.0;
-    const double L0 = in * (t1 * t2 * t3 * (1.0 / 6.0));
-    const double L1 = in * (t * t2 * t3 * 0.5);
-    const double L2 = in * (-t * t1 * t3 * 0.5);
-    const double L3 = in * (t * t1 * t2 * (1.0 / 6.0));
-    const double* Tk = tab + tab_off + (inside ? k : 0) * nrad;
-    // real Y_lm, l <= 2 (no Condon-Shortley phase; order fixed in include/gint.h)
-    const double Y00 = 0.28209479177387814;
-    const double c1 = 0.48860251190291992 * lnz;
-    const double c2a = 1.0925484305920792, c2b = 0.31539156525252005 * lnz, c2c = 0.54627421529603959;
-    int mu = 0;
-    for (int f = 0; f < nrad; f++) {
-        const double fv = Tk[f] * L0 + Tk[nrad + f] * L1 + Tk[2 * nrad + f] * L2 + Tk[3 * nrad + f] * L3;
-        const int l = __ldg(meta + 4 + f);
+    const double a23 = t2 * t3, b01 = t * t1;
+    const double sq = s_sqrtw[p];
+    const double L0 = (t1 * a23) * (sq * (1.0 / 6.0));
+    const double L1 = (t * a23) * (sq * 0.5);
+    const double L2 = (b01 * t3) * (sq * -0.5);
+    const double L3 = (b01 * t2) * (sq * (1.0 / 6.0));
+    const double* Tk = tab + tab_off + k * nradp;
+    // store addressing
+    const int row0 = en->row0;
+    double* out = psi_region + ((lane >> 4) * kChunkDoubles + ((lane >> 3) & 1) * 64 + (lane & 3) * 2 + ((lane >> 2) & 1));
+    const int gstride = P.nstage * kChunkDoubles;
+    int R = row0;
+    auto put = [&](double v) {
+        out[(R >> 5) * gstride + ((R >> 3) & 3) * 128 + (R & 7) * 8] = v;
+        R++;
+    };
+    auto emit = [&](int l, double fv) {
         if (l == 0) {
-            put(mu, fv * Y00);
-            mu += 1;
+            put(fv);
         } else if (l == 1) {
-            const double g1 = fv * c1;
-            put(mu, g1 * y);
-            put(mu + 1, g1 * z);
-            put(mu + 2, g1 * x);
-            mu += 3;
+            put(fv * y);
+            put(fv * z);
+            put(fv * x);
         } else {
-            const double ga = fv * c2a;
-            put(mu, ga * (x * y));
-            put(mu + 1, ga * (y * z));
-            put(mu + 2, (fv * c2b) * (3.0 * z * z - 1.0));
-            put(mu + 3, ga * (x * z));
-            put(mu + 4, (fv * c2c) * (x * x - y * y));
-            mu += 5;
+            // table carries 1/2 sqrt(15/pi); ratios: 1/4 sqrt(5/pi) / that = 1/(2 sqrt 3), 1/4 sqrt(15/pi) / that = 1/2
+            put(fv * (x * y));
+            put(fv * (y * z));
+            put(fv * (fma(3.0 * z, z, -lnz) * 0.28867513459481288));
+            put(fv * (x * z));
+            put(fv * (fma(x, x, -(y * y)) * 0.5));
         }
+    };
+    for (int f = 0; f < nradp; f += 2) {
+        const double2 T0 = *reinterpret_cast<const double2*>(Tk + f);
+        const double2 T1 = *reinterpret_cast<const double2*>(Tk + nradp + f);
+        const double2 T2 = *reinterpret_cast<const double2*>(Tk + 2 * nradp + f);
+        const double2 T3 = *reinterpret_cast<const double2*>(Tk + 3 * nradp + f);
+        const int l0 = __ldg(meta + 4 + f);
+        const int l1 = (f + 1 < 8) ? __ldg(meta + 4 + f + 1) : -1;
+        emit(l0, fma(T0.x, L0, fma(T1.x, L1, fma(T2.x, L2, T3.x * L3))));
+        if (l1 >= 0) emit(l1, fma(T0.y, L0, fma(T1.y, L1, fma(T2.y, L2, T3.y * L3))));
     }
 }
 
@@ -135,16 +168,14 @@ __global__ void __launch_bounds__(kThreads, 1)
 gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__ V, double* __restrict__ H) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const SmemLayout L = smem_layout(TAB_SMEM ? (size_t)P.tab_doubles * sizeof(double) : 0);
+    const SmemLayout L = smem_layout(TAB_SMEM ? (size_t)P.tab_doubles * sizeof(double) : 0, P.nring);
+    uint64_t* s_full = reinterpret_cast<uint64_t*>(smem_raw + L.bar);         // [8]
+    uint64_t* s_empty = s_full + 8;                                           // [8]
+    ItemDesc* s_desc = reinterpret_cast<ItemDesc*>(smem_raw + L.desc);        // [3]
+    double* s_off = reinterpret_cast<double*>(smem_raw + L.off);              // [3][512] Cartesian offset of a point slot
     double* s_tab = reinterpret_cast<double*>(smem_raw + L.tab);
-    double* s_off = reinterpret_cast<double*>(smem_raw + L.off);      // [3][512] Cartesian offset of a point slot
-    double* s_w = reinterpret_cast<double*>(smem_raw + L.w);          // [2][32]  V dV of the slice's points
-    uint8_t* s_gmask = smem_raw + L.gmask;                            // [slot][k-step] fragment activity nibbles
-    EvalTask* s_tasks = reinterpret_cast<EvalTask*>(smem_raw + L.tasks);
-    WorkItem* s_item = reinterpret_cast<WorkItem*>(smem_raw + L.item);
-    Region* s_region = reinterpret_cast<Region*>(smem_raw + L.item + sizeof(WorkItem));
-    int* s_misc = reinterpret_cast<int*>(smem_raw + L.misc);
-    double* s_phi = reinterpret_cast<double*>(smem_raw + L.phi);      // [2][slot*32 + row][kLD]
+    unsigned char* s_ring = smem_raw + L.ring;                                // [nring][slot][4 KB]
+    const int nring = P.nring;
 
     if (TAB_SMEM) {
         for (int i = tid; i < P.tab_doubles; i += kThreads) s_tab[i] = __ldg(P.tab + i);
@@ -155,121 +186,252 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
         for (int k = 0; k < 3; k++)
             s_off[k * kMaxRegionPoints + p] = c.x * P.estep[k] + c.y * P.estep[3 + k] + c.z * P.estep[6 + k];
     }
-    const int frow = lane >> 2, fk = lane & 3;
-
-    while (true) {
-        if (tid == 0) s_misc[0] = (int)atomicAdd(P.counter, 1u);
-        __syncthreads();   // also: every warp has finished the previous item (flush reads s_item / s_region)
-        const int item = s_misc[0];
-        if (item >= P.nitems) break;
-        // ---------------- stage the item ---------------------------------------------------------
-        if (tid < (int)(sizeof(WorkItem) / 4))
-            reinterpret_cast<uint32_t*>(s_item)[tid] = __ldg(reinterpret_cast<const uint32_t*>(P.items + item) + tid);
-        __syncthreads();
-        const int ntask = s_item->ntask, ntile = s_item->ntile, nslot = s_item->nslot;
-        const uint32_t slice_mask = s_item->slice_mask;
-        const Region* greg = P.regions + s_item->region;
-        if (tid < (int)(sizeof(Region) / 4))
-            reinterpret_cast<uint32_t*>(s_region)[tid] = __ldg(reinterpret_cast<const uint32_t*>(greg) + tid);
-        for (int i = tid; i < ntask * (int)(sizeof(EvalTask) / 4); i += kThreads)
-            reinterpret_cast<uint32_t*>(s_tasks)[i] = __ldg(reinterpret_cast<const uint32_t*>(P.tasks + s_item->task0) + i);
-        {
-            const int wpr = P.nks_pad >> 2;   // 32-bit words per group row of activity bytes
-            const int gmask_off = __ldg(&greg->gmask_off);
-            for (int i = tid; i < nslot * wpr; i += kThreads) {
-                const int slot = i / wpr, wd = i - slot * wpr;
-                reinterpret_cast<uint32_t*>(s_gmask + slot * kMaxKsteps)[wd] =
-                    __ldg(reinterpret_cast<const uint32_t*>(P.gmask + gmask_off + (int)s_item->slot_group[slot] * P.nks_pad) + wd);
-            }
+    if (tid == 0) {
+        for (int i = 0; i < nring; i++) {
+            mbar_init(smem_u32(s_full + i), 1);
+            mbar_init(smem_u32(s_empty + i), kConsumerWarps);
         }
-        __syncthreads();
-        const int ox = s_region->origin[0], oy = s_region->origin[1], oz = s_region->origin[2];
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    fence_proxy_async();
 
-        auto evaluate = [&](int slice, int b) {
-            double* buf = s_phi + b * kBufDoubles;
-            if (warp == kWarps - 1) {   // w = V dV of the slice's points (0 outside the mesh)
-                const int p = slice * kSlicePts + lane;
-                const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
-                const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
-                double wv = 0.0;
-                if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
-                    wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
-                s_w[b * kSlicePts + lane] = wv;
-            }
-            for (int t = warp; t < ntask; t += kWarps) {
-                const EvalTask tk = s_tasks[t];
-                eval_task(P, tab, P.entries + tk.entry, tk, slice, lane, s_off, buf);
-            }
-        };
+    // ---- producer warp: take the next item from the queue and stage its descriptor ---------------
+    auto prepare = [&](ItemDesc* d) {
+        unsigned int it = 0;
+        if (lane == 0) it = atomicAdd(P.counter, 1u);
+        it = __shfl_sync(0xffffffffu, it, 0);
+        if (it >= (unsigned int)P.nitems) {
+            if (lane == 0) d->valid = 0;
+            __syncwarp();
+            return;
+        }
+        if (lane < (int)(sizeof(WorkItem) / 4))
+            reinterpret_cast<uint32_t*>(&d->item)[lane] = __ldg(reinterpret_cast<const uint32_t*>(P.items + it) + lane);
+        __syncwarp();
+        const Region* greg = P.regions + d->item.region;
+        if (lane < (int)(sizeof(Region) / 4))
+            reinterpret_cast<uint32_t*>(&d->region)[lane] = __ldg(reinterpret_cast<const uint32_t*>(greg) + lane);
+        __syncwarp();
+        const int wpr = P.nks_pad >> 2;   // 32-bit words per group row of activity bytes
+        const int nslot = d->item.nslot;
+        for (int i = lane; i < nslot * wpr; i += 32) {
+            const int slot = i / wpr, wd = i - slot * wpr;
+            reinterpret_cast<uint32_t*>(d->gmask[slot])[wd] = __ldg(
+                reinterpret_cast<const uint32_t*>(P.gmask + d->region.gmask_off + (int)d->item.slot_group[slot] * P.nks_pad) + wd);
+        }
+        const int ox = d->region.origin[0], oy = d->region.origin[1], oz = d->region.origin[2];
+        for (int p = lane; p < P.nslice * kSlicePts; p += 32) {   // w = V dV of the region's points (0 outside the mesh)
+            const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
+            const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
+            double wv = 0.0;
+            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
+                wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
+            d->sqrtw[p] = sqrt(fabs(wv));
+            const unsigned int neg = __ballot_sync(0xffffffffu, wv < 0.0);
+            if (lane == 0) d->sign[p >> 5] = neg;
+        }
+        if (lane == 0) {
+            d->valid = 1;
+            d->evaluated = 0;
+        }
+        __syncwarp();
+    };
 
+    // ---- consumers: phase 1, evaluate this item's share of its region's psi ----------------------
+    auto evaluate = [&](const ItemDesc* d, int w, int nw) {
+        const int ntask = d->region.ntask, nshare = d->region.nitem, share = d->item.share;
+        const uint32_t* tasks = P.etasks + d->region.task_off;
+        const Entry* entries = P.entries + d->region.entry0;
+        double* psi_region = P.psi + (size_t)d->region.psi_chunk0 * kChunkDoubles;
+        for (int t = share + nshare * w; t < ntask; t += nshare * nw) {
+            const uint32_t tk = __ldg(tasks + t);
+            const int slice = (int)(tk >> 16);
+            eval_task(P, tab, entries + (tk & 0xFFFFu), slice, lane, s_off, d->sqrtw,
+                      psi_region + (size_t)(2 * slice) * kChunkDoubles);
+        }
+    };
+    auto publish = [&](const ItemDesc* d) {   // after bar_consumers(): every consumer's stores precede the fence
+        __threadfence();
+        fence_proxy_async();
+        atomicAdd(P.ready + d->item.region, 1u);
+    };
+
+    __syncthreads();
+    if (warp == kConsumerWarps) {
+        prepare(&s_desc[0]);
+        prepare(&s_desc[1]);
+    }
+    __syncthreads();
+    if (warp < kConsumerWarps && s_desc[0].valid) {
+        evaluate(&s_desc[0], warp, kConsumerWarps);
+        bar_consumers();
+        if (tid == 0) publish(&s_desc[0]);
+    }
+
+    uint32_t nstage_done = 0;   // stages streamed so far (same count in every warp): ring slot and phase parity
+    const int frow = lane >> 2, fk = lane & 3;
+    for (int iter = 0;; iter++) {
+        __syncthreads();   // previous item finished by all warps: its descriptor slot and the ring are free
+        const ItemDesc* cur = &s_desc[iter % kDescSlots];
+        if (!cur->valid) break;
+        const ItemDesc* nxt = &s_desc[(iter + 1) % kDescSlots];
+        const uint32_t stage_mask = cur->item.stage_mask;
+
+        if (warp == kConsumerWarps) {
+            // ================= producer warp =================
+            const unsigned char* psi_bytes = reinterpret_cast<const unsigned char*>(P.psi) +
+                                             (size_t)cur->region.psi_chunk0 * kChunkBytes;
+            const int nslot = cur->item.nslot, nst = P.nstage;
+            const unsigned int* flag = P.ready + cur->item.region;
+            const unsigned int need = (unsigned int)cur->region.nitem;
+            uint32_t todo = stage_mask, n = nstage_done;
+            auto issue = [&](int s) {   // lane 0
+                const uint32_t slot_r = n % (uint32_t)nring, ph = (n / (uint32_t)nring) & 1u;
+                mbar_wait(smem_u32(s_empty + slot_r), ph ^ 1u);
+                uint32_t act = 0;
+                for (int q = 0; q < nslot; q++)
+                    if (*reinterpret_cast<const uint32_t*>(&cur->gmask[q][s * kStageKsteps])) act |= 1u << q;
+                const uint32_t bar = smem_u32(s_full + slot_r);
+                if (act) mbar_arrive_expect_tx(bar, (uint32_t)__popc(act) * kChunkBytes);
+                else mbar_arrive(bar);
+                const uint32_t dst0 = smem_u32(s_ring + (size_t)slot_r * kStageBytes);
+                for (int q = 0; q < nslot; q++)
+                    if ((act >> q) & 1u)
+                        bulk_g2s(dst0 + q * kChunkBytes,
+                                 psi_bytes + ((size_t)cur->item.slot_group[q] * nst + s) * kChunkBytes, kChunkBytes, bar);
+                n++;
+            };
+            // Common case: every share of the region is already published -> fill the ring first, then
+            // prefetch the next descriptor.  Otherwise take the next item first (it may be the missing
+            // share, and nobody else may be left to take it) and wait afterwards.
+            int ok = 0;
+            if (lane == 0) ok = ld_acquire(flag) >= need;
+            ok = __shfl_sync(0xffffffffu, ok, 0);
+            if (ok && lane == 0) {
+                fence_proxy_async();
+                for (int i = 0; i < nring && todo; i++) {
+                    const int s = __ffs(todo) - 1;
+                    todo &= todo - 1;
+                    issue(s);
+                }
+            }
+            __syncwarp();
+            ItemDesc* pre = &s_desc[(iter + 2) % kDescSlots];
+            if (nxt->valid) {
+                prepare(pre);
+                if (pre->valid && pre->item.region == cur->item.region) {
+                    // this CTA would hold an unevaluated share of the region it is about to wait for
+                    evaluate(pre, 0, 1);
+                    __syncwarp();
+                    if (lane == 0) {
+                        publish(pre);
+                        pre->evaluated = 1;
+                    }
+                }
+            } else if (lane == 0) {
+                pre->valid = 0;
+            }
+            __syncwarp();
+            if (lane == 0) {
+                if (!ok) {
+                    while (ld_acquire(flag) < need) __nanosleep(64);
+                    fence_proxy_async();
+                }
+                while (todo) {
+                    const int s = __ffs(todo) - 1;
+                    todo &= todo - 1;
+                    issue(s);
+                }
+            }
+            nstage_done += __popc(stage_mask);
+            continue;
+        }
+
+        // ================= consumer warps =================
+        if (nxt->valid && !nxt->evaluated) {
+            evaluate(nxt, warp, kConsumerWarps);
+            bar_consumers();
+            if (tid == 0) publish(nxt);
+        }
+        const int sa = cur->item.tiles[warp][0], sb = cur->item.tiles[warp][1];
+        const bool has_tile = sa != 0xFF;
+        const bool diag = sa == sb;
+        const uint32_t tile_mask = diag ? 0x8CEFu : 0xFFFFu;   // diagonal tile: fragments i <= j only (bit 4i+j)
         double acc[4][4][2];
 #pragma unroll
         for (int i = 0; i < 4; i++)
 #pragma unroll
             for (int j = 0; j < 4; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
-        const bool has_tile = warp < ntile;
-        const int sa = has_tile ? s_item->tiles[warp][0] : 0, sb = has_tile ? s_item->tiles[warp][1] : 0;
-        const uint32_t tile_mask = (sa == sb) ? 0x8CEFu : 0xFFFFu;   // diagonal tile: fragments i <= j only
 
-        // ---------------- stream the slices ------------------------------------------------------
-        uint32_t todo = slice_mask;
-        int cur = __ffs(todo) - 1;
-        todo &= todo - 1;
-        int b = 0;
-        evaluate(cur, 0);
-        __syncthreads();
-        while (true) {
-            const int next = todo ? __ffs(todo) - 1 : -1;
+        uint32_t todo = stage_mask, n = nstage_done;
+        while (todo) {
+            const int s = __ffs(todo) - 1;
             todo &= todo - 1;
-            if (next >= 0) evaluate(next, b ^ 1);
+            const uint32_t slot_r = n % (uint32_t)nring, ph = (n / (uint32_t)nring) & 1u;
+            n++;
+            mbar_wait(smem_u32(s_full + slot_r), ph);
             if (has_tile) {
-                const double* bufp = s_phi + b * kBufDoubles;
-                const double* pa = bufp + (sa * kGroupRows + frow) * kLD + fk;
-                const double* pb = bufp + (sb * kGroupRows + frow) * kLD + fk;
-                const double* pw = s_w + b * kSlicePts + fk;
-                const uint2 ra8 = *reinterpret_cast<const uint2*>(s_gmask + sa * kMaxKsteps + cur * kSliceKsteps);
-                const uint2 ca8 = *reinterpret_cast<const uint2*>(s_gmask + sb * kMaxKsteps + cur * kSliceKsteps);
-#pragma unroll 1
-                for (int ks = 0; ks < kSliceKsteps; ks++) {
-                    const uint32_t rw = (ks < 4) ? ra8.x : ra8.y, cw = (ks < 4) ? ca8.x : ca8.y;
-                    const uint32_t ra = (rw >> (8 * (ks & 3))) & 0xFu, ca = (cw >> (8 * (ks & 3))) & 0xFu;
+                const uint32_t ma = *reinterpret_cast<const uint32_t*>(&cur->gmask[sa][s * kStageKsteps]);
+                const uint32_t mb = *reinterpret_cast<const uint32_t*>(&cur->gmask[sb][s * kStageKsteps]);
+                const unsigned char* stage = s_ring + (size_t)slot_r * kStageBytes;
+                const double2* pa = reinterpret_cast<const double2*>(stage + sa * kChunkBytes) + lane;
+                const double2* pb = reinterpret_cast<const double2*>(stage + sb * kChunkBytes) + lane;
+                // sign bits of V dV at this lane's four points (k-step ks: bit 4 ks + fk of the stage's 16)
+                const uint32_t sg = (cur->sign[s >> 1] >> ((s & 1) * 16 + fk));
+#pragma unroll
+                for (int kp = 0; kp < 2; kp++) {
+                    const uint32_t ra0 = (ma >> (16 * kp)) & 0xFu, ra1 = (ma >> (16 * kp + 8)) & 0xFu;
+                    const uint32_t ca0 = (mb >> (16 * kp)) & 0xFu, ca1 = (mb >> (16 * kp + 8)) & 0xFu;
                     // pair mask: bit 4i+j <=> row fragment i and column fragment j both active
-                    const uint32_t spread = (ra & 1u) | ((ra & 2u) << 3) | ((ra & 4u) << 6) | ((ra & 8u) << 9);
-                    const uint32_t pm = (ca * spread) & tile_mask;
-                    if (pm == 0u) continue;
-                    const double wv = pw[4 * ks];
-                    double a[4], bb[4];
+                    const uint32_t sp0 = (ra0 & 1u) | ((ra0 & 2u) << 3) | ((ra0 & 4u) << 6) | ((ra0 & 8u) << 9);
+                    const uint32_t sp1 = (ra1 & 1u) | ((ra1 & 2u) << 3) | ((ra1 & 4u) << 6) | ((ra1 & 8u) << 9);
+                    const uint32_t pm0 = (ca0 * sp0) & tile_mask, pm1 = (ca1 * sp1) & tile_mask;
+                    if ((pm0 | pm1) == 0u) continue;
+                    const uint32_t rows = ra0 | ra1, cols = ca0 | ca1;
+                    double2 a[4], b[4];
 #pragma unroll
                     for (int i = 0; i < 4; i++) {
-                        a[i] = pa[(8 * i) * kLD + 4 * ks];
-                        bb[i] = wv * pb[(8 * i) * kLD + 4 * ks];
+                        a[i] = make_double2(0.0, 0.0);
+                        if ((rows >> i) & 1u) a[i] = pa[(i * 2 + kp) * 32];
                     }
-                    if (pm == 0xFFFFu) {
+                    const uint32_t x0 = ((sg >> (8 * kp)) & 1u) << 31, x1 = ((sg >> (8 * kp + 4)) & 1u) << 31;
+#pragma unroll
+                    for (int j = 0; j < 4; j++) {
+                        b[j] = make_double2(0.0, 0.0);
+                        if ((cols >> j) & 1u) b[j] = diag ? a[j] : pb[(j * 2 + kp) * 32];
+                        b[j].x = __hiloint2double(__double2hiint(b[j].x) ^ x0, __double2loint(b[j].x));
+                        b[j].y = __hiloint2double(__double2hiint(b[j].y) ^ x1, __double2loint(b[j].y));
+                    }
+                    if (pm0 == tile_mask && pm1 == tile_mask && !diag) {
 #pragma unroll
                         for (int i = 0; i < 4; i++)
 #pragma unroll
-                            for (int j = 0; j < 4; j++) dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i], bb[j]);
+                            for (int j = 0; j < 4; j++) {
+                                dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
+                                dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
+                            }
                     } else {
 #pragma unroll
                         for (int i = 0; i < 4; i++)
 #pragma unroll
-                            for (int j = 0; j < 4; j++)
-                                dmma8x8x4_if(acc[i][j][0], acc[i][j][1], a[i], bb[j], pm & (1u << (4 * i + j)));
+                            for (int j = 0; j < 4; j++) {
+                                if (pm0 & (1u << (4 * i + j))) dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
+                                if (pm1 & (1u << (4 * i + j))) dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
+                            }
                     }
                 }
             }
-            __syncthreads();
-            if (next < 0) break;
-            cur = next;
-            b ^= 1;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(s_empty + slot_r));
         }
+        nstage_done = n;
 
         // ---------------- flush: add the tile into the canonical H blocks ---------------------------
         if (has_tile) {
-            const int ga = s_item->slot_group[sa], gb = s_item->slot_group[sb];
-            const uint32_t* rinfo = P.rowinfo + s_region->rowinfo_off;
-            const uint32_t* pair = P.pair + s_region->pair_off;
-            const int m = s_region->nentry;
+            const int ga = cur->item.slot_group[sa], gb = cur->item.slot_group[sb];
+            const uint32_t* rinfo = P.rowinfo + cur->region.rowinfo_off;
+            const uint32_t* pair = P.pair + cur->region.pair_off;
+            const int m = cur->region.nentry;
 #pragma unroll
             for (int i = 0; i < 4; i++) {
                 const int row = ga * kGroupRows + 8 * i + frow;
@@ -278,7 +440,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                 const int ea = ri & 0xFFF, mu = (ri >> 12) & 0xFF, nI = ri >> 20;
 #pragma unroll
                 for (int j = 0; j < 4; j++) {
-                    if (sa == sb && i > j) continue;
+                    if (diag && i > j) continue;
 #pragma unroll
                     for (int h = 0; h < 2; h++) {
                         const double v = acc[i][j][h];
@@ -296,7 +458,6 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                 }
             }
         }
-        // loop-top __syncthreads separates the flush from the next item's staging
     }
 }
 
@@ -332,7 +493,8 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t smem_bytes, bool tab_smem,
     if (ev) cudaEventRecord(ev[0], stream);
     cudaError_t e = cudaMemsetAsync(H, 0, h_len * sizeof(double), stream);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int), stream);
+    // queue head and per-region share counters live in one allocation: counter[0], ready[nregions]
+    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * (size_t)(1 + P.nregions), stream);
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[1], stream);
     if (P.nitems > 0) {

@@ -61,7 +61,6 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.nranks = nranks;
     P.species.assign(species, species + nspecies);
     double rc_max = 0;
-    int tab_off = 0;
     for (int s = 0; s < nspecies; s++) {
         SpeciesHost& sp = P.species[s];
         if (!(sp.rcut > 0) || !(sp.dr > 0) || sp.nrad <= 0 || sp.ntab < 4) { err = "bad species"; return GINT_EINVAL; }
@@ -76,8 +75,6 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         if (sp.norb > kMaxOrbPerAtom) { err = "too many orbitals per atom"; return GINT_EUNSUPPORTED; }
         for (double v : sp.table)
             if (!std::isfinite(v)) { err = "table not finite"; return GINT_EINVAL; }
-        sp.tab_offset = tab_off;
-        tab_off += sp.ntab * sp.nrad;
         rc_max = std::max(rc_max, sp.rcut);
     }
     P.atom_species.assign(atom_species, atom_species + natom);
@@ -191,29 +188,43 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         }
     }
 
-    // ---- packed radial tables (node-major: [k][nrad]) ---------------------------
-    P.tab_packed.resize((size_t)tab_off);
-    for (int s = 0; s < nspecies; s++) {
-        const SpeciesHost& sp = P.species[s];
-        for (int k = 0; k < sp.ntab; k++)
-            for (int f = 0; f < sp.nrad; f++)
-                P.tab_packed[(size_t)sp.tab_offset + (size_t)k * sp.nrad + f] = sp.table[(size_t)f * sp.ntab + k];
-        P.sp_meta.push_back(sp.tab_offset);
-        P.sp_meta.push_back(sp.ntab);
-        P.sp_meta.push_back(sp.nrad);
-        P.sp_meta.push_back(sp.norb);
-        for (int k = 0; k < 8; k++) P.sp_meta.push_back(k < sp.nrad ? sp.l[k] : -1);
-        P.sp_real.push_back(sp.rcut * sp.rcut);
-        P.sp_real.push_back(1.0 / sp.dr);
+    // ---- packed radial tables: node-major [ntab+4][nradp], pre-multiplied by the Y_lm constant -------
+    // l=0: 1/(2 sqrt(pi)); l=1: sqrt(3/4pi); l=2: 1/2 sqrt(15/pi) (the kernel applies the two remaining
+    // l=2 ratios to the angular polynomials).  Four zero nodes follow the table: the stencil of a point
+    // outside the sphere is redirected there, so phi == 0 exactly for r >= rcut.
+    {
+        const double ylm_c[3] = {0.28209479177387814, 0.48860251190291992, 1.0925484305920792};
+        size_t off = 0;
+        for (int s = 0; s < nspecies; s++) {
+            SpeciesHost& sp = P.species[s];
+            const int nradp = (sp.nrad + 1) & ~1;
+            sp.tab_offset = (int)off;
+            P.tab_packed.resize(off + (size_t)(sp.ntab + 4) * nradp, 0.0);
+            for (int k = 0; k < sp.ntab; k++)
+                for (int f = 0; f < sp.nrad; f++)
+                    P.tab_packed[off + (size_t)k * nradp + f] = sp.table[(size_t)f * sp.ntab + k] * ylm_c[sp.l[f]];
+            off = P.tab_packed.size();
+            P.sp_meta.push_back(sp.tab_offset);
+            P.sp_meta.push_back(sp.ntab);
+            P.sp_meta.push_back(nradp);
+            P.sp_meta.push_back(sp.norb);
+            for (int k = 0; k < 8; k++) P.sp_meta.push_back(k < sp.nrad ? sp.l[k] : -1);
+            P.sp_real.push_back(sp.rcut * sp.rcut);
+            P.sp_real.push_back(1.0 / sp.dr);
+        }
     }
-    const size_t table_bytes_all = P.tab_packed.size() * sizeof(double);
-    P.tables_in_smem = table_bytes_all <= 64 * 1024;
-
-    // smem: the radial tables go to shared memory when the phi double buffer leaves room for them
-    if (P.tables_in_smem && smem_layout(table_bytes_all).total > kSmemLimit) P.tables_in_smem = false;
-    const size_t table_bytes = P.tables_in_smem ? table_bytes_all : 0;
-    P.smem_bytes = smem_layout(table_bytes).total;
-    if (P.smem_bytes > kSmemLimit) { err = "internal: shared-memory layout exceeds 227 KB"; return GINT_EUNSUPPORTED; }
+    // shared memory: as many ring stages as fit next to the tables (3..6); tables stay in global memory
+    // (L1/L2-cached) when even three stages do not fit
+    {
+        const size_t table_bytes_all = P.tab_packed.size() * sizeof(double);
+        P.tables_in_smem = false;
+        P.nring = 0;
+        for (int nr = 6; nr >= 3 && !P.nring; nr--)
+            if (smem_layout(table_bytes_all, nr).total <= kSmemLimit) { P.nring = nr; P.tables_in_smem = true; }
+        if (!P.nring) P.nring = 6;
+        P.smem_bytes = smem_layout(P.tables_in_smem ? table_bytes_all : 0, P.nring).total;
+        if (P.smem_bytes > kSmemLimit) { err = "internal: shared-memory layout exceeds 227 KB"; return GINT_EUNSUPPORTED; }
+    }
 
     // ---- point order inside a region: k-steps of 4 points, slices of 8 k-steps -----------------
     const int bx = P.bcell[0], by = P.bcell[1], bz = P.bcell[2];
@@ -233,6 +244,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         P.nks = (P.npts + kKstepPts - 1) / kKstepPts;
         P.nslice = (P.nks + kSliceKsteps - 1) / kSliceKsteps;
         P.nks_pad = P.nslice * kSliceKsteps;
+        P.nstage = P.nks_pad / kStageKsteps;
         while ((int)order.size() < P.nks_pad * kKstepPts) order.push_back({0, 0, 0, 0});
         P.slot_xyz.resize(order.size() * 4);
         for (size_t i = 0; i < order.size(); i++)
@@ -360,10 +372,10 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     for (size_t i = 0; i < tmp.size(); i++) P.entries[i] = tmp[i].e;
 
     // ---- per region: rows, fragment / group activity, row info, pair table, tiles, work items -----
-    struct ItemCost { double cost; };
-    std::vector<double> item_cost;
-    double exec_dmma = 0, flush_elems = 0, phi_tasks = 0, max_rows = 0;
-    const int nks_pad = P.nks_pad, nslice = P.nslice;
+    struct RegionItems { int region; double cost; std::vector<WorkItem> items; };
+    std::vector<RegionItems> region_items;
+    double exec_dmma = 0, flush_elems = 0, n_etask = 0, max_rows = 0, chunk_loads = 0;
+    const int nks_pad = P.nks_pad, nslice = P.nslice, nstage = P.nstage;
     size_t pos = 0;
     while (pos < tmp.size()) {
         size_t end = pos;
@@ -372,6 +384,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         const int m = (int)(end - pos);
         if (m > 4095) { err = "more than 4095 atom images touch one region"; return GINT_EUNSUPPORTED; }
         Region R;
+        std::memset(&R, 0, sizeof(R));
         const int c3 = (int)(c % P.ncell[2]), c2 = (int)((c / P.ncell[2]) % P.ncell[1]), c1 = (int)(c / ((int64_t)P.ncell[1] * P.ncell[2]));
         R.origin[0] = c1 * bx;
         R.origin[1] = c2 * by;
@@ -386,13 +399,25 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         max_rows = std::max(max_rows, (double)rows);
         R.nrow = rows;
         R.nentry = m;
+        R.entry0 = (int32_t)pos;
+        R.ngroup = ngroup;
         R.gmask_off = (int32_t)P.gmask.size();
         R.rowinfo_off = (int32_t)P.rowinfo.size();
         R.pair_off = (int32_t)P.pair.size();
-        if (P.gmask.size() + (size_t)ngroup * nks_pad > 0x7FFFFFFFu || P.pair.size() + (size_t)m * m > 0x7FFFFFFFu) {
+        R.task_off = (int32_t)P.etasks.size();
+        R.psi_chunk0 = P.psi_chunks;
+        if (P.gmask.size() + (size_t)ngroup * nks_pad > 0x7FFFFFFFu || P.pair.size() + (size_t)m * m > 0x7FFFFFFFu ||
+            P.etasks.size() + (size_t)m * nslice > 0x7FFFFFFFu) {
             err = "plan tables exceed 2^31 entries";
             return GINT_EUNSUPPORTED;
         }
+        // evaluation tasks: (entry, 32-point slice) pairs with at least one point inside the sphere
+        for (int s = 0; s < nslice; s++)
+            for (int i = 0; i < m; i++) {
+                const Entry& e = P.entries[pos + i];
+                if ((e.kmask[(s * kSliceKsteps) >> 5] >> ((s * kSliceKsteps) & 31)) & 0xFFu) P.etasks.push_back(pack_etask(i, s));
+            }
+        R.ntask = (int32_t)P.etasks.size() - R.task_off;
         // fragment activity: OR of the k-step masks of the entries that own rows of the fragment
         std::vector<std::array<uint32_t, 4>> fmask((size_t)ngroup * 4, std::array<uint32_t, 4>{0, 0, 0, 0});
         P.rowinfo.resize(P.rowinfo.size() + (size_t)ngroup * kGroupRows, kNoBlock);
@@ -426,10 +451,10 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 if (off != kNoBlock && !canonical) off |= kPairTransposed;
                 P.pair[(size_t)R.pair_off + (size_t)a * m + b] = off;
             }
-        // tiles (group gi <= gj) and their cost per slice
-        auto tile_slice_cost = [&](int gi, int gj, int s) {
+        // tiles (group gi <= gj) and their cost (DMMAs) per stage
+        auto tile_stage_cost = [&](int gi, int gj, int st) {
             int n = 0;
-            for (int ks = s * kSliceKsteps; ks < (s + 1) * kSliceKsteps; ks++) {
+            for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) {
                 const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
                 if (gi != gj) n += __builtin_popcount(ra) * __builtin_popcount(ca);
                 else
@@ -444,7 +469,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         for (int gi = 0; gi < ngroup; gi++)
             for (int gj = gi; gj < ngroup; gj++) {
                 int n = 0;
-                for (int s = 0; s < nslice; s++) n += tile_slice_cost(gi, gj, s);
+                for (int st = 0; st < nstage; st++) n += tile_stage_cost(gi, gj, st);
                 tcost[(size_t)gi][(size_t)gj] = n;
             }
         std::vector<Proto> protos;
@@ -469,7 +494,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 }
             }
         }
-        // greedy merge of small proto-items (fewer phi evaluations, fewer items)
+        // greedy merge of small proto-items (fewer items, fewer chunk loads)
         for (bool merged = true; merged;) {
             merged = false;
             int best_a = -1, best_b = -1, best_union = 1 << 30;
@@ -489,76 +514,70 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 merged = true;
             }
         }
+        if (protos.size() > 32767) { err = "internal: too many work items in one region"; return GINT_EUNSUPPORTED; }
         const int region_index = (int)P.regions.size();
+        RegionItems ri;
+        ri.region = region_index;
+        ri.cost = 0;
         for (Proto& p : protos) {
             std::sort(p.groups.begin(), p.groups.end());
             WorkItem w;
             std::memset(&w, 0, sizeof(w));
+            std::memset(w.tiles, 0xFF, sizeof(w.tiles));
             w.region = region_index;
+            w.share = (int16_t)ri.items.size();
             w.nslot = (int32_t)p.groups.size();
             for (size_t s = 0; s < p.groups.size(); s++) w.slot_group[s] = (uint8_t)p.groups[s];
             auto slot_of = [&](int g) { return (int)(std::find(p.groups.begin(), p.groups.end(), g) - p.groups.begin()); };
-            // heaviest tiles first: warp w takes tile w
+            // heaviest tiles first onto the least loaded scheduler (consumer warp w runs on SM sub-partition w % 4)
             std::sort(p.tiles.begin(), p.tiles.end(), [&](const std::pair<int, int>& a, const std::pair<int, int>& b) {
                 return tcost[(size_t)a.first][(size_t)a.second] > tcost[(size_t)b.first][(size_t)b.second];
             });
             w.ntile = (int16_t)p.tiles.size();
-            double cost = 0;
+            double load[4] = {0, 0, 0, 0};
+            int used[4] = {0, 0, 0, 0};
             for (size_t t = 0; t < p.tiles.size(); t++) {
-                w.tiles[t][0] = (uint8_t)slot_of(p.tiles[t].first);
-                w.tiles[t][1] = (uint8_t)slot_of(p.tiles[t].second);
-                cost += tcost[(size_t)p.tiles[t].first][(size_t)p.tiles[t].second];
-                for (int s = 0; s < nslice; s++)
-                    if (tile_slice_cost(p.tiles[t].first, p.tiles[t].second, s) > 0) w.slice_mask |= 1u << s;
+                int q = -1;
+                for (int k = 0; k < 4; k++)   // sub-partition 3 also hosts the producer warp: three consumers there
+                    if (used[k] < (k == 3 ? 3 : 4) && (q < 0 || load[k] < load[q])) q = k;
+                const int warp = q + 4 * used[q];
+                used[q]++;
+                const double tc = tcost[(size_t)p.tiles[t].first][(size_t)p.tiles[t].second];
+                load[q] += tc;
+                w.tiles[warp][0] = (uint8_t)slot_of(p.tiles[t].first);
+                w.tiles[warp][1] = (uint8_t)slot_of(p.tiles[t].second);
+                exec_dmma += tc;
+                for (int st = 0; st < nstage; st++)
+                    if (tile_stage_cost(p.tiles[t].first, p.tiles[t].second, st) > 0) w.stage_mask |= 1u << st;
             }
-            exec_dmma += cost;
+            ri.cost += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
             flush_elems += 1024.0 * (double)p.tiles.size();
-            // evaluation tasks: entries owning rows in the item's groups
-            w.task0 = (int32_t)P.tasks.size();
-            int ntask = 0;
-            for (int i = 0; i < m; i++) {
-                const Entry& e = P.entries[pos + i];
-                const int g0 = e.row0 >> 5, g1 = (e.row0 + e.norb - 1) >> 5;
-                EvalTask t;
-                std::memset(&t, 0, sizeof(t));
-                t.entry = (int32_t)(pos + i);
-                t.row0 = (int16_t)e.row0;
-                bool any = false;
-                for (int k = 0; k < 3; k++) {
-                    t.slot[k] = -1;
-                    const int g = g0 + k;
-                    if (g > g1) continue;
-                    const int s = slot_of(g);
-                    if (s < (int)p.groups.size()) { t.slot[k] = (int8_t)s; any = true; }
-                }
-                if (!any) continue;
-                P.tasks.push_back(t);
-                ntask++;
-                for (int s = 0; s < nslice; s++)
-                    if (((w.slice_mask >> s) & 1u) && ((e.kmask[(s * kSliceKsteps) >> 5] >> ((s * kSliceKsteps) & 31)) & 0xFFu)) {
-                        phi_tasks += 1;
-                        cost += 12.0;   // one (entry, slice) phi evaluation ~ 12 DMMA issue times of FP64 pipe
+            for (int st = 0; st < nstage; st++)
+                if ((w.stage_mask >> st) & 1u)
+                    for (int g : p.groups) {
+                        bool act = false;
+                        for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) act = act || gm[(size_t)g * nks_pad + ks];
+                        if (act) chunk_loads += 1;
                     }
-            }
-            if (ntask > kMaxTasksPerItem) { err = "internal: too many evaluation tasks in one work item"; return GINT_EUNSUPPORTED; }
-            w.ntask = (int16_t)ntask;
-            P.items.push_back(w);
-            item_cost.push_back(cost);
+            ri.items.push_back(w);
+        }
+        R.nitem = (int32_t)ri.items.size();
+        if (R.nitem > 0) {
+            P.psi_chunks += (int64_t)ngroup * nstage;
+            n_etask += R.ntask;
+            region_items.push_back(std::move(ri));
+        } else {
+            R.ntask = 0;
         }
         P.regions.push_back(R);
         pos = end;
     }
     tmp.clear();
     tmp.shrink_to_fit();
-    // longest-processing-time-first order for the dynamic queue
-    {
-        std::vector<size_t> idx(P.items.size());
-        std::iota(idx.begin(), idx.end(), size_t(0));
-        std::stable_sort(idx.begin(), idx.end(), [&](size_t a, size_t b) { return item_cost[a] > item_cost[b]; });
-        std::vector<WorkItem> sorted(P.items.size());
-        for (size_t i = 0; i < idx.size(); i++) sorted[i] = P.items[idx[i]];
-        P.items.swap(sorted);
-    }
+    // queue order: heaviest regions first, the items of a region consecutive (their CTAs share its psi)
+    std::stable_sort(region_items.begin(), region_items.end(), [](const RegionItems& a, const RegionItems& b) { return a.cost > b.cost; });
+    for (const RegionItems& ri : region_items)
+        for (const WorkItem& w : ri.items) P.items.push_back(w);
 
     double fpt = 0, fsym = 0;
     for (int32_t n : npoint_orb) {
@@ -576,7 +595,11 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[8] = fpt;
     P.stats[9] = fsym;
     P.stats[10] = n_insphere;
-    P.stats[11] = phi_tasks * kSlicePts;
+    P.stats[11] = n_etask * kSlicePts;
+    P.stats[12] = (double)P.psi_chunks * kChunkBytes;
+    P.stats[13] = chunk_loads * kChunkBytes;
+    P.stats[14] = (double)P.nring;
+    P.stats[15] = (double)P.regions.size();
     return GINT_OK;
 }
 

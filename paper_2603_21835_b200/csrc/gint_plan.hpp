@@ -7,20 +7,26 @@
 // -- PAPER.md:380 (Sec. 3.3.1), Fig. 2 at PAPER.md:368.
 //
 // A *region* is this build's BigGrid: a box of up to 512 mesh points.  Its points
-// are ordered into k-steps of 4 points (the K of one DMMA.8x8x4) and slices of 8
-// k-steps.  Every (atom image, region) pair whose sphere holds a point of the
-// region is an *entry*; entries are sorted densest first and their orbitals are
-// packed into consecutive *rows* of the region's phi matrix.  Rows are cut into
+// are ordered into k-steps of 4 points (the K of one DMMA.8x8x4), stages of 4
+// k-steps (16 points, one shared-memory pipeline stage of the contraction) and
+// evaluation slices of 2 stages (32 points, one lane per point).  Every (atom
+// image, region) pair whose sphere holds a point of the region is an *entry*;
+// entries are sorted densest first and their orbitals are packed into consecutive
+// *rows* of the region's psi matrix, psi = phi sqrt(|V dV|).  Rows are cut into
 // fragments of 8 (one DMMA operand) and groups of 32 (one warp-tile edge).  The
-// upper triangle of the region's  C = phi diag(V dV) phi^T  is cut into 32x32
-// tiles; tiles are packed 16 at a time (one per warp) into *work items* so that
-// an item touches at most kMaxSlots row groups.  An item is what one CTA keeps
-// register-resident while it streams the region's points through shared memory.
+// upper triangle of the region's  C = psi diag(sign V) psi^T  is cut into 32x32
+// tiles; tiles are packed 15 at a time (one per consumer warp) into *work items*
+// that touch at most kMaxSlots row groups.  The items of a region are consecutive
+// in the work queue; the CTA that takes item q of n evaluates share q of the
+// region's psi (phase 1), writes it to the psi scratch buffer in global memory
+// (L2-resident between the sibling CTAs) and later streams the groups its tiles
+// need back through shared memory with bulk copies (phase 2).
 //
 // Output of the plan (plain arrays, uploaded verbatim by gint_api.cu):
 //   * block table (I,J,R) sorted, offsets, mirror list
-//   * regions, entries, per-group k-step activity bytes, row info, pair->block table
-//   * work items (tile lists, slot maps, evaluation tasks), sorted by cost
+//   * regions, entries, evaluation tasks, per-group k-step activity bytes, row info,
+//     pair->block table
+//   * work items (tile lists, slot maps), region-major, heaviest regions first
 #pragma once
 #include <cstddef>
 #include <cstdint>
@@ -38,15 +44,18 @@ namespace gint {
 constexpr int kMaxOrbPerAtom = 64;
 constexpr int kMaxRegionPoints = 512;          // mesh points of one region
 constexpr int kKstepPts = 4;                   // K of DMMA.8x8x4
-constexpr int kSliceKsteps = 8;                // k-steps per shared-memory slice
-constexpr int kSlicePts = kKstepPts * kSliceKsteps;   // 32
+constexpr int kStageKsteps = 4;                // k-steps per pipeline stage
+constexpr int kStagePts = kKstepPts * kStageKsteps;     // 16
+constexpr int kSlicePts = 32;                  // points of one evaluation task (one lane per point)
+constexpr int kSliceKsteps = kSlicePts / kKstepPts;     // 8
 constexpr int kMaxKsteps = kMaxRegionPoints / kKstepPts;   // 128
-constexpr int kMaxSlices = kMaxKsteps / kSliceKsteps;      // 16
+constexpr int kMaxStages = kMaxKsteps / kStageKsteps;      // 32
 constexpr int kGroupRows = 32;                 // rows of one row group = warp-tile edge
 constexpr int kMaxSlots = 8;                   // row groups one work item may touch
-constexpr int kTilesPerItem = 16;              // one 32x32 tile per warp
+constexpr int kTilesPerItem = 15;              // one 32x32 tile per consumer warp (warp 15 is the producer)
 constexpr int kMaxGroups = 40;                 // row groups per region (<= 1280 orbitals listed)
-constexpr int kMaxTasksPerItem = 264;        // 8 groups x 32 rows of 1-orbital atoms + stragglers
+constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 512: psi of one (group, stage), fragment order
+constexpr int kChunkBytes = kChunkDoubles * 8;             // 4096
 constexpr uint32_t kNoBlock = 0xFFFFFFFFu;
 constexpr uint32_t kPairTransposed = 0x80000000u;
 
@@ -71,35 +80,35 @@ struct Entry {
 };
 static_assert(sizeof(Entry) == 64, "Entry layout is shared with the device");
 
-struct Region {          // 32 bytes
+struct Region {          // 64 bytes
     int32_t origin[3];   // mesh index of the region's first point
     int32_t nrow;        // orbitals listed
     int32_t gmask_off;   // into gmask: [ngroup][nks_pad] bytes, low nibble = fragment activity of a k-step
     int32_t rowinfo_off; // into rowinfo: [ngroup*32]
     int32_t pair_off;    // into pair: [nentry][nentry]
     int32_t nentry;
+    int32_t entry0;      // first entry of the region in entries
+    int32_t task_off;    // into etasks
+    int32_t ntask;       // evaluation tasks (entry, 32-point slice) with a point inside the sphere
+    int32_t nitem;       // work items of the region = number of evaluation shares
+    int64_t psi_chunk0;  // first 4 KB chunk of the region in the psi scratch: chunk(g, s) = psi_chunk0 + g*nstage + s
+    int32_t ngroup;
+    int32_t pad;
 };
-static_assert(sizeof(Region) == 32, "Region layout is shared with the device");
+static_assert(sizeof(Region) == 64, "Region layout is shared with the device");
 
-// One evaluation task of a work item: the orbitals of one entry that fall into the item's row groups.
-struct EvalTask {        // 12 bytes
-    int32_t entry;       // index into entries
-    int16_t row0;        // region row of the entry's first orbital
-    int8_t slot[3];      // shared-memory slot of row group (row0>>5)+k, -1 = group not needed by the item
-    int8_t pad[3];
-};
-static_assert(sizeof(EvalTask) == 12, "EvalTask layout is shared with the device");
+// evaluation task word: entry index within the region | slice << 16
+inline uint32_t pack_etask(int e, int slice) { return (uint32_t)e | ((uint32_t)slice << 16); }
 
 struct WorkItem {        // 64 bytes
     int32_t region;
-    int32_t task0;       // first EvalTask
-    int16_t ntask;
+    int16_t share;       // index of the item within its region: evaluates tasks t = share (mod nitem)
     int16_t ntile;
-    uint32_t slice_mask; // bit s: slice s holds work for this item
-    uint8_t tiles[kTilesPerItem][2];   // (slot of row group, slot of column group), row group <= column group
+    uint32_t stage_mask; // bit s: stage s (16 points) holds work for this item
+    uint8_t tiles[16][2];              // per consumer warp: (slot of row group, slot of column group), 0xFF = no tile
     uint8_t slot_group[kMaxSlots];     // region row group held by each slot
     int32_t nslot;
-    int32_t pad;
+    int32_t pad[2];
 };
 static_assert(sizeof(WorkItem) == 64, "WorkItem layout is shared with the device");
 
@@ -124,7 +133,7 @@ struct Plan {
     double dV = 0;
     double estep[9];             // mesh step vectors e_d = a_d / N_d (rows)
     // region point order
-    int npts = 0, nks = 0, nks_pad = 0, nslice = 0;
+    int npts = 0, nks = 0, nks_pad = 0, nslice = 0, nstage = 0;   // nks_pad = 8*nslice = 4*nstage
     std::vector<uint8_t> slot_xyz;              // [nslice*32][4]: ix, iy, iz, valid
     // blocks
     std::vector<int32_t> blk_i, blk_j, blk_R;   // blk_R [nblk][3]
@@ -142,37 +151,49 @@ struct Plan {
     std::vector<uint32_t> rowinfo;
     std::vector<uint32_t> pair;
     std::vector<WorkItem> items;
-    std::vector<EvalTask> tasks;
-    // packed radial tables for the device: per species [ntab][nrad] (node-major)
+    std::vector<uint32_t> etasks;               // evaluation tasks, region-major
+    int64_t psi_chunks = 0;                     // 4 KB chunks of the psi scratch buffer
+    // packed radial tables for the device: per species [ntab+4][nradp] (node-major, nradp = nrad rounded up
+    // to even, every function pre-multiplied by its Y_lm constant, four zero nodes appended)
     std::vector<double> tab_packed;
-    std::vector<int32_t> sp_meta;               // per species: tab_offset, ntab, nrad, norb, l[0..7] (12 ints)
+    std::vector<int32_t> sp_meta;               // per species: tab_offset, ntab, nradp, norb, l[0..7] (12 ints)
     std::vector<double> sp_real;                // per species: rcut^2, 1/dr
     // statistics
-    double stats[12] = {0};
+    double stats[16] = {0};
     size_t smem_bytes = 0;
     bool tables_in_smem = true;
+    int nring = 0;                              // pipeline stages of the psi ring in shared memory
 };
 
 constexpr size_t kSmemLimit = 232448;   // 227 KB opt-in limit per CTA on sm_100
-constexpr int kPhiLD = kSlicePts + 4;   // row stride of the phi slice in doubles (conflict-free fragment loads)
+constexpr int kDescSlots = 3;           // item descriptors in flight: current, next (being evaluated), prefetched
+
+// Per-item descriptor staged in shared memory by the producer warp.
+struct ItemDesc {
+    WorkItem item;                                  // 64
+    Region region;                                  // 64
+    uint8_t gmask[kMaxSlots][kMaxKsteps];           // 1024: fragment activity nibbles of the item's slots
+    uint32_t sign[kMaxRegionPoints / 32];           // 64: bit p = sign bit of V dV at point slot p
+    int32_t valid;                                  // 0 = queue exhausted
+    int32_t evaluated;                              // 1 = the producer warp already evaluated and published the share
+    int32_t pad[14];
+    double sqrtw[kMaxRegionPoints];                 // 4096: sqrt(|V dV|), 0 outside the mesh
+};
+static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
 // Shared-memory carve-up of the integration kernel (bytes); used by host and device.
 struct SmemLayout {
-    uint32_t tab, off, w, gmask, tasks, item, misc, phi, total;
+    uint32_t bar, desc, off, tab, ring, total;
 };
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
-GINT_HD inline SmemLayout smem_layout(size_t table_bytes) {
-    auto al = [](size_t x) { return smem_align(x); };
+GINT_HD inline SmemLayout smem_layout(size_t table_bytes, int nring) {
     SmemLayout L;
     uint32_t o = 0;
-    L.tab = o;   o += al(table_bytes);
-    L.off = o;   o += al((size_t)3 * kMaxRegionPoints * sizeof(double));
-    L.w = o;     o += al((size_t)2 * kSlicePts * sizeof(double));
-    L.gmask = o; o += al((size_t)kMaxSlots * kMaxKsteps);
-    L.tasks = o; o += al((size_t)kMaxTasksPerItem * sizeof(EvalTask));
-    L.item = o;  o += al(sizeof(WorkItem) + sizeof(Region));
-    L.misc = o;  o += 128;
-    L.phi = o;   o += al((size_t)2 * kMaxSlots * kGroupRows * kPhiLD * sizeof(double));
+    L.bar = o;   o += 256;                                           // mbarriers: full[8], empty[8]; misc words
+    L.desc = o;  o += smem_align((size_t)kDescSlots * sizeof(ItemDesc));
+    L.off = o;   o += smem_align((size_t)3 * kMaxRegionPoints * sizeof(double));
+    L.tab = o;   o += smem_align(table_bytes);
+    L.ring = o;  o += (uint32_t)nring * kMaxSlots * kChunkBytes;
     L.total = o;
     return L;
 }
