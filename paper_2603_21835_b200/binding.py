@@ -23,7 +23,7 @@ EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
-              "regions")
+              "regions", "ksteps_full", "ksteps_partial", "dmma_in_partial_ksteps", "stage_visits", "s20", "s21", "s22", "s23")
 
 
 class GintError(RuntimeError):
@@ -116,8 +116,8 @@ class GintContext:
         return iat[:n], jat[:n], R[:n], off
 
     def gint_get_stats(self) -> dict:
-        s = np.zeros(16, dtype=np.float64)
-        n = _check(_lib.gint_get_stats(self._h, _ptr(s, ctypes.c_double), 16), "gint_get_stats")
+        s = np.zeros(24, dtype=np.float64)
+        n = _check(_lib.gint_get_stats(self._h, _ptr(s, ctypes.c_double), 24), "gint_get_stats")
         return {STAT_NAMES[i]: float(s[i]) for i in range(n)}
 
     def gint_set_profiling(self, on: bool = True):

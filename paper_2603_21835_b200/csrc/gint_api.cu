@@ -1,6 +1,7 @@
 // gint_api.cu -- extern "C" boundary of libgint_b200.so (declared in include/gint.h).
 #include <cuda_runtime.h>
 
+#include <cstdio>
 #include <cstring>
 #include <new>
 #include <string>
@@ -52,6 +53,23 @@ cudaError_t upload(gint_ctx* ctx, const std::vector<T>& host, const T** dev_out)
 void release(gint_ctx* ctx) {
     if (ctx->device >= 0) {
         cudaSetDevice(ctx->device);
+#ifdef GINT_TIMING
+        if (ctx->dev.ready) {
+            std::vector<long long> tm(24 * 256);
+            cudaDeviceSynchronize();
+            cudaMemcpy(tm.data(), ctx->dev.ready + ctx->dev.nregions + 1, tm.size() * 8, cudaMemcpyDeviceToHost);
+            const char* names[3] = {"consumer w0: topbar eval pub fullwait contract flush items -", "consumer w5: topbar eval pub fullwait contract flush items -",
+                                    "producer   : topbar emptywait poll nslow - - - -"};
+            for (int r = 0; r < 3; r++) {
+                fprintf(stderr, "[timing] %s\n", names[r]);
+                for (int b : {0, 1, 73, 147}) {
+                    fprintf(stderr, "   cta %3d:", b);
+                    for (int k = 0; k < 8; k++) fprintf(stderr, " %10.3f", (k == 6 || (r == 2 && k == 3)) ? (double)tm[24 * b + 8 * r + k] : tm[24 * b + 8 * r + k] / 1.965e6);
+                    fprintf(stderr, "\n");
+                }
+            }
+        }
+#endif
         for (void* p : ctx->allocs) cudaFree(p);
         if (ctx->have_events)
             for (int i = 0; i < 4; i++) cudaEventDestroy(ctx->ev[i]);
@@ -136,7 +154,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     UP(P.sp_real, &D.sp_real)
 #undef UP
     void* ctr = nullptr;   // queue head + one share counter per region
-    if ((e = cudaMalloc(&ctr, sizeof(unsigned int) * (P.regions.size() + 1) + 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counters"); }
+    if ((e = cudaMalloc(&ctr, sizeof(unsigned int) * (P.regions.size() + 2) + 64 + 24 * 8 * 256)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counters"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
     D.ready = D.counter + 1;
@@ -155,6 +173,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     D.nstage = P.nstage;
     D.nregions = (int32_t)P.regions.size();
     D.nring = P.nring;
+    D.never = 0;
     D.nitems = (int32_t)P.items.size();
     D.nmirror = (int32_t)P.mirror.size();
     D.tab_doubles = (int32_t)P.tab_packed.size();
@@ -247,7 +266,7 @@ int gint_get_kernel_ms(gint_ctx* ctx, double* ms) {
 
 int gint_get_stats(const gint_ctx* ctx, double* stats, int32_t n) {
     if (!ctx || !stats) return fail(GINT_EINVAL, "null argument");
-    const int m = n < 16 ? n : 16;
+    const int m = n < 24 ? n : 24;
     for (int i = 0; i < m; i++) stats[i] = ctx->plan.stats[i];
     return m;
 }

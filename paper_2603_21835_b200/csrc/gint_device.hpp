@@ -35,6 +35,7 @@ struct DevicePlan {
     int32_t nitems, nmirror, nregions;
     int32_t tab_doubles;
     int32_t nring;
+    int32_t never;            // always 0: a branch condition the compiler cannot fold (see DMMA_IF in gint_kernels.cu)
 };
 
 cudaError_t configure_kernels(size_t smem_bytes, bool tab_smem);

@@ -34,6 +34,18 @@ namespace gint {
 
 namespace {
 
+#ifdef GINT_TIMING   // development only: per-CTA clock64 breakdown written behind the ready counters
+#define TIMER_DECL long long tm_[8] = {0, 0, 0, 0, 0, 0, 0, 0}; long long t0_ = 0; (void)t0_;
+#define TIMER_START t0_ = clock64();
+#define TIMER_ADD(k) tm_[k] += clock64() - t0_;
+#define TIMER_COUNT(k) tm_[k] += 1;
+#else
+#define TIMER_DECL
+#define TIMER_START
+#define TIMER_ADD(k)
+#define TIMER_COUNT(k)
+#endif
+
 constexpr int kConsumerWarps = kTilesPerItem;          // 15
 constexpr int kConsumerThreads = kConsumerWarps * 32;  // 480
 constexpr int kThreads = kConsumerThreads + 32;        // + 1 producer warp
@@ -44,6 +56,61 @@ __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, doub
                  : "+d"(c0), "+d"(c1)
                  : "d"(a), "d"(b));
 }
+
+// DMMA under a warp-uniform condition.  A predicated-off DMMA still holds the FP64 tensor pipe for its
+// 16 cycles (measured), and ptxas if-converts a plain `if` around one into exactly that; the never-taken
+// back edge (again is always 0 at run time) makes the block a loop, which is not if-converted.
+#define DMMA_IF(cond, c0, c1, a, b, again) \
+    if (cond) {                            \
+        do {                               \
+            dmma8x8x4(c0, c1, a, b);       \
+        } while (again);                   \
+    }
+
+// One k-step of an off-diagonal tile: row fragments ra x column fragments ca (4-bit masks).  The code
+// is selected by the column pattern (a jump on a warp-uniform value), the rows are guarded one by one.
+#define KROW(i, body)                                  \
+    if (ra & (1u << i)) {                              \
+        do { body } while (never);                     \
+    }
+#define KD(i, j) dmma8x8x4(acc[i][j][0], acc[i][j][1], a##i, b##j);
+#define KCASE(c, r0, r1, r2, r3) \
+    case c:                      \
+        KROW(0, r0) KROW(1, r1) KROW(2, r2) KROW(3, r3) break;
+__device__ __forceinline__ void kstep_rect(double (&acc)[4][4][2], uint32_t ra, uint32_t ca, double a0, double a1, double a2,
+                                           double a3, double b0, double b1, double b2, double b3, int never) {
+    switch (ca) {
+        KCASE(1, KD(0, 0), KD(1, 0), KD(2, 0), KD(3, 0))
+        KCASE(2, KD(0, 1), KD(1, 1), KD(2, 1), KD(3, 1))
+        KCASE(3, KD(0, 0) KD(0, 1), KD(1, 0) KD(1, 1), KD(2, 0) KD(2, 1), KD(3, 0) KD(3, 1))
+        KCASE(4, KD(0, 2), KD(1, 2), KD(2, 2), KD(3, 2))
+        KCASE(5, KD(0, 0) KD(0, 2), KD(1, 0) KD(1, 2), KD(2, 0) KD(2, 2), KD(3, 0) KD(3, 2))
+        KCASE(6, KD(0, 1) KD(0, 2), KD(1, 1) KD(1, 2), KD(2, 1) KD(2, 2), KD(3, 1) KD(3, 2))
+        KCASE(7, KD(0, 0) KD(0, 1) KD(0, 2), KD(1, 0) KD(1, 1) KD(1, 2), KD(2, 0) KD(2, 1) KD(2, 2), KD(3, 0) KD(3, 1) KD(3, 2))
+        KCASE(8, KD(0, 3), KD(1, 3), KD(2, 3), KD(3, 3))
+        KCASE(9, KD(0, 0) KD(0, 3), KD(1, 0) KD(1, 3), KD(2, 0) KD(2, 3), KD(3, 0) KD(3, 3))
+        KCASE(10, KD(0, 1) KD(0, 3), KD(1, 1) KD(1, 3), KD(2, 1) KD(2, 3), KD(3, 1) KD(3, 3))
+        KCASE(11, KD(0, 0) KD(0, 1) KD(0, 3), KD(1, 0) KD(1, 1) KD(1, 3), KD(2, 0) KD(2, 1) KD(2, 3), KD(3, 0) KD(3, 1) KD(3, 3))
+        KCASE(12, KD(0, 2) KD(0, 3), KD(1, 2) KD(1, 3), KD(2, 2) KD(2, 3), KD(3, 2) KD(3, 3))
+        KCASE(13, KD(0, 0) KD(0, 2) KD(0, 3), KD(1, 0) KD(1, 2) KD(1, 3), KD(2, 0) KD(2, 2) KD(2, 3), KD(3, 0) KD(3, 2) KD(3, 3))
+        KCASE(14, KD(0, 1) KD(0, 2) KD(0, 3), KD(1, 1) KD(1, 2) KD(1, 3), KD(2, 1) KD(2, 2) KD(2, 3), KD(3, 1) KD(3, 2) KD(3, 3))
+        KCASE(15, KD(0, 0) KD(0, 1) KD(0, 2) KD(0, 3), KD(1, 0) KD(1, 1) KD(1, 2) KD(1, 3), KD(2, 0) KD(2, 1) KD(2, 2) KD(2, 3),
+              KD(3, 0) KD(3, 1) KD(3, 2) KD(3, 3))
+        default: break;
+    }
+}
+// One k-step of a diagonal tile (row group == column group): fragment pairs i <= j with both active.
+__device__ __forceinline__ void kstep_diag(double (&acc)[4][4][2], uint32_t ra, double a0, double a1, double a2, double a3,
+                                           double b0, double b1, double b2, double b3, int never) {
+    KROW(0, KD(0, 0) DMMA_IF(ra & 2u, acc[0][1][0], acc[0][1][1], a0, b1, never) DMMA_IF(ra & 4u, acc[0][2][0], acc[0][2][1], a0, b2, never)
+                DMMA_IF(ra & 8u, acc[0][3][0], acc[0][3][1], a0, b3, never))
+    KROW(1, KD(1, 1) DMMA_IF(ra & 4u, acc[1][2][0], acc[1][2][1], a1, b2, never) DMMA_IF(ra & 8u, acc[1][3][0], acc[1][3][1], a1, b3, never))
+    KROW(2, KD(2, 2) DMMA_IF(ra & 8u, acc[2][3][0], acc[2][3][1], a2, b3, never))
+    KROW(3, KD(3, 3))
+}
+#undef KROW
+#undef KD
+#undef KCASE
 
 // ---- mbarrier / bulk-copy helpers (shared::cta addresses) --------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -76,6 +143,11 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
     unsigned int v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned int ld_relaxed(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void bar_consumers() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory"); }
@@ -172,10 +244,12 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
     uint64_t* s_full = reinterpret_cast<uint64_t*>(smem_raw + L.bar);         // [8]
     uint64_t* s_empty = s_full + 8;                                           // [8]
     ItemDesc* s_desc = reinterpret_cast<ItemDesc*>(smem_raw + L.desc);        // [3]
+    double* s_sqrtw = reinterpret_cast<double*>(smem_raw + L.sqrtw);          // [2][512] sqrt(|V dV|) of a region's points
     double* s_off = reinterpret_cast<double*>(smem_raw + L.off);              // [3][512] Cartesian offset of a point slot
     double* s_tab = reinterpret_cast<double*>(smem_raw + L.tab);
     unsigned char* s_ring = smem_raw + L.ring;                                // [nring][slot][4 KB]
     const int nring = P.nring;
+    const int never = P.never;   // always 0; see DMMA_IF
 
     if (TAB_SMEM) {
         for (int i = tid; i < P.tab_doubles; i += kThreads) s_tab[i] = __ldg(P.tab + i);
@@ -196,7 +270,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
     fence_proxy_async();
 
     // ---- producer warp: take the next item from the queue and stage its descriptor ---------------
-    auto prepare = [&](ItemDesc* d) {
+    auto prepare = [&](ItemDesc* d, double* sqrtw) {
         unsigned int it = 0;
         if (lane == 0) it = atomicAdd(P.counter, 1u);
         it = __shfl_sync(0xffffffffu, it, 0);
@@ -219,6 +293,15 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
             reinterpret_cast<uint32_t*>(d->gmask[slot])[wd] = __ldg(
                 reinterpret_cast<const uint32_t*>(P.gmask + d->region.gmask_off + (int)d->item.slot_group[slot] * P.nks_pad) + wd);
         }
+        for (int i = lane; i < nslot * kGroupRows; i += 32)
+            d->rinfo[i >> 5][i & 31] = __ldg(P.rowinfo + d->region.rowinfo_off + (int)d->item.slot_group[i >> 5] * kGroupRows + (i & 31));
+        __syncwarp();
+        {   // stage lane: which slots hold an active k-step there
+            uint32_t a = 0;
+            for (int q = 0; q < nslot; q++)
+                if (lane < P.nstage && *reinterpret_cast<const uint32_t*>(&d->gmask[q][lane * kStageKsteps])) a |= 1u << q;
+            d->act[lane] = (uint8_t)a;
+        }
         const int ox = d->region.origin[0], oy = d->region.origin[1], oz = d->region.origin[2];
         for (int p = lane; p < P.nslice * kSlicePts; p += 32) {   // w = V dV of the region's points (0 outside the mesh)
             const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
@@ -226,7 +309,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
             double wv = 0.0;
             if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
                 wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
-            d->sqrtw[p] = sqrt(fabs(wv));
+            sqrtw[p] = sqrt(fabs(wv));
             const unsigned int neg = __ballot_sync(0xffffffffu, wv < 0.0);
             if (lane == 0) d->sign[p >> 5] = neg;
         }
@@ -238,7 +321,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
     };
 
     // ---- consumers: phase 1, evaluate this item's share of its region's psi ----------------------
-    auto evaluate = [&](const ItemDesc* d, int w, int nw) {
+    auto evaluate = [&](const ItemDesc* d, const double* sqrtw, int w, int nw) {
         const int ntask = d->region.ntask, nshare = d->region.nitem, share = d->item.share;
         const uint32_t* tasks = P.etasks + d->region.task_off;
         const Entry* entries = P.entries + d->region.entry0;
@@ -246,7 +329,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
         for (int t = share + nshare * w; t < ntask; t += nshare * nw) {
             const uint32_t tk = __ldg(tasks + t);
             const int slice = (int)(tk >> 16);
-            eval_task(P, tab, entries + (tk & 0xFFFFu), slice, lane, s_off, d->sqrtw,
+            eval_task(P, tab, entries + (tk & 0xFFFFu), slice, lane, s_off, sqrtw,
                       psi_region + (size_t)(2 * slice) * kChunkDoubles);
         }
     };
@@ -258,20 +341,23 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
 
     __syncthreads();
     if (warp == kConsumerWarps) {
-        prepare(&s_desc[0]);
-        prepare(&s_desc[1]);
+        prepare(&s_desc[0], s_sqrtw);
+        prepare(&s_desc[1], s_sqrtw + kMaxRegionPoints);
     }
     __syncthreads();
     if (warp < kConsumerWarps && s_desc[0].valid) {
-        evaluate(&s_desc[0], warp, kConsumerWarps);
+        evaluate(&s_desc[0], s_sqrtw, warp, kConsumerWarps);
         bar_consumers();
         if (tid == 0) publish(&s_desc[0]);
     }
 
+    TIMER_DECL
     uint32_t nstage_done = 0;   // stages streamed so far (same count in every warp): ring slot and phase parity
     const int frow = lane >> 2, fk = lane & 3;
     for (int iter = 0;; iter++) {
+        TIMER_START
         __syncthreads();   // previous item finished by all warps: its descriptor slot and the ring are free
+        TIMER_ADD(0)
         const ItemDesc* cur = &s_desc[iter % kDescSlots];
         if (!cur->valid) break;
         const ItemDesc* nxt = &s_desc[(iter + 1) % kDescSlots];
@@ -285,20 +371,23 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
             const unsigned int* flag = P.ready + cur->item.region;
             const unsigned int need = (unsigned int)cur->region.nitem;
             uint32_t todo = stage_mask, n = nstage_done;
-            auto issue = [&](int s) {   // lane 0
+            // lane q copies the chunks of slot q; lane 0 also owns the barriers
+            const unsigned char* src_lane = psi_bytes + (size_t)(lane < nslot ? cur->item.slot_group[lane] : 0) * nst * kChunkBytes;
+            auto issue = [&](int s) {   // whole warp
                 const uint32_t slot_r = n % (uint32_t)nring, ph = (n / (uint32_t)nring) & 1u;
-                mbar_wait(smem_u32(s_empty + slot_r), ph ^ 1u);
-                uint32_t act = 0;
-                for (int q = 0; q < nslot; q++)
-                    if (*reinterpret_cast<const uint32_t*>(&cur->gmask[q][s * kStageKsteps])) act |= 1u << q;
+                const uint32_t act = cur->act[s];
                 const uint32_t bar = smem_u32(s_full + slot_r);
-                if (act) mbar_arrive_expect_tx(bar, (uint32_t)__popc(act) * kChunkBytes);
-                else mbar_arrive(bar);
-                const uint32_t dst0 = smem_u32(s_ring + (size_t)slot_r * kStageBytes);
-                for (int q = 0; q < nslot; q++)
-                    if ((act >> q) & 1u)
-                        bulk_g2s(dst0 + q * kChunkBytes,
-                                 psi_bytes + ((size_t)cur->item.slot_group[q] * nst + s) * kChunkBytes, kChunkBytes, bar);
+                if (lane == 0) {
+                    TIMER_START
+                    mbar_wait(smem_u32(s_empty + slot_r), ph ^ 1u);
+                    TIMER_ADD(1)
+                    if (act) mbar_arrive_expect_tx(bar, (uint32_t)__popc(act) * kChunkBytes);
+                    else mbar_arrive(bar);
+                }
+                __syncwarp();
+                if ((act >> lane) & 1u)
+                    bulk_g2s(smem_u32(s_ring + (size_t)slot_r * kStageBytes) + lane * kChunkBytes,
+                             src_lane + (size_t)s * kChunkBytes, kChunkBytes, bar);
                 n++;
             };
             // Common case: every share of the region is already published -> fill the ring first, then
@@ -307,7 +396,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
             int ok = 0;
             if (lane == 0) ok = ld_acquire(flag) >= need;
             ok = __shfl_sync(0xffffffffu, ok, 0);
-            if (ok && lane == 0) {
+            if (ok) {
                 fence_proxy_async();
                 for (int i = 0; i < nring && todo; i++) {
                     const int s = __ffs(todo) - 1;
@@ -315,13 +404,13 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                     issue(s);
                 }
             }
-            __syncwarp();
             ItemDesc* pre = &s_desc[(iter + 2) % kDescSlots];
             if (nxt->valid) {
-                prepare(pre);
+                double* sqrtw_pre = s_sqrtw + (iter & 1) * kMaxRegionPoints;
+                prepare(pre, sqrtw_pre);
                 if (pre->valid && pre->item.region == cur->item.region) {
                     // this CTA would hold an unevaluated share of the region it is about to wait for
-                    evaluate(pre, 0, 1);
+                    evaluate(pre, sqrtw_pre, 0, 1);
                     __syncwarp();
                     if (lane == 0) {
                         publish(pre);
@@ -332,16 +421,21 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                 pre->valid = 0;
             }
             __syncwarp();
-            if (lane == 0) {
-                if (!ok) {
-                    while (ld_acquire(flag) < need) __nanosleep(64);
-                    fence_proxy_async();
+            if (!ok) {
+                if (lane == 0) {
+                    TIMER_START
+                    TIMER_COUNT(3)
+                    while (ld_relaxed(flag) < need) __nanosleep(100);
+                    TIMER_ADD(2)
+                    (void)ld_acquire(flag);
                 }
-                while (todo) {
-                    const int s = __ffs(todo) - 1;
-                    todo &= todo - 1;
-                    issue(s);
-                }
+                __syncwarp();
+                fence_proxy_async();
+            }
+            while (todo) {
+                const int s = __ffs(todo) - 1;
+                todo &= todo - 1;
+                issue(s);
             }
             nstage_done += __popc(stage_mask);
             continue;
@@ -349,14 +443,16 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
 
         // ================= consumer warps =================
         if (nxt->valid && !nxt->evaluated) {
-            evaluate(nxt, warp, kConsumerWarps);
+            TIMER_START
+            evaluate(nxt, s_sqrtw + ((iter + 1) & 1) * kMaxRegionPoints, warp, kConsumerWarps);
+            TIMER_ADD(1)
             bar_consumers();
             if (tid == 0) publish(nxt);
+            TIMER_ADD(2)
         }
         const int sa = cur->item.tiles[warp][0], sb = cur->item.tiles[warp][1];
         const bool has_tile = sa != 0xFF;
         const bool diag = sa == sb;
-        const uint32_t tile_mask = diag ? 0x8CEFu : 0xFFFFu;   // diagonal tile: fragments i <= j only (bit 4i+j)
         double acc[4][4][2];
 #pragma unroll
         for (int i = 0; i < 4; i++)
@@ -369,7 +465,10 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
             todo &= todo - 1;
             const uint32_t slot_r = n % (uint32_t)nring, ph = (n / (uint32_t)nring) & 1u;
             n++;
+            TIMER_START
             mbar_wait(smem_u32(s_full + slot_r), ph);
+            TIMER_ADD(3)
+            TIMER_START
             if (has_tile) {
                 const uint32_t ma = *reinterpret_cast<const uint32_t*>(&cur->gmask[sa][s * kStageKsteps]);
                 const uint32_t mb = *reinterpret_cast<const uint32_t*>(&cur->gmask[sb][s * kStageKsteps]);
@@ -382,11 +481,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                 for (int kp = 0; kp < 2; kp++) {
                     const uint32_t ra0 = (ma >> (16 * kp)) & 0xFu, ra1 = (ma >> (16 * kp + 8)) & 0xFu;
                     const uint32_t ca0 = (mb >> (16 * kp)) & 0xFu, ca1 = (mb >> (16 * kp + 8)) & 0xFu;
-                    // pair mask: bit 4i+j <=> row fragment i and column fragment j both active
-                    const uint32_t sp0 = (ra0 & 1u) | ((ra0 & 2u) << 3) | ((ra0 & 4u) << 6) | ((ra0 & 8u) << 9);
-                    const uint32_t sp1 = (ra1 & 1u) | ((ra1 & 2u) << 3) | ((ra1 & 4u) << 6) | ((ra1 & 8u) << 9);
-                    const uint32_t pm0 = (ca0 * sp0) & tile_mask, pm1 = (ca1 * sp1) & tile_mask;
-                    if ((pm0 | pm1) == 0u) continue;
+                    if (((ra0 && ca0) || (ra1 && ca1)) == false) continue;
                     const uint32_t rows = ra0 | ra1, cols = ca0 | ca1;
                     double2 a[4], b[4];
 #pragma unroll
@@ -402,40 +497,41 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                         b[j].x = __hiloint2double(__double2hiint(b[j].x) ^ x0, __double2loint(b[j].x));
                         b[j].y = __hiloint2double(__double2hiint(b[j].y) ^ x1, __double2loint(b[j].y));
                     }
-                    if (pm0 == tile_mask && pm1 == tile_mask && !diag) {
+                    if (!diag) {
+                        if ((ra0 & ca0 & ra1 & ca1) == 0xFu) {
 #pragma unroll
-                        for (int i = 0; i < 4; i++)
+                            for (int i = 0; i < 4; i++)
 #pragma unroll
-                            for (int j = 0; j < 4; j++) {
-                                dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
-                                dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
-                            }
+                                for (int j = 0; j < 4; j++) {
+                                    dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
+                                    dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
+                                }
+                        } else {
+                            kstep_rect(acc, ra0, ca0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
+                            kstep_rect(acc, ra1, ca1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
+                        }
                     } else {
-#pragma unroll
-                        for (int i = 0; i < 4; i++)
-#pragma unroll
-                            for (int j = 0; j < 4; j++) {
-                                if (pm0 & (1u << (4 * i + j))) dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
-                                if (pm1 & (1u << (4 * i + j))) dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
-                            }
+                        kstep_diag(acc, ra0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
+                        kstep_diag(acc, ra1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
                     }
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(s_empty + slot_r));
+            TIMER_ADD(4)
         }
         nstage_done = n;
+        TIMER_START
 
         // ---------------- flush: add the tile into the canonical H blocks ---------------------------
         if (has_tile) {
             const int ga = cur->item.slot_group[sa], gb = cur->item.slot_group[sb];
-            const uint32_t* rinfo = P.rowinfo + cur->region.rowinfo_off;
             const uint32_t* pair = P.pair + cur->region.pair_off;
             const int m = cur->region.nentry;
 #pragma unroll
             for (int i = 0; i < 4; i++) {
                 const int row = ga * kGroupRows + 8 * i + frow;
-                const uint32_t ri = __ldg(rinfo + row);
+                const uint32_t ri = cur->rinfo[sa][8 * i + frow];
                 if (ri == kNoBlock) continue;
                 const int ea = ri & 0xFFF, mu = (ri >> 12) & 0xFF, nI = ri >> 20;
 #pragma unroll
@@ -447,7 +543,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                         if (v == 0.0) continue;
                         const int col = gb * kGroupRows + 8 * j + 2 * fk + h;
                         if (row > col) continue;
-                        const uint32_t ci = __ldg(rinfo + col);
+                        const uint32_t ci = cur->rinfo[sb][8 * j + 2 * fk + h];
                         if (ci == kNoBlock) continue;
                         const int eb = ci & 0xFFF, nu = (ci >> 12) & 0xFF, nJ = ci >> 20;
                         const uint32_t pr = __ldg(pair + ea * m + eb);
@@ -458,7 +554,15 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                 }
             }
         }
+        TIMER_ADD(5)
+        TIMER_COUNT(6)
     }
+#ifdef GINT_TIMING
+    if (lane == 0 && (warp == 0 || warp == 5 || warp == kConsumerWarps)) {
+        long long* out = reinterpret_cast<long long*>(P.ready + P.nregions + 1) + 24 * blockIdx.x + (warp == 0 ? 0 : (warp == 5 ? 8 : 16));
+        for (int k = 0; k < 8; k++) out[k] = tm_[k];
+    }
+#endif
 }
 
 // H(J,I,-R) = H(I,J,R)^T for every non-canonical block; lower <- upper for (I,I,0).

@@ -375,6 +375,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     struct RegionItems { int region; double cost; std::vector<WorkItem> items; };
     std::vector<RegionItems> region_items;
     double exec_dmma = 0, flush_elems = 0, n_etask = 0, max_rows = 0, chunk_loads = 0;
+    double ks_full = 0, ks_part = 0, dmma_part = 0, stage_visits = 0;
     const int nks_pad = P.nks_pad, nslice = P.nslice, nstage = P.nstage;
     size_t pos = 0;
     while (pos < tmp.size()) {
@@ -547,10 +548,22 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 w.tiles[warp][0] = (uint8_t)slot_of(p.tiles[t].first);
                 w.tiles[warp][1] = (uint8_t)slot_of(p.tiles[t].second);
                 exec_dmma += tc;
+                for (int ks = 0; ks < nks_pad; ks++) {
+                    const int gi = p.tiles[t].first, gj = p.tiles[t].second;
+                    const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
+                    int nd = 0;
+                    if (gi != gj) nd = __builtin_popcount(ra) * __builtin_popcount(ca);
+                    else
+                        for (int i = 0; i < 4; i++)
+                            if ((ra >> i) & 1u) nd += __builtin_popcount(ca >> i);
+                    if (gi != gj && nd == 16) ks_full += 1;
+                    else if (nd > 0) { ks_part += 1; dmma_part += nd; }
+                }
                 for (int st = 0; st < nstage; st++)
                     if (tile_stage_cost(p.tiles[t].first, p.tiles[t].second, st) > 0) w.stage_mask |= 1u << st;
             }
             ri.cost += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
+            stage_visits += __builtin_popcount(w.stage_mask);
             flush_elems += 1024.0 * (double)p.tiles.size();
             for (int st = 0; st < nstage; st++)
                 if ((w.stage_mask >> st) & 1u)
@@ -600,6 +613,10 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[13] = chunk_loads * kChunkBytes;
     P.stats[14] = (double)P.nring;
     P.stats[15] = (double)P.regions.size();
+    P.stats[16] = ks_full;
+    P.stats[17] = ks_part;
+    P.stats[18] = dmma_part;
+    P.stats[19] = stage_visits;
     return GINT_OK;
 }
 

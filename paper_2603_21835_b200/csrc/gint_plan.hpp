@@ -159,7 +159,7 @@ struct Plan {
     std::vector<int32_t> sp_meta;               // per species: tab_offset, ntab, nradp, norb, l[0..7] (12 ints)
     std::vector<double> sp_real;                // per species: rcut^2, 1/dr
     // statistics
-    double stats[16] = {0};
+    double stats[24] = {0};
     size_t smem_bytes = 0;
     bool tables_in_smem = true;
     int nring = 0;                              // pipeline stages of the psi ring in shared memory
@@ -174,16 +174,17 @@ struct ItemDesc {
     Region region;                                  // 64
     uint8_t gmask[kMaxSlots][kMaxKsteps];           // 1024: fragment activity nibbles of the item's slots
     uint32_t sign[kMaxRegionPoints / 32];           // 64: bit p = sign bit of V dV at point slot p
+    uint8_t act[kMaxStages];                        // 32: bit q = slot q has an active k-step in the stage
+    uint32_t rinfo[kMaxSlots][kGroupRows];          // 1024: row info words of the item's slots (flush)
     int32_t valid;                                  // 0 = queue exhausted
     int32_t evaluated;                              // 1 = the producer warp already evaluated and published the share
-    int32_t pad[14];
-    double sqrtw[kMaxRegionPoints];                 // 4096: sqrt(|V dV|), 0 outside the mesh
+    int32_t pad[6];
 };
 static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
 // Shared-memory carve-up of the integration kernel (bytes); used by host and device.
 struct SmemLayout {
-    uint32_t bar, desc, off, tab, ring, total;
+    uint32_t bar, desc, sqrtw, off, tab, ring, total;
 };
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
 GINT_HD inline SmemLayout smem_layout(size_t table_bytes, int nring) {
@@ -191,6 +192,7 @@ GINT_HD inline SmemLayout smem_layout(size_t table_bytes, int nring) {
     uint32_t o = 0;
     L.bar = o;   o += 256;                                           // mbarriers: full[8], empty[8]; misc words
     L.desc = o;  o += smem_align((size_t)kDescSlots * sizeof(ItemDesc));
+    L.sqrtw = o; o += smem_align((size_t)2 * kMaxRegionPoints * sizeof(double));   // sqrt(|V dV|), two items in flight
     L.off = o;   o += smem_align((size_t)3 * kMaxRegionPoints * sizeof(double));
     L.tab = o;   o += smem_align(table_bytes);
     L.ring = o;  o += (uint32_t)nring * kMaxSlots * kChunkBytes;
