@@ -101,8 +101,10 @@ int gint_get_blocks(const gint_ctx *ctx, int32_t *iat, int32_t *jat, int32_t *R,
  *   V_dev   device pointer, [N1][N2][N3] doubles, third index fastest; read only
  *   H_dev   device pointer, h_len doubles; OVERWRITTEN (not accumulated into)
  *   stream  cudaStream_t (as void*), NULL = legacy default stream
- * Asynchronous: enqueues a memset, the integration kernel and the mirror kernel
- * on `stream`; no host synchronisation, no allocation, no host<->device copy.
+ * Asynchronous: enqueues two memsets, the psi kernel, the contraction kernel and the
+ * mirror kernel on `stream`; no host synchronisation, no allocation, no host<->device
+ * copy.  The context owns a device scratch buffer for psi (stats[12] bytes; 8.5 GB for
+ * the 512-atom Si-like workload).
  * With nranks > 1 H holds this rank's partial sum (sum over ranks = full H).
  * Kernel faults surface at the caller's next synchronisation. */
 int gint_vlocal(gint_ctx *ctx, const double *V_dev, double *H_dev, void *stream);
@@ -112,12 +114,13 @@ int gint_vlocal(gint_ctx *ctx, const double *V_dev, double *H_dev, void *stream)
 int gint_vlocal_host(gint_ctx *ctx, const double *V_host, double *H_host);
 
 /* Per-kernel timing on the launch stream.  After gint_set_profiling(ctx, 1) every
- * gint_vlocal call records CUDA events around its integration kernel and its mirror
- * kernel on `stream`; gint_get_kernel_ms synchronises on the last call's events and
- * returns their durations in milliseconds (ms[0] integration, ms[1] mirror, ms[2] whole
- * call incl. the memsets).  Used by bench.py for the roofline's per-launch duration. */
+ * gint_vlocal call records CUDA events around its kernels on `stream`;
+ * gint_get_kernel_ms synchronises on the last call's events and returns durations in
+ * milliseconds: ms[0] contraction kernel, ms[1] mirror kernel, ms[2] whole call incl. the
+ * memsets, ms[3] psi (orbital evaluation) kernel.  Used by bench.py for the roofline's
+ * per-launch duration. */
 int gint_set_profiling(gint_ctx *ctx, int32_t on);
-int gint_get_kernel_ms(gint_ctx *ctx, double *ms /* [3] */);
+int gint_get_kernel_ms(gint_ctx *ctx, double *ms /* [4] */);
 
 /* Statistics of the setup (all host-side, valid for host-only contexts too).
  * stats[0] big cells (regions) total, empty ones included      stats[1] work items

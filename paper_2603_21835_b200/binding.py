@@ -23,7 +23,7 @@ EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
-              "regions", "ksteps_full", "ksteps_partial", "dmma_in_partial_ksteps", "stage_visits", "s20", "s21", "s22", "s23")
+              "regions", "ksteps_full", "ksteps_partial", "dmma_in_partial_ksteps", "stage_visits", "dmma_max_sched_item", "dmma_max_sched_stage", "dmma_max_warp_stage", "s23")
 
 
 class GintError(RuntimeError):
@@ -124,10 +124,10 @@ class GintContext:
         _check(_lib.gint_set_profiling(self._h, 1 if on else 0), "gint_set_profiling")
 
     def gint_get_kernel_ms(self):
-        """(integration kernel ms, mirror kernel ms, whole call ms) of the last gint_vlocal call."""
-        ms = np.zeros(3, dtype=np.float64)
+        """(contraction kernel ms, mirror kernel ms, whole call ms, psi kernel ms) of the last gint_vlocal call."""
+        ms = np.zeros(4, dtype=np.float64)
         _check(_lib.gint_get_kernel_ms(self._h, _ptr(ms, ctypes.c_double)), "gint_get_kernel_ms")
-        return float(ms[0]), float(ms[1]), float(ms[2])
+        return float(ms[0]), float(ms[1]), float(ms[2]), float(ms[3])
 
     def gint_get_cell_lists(self):
         nc, ne = ctypes.c_int64(), ctypes.c_int64()

@@ -2,6 +2,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -18,9 +19,10 @@ struct gint_ctx {
     int device = -1;
     int nsm = 0;
     std::vector<void*> allocs;
+    size_t psi_smem = 0, contract_smem = 0;
     bool profiling = false;
     bool have_events = false;
-    cudaEvent_t ev[4];
+    cudaEvent_t ev[5];
     double* V_scratch = nullptr;   // gint_vlocal_host only
     double* H_scratch = nullptr;
 };
@@ -54,17 +56,17 @@ void release(gint_ctx* ctx) {
     if (ctx->device >= 0) {
         cudaSetDevice(ctx->device);
 #ifdef GINT_TIMING
-        if (ctx->dev.ready) {
+        if (ctx->dev.counter) {
             std::vector<long long> tm(24 * 256);
             cudaDeviceSynchronize();
-            cudaMemcpy(tm.data(), ctx->dev.ready + ctx->dev.nregions + 1, tm.size() * 8, cudaMemcpyDeviceToHost);
-            const char* names[3] = {"consumer w0: topbar eval pub fullwait contract flush items -", "consumer w5: topbar eval pub fullwait contract flush items -",
-                                    "producer   : topbar emptywait poll nslow - - - -"};
+            cudaMemcpy(tm.data(), ctx->dev.counter + 16, tm.size() * 8, cudaMemcpyDeviceToHost);
+            const char* names[3] = {"consumer w0: descwait - - fullwait contract flush items -", "consumer w5: descwait - - fullwait contract flush items -",
+                                    "producer   : - emptywait prepare - - - items -"};
             for (int r = 0; r < 3; r++) {
                 fprintf(stderr, "[timing] %s\n", names[r]);
                 for (int b : {0, 1, 73, 147}) {
                     fprintf(stderr, "   cta %3d:", b);
-                    for (int k = 0; k < 8; k++) fprintf(stderr, " %10.3f", (k == 6 || (r == 2 && k == 3)) ? (double)tm[24 * b + 8 * r + k] : tm[24 * b + 8 * r + k] / 1.965e6);
+                    for (int k = 0; k < 8; k++) fprintf(stderr, " %10.3f", (k == 6) ? (double)tm[24 * b + 8 * r + k] : tm[24 * b + 8 * r + k] / 1.965e6);
                     fprintf(stderr, "\n");
                 }
             }
@@ -72,7 +74,7 @@ void release(gint_ctx* ctx) {
 #endif
         for (void* p : ctx->allocs) cudaFree(p);
         if (ctx->have_events)
-            for (int i = 0; i < 4; i++) cudaEventDestroy(ctx->ev[i]);
+            for (int i = 0; i < 5; i++) cudaEventDestroy(ctx->ev[i]);
         if (ctx->V_scratch) cudaFree(ctx->V_scratch);
         if (ctx->H_scratch) cudaFree(ctx->H_scratch);
     }
@@ -153,11 +155,21 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     UP(P.sp_meta, &D.sp_meta)
     UP(P.sp_real, &D.sp_real)
 #undef UP
-    void* ctr = nullptr;   // queue head + one share counter per region
-    if ((e = cudaMalloc(&ctr, sizeof(unsigned int) * (P.regions.size() + 2) + 64 + 24 * 8 * 256)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counters"); }
+    void* ctr = nullptr;   // queue head (+ development timing area)
+    if ((e = cudaMalloc(&ctr, 64 + 24 * 8 * 256)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
-    D.ready = D.counter + 1;
+    void* sgn = nullptr;
+    if ((e = cudaMalloc(&sgn, sizeof(uint32_t) * 16 * (P.regions.size() + 1))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc sign"); }
+    ctx->allocs.push_back(sgn);
+    D.sign = reinterpret_cast<uint32_t*>(sgn);
+    {
+        std::vector<int32_t> work;
+        for (size_t r = 0; r < P.regions.size(); r++)
+            if (P.regions[r].nitem > 0) work.push_back((int32_t)r);
+        D.nwork_regions = (int32_t)work.size();
+        if ((e = upload(ctx, work, &D.work_regions)) != cudaSuccess) { release(ctx); return fail_cuda(e, "upload work_regions"); }
+    }
     // psi scratch: zero-filled once; rows and slices that no evaluation task writes stay zero for good
     void* psi = nullptr;
     const size_t psi_bytes = (size_t)P.psi_chunks * gint::kChunkBytes;
@@ -174,10 +186,16 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     D.nregions = (int32_t)P.regions.size();
     D.nring = P.nring;
     D.never = 0;
+    D.debug = 0;
+#ifdef GINT_TIMING
+    if (const char* dbg = getenv("GINT_DEBUG")) D.debug = atoi(dbg);
+#endif
     D.nitems = (int32_t)P.items.size();
     D.nmirror = (int32_t)P.mirror.size();
     D.tab_doubles = (int32_t)P.tab_packed.size();
-    if ((e = gint::configure_kernels(P.smem_bytes, P.tables_in_smem)) != cudaSuccess) {
+    ctx->psi_smem = gint::psi_kernel_smem(P.tables_in_smem ? P.tab_packed.size() * sizeof(double) : 0);
+    ctx->contract_smem = gint::contract_kernel_smem(P.nring);
+    if ((e = gint::configure_kernels(ctx->psi_smem, ctx->contract_smem, P.tables_in_smem)) != cudaSuccess) {
         release(ctx);
         return fail_cuda(e, "cudaFuncSetAttribute");
     }
@@ -206,7 +224,7 @@ int gint_get_blocks(const gint_ctx* ctx, int32_t* iat, int32_t* jat, int32_t* R,
 int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream) {
     if (!ctx || !V_dev || !H_dev) return fail(GINT_EINVAL, "null argument");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
-    cudaError_t e = gint::launch_vlocal(ctx->dev, ctx->plan.smem_bytes, ctx->plan.tables_in_smem, ctx->nsm,
+    cudaError_t e = gint::launch_vlocal(ctx->dev, ctx->psi_smem, ctx->contract_smem, ctx->plan.tables_in_smem, ctx->nsm,
                                         (size_t)ctx->plan.blk_off.back(), V_dev, H_dev,
                                         reinterpret_cast<cudaStream_t>(stream), ctx->profiling ? ctx->ev : nullptr);
     if (e != cudaSuccess) return fail_cuda(e, "gint_vlocal launch");
@@ -239,7 +257,7 @@ int gint_set_profiling(gint_ctx* ctx, int32_t on) {
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
     if (on && !ctx->have_events) {
         cudaSetDevice(ctx->device);
-        for (int i = 0; i < 4; i++) {
+        for (int i = 0; i < 5; i++) {
             cudaError_t e = cudaEventCreate(&ctx->ev[i]);
             if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
         }
@@ -252,15 +270,17 @@ int gint_set_profiling(gint_ctx* ctx, int32_t on) {
 int gint_get_kernel_ms(gint_ctx* ctx, double* ms) {
     if (!ctx || !ms) return fail(GINT_EINVAL, "null argument");
     if (!ctx->profiling || !ctx->have_events) return fail(GINT_EINVAL, "profiling is off");
-    cudaError_t e = cudaEventSynchronize(ctx->ev[3]);
+    cudaError_t e = cudaEventSynchronize(ctx->ev[4]);
     if (e != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
-    float a = 0, b = 0, c = 0;
-    cudaEventElapsedTime(&a, ctx->ev[1], ctx->ev[2]);
-    cudaEventElapsedTime(&b, ctx->ev[2], ctx->ev[3]);
-    cudaEventElapsedTime(&c, ctx->ev[0], ctx->ev[3]);
+    float a = 0, b = 0, c = 0, d = 0;
+    cudaEventElapsedTime(&a, ctx->ev[2], ctx->ev[3]);
+    cudaEventElapsedTime(&b, ctx->ev[3], ctx->ev[4]);
+    cudaEventElapsedTime(&c, ctx->ev[0], ctx->ev[4]);
+    cudaEventElapsedTime(&d, ctx->ev[1], ctx->ev[2]);
     ms[0] = a;
     ms[1] = b;
     ms[2] = c;
+    ms[3] = d;
     return GINT_OK;
 }
 

@@ -27,21 +27,25 @@ struct DevicePlan {
     const MirrorItem* mirror;
     double* psi;              // scratch: psi_chunks x 512 doubles, zero-filled once at setup
     unsigned int* counter;    // work-queue head, reset before every launch
-    unsigned int* ready;      // per region: evaluation shares published, reset before every launch
+    uint32_t* sign;           // [nregions][16]: sign bits of V at the region's point slots (written by gint_psi_kernel)
+    const int32_t* work_regions;   // indices of the regions that own work items
     double estep[9];          // mesh step vectors a_d / N_d (rows)
     double dV;
     int32_t ngrid[3];
     int32_t nks_pad, nslice, nstage;
-    int32_t nitems, nmirror, nregions;
+    int32_t nitems, nmirror, nregions, nwork_regions;
     int32_t tab_doubles;
     int32_t nring;
+    int32_t debug;            // development builds (GINT_TIMING) only: 1 skip contraction, 2 skip evaluation, 4 skip flush
     int32_t never;            // always 0: a branch condition the compiler cannot fold (see DMMA_IF in gint_kernels.cu)
 };
 
-cudaError_t configure_kernels(size_t smem_bytes, bool tab_smem);
-// ev: nullptr, or 4 events recorded at call start / before main / after main / after mirror
-cudaError_t launch_vlocal(const DevicePlan& P, size_t smem_bytes, bool tab_smem, int nsm, size_t h_len,
-                          const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev);
+size_t psi_kernel_smem(size_t table_bytes);
+size_t contract_kernel_smem(int nring);
+cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool tab_smem);
+// ev: nullptr, or 5 events recorded at call start / before psi / before contraction / after it / after mirror
+cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
+                          size_t h_len, const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev);
 cudaError_t measure_dmma_peak(double seconds, int nsm, double* tflops);
 
 }  // namespace gint

@@ -2,28 +2,26 @@
 //
 //   H_mu,nu(R) = sum_g phi_mu(r_g - tau_I) V(r_g) phi_nu(r_g - tau_J - R) dV   (Eq. 45)
 //
-// Output-stationary design.  One persistent CTA per SM pulls work items from a global
-// queue.  A work item is a set of up to 15 32x32 tiles (one per consumer warp) of the
-// upper triangle of one region's  C = psi diag(sign V) psi^T,  psi = phi sqrt(|V dV|)
-// (the paper's per-BigGrid dense contraction, with the V dV weighting
-// of Eq. 45 folded into the operand).  The items of a region sit next to each other in
-// the queue and share its psi through the L2 cache:
+// Two kernels per call, both behind gint_vlocal (plus a tiny mirror kernel):
 //
-//   phase 1 (evaluate)  the CTA that takes item q of n evaluates share q of the region's
-//       (atom image, 32-point slice) tasks -- Eq. 1: 4-point Lagrange radial table x real
-//       Y_lm, one lane per mesh point -- and stores psi to a global scratch buffer in DMMA
-//       fragment order, then publishes the share (release counter per region).  Phase 1 of
-//       item i+1 runs before phase 2 of item i, so sibling shares are ready when needed.
-//   phase 2 (contract)  a producer warp streams the row groups the item's tiles need back
-//       through a ring of shared-memory stages (16 points each) with cp.async.bulk +
-//       mbarrier; 15 consumer warps keep one 32x32 tile each in registers and issue
-//       mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has no FP64 kind).  (fragment,
-//       k-step) pairs that hold no in-sphere point are skipped by warp-uniform branches on
-//       host-built activity nibbles (a predicated-off DMMA still costs its 16 pipe cycles).
-//   flush   after the last stage the warp adds its tile into the canonical H blocks with
-//       red.global.add.f64 (once per item, not once per BigGrid).
-// A second kernel writes every non-canonical block as the transpose of its partner,
-// H(J,I,-R) = H(I,J,R)^T, and symmetrises the (I,I,0) blocks.
+//   gint_psi_kernel     psi = phi sqrt(|V dV|) for every (atom image, mesh point) pair listed by
+//       the plan, evaluated exactly once -- Eq. 1: 4-point Lagrange radial table x real Y_lm, one
+//       lane per mesh point -- and stored to a scratch buffer in DMMA fragment order, together
+//       with the sign bits of V per region.  The V dV weighting of Eq. 45 is thereby folded into
+//       the operand: C = psi diag(sign V) psi^T.
+//   gint_vlocal_kernel  output-stationary contraction (the paper's per-BigGrid dense contraction,
+//       PAPER.md:380, 413).  One persistent CTA per SM pulls work items from a global queue; a
+//       work item is a set of up to 15 32x32 tiles (one per consumer warp) of the upper triangle
+//       of one region's C.  A producer warp stages the item descriptor and streams the row groups
+//       the tiles need through a ring of shared-memory stages (16 points each) with
+//       cp.async.bulk + mbarrier, running ahead across item boundaries; the 15 consumer warps
+//       keep their tile in registers and issue mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has
+//       no FP64 kind).  (fragment, k-step) pairs that hold no in-sphere point are skipped by
+//       warp-uniform branches on host-built activity nibbles (a predicated-off DMMA still costs
+//       its 16 pipe cycles).  After the last stage the warp adds its tile into the canonical H
+//       blocks with red.global.add.f64 (once per item, not once per BigGrid).
+//   gint_mirror_kernel  writes every non-canonical block as the transpose of its partner,
+//       H(J,I,-R) = H(I,J,R)^T, and symmetrises the (I,I,0) blocks.
 #include <cuda_runtime.h>
 
 #include <cstdint>
@@ -140,17 +138,6 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                  : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
-__device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
-    unsigned int v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ unsigned int ld_relaxed(const unsigned int* p) {
-    unsigned int v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void bar_consumers() { asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory"); }
 
 __device__ __forceinline__ double rsqrt_seed(double x) {
     double y;
@@ -234,300 +221,299 @@ __device__ __forceinline__ void eval_task(const DevicePlan& P, const double* __r
 }
 
 }  // namespace
+// ---- kernel 1: psi = phi sqrt(|V dV|) of every region, evaluated once ---------------------------
+// One CTA per region (with work): stage sqrt(|V dV|) of the region's points and their sign bits, then
+// the warps walk the region's (atom image, 32-point slice) tasks.  Plenty of warps per SM (4 CTAs of 8
+// warps) hide the table and entry latencies; the output is 8.5 GB at si512_dzp, so the kernel runs at
+// the HBM write rate.
+constexpr int kEvalThreads = 256;
+
+struct EvalSmem {
+    uint32_t off, xyz, sqrtw, tab, total;
+};
+GINT_HD inline EvalSmem eval_smem(size_t table_bytes) {
+    EvalSmem L;
+    uint32_t o = 0;
+    L.off = o;   o += 3 * kMaxRegionPoints * 8;
+    L.xyz = o;   o += kMaxRegionPoints * 4;
+    L.sqrtw = o; o += kMaxRegionPoints * 8;
+    L.tab = o;   o += smem_align(table_bytes);
+    L.total = o;
+    return L;
+}
 
 template <bool TAB_SMEM>
-__global__ void __launch_bounds__(kThreads, 1)
-gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__ V, double* __restrict__ H) {
+__global__ void __launch_bounds__(kEvalThreads, 3)
+gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__ V) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const SmemLayout L = smem_layout(TAB_SMEM ? (size_t)P.tab_doubles * sizeof(double) : 0, P.nring);
-    uint64_t* s_full = reinterpret_cast<uint64_t*>(smem_raw + L.bar);         // [8]
-    uint64_t* s_empty = s_full + 8;                                           // [8]
-    ItemDesc* s_desc = reinterpret_cast<ItemDesc*>(smem_raw + L.desc);        // [3]
-    double* s_sqrtw = reinterpret_cast<double*>(smem_raw + L.sqrtw);          // [2][512] sqrt(|V dV|) of a region's points
-    double* s_off = reinterpret_cast<double*>(smem_raw + L.off);              // [3][512] Cartesian offset of a point slot
+    const EvalSmem L = eval_smem(TAB_SMEM ? (size_t)P.tab_doubles * sizeof(double) : 0);
+    double* s_off = reinterpret_cast<double*>(smem_raw + L.off);
+    uchar4* s_xyz = reinterpret_cast<uchar4*>(smem_raw + L.xyz);
+    double* s_sqrtw = reinterpret_cast<double*>(smem_raw + L.sqrtw);
     double* s_tab = reinterpret_cast<double*>(smem_raw + L.tab);
+    if (TAB_SMEM) {
+        for (int i = tid; i < P.tab_doubles; i += kEvalThreads) s_tab[i] = __ldg(P.tab + i);
+    }
+    const double* tab = TAB_SMEM ? s_tab : P.tab;
+    const int npt = P.nslice * kSlicePts;
+    for (int p = tid; p < npt; p += kEvalThreads) {
+        const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
+        for (int k = 0; k < 3; k++)
+            s_off[k * kMaxRegionPoints + p] = c.x * P.estep[k] + c.y * P.estep[3 + k] + c.z * P.estep[6 + k];
+        s_xyz[p] = c;
+    }
+    for (int r = blockIdx.x; r < P.nwork_regions; r += gridDim.x) {
+        __syncthreads();   // previous region's sqrtw no longer read (first pass: tables and offsets staged)
+        const int reg_index = __ldg(P.work_regions + r);
+        const Region* reg = P.regions + reg_index;
+        const int ox = __ldg(&reg->origin[0]), oy = __ldg(&reg->origin[1]), oz = __ldg(&reg->origin[2]);
+        for (int p = tid; p < npt; p += kEvalThreads) {   // npt is a multiple of 32: whole warps
+            const uchar4 c = s_xyz[p];
+            const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
+            double wv = 0.0;
+            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
+                wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
+            s_sqrtw[p] = sqrt(fabs(wv));
+            const unsigned int neg = __ballot_sync(0xffffffffu, wv < 0.0);
+            if (lane == 0) P.sign[(size_t)reg_index * (kMaxRegionPoints / 32) + (p >> 5)] = neg;
+        }
+        __syncthreads();
+        const int ntask = __ldg(&reg->ntask);
+        const uint32_t* tasks = P.etasks + __ldg(&reg->task_off);
+        const Entry* entries = P.entries + __ldg(&reg->entry0);
+        double* psi_region = P.psi + (size_t)__ldg(&reg->psi_chunk0) * kChunkDoubles;
+        for (int t = warp; t < ntask; t += kEvalThreads / 32) {
+            const uint32_t tk = __ldg(tasks + t);
+            const int slice = (int)(tk >> 16);
+            eval_task(P, tab, entries + (tk & 0xFFFFu), slice, lane, s_off, s_sqrtw,
+                      psi_region + (size_t)(2 * slice) * kChunkDoubles);
+        }
+    }
+}
+
+// ---- kernel 2: contraction -------------------------------------------------------------------
+struct ContractSmem {
+    uint32_t bar, desc, ring, total;
+};
+GINT_HD inline ContractSmem contract_smem(int nring) {
+    ContractSmem L;
+    uint32_t o = 0;
+    L.bar = o;   o += 256;   // mbarriers: full[8], empty[8], desc_full[4], desc_empty[4]
+    L.desc = o;  o += smem_align((size_t)kDescSlots * sizeof(ItemDesc));
+    L.ring = o;  o += (uint32_t)nring * kStageBytes;
+    L.total = o;
+    return L;
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const ContractSmem L = contract_smem(P.nring);
+    uint64_t* s_full = reinterpret_cast<uint64_t*>(smem_raw + L.bar);         // [8] stage filled (tx bytes)
+    uint64_t* s_empty = s_full + 8;                                           // [8] stage released by the 15 consumer warps
+    uint64_t* s_dfull = s_full + 16;                                          // [4] descriptor staged
+    uint64_t* s_dempty = s_full + 20;                                         // [4] descriptor released
+    ItemDesc* s_desc = reinterpret_cast<ItemDesc*>(smem_raw + L.desc);        // [3]
     unsigned char* s_ring = smem_raw + L.ring;                                // [nring][slot][4 KB]
     const int nring = P.nring;
     const int never = P.never;   // always 0; see DMMA_IF
 
-    if (TAB_SMEM) {
-        for (int i = tid; i < P.tab_doubles; i += kThreads) s_tab[i] = __ldg(P.tab + i);
-    }
-    const double* tab = TAB_SMEM ? s_tab : P.tab;
-    for (int p = tid; p < P.nslice * kSlicePts; p += kThreads) {
-        const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
-        for (int k = 0; k < 3; k++)
-            s_off[k * kMaxRegionPoints + p] = c.x * P.estep[k] + c.y * P.estep[3 + k] + c.z * P.estep[6 + k];
-    }
     if (tid == 0) {
         for (int i = 0; i < nring; i++) {
             mbar_init(smem_u32(s_full + i), 1);
             mbar_init(smem_u32(s_empty + i), kConsumerWarps);
         }
+        for (int i = 0; i < kDescSlots; i++) {
+            mbar_init(smem_u32(s_dfull + i), 1);
+            mbar_init(smem_u32(s_dempty + i), kConsumerWarps);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     fence_proxy_async();
-
-    // ---- producer warp: take the next item from the queue and stage its descriptor ---------------
-    auto prepare = [&](ItemDesc* d, double* sqrtw) {
-        unsigned int it = 0;
-        if (lane == 0) it = atomicAdd(P.counter, 1u);
-        it = __shfl_sync(0xffffffffu, it, 0);
-        if (it >= (unsigned int)P.nitems) {
-            if (lane == 0) d->valid = 0;
-            __syncwarp();
-            return;
-        }
-        if (lane < (int)(sizeof(WorkItem) / 4))
-            reinterpret_cast<uint32_t*>(&d->item)[lane] = __ldg(reinterpret_cast<const uint32_t*>(P.items + it) + lane);
-        __syncwarp();
-        const Region* greg = P.regions + d->item.region;
-        if (lane < (int)(sizeof(Region) / 4))
-            reinterpret_cast<uint32_t*>(&d->region)[lane] = __ldg(reinterpret_cast<const uint32_t*>(greg) + lane);
-        __syncwarp();
-        const int wpr = P.nks_pad >> 2;   // 32-bit words per group row of activity bytes
-        const int nslot = d->item.nslot;
-        for (int i = lane; i < nslot * wpr; i += 32) {
-            const int slot = i / wpr, wd = i - slot * wpr;
-            reinterpret_cast<uint32_t*>(d->gmask[slot])[wd] = __ldg(
-                reinterpret_cast<const uint32_t*>(P.gmask + d->region.gmask_off + (int)d->item.slot_group[slot] * P.nks_pad) + wd);
-        }
-        for (int i = lane; i < nslot * kGroupRows; i += 32)
-            d->rinfo[i >> 5][i & 31] = __ldg(P.rowinfo + d->region.rowinfo_off + (int)d->item.slot_group[i >> 5] * kGroupRows + (i & 31));
-        __syncwarp();
-        {   // stage lane: which slots hold an active k-step there
-            uint32_t a = 0;
-            for (int q = 0; q < nslot; q++)
-                if (lane < P.nstage && *reinterpret_cast<const uint32_t*>(&d->gmask[q][lane * kStageKsteps])) a |= 1u << q;
-            d->act[lane] = (uint8_t)a;
-        }
-        const int ox = d->region.origin[0], oy = d->region.origin[1], oz = d->region.origin[2];
-        for (int p = lane; p < P.nslice * kSlicePts; p += 32) {   // w = V dV of the region's points (0 outside the mesh)
-            const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[p];
-            const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
-            double wv = 0.0;
-            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
-                wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
-            sqrtw[p] = sqrt(fabs(wv));
-            const unsigned int neg = __ballot_sync(0xffffffffu, wv < 0.0);
-            if (lane == 0) d->sign[p >> 5] = neg;
-        }
-        if (lane == 0) {
-            d->valid = 1;
-            d->evaluated = 0;
-        }
-        __syncwarp();
-    };
-
-    // ---- consumers: phase 1, evaluate this item's share of its region's psi ----------------------
-    auto evaluate = [&](const ItemDesc* d, const double* sqrtw, int w, int nw) {
-        const int ntask = d->region.ntask, nshare = d->region.nitem, share = d->item.share;
-        const uint32_t* tasks = P.etasks + d->region.task_off;
-        const Entry* entries = P.entries + d->region.entry0;
-        double* psi_region = P.psi + (size_t)d->region.psi_chunk0 * kChunkDoubles;
-        for (int t = share + nshare * w; t < ntask; t += nshare * nw) {
-            const uint32_t tk = __ldg(tasks + t);
-            const int slice = (int)(tk >> 16);
-            eval_task(P, tab, entries + (tk & 0xFFFFu), slice, lane, s_off, sqrtw,
-                      psi_region + (size_t)(2 * slice) * kChunkDoubles);
-        }
-    };
-    auto publish = [&](const ItemDesc* d) {   // after bar_consumers(): every consumer's stores precede the fence
-        __threadfence();
-        fence_proxy_async();
-        atomicAdd(P.ready + d->item.region, 1u);
-    };
-
     __syncthreads();
-    if (warp == kConsumerWarps) {
-        prepare(&s_desc[0], s_sqrtw);
-        prepare(&s_desc[1], s_sqrtw + kMaxRegionPoints);
-    }
-    __syncthreads();
-    if (warp < kConsumerWarps && s_desc[0].valid) {
-        evaluate(&s_desc[0], s_sqrtw, warp, kConsumerWarps);
-        bar_consumers();
-        if (tid == 0) publish(&s_desc[0]);
-    }
-
     TIMER_DECL
-    uint32_t nstage_done = 0;   // stages streamed so far (same count in every warp): ring slot and phase parity
-    const int frow = lane >> 2, fk = lane & 3;
-    for (int iter = 0;; iter++) {
-        TIMER_START
-        __syncthreads();   // previous item finished by all warps: its descriptor slot and the ring are free
-        TIMER_ADD(0)
-        const ItemDesc* cur = &s_desc[iter % kDescSlots];
-        if (!cur->valid) break;
-        const ItemDesc* nxt = &s_desc[(iter + 1) % kDescSlots];
-        const uint32_t stage_mask = cur->item.stage_mask;
 
-        if (warp == kConsumerWarps) {
-            // ================= producer warp =================
+    if (warp == kConsumerWarps) {
+        // ================= producer warp =================
+        // take the next item from the queue and stage its descriptor
+        auto prepare = [&](ItemDesc* d) {
+            unsigned int it = 0;
+            if (lane == 0) it = atomicAdd(P.counter, 1u);
+            it = __shfl_sync(0xffffffffu, it, 0);
+            if (it >= (unsigned int)P.nitems) {
+                if (lane == 0) d->valid = 0;
+                __syncwarp();
+                return;
+            }
+            reinterpret_cast<uint32_t*>(&d->item)[lane] = __ldg(reinterpret_cast<const uint32_t*>(P.items + it) + lane);   // 128 B
+            __syncwarp();
+            const int wpr = P.nks_pad >> 2;   // 32-bit words per group row of activity bytes
+            const int nslot = d->item.nslot;
+            for (int i = lane; i < nslot * wpr; i += 32) {
+                const int slot = i / wpr, wd = i - slot * wpr;
+                reinterpret_cast<uint32_t*>(d->gmask[slot])[wd] = __ldg(
+                    reinterpret_cast<const uint32_t*>(P.gmask + d->item.reg.gmask_off + (int)d->item.slot_group[slot] * P.nks_pad) + wd);
+            }
+            for (int i = lane; i < nslot * kGroupRows; i += 32)
+                d->rinfo[i >> 5][i & 31] = __ldg(P.rowinfo + d->item.reg.rowinfo_off + (int)d->item.slot_group[i >> 5] * kGroupRows + (i & 31));
+            if (lane < kMaxRegionPoints / 32) d->sign[lane] = P.sign[(size_t)d->item.region * (kMaxRegionPoints / 32) + lane];
+            __syncwarp();
+            {   // stage lane: which slots hold an active k-step there
+                uint32_t a = 0;
+                for (int q = 0; q < nslot; q++)
+                    if (lane < P.nstage && *reinterpret_cast<const uint32_t*>(&d->gmask[q][lane * kStageKsteps])) a |= 1u << q;
+                d->act[lane] = (uint8_t)a;
+            }
+            if (lane == 0) d->valid = 1;
+            __syncwarp();
+        };
+        uint32_t rs = 0, rph = 0;   // ring slot and phase of the next stage to fill
+        auto acquire_desc = [&](int i) {   // wait until the consumers released slot i % 3, stage item, publish
+            const int ds = i % kDescSlots;
+            if (lane == 0) mbar_wait(smem_u32(s_dempty + ds), (((uint32_t)i / kDescSlots) & 1u) ^ 1u);
+            __syncwarp();
+            prepare(&s_desc[ds]);
+            if (lane == 0) mbar_arrive(smem_u32(s_dfull + ds));
+            __syncwarp();
+        };
+        acquire_desc(0);
+        for (int i = 0;; i++) {
+            const ItemDesc* cur = &s_desc[i % kDescSlots];
+            if (!cur->valid) break;
+            const int nslot = cur->item.nslot;
             const unsigned char* psi_bytes = reinterpret_cast<const unsigned char*>(P.psi) +
-                                             (size_t)cur->region.psi_chunk0 * kChunkBytes;
-            const int nslot = cur->item.nslot, nst = P.nstage;
-            const unsigned int* flag = P.ready + cur->item.region;
-            const unsigned int need = (unsigned int)cur->region.nitem;
-            uint32_t todo = stage_mask, n = nstage_done;
+                                             (size_t)cur->item.reg.psi_chunk0 * kChunkBytes;
             // lane q copies the chunks of slot q; lane 0 also owns the barriers
-            const unsigned char* src_lane = psi_bytes + (size_t)(lane < nslot ? cur->item.slot_group[lane] : 0) * nst * kChunkBytes;
+            const unsigned char* src_lane = psi_bytes + (size_t)(lane < nslot ? cur->item.slot_group[lane] : 0) * P.nstage * kChunkBytes;
+            uint32_t todo = cur->item.stage_mask;
             auto issue = [&](int s) {   // whole warp
-                const uint32_t slot_r = n % (uint32_t)nring, ph = (n / (uint32_t)nring) & 1u;
                 const uint32_t act = cur->act[s];
-                const uint32_t bar = smem_u32(s_full + slot_r);
+                const uint32_t bar = smem_u32(s_full + rs);
                 if (lane == 0) {
                     TIMER_START
-                    mbar_wait(smem_u32(s_empty + slot_r), ph ^ 1u);
+                    mbar_wait(smem_u32(s_empty + rs), rph ^ 1u);
                     TIMER_ADD(1)
                     if (act) mbar_arrive_expect_tx(bar, (uint32_t)__popc(act) * kChunkBytes);
                     else mbar_arrive(bar);
                 }
                 __syncwarp();
                 if ((act >> lane) & 1u)
-                    bulk_g2s(smem_u32(s_ring + (size_t)slot_r * kStageBytes) + lane * kChunkBytes,
+                    bulk_g2s(smem_u32(s_ring + (size_t)rs * kStageBytes) + lane * kChunkBytes,
                              src_lane + (size_t)s * kChunkBytes, kChunkBytes, bar);
-                n++;
+                if (++rs == (uint32_t)nring) { rs = 0; rph ^= 1u; }
             };
-            // Common case: every share of the region is already published -> fill the ring first, then
-            // prefetch the next descriptor.  Otherwise take the next item first (it may be the missing
-            // share, and nobody else may be left to take it) and wait afterwards.
-            int ok = 0;
-            if (lane == 0) ok = ld_acquire(flag) >= need;
-            ok = __shfl_sync(0xffffffffu, ok, 0);
-            if (ok) {
-                fence_proxy_async();
-                for (int i = 0; i < nring && todo; i++) {
-                    const int s = __ffs(todo) - 1;
-                    todo &= todo - 1;
-                    issue(s);
-                }
+            for (int k = 0; k < nring && todo; k++) {
+                const int s = __ffs(todo) - 1;
+                todo &= todo - 1;
+                issue(s);
             }
-            ItemDesc* pre = &s_desc[(iter + 2) % kDescSlots];
-            if (nxt->valid) {
-                double* sqrtw_pre = s_sqrtw + (iter & 1) * kMaxRegionPoints;
-                prepare(pre, sqrtw_pre);
-                if (pre->valid && pre->item.region == cur->item.region) {
-                    // this CTA would hold an unevaluated share of the region it is about to wait for
-                    evaluate(pre, sqrtw_pre, 0, 1);
-                    __syncwarp();
-                    if (lane == 0) {
-                        publish(pre);
-                        pre->evaluated = 1;
-                    }
-                }
-            } else if (lane == 0) {
-                pre->valid = 0;
-            }
-            __syncwarp();
-            if (!ok) {
-                if (lane == 0) {
-                    TIMER_START
-                    TIMER_COUNT(3)
-                    while (ld_relaxed(flag) < need) __nanosleep(100);
-                    TIMER_ADD(2)
-                    (void)ld_acquire(flag);
-                }
-                __syncwarp();
-                fence_proxy_async();
-            }
+            TIMER_START
+            acquire_desc(i + 1);   // overlaps with the stages just issued
+            TIMER_ADD(2)
             while (todo) {
                 const int s = __ffs(todo) - 1;
                 todo &= todo - 1;
                 issue(s);
             }
-            nstage_done += __popc(stage_mask);
-            continue;
+            TIMER_COUNT(6)
         }
-
+    } else {
         // ================= consumer warps =================
-        if (nxt->valid && !nxt->evaluated) {
+        const int frow = lane >> 2, fk = lane & 3;
+        uint32_t cs = 0, cph = 0;   // ring slot and phase of the next stage to consume
+        for (int it = 0;; it++) {
+            const int ds = it % kDescSlots;
             TIMER_START
-            evaluate(nxt, s_sqrtw + ((iter + 1) & 1) * kMaxRegionPoints, warp, kConsumerWarps);
-            TIMER_ADD(1)
-            bar_consumers();
-            if (tid == 0) publish(nxt);
-            TIMER_ADD(2)
-        }
-        const int sa = cur->item.tiles[warp][0], sb = cur->item.tiles[warp][1];
-        const bool has_tile = sa != 0xFF;
-        const bool diag = sa == sb;
-        double acc[4][4][2];
+            mbar_wait(smem_u32(s_dfull + ds), ((uint32_t)it / kDescSlots) & 1u);
+            TIMER_ADD(0)
+            const ItemDesc* cur = &s_desc[ds];
+            if (!cur->valid) break;
+            const int sa = cur->item.tiles[warp][0], sb = cur->item.tiles[warp][1];
+            const bool has_tile = sa != 0xFF;
+            const bool diag = sa == sb;
+            double acc[4][4][2];
 #pragma unroll
-        for (int i = 0; i < 4; i++)
+            for (int i = 0; i < 4; i++)
 #pragma unroll
-            for (int j = 0; j < 4; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+                for (int j = 0; j < 4; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-        uint32_t todo = stage_mask, n = nstage_done;
-        while (todo) {
-            const int s = __ffs(todo) - 1;
-            todo &= todo - 1;
-            const uint32_t slot_r = n % (uint32_t)nring, ph = (n / (uint32_t)nring) & 1u;
-            n++;
-            TIMER_START
-            mbar_wait(smem_u32(s_full + slot_r), ph);
-            TIMER_ADD(3)
-            TIMER_START
-            if (has_tile) {
-                const uint32_t ma = *reinterpret_cast<const uint32_t*>(&cur->gmask[sa][s * kStageKsteps]);
-                const uint32_t mb = *reinterpret_cast<const uint32_t*>(&cur->gmask[sb][s * kStageKsteps]);
-                const unsigned char* stage = s_ring + (size_t)slot_r * kStageBytes;
-                const double2* pa = reinterpret_cast<const double2*>(stage + sa * kChunkBytes) + lane;
-                const double2* pb = reinterpret_cast<const double2*>(stage + sb * kChunkBytes) + lane;
-                // sign bits of V dV at this lane's four points (k-step ks: bit 4 ks + fk of the stage's 16)
-                const uint32_t sg = (cur->sign[s >> 1] >> ((s & 1) * 16 + fk));
+            uint32_t todo = cur->item.stage_mask;
+            while (todo) {
+                const int s = __ffs(todo) - 1;
+                todo &= todo - 1;
+                TIMER_START
+                mbar_wait(smem_u32(s_full + cs), cph);
+                TIMER_ADD(3)
+                TIMER_START
+#ifdef GINT_TIMING
+                if (has_tile && !(P.debug & 1)) {
+#else
+                if (has_tile) {
+#endif
+                    const uint32_t ma = *reinterpret_cast<const uint32_t*>(&cur->gmask[sa][s * kStageKsteps]);
+                    const uint32_t mb = *reinterpret_cast<const uint32_t*>(&cur->gmask[sb][s * kStageKsteps]);
+                    const unsigned char* stage = s_ring + (size_t)cs * kStageBytes;
+                    const double2* pa = reinterpret_cast<const double2*>(stage + sa * kChunkBytes) + lane;
+                    const double2* pb = reinterpret_cast<const double2*>(stage + sb * kChunkBytes) + lane;
+                    // sign bits of V dV at this lane's four points (k-step ks: bit 4 ks + fk of the stage's 16)
+                    const uint32_t sg = (cur->sign[s >> 1] >> ((s & 1) * 16 + fk));
 #pragma unroll
-                for (int kp = 0; kp < 2; kp++) {
-                    const uint32_t ra0 = (ma >> (16 * kp)) & 0xFu, ra1 = (ma >> (16 * kp + 8)) & 0xFu;
-                    const uint32_t ca0 = (mb >> (16 * kp)) & 0xFu, ca1 = (mb >> (16 * kp + 8)) & 0xFu;
-                    if (((ra0 && ca0) || (ra1 && ca1)) == false) continue;
-                    const uint32_t rows = ra0 | ra1, cols = ca0 | ca1;
-                    double2 a[4], b[4];
+                    for (int kp = 0; kp < 2; kp++) {
+                        const uint32_t ra0 = (ma >> (16 * kp)) & 0xFu, ra1 = (ma >> (16 * kp + 8)) & 0xFu;
+                        const uint32_t ca0 = (mb >> (16 * kp)) & 0xFu, ca1 = (mb >> (16 * kp + 8)) & 0xFu;
+                        if (((ra0 && ca0) || (ra1 && ca1)) == false) continue;
+                        const uint32_t rows = ra0 | ra1, cols = ca0 | ca1;
+                        double2 a[4], b[4];
 #pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        a[i] = make_double2(0.0, 0.0);
-                        if ((rows >> i) & 1u) a[i] = pa[(i * 2 + kp) * 32];
-                    }
-                    const uint32_t x0 = ((sg >> (8 * kp)) & 1u) << 31, x1 = ((sg >> (8 * kp + 4)) & 1u) << 31;
-#pragma unroll
-                    for (int j = 0; j < 4; j++) {
-                        b[j] = make_double2(0.0, 0.0);
-                        if ((cols >> j) & 1u) b[j] = diag ? a[j] : pb[(j * 2 + kp) * 32];
-                        b[j].x = __hiloint2double(__double2hiint(b[j].x) ^ x0, __double2loint(b[j].x));
-                        b[j].y = __hiloint2double(__double2hiint(b[j].y) ^ x1, __double2loint(b[j].y));
-                    }
-                    if (!diag) {
-                        if ((ra0 & ca0 & ra1 & ca1) == 0xFu) {
-#pragma unroll
-                            for (int i = 0; i < 4; i++)
-#pragma unroll
-                                for (int j = 0; j < 4; j++) {
-                                    dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
-                                    dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
-                                }
-                        } else {
-                            kstep_rect(acc, ra0, ca0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
-                            kstep_rect(acc, ra1, ca1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
+                        for (int i = 0; i < 4; i++) {
+                            a[i] = make_double2(0.0, 0.0);
+                            if ((rows >> i) & 1u) a[i] = pa[(i * 2 + kp) * 32];
                         }
-                    } else {
-                        kstep_diag(acc, ra0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
-                        kstep_diag(acc, ra1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
+                        const uint32_t x0 = ((sg >> (8 * kp)) & 1u) << 31, x1 = ((sg >> (8 * kp + 4)) & 1u) << 31;
+#pragma unroll
+                        for (int j = 0; j < 4; j++) {
+                            b[j] = make_double2(0.0, 0.0);
+                            if ((cols >> j) & 1u) b[j] = diag ? a[j] : pb[(j * 2 + kp) * 32];
+                            b[j].x = __hiloint2double(__double2hiint(b[j].x) ^ x0, __double2loint(b[j].x));
+                            b[j].y = __hiloint2double(__double2hiint(b[j].y) ^ x1, __double2loint(b[j].y));
+                        }
+                        if (!diag) {
+                            if ((ra0 & ca0 & ra1 & ca1) == 0xFu) {
+#pragma unroll
+                                for (int i = 0; i < 4; i++)
+#pragma unroll
+                                    for (int j = 0; j < 4; j++) {
+                                        dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
+                                        dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
+                                    }
+                            } else {
+                                kstep_rect(acc, ra0, ca0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
+                                kstep_rect(acc, ra1, ca1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
+                            }
+                        } else {
+                            kstep_diag(acc, ra0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
+                            kstep_diag(acc, ra1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
+                        }
                     }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(s_empty + cs));
+                if (++cs == (uint32_t)nring) { cs = 0; cph ^= 1u; }
+                TIMER_ADD(4)
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(s_empty + slot_r));
-            TIMER_ADD(4)
-        }
-        nstage_done = n;
-        TIMER_START
+            TIMER_START
 
         // ---------------- flush: add the tile into the canonical H blocks ---------------------------
+#ifdef GINT_TIMING
+        if (has_tile && !(P.debug & 4)) {
+#else
         if (has_tile) {
+#endif
             const int ga = cur->item.slot_group[sa], gb = cur->item.slot_group[sb];
-            const uint32_t* pair = P.pair + cur->region.pair_off;
-            const int m = cur->region.nentry;
+            const uint32_t* pair = P.pair + cur->item.reg.pair_off;
+            const int m = cur->item.reg.nentry;
 #pragma unroll
             for (int i = 0; i < 4; i++) {
                 const int row = ga * kGroupRows + 8 * i + frow;
@@ -554,12 +540,15 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, const double* __restric
                 }
             }
         }
-        TIMER_ADD(5)
-        TIMER_COUNT(6)
+            TIMER_ADD(5)
+            TIMER_COUNT(6)
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(s_dempty + ds));   // descriptor (row info, masks) no longer read
+        }
     }
 #ifdef GINT_TIMING
     if (lane == 0 && (warp == 0 || warp == 5 || warp == kConsumerWarps)) {
-        long long* out = reinterpret_cast<long long*>(P.ready + P.nregions + 1) + 24 * blockIdx.x + (warp == 0 ? 0 : (warp == 5 ? 8 : 16));
+        long long* out = reinterpret_cast<long long*>(P.counter + 16) + 24 * blockIdx.x + (warp == 0 ? 0 : (warp == 5 ? 8 : 16));
         for (int k = 0; k < 8; k++) out[k] = tm_[k];
     }
 #endif
@@ -586,37 +575,47 @@ __global__ void __launch_bounds__(256) gint_mirror_kernel(const MirrorItem* __re
 }
 
 // ---- launchers -----------------------------------------------------------------------
-cudaError_t configure_kernels(size_t smem_bytes, bool tab_smem) {
-    if (tab_smem)
-        return cudaFuncSetAttribute(gint_vlocal_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
-    return cudaFuncSetAttribute(gint_vlocal_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+size_t psi_kernel_smem(size_t table_bytes) { return eval_smem(table_bytes).total; }
+size_t contract_kernel_smem(int nring) { return contract_smem(nring).total; }
+
+cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool tab_smem) {
+    cudaError_t e = tab_smem ? cudaFuncSetAttribute(gint_psi_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psi_smem)
+                             : cudaFuncSetAttribute(gint_psi_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psi_smem);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(gint_vlocal_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)contract_smem_bytes);
 }
 
-cudaError_t launch_vlocal(const DevicePlan& P, size_t smem_bytes, bool tab_smem, int nsm, size_t h_len,
-                          const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev) {
+cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
+                          size_t h_len, const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev) {
     if (ev) cudaEventRecord(ev[0], stream);
     cudaError_t e = cudaMemsetAsync(H, 0, h_len * sizeof(double), stream);
     if (e != cudaSuccess) return e;
-    // queue head and per-region share counters live in one allocation: counter[0], ready[nregions]
-    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * (size_t)(1 + P.nregions), stream);
+    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int), stream);   // work-queue head
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[1], stream);
     if (P.nitems > 0) {
-        const int grid = P.nitems < nsm ? P.nitems : nsm;
+        const int pgrid = P.nwork_regions < 3 * nsm ? P.nwork_regions : 3 * nsm;
         if (tab_smem)
-            gint_vlocal_kernel<true><<<grid, kThreads, smem_bytes, stream>>>(P, V, H);
+            gint_psi_kernel<true><<<pgrid, kEvalThreads, psi_smem, stream>>>(P, V);
         else
-            gint_vlocal_kernel<false><<<grid, kThreads, smem_bytes, stream>>>(P, V, H);
+            gint_psi_kernel<false><<<pgrid, kEvalThreads, psi_smem, stream>>>(P, V);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[2], stream);
+    if (P.nitems > 0) {
+        const int grid = P.nitems < nsm ? P.nitems : nsm;
+        gint_vlocal_kernel<<<grid, kThreads, contract_smem_bytes, stream>>>(P, H);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    if (ev) cudaEventRecord(ev[3], stream);
     if (P.nmirror > 0) {
         const int wpb = 256 / 32;
         gint_mirror_kernel<<<(P.nmirror + wpb - 1) / wpb, 256, 0, stream>>>(P.mirror, P.nmirror, H);
         e = cudaGetLastError();
     }
-    if (ev) cudaEventRecord(ev[3], stream);
+    if (ev) cudaEventRecord(ev[4], stream);
     return e;
 }
 

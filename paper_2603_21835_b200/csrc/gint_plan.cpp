@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <array>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 
@@ -213,18 +214,9 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             P.sp_real.push_back(1.0 / sp.dr);
         }
     }
-    // shared memory: as many ring stages as fit next to the tables (3..6); tables stay in global memory
-    // (L1/L2-cached) when even three stages do not fit
-    {
-        const size_t table_bytes_all = P.tab_packed.size() * sizeof(double);
-        P.tables_in_smem = false;
-        P.nring = 0;
-        for (int nr = 6; nr >= 3 && !P.nring; nr--)
-            if (smem_layout(table_bytes_all, nr).total <= kSmemLimit) { P.nring = nr; P.tables_in_smem = true; }
-        if (!P.nring) P.nring = 6;
-        P.smem_bytes = smem_layout(P.tables_in_smem ? table_bytes_all : 0, P.nring).total;
-        if (P.smem_bytes > kSmemLimit) { err = "internal: shared-memory layout exceeds 227 KB"; return GINT_EUNSUPPORTED; }
-    }
+    P.tables_in_smem = P.tab_packed.size() * sizeof(double) <= kMaxTableSmem;
+    P.nring = kRingStages;
+    P.smem_bytes = 256 + smem_align((size_t)kDescSlots * sizeof(ItemDesc)) + (size_t)P.nring * kMaxSlots * kChunkBytes;
 
     // ---- point order inside a region: k-steps of 4 points, slices of 8 k-steps -----------------
     const int bx = P.bcell[0], by = P.bcell[1], bz = P.bcell[2];
@@ -375,7 +367,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     struct RegionItems { int region; double cost; std::vector<WorkItem> items; };
     std::vector<RegionItems> region_items;
     double exec_dmma = 0, flush_elems = 0, n_etask = 0, max_rows = 0, chunk_loads = 0;
-    double ks_full = 0, ks_part = 0, dmma_part = 0, stage_visits = 0;
+    double ks_full = 0, ks_part = 0, dmma_part = 0, stage_visits = 0, bal_item = 0, bal_stage = 0, bal_warp = 0;
     const int nks_pad = P.nks_pad, nslice = P.nslice, nstage = P.nstage;
     size_t pos = 0;
     while (pos < tmp.size()) {
@@ -563,6 +555,18 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                     if (tile_stage_cost(p.tiles[t].first, p.tiles[t].second, st) > 0) w.stage_mask |= 1u << st;
             }
             ri.cost += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
+            bal_item += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
+            for (int st = 0; st < nstage; st++) {
+                double ls[4] = {0, 0, 0, 0}, lw = 0;
+                for (int wp = 0; wp < 16; wp++) {
+                    if (w.tiles[wp][0] == 0xFF) continue;
+                    const double c = tile_stage_cost(p.groups[w.tiles[wp][0]], p.groups[w.tiles[wp][1]], st);
+                    ls[wp & 3] += c;
+                    lw = std::max(lw, c);
+                }
+                bal_stage += std::max(std::max(ls[0], ls[1]), std::max(ls[2], ls[3]));
+                bal_warp += lw;
+            }
             stage_visits += __builtin_popcount(w.stage_mask);
             flush_elems += 1024.0 * (double)p.tiles.size();
             for (int st = 0; st < nstage; st++)
@@ -590,7 +594,10 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     // queue order: heaviest regions first, the items of a region consecutive (their CTAs share its psi)
     std::stable_sort(region_items.begin(), region_items.end(), [](const RegionItems& a, const RegionItems& b) { return a.cost > b.cost; });
     for (const RegionItems& ri : region_items)
-        for (const WorkItem& w : ri.items) P.items.push_back(w);
+        for (WorkItem w : ri.items) {
+            w.reg = P.regions[(size_t)w.region];
+            P.items.push_back(w);
+        }
 
     double fpt = 0, fsym = 0;
     for (int32_t n : npoint_orb) {
@@ -604,7 +611,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[4] = 512.0 * exec_dmma;
     P.stats[5] = flush_elems;
     P.stats[6] = (double)P.smem_bytes;
-    P.stats[7] = 2;
+    P.stats[7] = 3;
     P.stats[8] = fpt;
     P.stats[9] = fsym;
     P.stats[10] = n_insphere;
@@ -617,6 +624,9 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[17] = ks_part;
     P.stats[18] = dmma_part;
     P.stats[19] = stage_visits;
+    P.stats[20] = bal_item;    // sum over items of the heaviest scheduler's DMMAs (perfect overlap inside an item)
+    P.stats[21] = bal_stage;   // same if the warps moved through the stages in lockstep
+    P.stats[22] = bal_warp;    // sum over (item, stage) of the heaviest single warp's DMMAs
     return GINT_OK;
 }
 

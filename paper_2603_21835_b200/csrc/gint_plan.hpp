@@ -100,7 +100,7 @@ static_assert(sizeof(Region) == 64, "Region layout is shared with the device");
 // evaluation task word: entry index within the region | slice << 16
 inline uint32_t pack_etask(int e, int slice) { return (uint32_t)e | ((uint32_t)slice << 16); }
 
-struct WorkItem {        // 64 bytes
+struct WorkItem {        // 128 bytes: 64 of its own + a copy of its region (one fetch instead of two dependent ones)
     int32_t region;
     int16_t share;       // index of the item within its region: evaluates tasks t = share (mod nitem)
     int16_t ntile;
@@ -109,8 +109,9 @@ struct WorkItem {        // 64 bytes
     uint8_t slot_group[kMaxSlots];     // region row group held by each slot
     int32_t nslot;
     int32_t pad[2];
+    Region reg;
 };
-static_assert(sizeof(WorkItem) == 64, "WorkItem layout is shared with the device");
+static_assert(sizeof(WorkItem) == 128, "WorkItem layout is shared with the device");
 
 struct MirrorItem {   // dst block (I,J,R) <- transpose of src block (J,I,-R); src == dst: symmetrise lower <- upper
     uint32_t dst, src;
@@ -166,39 +167,23 @@ struct Plan {
 };
 
 constexpr size_t kSmemLimit = 232448;   // 227 KB opt-in limit per CTA on sm_100
-constexpr int kDescSlots = 3;           // item descriptors in flight: current, next (being evaluated), prefetched
+constexpr int kDescSlots = 3;           // item descriptors in flight in the contraction kernel
 
 // Per-item descriptor staged in shared memory by the producer warp.
 struct ItemDesc {
-    WorkItem item;                                  // 64
-    Region region;                                  // 64
+    WorkItem item;                                  // 128 (item.reg = its region)
     uint8_t gmask[kMaxSlots][kMaxKsteps];           // 1024: fragment activity nibbles of the item's slots
     uint32_t sign[kMaxRegionPoints / 32];           // 64: bit p = sign bit of V dV at point slot p
     uint8_t act[kMaxStages];                        // 32: bit q = slot q has an active k-step in the stage
     uint32_t rinfo[kMaxSlots][kGroupRows];          // 1024: row info words of the item's slots (flush)
     int32_t valid;                                  // 0 = queue exhausted
-    int32_t evaluated;                              // 1 = the producer warp already evaluated and published the share
-    int32_t pad[6];
+    int32_t pad[7];
 };
 static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
-// Shared-memory carve-up of the integration kernel (bytes); used by host and device.
-struct SmemLayout {
-    uint32_t bar, desc, sqrtw, off, tab, ring, total;
-};
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
-GINT_HD inline SmemLayout smem_layout(size_t table_bytes, int nring) {
-    SmemLayout L;
-    uint32_t o = 0;
-    L.bar = o;   o += 256;                                           // mbarriers: full[8], empty[8]; misc words
-    L.desc = o;  o += smem_align((size_t)kDescSlots * sizeof(ItemDesc));
-    L.sqrtw = o; o += smem_align((size_t)2 * kMaxRegionPoints * sizeof(double));   // sqrt(|V dV|), two items in flight
-    L.off = o;   o += smem_align((size_t)3 * kMaxRegionPoints * sizeof(double));
-    L.tab = o;   o += smem_align(table_bytes);
-    L.ring = o;  o += (uint32_t)nring * kMaxSlots * kChunkBytes;
-    L.total = o;
-    return L;
-}
+constexpr int kRingStages = 6;          // 6 x 32 KB of psi in flight per SM
+constexpr size_t kMaxTableSmem = 56 * 1024;   // larger radial tables stay in global memory (L1/L2-cached)
 
 inline uint64_t pack_key(int I, int J, int r1, int r2, int r3) {
     return ((uint64_t)(uint32_t)I << 44) | ((uint64_t)(uint32_t)J << 24) | ((uint64_t)(uint32_t)(r1 + 128) << 16) |
