@@ -55,60 +55,72 @@ __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, doub
                  : "d"(a), "d"(b));
 }
 
-// DMMA under a warp-uniform condition.  A predicated-off DMMA still holds the FP64 tensor pipe for its
-// 16 cycles (measured), and ptxas if-converts a plain `if` around one into exactly that; the never-taken
-// back edge (again is always 0 at run time) makes the block a loop, which is not if-converted.
-#define DMMA_IF(cond, c0, c1, a, b, again) \
-    if (cond) {                            \
-        do {                               \
-            dmma8x8x4(c0, c1, a, b);       \
-        } while (again);                   \
-    }
-
-// One k-step of an off-diagonal tile: row fragments ra x column fragments ca (4-bit masks).  The code
-// is selected by the column pattern (a jump on a warp-uniform value), the rows are guarded one by one.
+// DMMAs under warp-uniform conditions.  A predicated-off DMMA still holds the FP64 tensor pipe for its
+// 16 cycles (measured), and ptxas if-converts a plain `if` around a few of them into exactly that; a
+// never-taken back edge (`never` is always 0 at run time) makes the guarded block a loop, which is not
+// if-converted.
+// One k-pair (two k-steps = a 2x2x2 box of mesh points) of an off-diagonal tile: row fragments ra x
+// column fragments ca (4-bit masks, OR over the two k-steps).  The code is selected by the column
+// pattern (a jump on a warp-uniform value), the rows are guarded one by one; .x / .y of an operand are
+// its values for the first / second k-step.
 #define KROW(i, body)                                  \
     if (ra & (1u << i)) {                              \
         do { body } while (never);                     \
     }
-#define KD(i, j) dmma8x8x4(acc[i][j][0], acc[i][j][1], a##i, b##j);
-#define KCASE(c, r0, r1, r2, r3) \
-    case c:                      \
-        KROW(0, r0) KROW(1, r1) KROW(2, r2) KROW(3, r3) break;
-__device__ __forceinline__ void kstep_rect(double (&acc)[4][4][2], uint32_t ra, uint32_t ca, double a0, double a1, double a2,
-                                           double a3, double b0, double b1, double b2, double b3, int never) {
+#define KX(i, j) dmma8x8x4(acc[i][j][0], acc[i][j][1], a##i.x, b##j.x);
+#define KY(i, j) dmma8x8x4(acc[i][j][0], acc[i][j][1], a##i.y, b##j.y);
+#define K1(i, p) KX(i, p) KY(i, p)
+#define K2(i, p, q) KX(i, p) KX(i, q) KY(i, p) KY(i, q)
+#define K3(i, p, q, r) KX(i, p) KX(i, q) KX(i, r) KY(i, p) KY(i, q) KY(i, r)
+#define K4(i) KX(i, 0) KX(i, 1) KX(i, 2) KX(i, 3) KY(i, 0) KY(i, 1) KY(i, 2) KY(i, 3)
+#define KCASE1(c, p) case c: KROW(0, K1(0, p)) KROW(1, K1(1, p)) KROW(2, K1(2, p)) KROW(3, K1(3, p)) break;
+#define KCASE2(c, p, q) case c: KROW(0, K2(0, p, q)) KROW(1, K2(1, p, q)) KROW(2, K2(2, p, q)) KROW(3, K2(3, p, q)) break;
+#define KCASE3(c, p, q, r) \
+    case c: KROW(0, K3(0, p, q, r)) KROW(1, K3(1, p, q, r)) KROW(2, K3(2, p, q, r)) KROW(3, K3(3, p, q, r)) break;
+__device__ __forceinline__ void kpair_rect(double (&acc)[4][4][2], uint32_t ra, uint32_t ca, double2 a0, double2 a1, double2 a2,
+                                           double2 a3, double2 b0, double2 b1, double2 b2, double2 b3, int never) {
     switch (ca) {
-        KCASE(1, KD(0, 0), KD(1, 0), KD(2, 0), KD(3, 0))
-        KCASE(2, KD(0, 1), KD(1, 1), KD(2, 1), KD(3, 1))
-        KCASE(3, KD(0, 0) KD(0, 1), KD(1, 0) KD(1, 1), KD(2, 0) KD(2, 1), KD(3, 0) KD(3, 1))
-        KCASE(4, KD(0, 2), KD(1, 2), KD(2, 2), KD(3, 2))
-        KCASE(5, KD(0, 0) KD(0, 2), KD(1, 0) KD(1, 2), KD(2, 0) KD(2, 2), KD(3, 0) KD(3, 2))
-        KCASE(6, KD(0, 1) KD(0, 2), KD(1, 1) KD(1, 2), KD(2, 1) KD(2, 2), KD(3, 1) KD(3, 2))
-        KCASE(7, KD(0, 0) KD(0, 1) KD(0, 2), KD(1, 0) KD(1, 1) KD(1, 2), KD(2, 0) KD(2, 1) KD(2, 2), KD(3, 0) KD(3, 1) KD(3, 2))
-        KCASE(8, KD(0, 3), KD(1, 3), KD(2, 3), KD(3, 3))
-        KCASE(9, KD(0, 0) KD(0, 3), KD(1, 0) KD(1, 3), KD(2, 0) KD(2, 3), KD(3, 0) KD(3, 3))
-        KCASE(10, KD(0, 1) KD(0, 3), KD(1, 1) KD(1, 3), KD(2, 1) KD(2, 3), KD(3, 1) KD(3, 3))
-        KCASE(11, KD(0, 0) KD(0, 1) KD(0, 3), KD(1, 0) KD(1, 1) KD(1, 3), KD(2, 0) KD(2, 1) KD(2, 3), KD(3, 0) KD(3, 1) KD(3, 3))
-        KCASE(12, KD(0, 2) KD(0, 3), KD(1, 2) KD(1, 3), KD(2, 2) KD(2, 3), KD(3, 2) KD(3, 3))
-        KCASE(13, KD(0, 0) KD(0, 2) KD(0, 3), KD(1, 0) KD(1, 2) KD(1, 3), KD(2, 0) KD(2, 2) KD(2, 3), KD(3, 0) KD(3, 2) KD(3, 3))
-        KCASE(14, KD(0, 1) KD(0, 2) KD(0, 3), KD(1, 1) KD(1, 2) KD(1, 3), KD(2, 1) KD(2, 2) KD(2, 3), KD(3, 1) KD(3, 2) KD(3, 3))
-        KCASE(15, KD(0, 0) KD(0, 1) KD(0, 2) KD(0, 3), KD(1, 0) KD(1, 1) KD(1, 2) KD(1, 3), KD(2, 0) KD(2, 1) KD(2, 2) KD(2, 3),
-              KD(3, 0) KD(3, 1) KD(3, 2) KD(3, 3))
+        KCASE1(1, 0)
+        KCASE1(2, 1)
+        KCASE2(3, 0, 1)
+        KCASE1(4, 2)
+        KCASE2(5, 0, 2)
+        KCASE2(6, 1, 2)
+        KCASE3(7, 0, 1, 2)
+        KCASE1(8, 3)
+        KCASE2(9, 0, 3)
+        KCASE2(10, 1, 3)
+        KCASE3(11, 0, 1, 3)
+        KCASE2(12, 2, 3)
+        KCASE3(13, 0, 2, 3)
+        KCASE3(14, 1, 2, 3)
+        case 15: KROW(0, K4(0)) KROW(1, K4(1)) KROW(2, K4(2)) KROW(3, K4(3)) break;
         default: break;
     }
 }
-// One k-step of a diagonal tile (row group == column group): fragment pairs i <= j with both active.
-__device__ __forceinline__ void kstep_diag(double (&acc)[4][4][2], uint32_t ra, double a0, double a1, double a2, double a3,
-                                           double b0, double b1, double b2, double b3, int never) {
-    KROW(0, KD(0, 0) DMMA_IF(ra & 2u, acc[0][1][0], acc[0][1][1], a0, b1, never) DMMA_IF(ra & 4u, acc[0][2][0], acc[0][2][1], a0, b2, never)
-                DMMA_IF(ra & 8u, acc[0][3][0], acc[0][3][1], a0, b3, never))
-    KROW(1, KD(1, 1) DMMA_IF(ra & 4u, acc[1][2][0], acc[1][2][1], a1, b2, never) DMMA_IF(ra & 8u, acc[1][3][0], acc[1][3][1], a1, b3, never))
-    KROW(2, KD(2, 2) DMMA_IF(ra & 8u, acc[2][3][0], acc[2][3][1], a2, b3, never))
-    KROW(3, KD(3, 3))
+// One k-pair of a diagonal tile (row group == column group): fragment pairs i <= j with both active.
+#define KXY_IF(cond, i, j) \
+    if (cond) {            \
+        do { KX(i, j) KY(i, j) } while (never); \
+    }
+__device__ __forceinline__ void kpair_diag(double (&acc)[4][4][2], uint32_t ra, double2 a0, double2 a1, double2 a2, double2 a3,
+                                           double2 b0, double2 b1, double2 b2, double2 b3, int never) {
+    KROW(0, K1(0, 0) KXY_IF(ra & 2u, 0, 1) KXY_IF(ra & 4u, 0, 2) KXY_IF(ra & 8u, 0, 3))
+    KROW(1, K1(1, 1) KXY_IF(ra & 4u, 1, 2) KXY_IF(ra & 8u, 1, 3))
+    KROW(2, K1(2, 2) KXY_IF(ra & 8u, 2, 3))
+    KROW(3, K1(3, 3))
 }
 #undef KROW
-#undef KD
-#undef KCASE
+#undef KX
+#undef KY
+#undef K1
+#undef K2
+#undef K3
+#undef K4
+#undef KCASE1
+#undef KCASE2
+#undef KCASE3
+#undef KXY_IF
 
 // ---- mbarrier / bulk-copy helpers (shared::cta addresses) --------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -459,42 +471,37 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
                     const double2* pb = reinterpret_cast<const double2*>(stage + sb * kChunkBytes) + lane;
                     // sign bits of V dV at this lane's four points (k-step ks: bit 4 ks + fk of the stage's 16)
                     const uint32_t sg = (cur->sign[s >> 1] >> ((s & 1) * 16 + fk));
-#pragma unroll
+#pragma unroll 1
                     for (int kp = 0; kp < 2; kp++) {
-                        const uint32_t ra0 = (ma >> (16 * kp)) & 0xFu, ra1 = (ma >> (16 * kp + 8)) & 0xFu;
-                        const uint32_t ca0 = (mb >> (16 * kp)) & 0xFu, ca1 = (mb >> (16 * kp + 8)) & 0xFu;
-                        if (((ra0 && ca0) || (ra1 && ca1)) == false) continue;
-                        const uint32_t rows = ra0 | ra1, cols = ca0 | ca1;
-                        double2 a[4], b[4];
-#pragma unroll
-                        for (int i = 0; i < 4; i++) {
-                            a[i] = make_double2(0.0, 0.0);
-                            if ((rows >> i) & 1u) a[i] = pa[(i * 2 + kp) * 32];
-                        }
+                        const uint32_t ra = ((ma >> (16 * kp)) | (ma >> (16 * kp + 8))) & 0xFu;
+                        const uint32_t ca = ((mb >> (16 * kp)) | (mb >> (16 * kp + 8))) & 0xFu;
+                        if (ra == 0u || ca == 0u) continue;
+                        // operands of both k-steps; fragments outside the masks may hold stale data and are not used
+                        const double2 a0 = pa[(0 * 2 + kp) * 32], a1 = pa[(1 * 2 + kp) * 32], a2 = pa[(2 * 2 + kp) * 32],
+                                      a3 = pa[(3 * 2 + kp) * 32];
+                        double2 b0 = pb[(0 * 2 + kp) * 32], b1 = pb[(1 * 2 + kp) * 32], b2 = pb[(2 * 2 + kp) * 32],
+                                b3 = pb[(3 * 2 + kp) * 32];
                         const uint32_t x0 = ((sg >> (8 * kp)) & 1u) << 31, x1 = ((sg >> (8 * kp + 4)) & 1u) << 31;
-#pragma unroll
-                        for (int j = 0; j < 4; j++) {
-                            b[j] = make_double2(0.0, 0.0);
-                            if ((cols >> j) & 1u) b[j] = diag ? a[j] : pb[(j * 2 + kp) * 32];
-                            b[j].x = __hiloint2double(__double2hiint(b[j].x) ^ x0, __double2loint(b[j].x));
-                            b[j].y = __hiloint2double(__double2hiint(b[j].y) ^ x1, __double2loint(b[j].y));
-                        }
+#define SIGN_FLIP(v)                                                                 \
+    v.x = __hiloint2double(__double2hiint(v.x) ^ x0, __double2loint(v.x)); \
+    v.y = __hiloint2double(__double2hiint(v.y) ^ x1, __double2loint(v.y));
+                        SIGN_FLIP(b0) SIGN_FLIP(b1) SIGN_FLIP(b2) SIGN_FLIP(b3)
+#undef SIGN_FLIP
                         if (!diag) {
-                            if ((ra0 & ca0 & ra1 & ca1) == 0xFu) {
-#pragma unroll
-                                for (int i = 0; i < 4; i++)
-#pragma unroll
-                                    for (int j = 0; j < 4; j++) {
-                                        dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
-                                        dmma8x8x4(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
-                                    }
+                            if ((ra & ca) == 0xFu) {
+#define FX(i, j) dmma8x8x4(acc[i][j][0], acc[i][j][1], a##i.x, b##j.x);
+#define FY(i, j) dmma8x8x4(acc[i][j][0], acc[i][j][1], a##i.y, b##j.y);
+                                FX(0, 0) FX(0, 1) FX(0, 2) FX(0, 3) FX(1, 0) FX(1, 1) FX(1, 2) FX(1, 3)
+                                FX(2, 0) FX(2, 1) FX(2, 2) FX(2, 3) FX(3, 0) FX(3, 1) FX(3, 2) FX(3, 3)
+                                FY(0, 0) FY(0, 1) FY(0, 2) FY(0, 3) FY(1, 0) FY(1, 1) FY(1, 2) FY(1, 3)
+                                FY(2, 0) FY(2, 1) FY(2, 2) FY(2, 3) FY(3, 0) FY(3, 1) FY(3, 2) FY(3, 3)
+#undef FX
+#undef FY
                             } else {
-                                kstep_rect(acc, ra0, ca0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
-                                kstep_rect(acc, ra1, ca1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
+                                kpair_rect(acc, ra, ca, a0, a1, a2, a3, b0, b1, b2, b3, never);
                             }
                         } else {
-                            kstep_diag(acc, ra0, a[0].x, a[1].x, a[2].x, a[3].x, b[0].x, b[1].x, b[2].x, b[3].x, never);
-                            kstep_diag(acc, ra1, a[0].y, a[1].y, a[2].y, a[3].y, b[0].y, b[1].y, b[2].y, b[3].y, never);
+                            kpair_diag(acc, ra, a0, a1, a2, a3, b0, b1, b2, b3, never);
                         }
                     }
                 }

@@ -445,14 +445,17 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 P.pair[(size_t)R.pair_off + (size_t)a * m + b] = off;
             }
         // tiles (group gi <= gj) and their cost (DMMAs) per stage
+        // the kernel decides per k-pair (2 k-steps, a 2x2x2 box of mesh points): a fragment pair is
+        // executed for both k-steps if either holds an in-sphere point of both fragments' rows
         auto tile_stage_cost = [&](int gi, int gj, int st) {
             int n = 0;
-            for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) {
-                const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
-                if (gi != gj) n += __builtin_popcount(ra) * __builtin_popcount(ca);
+            for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks += 2) {
+                const unsigned ra = gm[(size_t)gi * nks_pad + ks] | gm[(size_t)gi * nks_pad + ks + 1];
+                const unsigned ca = gm[(size_t)gj * nks_pad + ks] | gm[(size_t)gj * nks_pad + ks + 1];
+                if (gi != gj) n += 2 * __builtin_popcount(ra) * __builtin_popcount(ca);
                 else
                     for (int i = 0; i < 4; i++)
-                        if ((ra >> i) & 1u) n += __builtin_popcount(ca >> i);
+                        if ((ra >> i) & 1u) n += 2 * __builtin_popcount(ca >> i);
             }
             return n;
         };
@@ -540,15 +543,16 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 w.tiles[warp][0] = (uint8_t)slot_of(p.tiles[t].first);
                 w.tiles[warp][1] = (uint8_t)slot_of(p.tiles[t].second);
                 exec_dmma += tc;
-                for (int ks = 0; ks < nks_pad; ks++) {
+                for (int ks = 0; ks < nks_pad; ks += 2) {
                     const int gi = p.tiles[t].first, gj = p.tiles[t].second;
-                    const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
+                    const unsigned ra = gm[(size_t)gi * nks_pad + ks] | gm[(size_t)gi * nks_pad + ks + 1];
+                    const unsigned ca = gm[(size_t)gj * nks_pad + ks] | gm[(size_t)gj * nks_pad + ks + 1];
                     int nd = 0;
-                    if (gi != gj) nd = __builtin_popcount(ra) * __builtin_popcount(ca);
+                    if (gi != gj) nd = 2 * __builtin_popcount(ra) * __builtin_popcount(ca);
                     else
                         for (int i = 0; i < 4; i++)
-                            if ((ra >> i) & 1u) nd += __builtin_popcount(ca >> i);
-                    if (gi != gj && nd == 16) ks_full += 1;
+                            if ((ra >> i) & 1u) nd += 2 * __builtin_popcount(ca >> i);
+                    if (gi != gj && nd == 32) ks_full += 1;
                     else if (nd > 0) { ks_part += 1; dmma_part += nd; }
                 }
                 for (int st = 0; st < nstage; st++)
