@@ -142,12 +142,14 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         release(ctx);                                                  \
         return fail_cuda(e, "upload " #vec);                           \
     }
-    UP(P.items, &D.items)
+    {
+        const gint::ItemDesc* dd = nullptr;
+        if ((e = upload(ctx, P.descs, &dd)) != cudaSuccess) { release(ctx); return fail_cuda(e, "upload descs"); }
+        D.descs = const_cast<gint::ItemDesc*>(dd);
+    }
     UP(P.regions, &D.regions)
     UP(P.entries, &D.entries)
     UP(P.etasks, &D.etasks)
-    UP(P.gmask, &D.gmask)
-    UP(P.rowinfo, &D.rowinfo)
     UP(P.pair, &D.pair)
     UP(P.slot_xyz, &D.slot_xyz)
     UP(P.mirror, &D.mirror)
@@ -159,10 +161,6 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     if ((e = cudaMalloc(&ctr, 64 + 24 * 8 * 256)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
-    void* sgn = nullptr;
-    if ((e = cudaMalloc(&sgn, sizeof(uint32_t) * 16 * (P.regions.size() + 1))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc sign"); }
-    ctx->allocs.push_back(sgn);
-    D.sign = reinterpret_cast<uint32_t*>(sgn);
     {
         std::vector<int32_t> work;
         for (size_t r = 0; r < P.regions.size(); r++)

@@ -13,12 +13,10 @@ namespace gint {
 
 // Kernel parameter block (passed by value as a __grid_constant__).
 struct DevicePlan {
-    const WorkItem* items;
+    ItemDesc* descs;          // one per work item, queue order; sign bits filled in by gint_psi_kernel
     const Region* regions;
     const Entry* entries;
     const uint32_t* etasks;   // evaluation tasks: entry within region | slice << 16
-    const uint8_t* gmask;
-    const uint32_t* rowinfo;
     const uint32_t* pair;
     const uint8_t* slot_xyz;  // [nslice*32][4]
     const double* tab;        // packed radial tables, per species [ntab+4][nradp]
@@ -27,7 +25,6 @@ struct DevicePlan {
     const MirrorItem* mirror;
     double* psi;              // scratch: psi_chunks x 512 doubles, zero-filled once at setup
     unsigned int* counter;    // work-queue head, reset before every launch
-    uint32_t* sign;           // [nregions][16]: sign bits of V at the region's point slots (written by gint_psi_kernel)
     const int32_t* work_regions;   // indices of the regions that own work items
     double estep[9];          // mesh step vectors a_d / N_d (rows)
     double dV;

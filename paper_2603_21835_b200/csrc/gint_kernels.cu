@@ -280,6 +280,7 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
         const int reg_index = __ldg(P.work_regions + r);
         const Region* reg = P.regions + reg_index;
         const int ox = __ldg(&reg->origin[0]), oy = __ldg(&reg->origin[1]), oz = __ldg(&reg->origin[2]);
+        const int item0 = __ldg(&reg->item0), nitem = __ldg(&reg->nitem);
         for (int p = tid; p < npt; p += kEvalThreads) {   // npt is a multiple of 32: whole warps
             const uchar4 c = s_xyz[p];
             const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
@@ -288,7 +289,8 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
                 wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
             s_sqrtw[p] = sqrt(fabs(wv));
             const unsigned int neg = __ballot_sync(0xffffffffu, wv < 0.0);
-            if (lane == 0) P.sign[(size_t)reg_index * (kMaxRegionPoints / 32) + (p >> 5)] = neg;
+            if (lane == 0)   // every work item of the region carries the sign bits in its descriptor
+                for (int q = 0; q < nitem; q++) P.descs[item0 + q].sign[p >> 5] = neg;
         }
         __syncthreads();
         const int ntask = __ldg(&reg->ntask);
@@ -349,50 +351,37 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
 
     if (warp == kConsumerWarps) {
         // ================= producer warp =================
-        // take the next item from the queue and stage its descriptor
-        auto prepare = [&](ItemDesc* d) {
-            unsigned int it = 0;
-            if (lane == 0) it = atomicAdd(P.counter, 1u);
-            it = __shfl_sync(0xffffffffu, it, 0);
-            if (it >= (unsigned int)P.nitems) {
-                if (lane == 0) d->valid = 0;
-                __syncwarp();
-                return;
-            }
-            reinterpret_cast<uint32_t*>(&d->item)[lane] = __ldg(reinterpret_cast<const uint32_t*>(P.items + it) + lane);   // 128 B
-            __syncwarp();
-            const int wpr = P.nks_pad >> 2;   // 32-bit words per group row of activity bytes
-            const int nslot = d->item.nslot;
-            for (int i = lane; i < nslot * wpr; i += 32) {
-                const int slot = i / wpr, wd = i - slot * wpr;
-                reinterpret_cast<uint32_t*>(d->gmask[slot])[wd] = __ldg(
-                    reinterpret_cast<const uint32_t*>(P.gmask + d->item.reg.gmask_off + (int)d->item.slot_group[slot] * P.nks_pad) + wd);
-            }
-            for (int i = lane; i < nslot * kGroupRows; i += 32)
-                d->rinfo[i >> 5][i & 31] = __ldg(P.rowinfo + d->item.reg.rowinfo_off + (int)d->item.slot_group[i >> 5] * kGroupRows + (i & 31));
-            if (lane < kMaxRegionPoints / 32) d->sign[lane] = P.sign[(size_t)d->item.region * (kMaxRegionPoints / 32) + lane];
-            __syncwarp();
-            {   // stage lane: which slots hold an active k-step there
-                uint32_t a = 0;
-                for (int q = 0; q < nslot; q++)
-                    if (lane < P.nstage && *reinterpret_cast<const uint32_t*>(&d->gmask[q][lane * kStageKsteps])) a |= 1u << q;
-                d->act[lane] = (uint8_t)a;
-            }
-            if (lane == 0) d->valid = 1;
-            __syncwarp();
-        };
+        // Descriptor i+1 is fetched (one bulk copy straight into the slot, completion on its own
+        // mbarrier) while the stages of item i are being streamed; the queue index is taken one more
+        // item ahead so that the atomic's latency is off the critical path as well.
         uint32_t rs = 0, rph = 0;   // ring slot and phase of the next stage to fill
-        auto acquire_desc = [&](int i) {   // wait until the consumers released slot i % 3, stage item, publish
+        auto fetch_desc = [&](int i, unsigned int it) {   // lane 0: item index it -> descriptor slot i % 3
             const int ds = i % kDescSlots;
-            if (lane == 0) mbar_wait(smem_u32(s_dempty + ds), (((uint32_t)i / kDescSlots) & 1u) ^ 1u);
-            __syncwarp();
-            prepare(&s_desc[ds]);
-            if (lane == 0) mbar_arrive(smem_u32(s_dfull + ds));
-            __syncwarp();
+            mbar_wait(smem_u32(s_dempty + ds), (((uint32_t)i / kDescSlots) & 1u) ^ 1u);
+            const uint32_t bar = smem_u32(s_dfull + ds);
+            if (it < (unsigned int)P.nitems) {
+                mbar_arrive_expect_tx(bar, (uint32_t)sizeof(ItemDesc));
+                bulk_g2s(smem_u32(&s_desc[ds]), P.descs + it, (uint32_t)sizeof(ItemDesc), bar);
+            } else {
+                s_desc[ds].valid = 0;
+                mbar_arrive(bar);
+            }
         };
-        acquire_desc(0);
+        unsigned int it_next = 0, it_after = 0;
+        if (lane == 0) {
+            it_next = atomicAdd(P.counter, 1u);
+            fetch_desc(0, it_next);
+            it_next = atomicAdd(P.counter, 1u);
+        }
         for (int i = 0;; i++) {
             const ItemDesc* cur = &s_desc[i % kDescSlots];
+            if (lane == 0) {
+                it_after = atomicAdd(P.counter, 1u);                    // index of item i+2, needed one item from now
+                mbar_wait(smem_u32(s_dfull + i % kDescSlots), ((uint32_t)i / kDescSlots) & 1u);
+                if (cur->valid) fetch_desc(i + 1, it_next);             // in flight while this item streams
+                it_next = it_after;
+            }
+            __syncwarp();
             if (!cur->valid) break;
             const int nslot = cur->item.nslot;
             const unsigned char* psi_bytes = reinterpret_cast<const unsigned char*>(P.psi) +
@@ -400,7 +389,9 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
             // lane q copies the chunks of slot q; lane 0 also owns the barriers
             const unsigned char* src_lane = psi_bytes + (size_t)(lane < nslot ? cur->item.slot_group[lane] : 0) * P.nstage * kChunkBytes;
             uint32_t todo = cur->item.stage_mask;
-            auto issue = [&](int s) {   // whole warp
+            while (todo) {
+                const int s = __ffs(todo) - 1;
+                todo &= todo - 1;
                 const uint32_t act = cur->act[s];
                 const uint32_t bar = smem_u32(s_full + rs);
                 if (lane == 0) {
@@ -415,19 +406,6 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
                     bulk_g2s(smem_u32(s_ring + (size_t)rs * kStageBytes) + lane * kChunkBytes,
                              src_lane + (size_t)s * kChunkBytes, kChunkBytes, bar);
                 if (++rs == (uint32_t)nring) { rs = 0; rph ^= 1u; }
-            };
-            for (int k = 0; k < nring && todo; k++) {
-                const int s = __ffs(todo) - 1;
-                todo &= todo - 1;
-                issue(s);
-            }
-            TIMER_START
-            acquire_desc(i + 1);   // overlaps with the stages just issued
-            TIMER_ADD(2)
-            while (todo) {
-                const int s = __ffs(todo) - 1;
-                todo &= todo - 1;
-                issue(s);
             }
             TIMER_COUNT(6)
         }

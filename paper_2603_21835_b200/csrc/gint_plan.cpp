@@ -216,6 +216,9 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     }
     P.tables_in_smem = P.tab_packed.size() * sizeof(double) <= kMaxTableSmem;
     P.nring = kRingStages;
+#ifdef GINT_TIMING
+    if (const char* e = getenv("GINT_NRING")) P.nring = std::min(P.nring, atoi(e));
+#endif
     P.smem_bytes = 256 + smem_align((size_t)kDescSlots * sizeof(ItemDesc)) + (size_t)P.nring * kMaxSlots * kChunkBytes;
 
     // ---- point order inside a region: k-steps of 4 points, slices of 8 k-steps -----------------
@@ -597,11 +600,34 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     tmp.shrink_to_fit();
     // queue order: heaviest regions first, the items of a region consecutive (their CTAs share its psi)
     std::stable_sort(region_items.begin(), region_items.end(), [](const RegionItems& a, const RegionItems& b) { return a.cost > b.cost; });
-    for (const RegionItems& ri : region_items)
+    for (const RegionItems& ri : region_items) {
+        P.regions[(size_t)ri.region].item0 = (int32_t)P.items.size();
         for (WorkItem w : ri.items) {
             w.reg = P.regions[(size_t)w.region];
             P.items.push_back(w);
         }
+    }
+    // descriptors: everything the contraction kernel needs for an item, contiguous (one bulk copy)
+    P.descs.resize(P.items.size());
+    for (size_t it = 0; it < P.items.size(); it++) {
+        ItemDesc& d = P.descs[it];
+        std::memset(&d, 0, sizeof(d));
+        d.item = P.items[it];
+        const Region& R = d.item.reg;
+        for (int q = 0; q < d.item.nslot; q++) {
+            const int g = d.item.slot_group[q];
+            std::memcpy(d.gmask[q], &P.gmask[(size_t)R.gmask_off + (size_t)g * nks_pad], (size_t)nks_pad);
+            std::memcpy(d.rinfo[q], &P.rowinfo[(size_t)R.rowinfo_off + (size_t)g * kGroupRows], sizeof(uint32_t) * kGroupRows);
+        }
+        for (int st = 0; st < nstage; st++) {
+            uint32_t a = 0;
+            for (int q = 0; q < d.item.nslot; q++)
+                for (int ks = 0; ks < kStageKsteps; ks++)
+                    if (d.gmask[q][st * kStageKsteps + ks]) a |= 1u << q;
+            d.act[st] = (uint8_t)a;
+        }
+        d.valid = 1;
+    }
 
     double fpt = 0, fsym = 0;
     for (int32_t n : npoint_orb) {

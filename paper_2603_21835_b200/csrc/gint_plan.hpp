@@ -93,7 +93,7 @@ struct Region {          // 64 bytes
     int32_t nitem;       // work items of the region = number of evaluation shares
     int64_t psi_chunk0;  // first 4 KB chunk of the region in the psi scratch: chunk(g, s) = psi_chunk0 + g*nstage + s
     int32_t ngroup;
-    int32_t pad;
+    int32_t item0;       // first work item of the region in queue order (its nitem items are consecutive)
 };
 static_assert(sizeof(Region) == 64, "Region layout is shared with the device");
 
@@ -120,6 +120,22 @@ struct MirrorItem {   // dst block (I,J,R) <- transpose of src block (J,I,-R); s
 
 // rowinfo word: entry index within the region | mu << 12 | norb << 20; kNoBlock for padding rows
 inline uint32_t pack_rowinfo(int e, int mu, int norb) { return (uint32_t)e | ((uint32_t)mu << 12) | ((uint32_t)norb << 20); }
+
+constexpr size_t kSmemLimit = 232448;   // 227 KB opt-in limit per CTA on sm_100
+constexpr int kDescSlots = 3;           // item descriptors in flight in the contraction kernel
+
+// Per-item descriptor: built by the host, completed by the psi kernel (sign bits), copied to shared
+// memory by the contraction kernel's producer warp with one bulk copy.
+struct ItemDesc {
+    WorkItem item;                                  // 128 (item.reg = its region)
+    uint8_t gmask[kMaxSlots][kMaxKsteps];           // 1024: fragment activity nibbles of the item's slots
+    uint32_t sign[kMaxRegionPoints / 32];           // 64: bit p = sign bit of V dV at point slot p
+    uint8_t act[kMaxStages];                        // 32: bit q = slot q has an active k-step in the stage
+    uint32_t rinfo[kMaxSlots][kGroupRows];          // 1024: row info words of the item's slots (flush)
+    int32_t valid;                                  // 0 = queue exhausted
+    int32_t pad[7];
+};
+static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
 struct Plan {
     // inputs
@@ -152,6 +168,7 @@ struct Plan {
     std::vector<uint32_t> rowinfo;
     std::vector<uint32_t> pair;
     std::vector<WorkItem> items;
+    std::vector<ItemDesc> descs;                // one per work item, queue order
     std::vector<uint32_t> etasks;               // evaluation tasks, region-major
     int64_t psi_chunks = 0;                     // 4 KB chunks of the psi scratch buffer
     // packed radial tables for the device: per species [ntab+4][nradp] (node-major, nradp = nrad rounded up
@@ -165,21 +182,6 @@ struct Plan {
     bool tables_in_smem = true;
     int nring = 0;                              // pipeline stages of the psi ring in shared memory
 };
-
-constexpr size_t kSmemLimit = 232448;   // 227 KB opt-in limit per CTA on sm_100
-constexpr int kDescSlots = 3;           // item descriptors in flight in the contraction kernel
-
-// Per-item descriptor staged in shared memory by the producer warp.
-struct ItemDesc {
-    WorkItem item;                                  // 128 (item.reg = its region)
-    uint8_t gmask[kMaxSlots][kMaxKsteps];           // 1024: fragment activity nibbles of the item's slots
-    uint32_t sign[kMaxRegionPoints / 32];           // 64: bit p = sign bit of V dV at point slot p
-    uint8_t act[kMaxStages];                        // 32: bit q = slot q has an active k-step in the stage
-    uint32_t rinfo[kMaxSlots][kGroupRows];          // 1024: row info words of the item's slots (flush)
-    int32_t valid;                                  // 0 = queue exhausted
-    int32_t pad[7];
-};
-static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
 constexpr int kRingStages = 6;          // 6 x 32 KB of psi in flight per SM
