@@ -57,18 +57,14 @@ void release(gint_ctx* ctx) {
         cudaSetDevice(ctx->device);
 #ifdef GINT_TIMING
         if (ctx->dev.counter) {
-            std::vector<long long> tm(24 * 256);
+            std::vector<long long> tm(16 * 16 * 8);
             cudaDeviceSynchronize();
             cudaMemcpy(tm.data(), ctx->dev.counter + 16, tm.size() * 8, cudaMemcpyDeviceToHost);
-            const char* names[3] = {"consumer w0: descwait - - fullwait contract flush items -", "consumer w5: descwait - - fullwait contract flush items -",
-                                    "producer   : - emptywait prepare - - - items -"};
-            for (int r = 0; r < 3; r++) {
-                fprintf(stderr, "[timing] %s\n", names[r]);
-                for (int b : {0, 1, 73, 147}) {
-                    fprintf(stderr, "   cta %3d:", b);
-                    for (int k = 0; k < 8; k++) fprintf(stderr, " %10.3f", (k == 6) ? (double)tm[24 * b + 8 * r + k] : tm[24 * b + 8 * r + k] / 1.965e6);
-                    fprintf(stderr, "\n");
-                }
+            fprintf(stderr, "[timing] cta 3, per warp (ms): descwait fullwait contract flush | warp 15 = producer: emptywait\n");
+            for (int w = 0; w < 16; w++) {
+                const long long* v = &tm[(16 * 3 + w) * 8];
+                fprintf(stderr, "   warp %2d (sched %d): %7.3f %7.3f %7.3f %7.3f   items %lld  wait@stage0 %7.3f @1-3 %7.3f\n", w, w & 3, v[0] / 1.965e6,
+                        (w == 15 ? v[1] : v[3]) / 1.965e6, v[4] / 1.965e6, v[5] / 1.965e6, v[6], v[1] / 1.965e6, v[2] / 1.965e6);
             }
         }
 #endif

@@ -13,7 +13,7 @@
 //       PAPER.md:380, 413).  One persistent CTA per SM pulls work items from a global queue; a
 //       work item is a set of up to 15 32x32 tiles (one per consumer warp) of the upper triangle
 //       of one region's C.  A producer warp stages the item descriptor and streams the row groups
-//       the tiles need through a ring of shared-memory stages (16 points each) with
+//       the tiles need through a ring of shared-memory stages (32 points each) with
 //       cp.async.bulk + mbarrier, running ahead across item boundaries; the 15 consumer warps
 //       keep their tile in registers and issue mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has
 //       no FP64 kind).  (fragment, k-step) pairs that hold no in-sphere point are skipped by
@@ -47,7 +47,7 @@ namespace {
 constexpr int kConsumerWarps = kTilesPerItem;          // 15
 constexpr int kConsumerThreads = kConsumerWarps * 32;  // 480
 constexpr int kThreads = kConsumerThreads + 32;        // + 1 producer warp
-constexpr int kStageBytes = kMaxSlots * kChunkBytes;   // 32 KB
+constexpr int kStageBytes = kMaxSlots * kChunkBytes;   // 64 KB
 
 __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -197,11 +197,11 @@ __device__ __forceinline__ void eval_task(const DevicePlan& P, const double* __r
     const double* Tk = tab + tab_off + k * nradp;
     // store addressing
     const int row0 = en->row0;
-    double* out = psi_region + ((lane >> 4) * kChunkDoubles + ((lane >> 3) & 1) * 64 + (lane & 3) * 2 + ((lane >> 2) & 1));
+    double* out = psi_region + ((lane / kStagePts) * kChunkDoubles + (((lane % kStagePts) >> 3) * 64) + (lane & 3) * 2 + ((lane >> 2) & 1));
     const int gstride = P.nstage * kChunkDoubles;
     int R = row0;
     auto put = [&](double v) {
-        out[(R >> 5) * gstride + ((R >> 3) & 3) * 128 + (R & 7) * 8] = v;
+        out[(R >> 5) * gstride + ((R >> 3) & 3) * (kStagePairs * 64) + (R & 7) * 8] = v;
         R++;
     };
     auto emit = [&](int l, double fv) {
@@ -301,7 +301,7 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
             const uint32_t tk = __ldg(tasks + t);
             const int slice = (int)(tk >> 16);
             eval_task(P, tab, entries + (tk & 0xFFFFu), slice, lane, s_off, s_sqrtw,
-                      psi_region + (size_t)(2 * slice) * kChunkDoubles);
+                      psi_region + (size_t)(slice * (kSlicePts / kStagePts)) * kChunkDoubles);
         }
     }
 }
@@ -430,35 +430,50 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
                 for (int j = 0; j < 4; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
 
             uint32_t todo = cur->item.stage_mask;
+            int nvis = 0;
+            (void)nvis;
             while (todo) {
                 const int s = __ffs(todo) - 1;
                 todo &= todo - 1;
                 TIMER_START
                 mbar_wait(smem_u32(s_full + cs), cph);
                 TIMER_ADD(3)
+#ifdef GINT_TIMING
+                if (nvis == 0) { TIMER_ADD(1) } else if (nvis < 4) { TIMER_ADD(2) }
+                nvis++;
+#endif
                 TIMER_START
 #ifdef GINT_TIMING
                 if (has_tile && !(P.debug & 1)) {
 #else
                 if (has_tile) {
 #endif
-                    const uint32_t ma = *reinterpret_cast<const uint32_t*>(&cur->gmask[sa][s * kStageKsteps]);
-                    const uint32_t mb = *reinterpret_cast<const uint32_t*>(&cur->gmask[sb][s * kStageKsteps]);
+                    // activity nibbles of the stage's k-steps, one byte each; k-pair kp = bytes 2 kp, 2 kp + 1
+                    const uint64_t ma8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sa][s * 8]);
+                    const uint64_t mb8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sb][s * 8]);
+                    const uint32_t ma = (uint32_t)((ma8 | (ma8 >> 8)) & 0x000F000F000F000Full) | (uint32_t)(((ma8 | (ma8 >> 8)) & 0x000F000F000F000Full) >> 28);
+                    const uint32_t mb = (uint32_t)((mb8 | (mb8 >> 8)) & 0x000F000F000F000Full) | (uint32_t)(((mb8 | (mb8 >> 8)) & 0x000F000F000F000Full) >> 28);
                     const unsigned char* stage = s_ring + (size_t)cs * kStageBytes;
                     const double2* pa = reinterpret_cast<const double2*>(stage + sa * kChunkBytes) + lane;
                     const double2* pb = reinterpret_cast<const double2*>(stage + sb * kChunkBytes) + lane;
                     // sign bits of V dV at this lane's four points (k-step ks: bit 4 ks + fk of the stage's 16)
-                    const uint32_t sg = (cur->sign[s >> 1] >> ((s & 1) * 16 + fk));
+                    const uint32_t sg = cur->sign[s] >> fk;
 #pragma unroll 1
-                    for (int kp = 0; kp < 2; kp++) {
-                        const uint32_t ra = ((ma >> (16 * kp)) | (ma >> (16 * kp + 8))) & 0xFu;
-                        const uint32_t ca = ((mb >> (16 * kp)) | (mb >> (16 * kp + 8))) & 0xFu;
+                    for (int kp = 0; kp < kStagePairs; kp++) {
+                        // packed above: pair 0 -> bits 0-3, pair 1 -> bits 16-19, pair 2 -> bits 4-7, pair 3 -> bits 20-23
+#ifdef GINT_TIMING
+                        const uint32_t ra = (P.debug & 8) ? 0xFu : (ma >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
+                        const uint32_t ca = (P.debug & 8) ? 0xFu : (mb >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
+#else
+                        const uint32_t ra = (ma >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
+                        const uint32_t ca = (mb >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
+#endif
                         if (ra == 0u || ca == 0u) continue;
                         // operands of both k-steps; fragments outside the masks may hold stale data and are not used
-                        const double2 a0 = pa[(0 * 2 + kp) * 32], a1 = pa[(1 * 2 + kp) * 32], a2 = pa[(2 * 2 + kp) * 32],
-                                      a3 = pa[(3 * 2 + kp) * 32];
-                        double2 b0 = pb[(0 * 2 + kp) * 32], b1 = pb[(1 * 2 + kp) * 32], b2 = pb[(2 * 2 + kp) * 32],
-                                b3 = pb[(3 * 2 + kp) * 32];
+                        const double2 a0 = pa[(0 * kStagePairs + kp) * 32], a1 = pa[(1 * kStagePairs + kp) * 32], a2 = pa[(2 * kStagePairs + kp) * 32],
+                                      a3 = pa[(3 * kStagePairs + kp) * 32];
+                        double2 b0 = pb[(0 * kStagePairs + kp) * 32], b1 = pb[(1 * kStagePairs + kp) * 32], b2 = pb[(2 * kStagePairs + kp) * 32],
+                                b3 = pb[(3 * kStagePairs + kp) * 32];
                         const uint32_t x0 = ((sg >> (8 * kp)) & 1u) << 31, x1 = ((sg >> (8 * kp + 4)) & 1u) << 31;
 #define SIGN_FLIP(v)                                                                 \
     v.x = __hiloint2double(__double2hiint(v.x) ^ x0, __double2loint(v.x)); \
@@ -499,30 +514,40 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
             const int ga = cur->item.slot_group[sa], gb = cur->item.slot_group[sb];
             const uint32_t* pair = P.pair + cur->item.reg.pair_off;
             const int m = cur->item.reg.nentry;
+            // this lane's 8 columns: j = 0..3, h = 0..1 -> column 8 j + 2 fk + h of the column group
+            uint32_t ci[4][2];
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                const uint2 c2 = *reinterpret_cast<const uint2*>(&cur->rinfo[sb][8 * j + 2 * fk]);
+                ci[j][0] = c2.x;
+                ci[j][1] = c2.y;
+            }
 #pragma unroll
             for (int i = 0; i < 4; i++) {
                 const int row = ga * kGroupRows + 8 * i + frow;
                 const uint32_t ri = cur->rinfo[sa][8 * i + frow];
-                if (ri == kNoBlock) continue;
                 const int ea = ri & 0xFFF, mu = (ri >> 12) & 0xFF, nI = ri >> 20;
+                // all pair-table look-ups of the row first (independent loads), then the reductions
+                uint32_t pr[4][2];
 #pragma unroll
-                for (int j = 0; j < 4; j++) {
-                    if (diag && i > j) continue;
+                for (int j = 0; j < 4; j++)
 #pragma unroll
                     for (int h = 0; h < 2; h++) {
-                        const double v = acc[i][j][h];
-                        if (v == 0.0) continue;
                         const int col = gb * kGroupRows + 8 * j + 2 * fk + h;
-                        if (row > col) continue;
-                        const uint32_t ci = cur->rinfo[sb][8 * j + 2 * fk + h];
-                        if (ci == kNoBlock) continue;
-                        const int eb = ci & 0xFFF, nu = (ci >> 12) & 0xFF, nJ = ci >> 20;
-                        const uint32_t pr = __ldg(pair + ea * m + eb);
-                        if (pr == kNoBlock) continue;
-                        const uint32_t idx = (pr & kPairTransposed) ? (uint32_t)(nu * nI + mu) : (uint32_t)(mu * nJ + nu);
-                        atomicAdd(H + (size_t)(pr & ~kPairTransposed) + idx, v);
+                        const bool ok = ri != kNoBlock && ci[j][h] != kNoBlock && row <= col && !(diag && i > j) &&
+                                        acc[i][j][h] != 0.0;
+                        pr[j][h] = ok ? __ldg(pair + ea * m + (int)(ci[j][h] & 0xFFF)) : kNoBlock;
                     }
-                }
+#pragma unroll
+                for (int j = 0; j < 4; j++)
+#pragma unroll
+                    for (int h = 0; h < 2; h++) {
+                        const uint32_t p2 = pr[j][h];
+                        if (p2 == kNoBlock) continue;
+                        const int nu = (ci[j][h] >> 12) & 0xFF, nJ = ci[j][h] >> 20;
+                        const uint32_t idx = (p2 & kPairTransposed) ? (uint32_t)(nu * nI + mu) : (uint32_t)(mu * nJ + nu);
+                        atomicAdd(H + (size_t)(p2 & ~kPairTransposed) + idx, acc[i][j][h]);
+                    }
             }
         }
             TIMER_ADD(5)
@@ -532,8 +557,8 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
         }
     }
 #ifdef GINT_TIMING
-    if (lane == 0 && (warp == 0 || warp == 5 || warp == kConsumerWarps)) {
-        long long* out = reinterpret_cast<long long*>(P.counter + 16) + 24 * blockIdx.x + (warp == 0 ? 0 : (warp == 5 ? 8 : 16));
+    if (lane == 0 && blockIdx.x < 16) {
+        long long* out = reinterpret_cast<long long*>(P.counter + 16) + (16 * blockIdx.x + warp) * 8;
         for (int k = 0; k < 8; k++) out[k] = tm_[k];
     }
 #endif

@@ -44,8 +44,9 @@ namespace gint {
 constexpr int kMaxOrbPerAtom = 64;
 constexpr int kMaxRegionPoints = 512;          // mesh points of one region
 constexpr int kKstepPts = 4;                   // K of DMMA.8x8x4
-constexpr int kStageKsteps = 4;                // k-steps per pipeline stage
-constexpr int kStagePts = kKstepPts * kStageKsteps;     // 16
+constexpr int kStageKsteps = 8;                // k-steps per pipeline stage
+constexpr int kStagePts = kKstepPts * kStageKsteps;     // 32
+constexpr int kStagePairs = kStageKsteps / 2;           // k-pairs (2x2x2 boxes) per stage
 constexpr int kSlicePts = 32;                  // points of one evaluation task (one lane per point)
 constexpr int kSliceKsteps = kSlicePts / kKstepPts;     // 8
 constexpr int kMaxKsteps = kMaxRegionPoints / kKstepPts;   // 128
@@ -54,8 +55,8 @@ constexpr int kGroupRows = 32;                 // rows of one row group = warp-t
 constexpr int kMaxSlots = 8;                   // row groups one work item may touch
 constexpr int kTilesPerItem = 15;              // one 32x32 tile per consumer warp (warp 15 is the producer)
 constexpr int kMaxGroups = 40;                 // row groups per region (<= 1280 orbitals listed)
-constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 512: psi of one (group, stage), fragment order
-constexpr int kChunkBytes = kChunkDoubles * 8;             // 4096
+constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 1024: psi of one (group, stage), fragment order
+constexpr int kChunkBytes = kChunkDoubles * 8;             // 8192
 constexpr uint32_t kNoBlock = 0xFFFFFFFFu;
 constexpr uint32_t kPairTransposed = 0x80000000u;
 
@@ -130,11 +131,12 @@ struct ItemDesc {
     WorkItem item;                                  // 128 (item.reg = its region)
     uint8_t gmask[kMaxSlots][kMaxKsteps];           // 1024: fragment activity nibbles of the item's slots
     uint32_t sign[kMaxRegionPoints / 32];           // 64: bit p = sign bit of V dV at point slot p
-    uint8_t act[kMaxStages];                        // 32: bit q = slot q has an active k-step in the stage
+    uint8_t act[32];                                // per stage (<= 32): bit q = slot q has an active k-step in the stage
     uint32_t rinfo[kMaxSlots][kGroupRows];          // 1024: row info words of the item's slots (flush)
     int32_t valid;                                  // 0 = queue exhausted
     int32_t pad[7];
 };
+static_assert(kSlicePts % kStagePts == 0 && kStageKsteps % 2 == 0 && kStageKsteps <= 8, "stage geometry");
 static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
 struct Plan {
@@ -184,7 +186,7 @@ struct Plan {
 };
 
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
-constexpr int kRingStages = 6;          // 6 x 32 KB of psi in flight per SM
+constexpr int kRingStages = 3;          // 3 x 64 KB of psi in flight per SM
 constexpr size_t kMaxTableSmem = 56 * 1024;   // larger radial tables stay in global memory (L1/L2-cached)
 
 inline uint64_t pack_key(int I, int J, int r1, int r2, int r3) {
