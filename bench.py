@@ -3,17 +3,18 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload si512_dzp] [--impl reference]
 
-A "step" is one gint_vlocal call = the whole hot path (V staging, phi evaluation,
-V*dV weighting, DMMA contraction, accumulation into H blocks, mirror) over the
-whole mesh.  Prints ONE JSON line (rank 0).
+A "step" is one gint_vlocal call = the whole hot path (psi kernel: V staging, phi
+evaluation, V*dV weighting; contraction kernel: DMMA contraction + accumulation into
+H blocks; mirror kernel) over the whole mesh.  Prints ONE JSON line (rank 0).
 
   value            FP64 TFLOP/s = F_sym / time, F_sym = sum_g n(g)(n(g)+1) useful flops
                    (the kernel exploits H(R) = H(-R)^T), inputs resident in HBM
   ms_per_step      ms per gint_vlocal call (CUDA events, L2 flushed between calls)
   e2e              same metric through gint_vlocal_host: pinned HOST V in, HOST H out,
                    both copies inside the timed region
-  roofline         integration kernel alone: achieved TFLOP/s (F_sym / its event-timed
-                   duration) over the FP64 tensor (DMMA.8x8x4) peak measured live
+  roofline         the dominant kernel (gint_vlocal_kernel, the contraction) alone: achieved
+                   TFLOP/s (F_sym / its event-timed duration) over the FP64 tensor (DMMA.8x8x4)
+                   peak measured live; the psi kernel's HBM figures ride along
   cpu_baseline     the CPU oracle, as it stands, on a bounded sample of the same workload
 
 N > 1 (torchrun): the big cells are sharded over ranks (strided slabs along a1), every
@@ -38,7 +39,7 @@ UNIT = "TFLOP/s"
 
 # DRAM traffic of the integration kernel per launch, from the ncu --set full capture
 # summarised in profiles/ (dram__bytes_read.sum + dram__bytes_write.sum); None = not captured.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"si512_dzp": 9.904e9 + 1.389e9}   # profiles/r01c_ncu_summary.md, gint_vlocal_kernel
 
 
 def measured_peaks():
@@ -261,6 +262,8 @@ def main():
     peak = max(peak_live, peak_rule)
     main_ms = float(np.mean([k[0] for k in kern_ms]))
     mirror_ms = float(np.mean([k[1] for k in kern_ms]))
+    psi_ms = float(np.mean([k[3] for k in kern_ms]))
+    psi_bytes = 8.0 * st["evaluated_pairs"] * (w.norb_total / w.natom) + 8.0 * float(np.prod(w.ngrid))
     F_rank = st["F_sym"]
     achieved = F_rank / (main_ms * 1e-3) * 1e-12
     hbm_bytes = 8.0 * float(np.prod(w.ngrid)) + 8.0 * ctx.h_len
@@ -269,6 +272,12 @@ def main():
         "traffic": NCU_TRAFFIC_BYTES.get(w.name),
         "kernel": "gint_vlocal_kernel", "kernel_ms": main_ms, "mirror_kernel_ms": mirror_ms,
         "kernel_share_of_step": main_ms / ms_per_step,
+        "psi_kernel": {"kernel": "gint_psi_kernel", "kernel_ms": psi_ms, "share_of_step": psi_ms / ms_per_step,
+                       "bound": "hbm", "algorithmic_bytes": psi_bytes,
+                       "achieved_gbs": psi_bytes / (psi_ms * 1e-3) * 1e-9, "peak_gbs": peaks["hbm_gbs"],
+                       "frac": psi_bytes / (psi_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"],
+                       "note": "writes psi = phi sqrt(|V dV|) once per listed (atom image, point) pair: "
+                               "8 B x orbitals x evaluated pairs, plus V read once"},
         "flops_per_launch": F_rank, "flops_accounting": "F_sym = sum_g n(g)(n(g)+1) (symmetry exploited); F_pt = %.4e" % F_pt,
         "executed_tensor_flops": st["executed_flops"],
         "peak_source": "live DMMA.8x8x4 register-resident microbenchmark (gint_measure_fp64_peak) %.2f; "
@@ -282,7 +291,9 @@ def main():
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "natom": w.natom, "norb": w.norb_total, "ngrid": [int(x) for x in w.ngrid],
-                   "nblocks": ctx.nblocks, "h_doubles": ctx.h_len, "bcell": [4, 4, 4],
+                   "nblocks": ctx.nblocks, "h_doubles": ctx.h_len,
+                   "bcell": [next(c for c in (8, 6, 4, int(n)) if int(n) % c == 0) for n in w.ngrid],
+                   "psi_scratch_bytes": st["psi_scratch_bytes"],
                    "l2": "flushed between timed iterations (256 MB write)", "parallelism": "cells sharded x%d" % world,
                    "input_sha256": w.sha256()[:16], "setup_s": setup_s, "wall_s_timed_region": wall},
         "clocks": clocks,
