@@ -39,7 +39,7 @@ UNIT = "TFLOP/s"
 
 # DRAM traffic of the integration kernel per launch, from the ncu --set full capture
 # summarised in profiles/ (dram__bytes_read.sum + dram__bytes_write.sum); None = not captured.
-NCU_TRAFFIC_BYTES = {"si512_dzp": 9.904e9 + 1.389e9}   # profiles/r01c_ncu_summary.md, gint_vlocal_kernel
+NCU_TRAFFIC_BYTES = {"si512_dzp": 13.608e9 + 1.584e9}   # profiles/r01c_ncu_summary.md, gint_vlocal_kernel
 
 
 def measured_peaks():
@@ -114,7 +114,7 @@ def run_reference(args, w, stats_fpt):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    frac_atoms = max(1, min(w.natom, args.ref_atoms))
+    frac_atoms = max(1, min(w.natom, args.ref_atoms or 32))
     times = []
     used = nblk = ntot = 0
     for i in range(args.warmup + args.steps):
@@ -145,7 +145,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="si512_dzp")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--ref-atoms", type=int, default=8, help="row atoms in the oracle sample")
+    ap.add_argument("--ref-atoms", type=int, default=0,
+                    help="row atoms in the oracle sample (default: 128 for the cpu_baseline leg, 32 per step for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -304,8 +305,8 @@ def main():
         "roofline": roofline,
     }
     if not args.no_cpu_baseline and world == 1:
-        dt, used, nblk, ntot = oracle_sample(w, min(w.natom, args.ref_atoms))
-        na = min(w.natom, args.ref_atoms)
+        na = min(w.natom, args.ref_atoms or 128)
+        dt, used, nblk, ntot = oracle_sample(w, na)
         cval = F_pt * na / w.natom / dt * 1e-12
         out["cpu_baseline"] = {
             "value": cval, "unit": UNIT, "cores": used, "kind": "oracle",
