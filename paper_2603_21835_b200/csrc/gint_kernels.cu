@@ -98,6 +98,34 @@ __device__ __forceinline__ void kpair_rect(double (&acc)[4][4][2], uint32_t ra, 
         default: break;
     }
 }
+// The same with all four row fragments active (the usual case: rows come from the denser groups):
+// straight-line code per column pattern, no row guards.
+#define KALL1(c, p) case c: K1(0, p) K1(1, p) K1(2, p) K1(3, p) break;
+#define KALL2(c, p, q) case c: K2(0, p, q) K2(1, p, q) K2(2, p, q) K2(3, p, q) break;
+#define KALL3(c, p, q, r) case c: K3(0, p, q, r) K3(1, p, q, r) K3(2, p, q, r) K3(3, p, q, r) break;
+__device__ __forceinline__ void kpair_rect_allrows(double (&acc)[4][4][2], uint32_t ca, double2 a0, double2 a1, double2 a2,
+                                                   double2 a3, double2 b0, double2 b1, double2 b2, double2 b3) {
+    switch (ca) {
+        KALL1(1, 0)
+        KALL1(2, 1)
+        KALL2(3, 0, 1)
+        KALL1(4, 2)
+        KALL2(5, 0, 2)
+        KALL2(6, 1, 2)
+        KALL3(7, 0, 1, 2)
+        KALL1(8, 3)
+        KALL2(9, 0, 3)
+        KALL2(10, 1, 3)
+        KALL3(11, 0, 1, 3)
+        KALL2(12, 2, 3)
+        KALL3(13, 0, 2, 3)
+        KALL3(14, 1, 2, 3)
+        default: break;
+    }
+}
+#undef KALL1
+#undef KALL2
+#undef KALL3
 // One k-pair of a diagonal tile (row group == column group): fragment pairs i <= j with both active.
 #define KXY_IF(cond, i, j) \
     if (cond) {            \
@@ -490,6 +518,8 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
                                 FY(2, 0) FY(2, 1) FY(2, 2) FY(2, 3) FY(3, 0) FY(3, 1) FY(3, 2) FY(3, 3)
 #undef FX
 #undef FY
+                            } else if (ra == 0xFu) {
+                                kpair_rect_allrows(acc, ca, a0, a1, a2, a3, b0, b1, b2, b3);
                             } else {
                                 kpair_rect(acc, ra, ca, a0, a1, a2, a3, b0, b1, b2, b3, never);
                             }

@@ -4,7 +4,6 @@
 #include <algorithm>
 #include <array>
 #include <cmath>
-#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <numeric>
@@ -556,7 +555,6 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                     else
                         for (int i = 0; i < 4; i++)
                             if ((ra >> i) & 1u) nd += 2 * __builtin_popcount(ca >> i);
-                    if (getenv("GINT_HIST") && gi != gj && nd > 0) { static double hist[256]; static long cnt = 0; hist[ra * 16 + ca] += nd; if (++cnt % 20000000 == 0) { double tot = 0; for (double h : hist) tot += h; fprintf(stderr, "HIST"); for (int q = 0; q < 256; q++) if (hist[q] > 0.004 * tot) fprintf(stderr, " %x:%x=%.1f%%", q >> 4, q & 15, 100 * hist[q] / tot); fprintf(stderr, "\n"); } }
                     if (gi != gj && nd == 32) ks_full += 1;
                     else if (nd > 0) { ks_part += 1; dmma_part += nd; }
                 }
