@@ -59,12 +59,12 @@ void release(gint_ctx* ctx) {
         if (ctx->dev.counter) {
             std::vector<long long> tm(16 * 16 * 8);
             cudaDeviceSynchronize();
-            cudaMemcpy(tm.data(), ctx->dev.counter + 16, tm.size() * 8, cudaMemcpyDeviceToHost);
+            cudaMemcpy(tm.data(), ctx->dev.counter + 272, tm.size() * 8, cudaMemcpyDeviceToHost);
             fprintf(stderr, "[timing] cta 3, per warp (ms): descwait fullwait contract flush | warp 15 = producer: emptywait\n");
-            for (int w = 0; w < 16; w++) {
+            for (int w = 0; w < 8; w++) {
                 const long long* v = &tm[(16 * 3 + w) * 8];
                 fprintf(stderr, "   warp %2d (sched %d): %7.3f %7.3f %7.3f %7.3f   items %lld  wait@stage0 %7.3f @1-3 %7.3f\n", w, w & 3, v[0] / 1.965e6,
-                        (w == 15 ? v[1] : v[3]) / 1.965e6, v[4] / 1.965e6, v[5] / 1.965e6, v[6], v[1] / 1.965e6, v[2] / 1.965e6);
+                        (v[3] == 0 ? v[1] : v[3]) / 1.965e6, v[4] / 1.965e6, v[5] / 1.965e6, v[6], v[1] / 1.965e6, v[2] / 1.965e6);
             }
         }
 #endif
@@ -154,7 +154,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     UP(P.sp_real, &D.sp_real)
 #undef UP
     void* ctr = nullptr;   // queue head (+ development timing area)
-    if ((e = cudaMalloc(&ctr, 64 + 24 * 8 * 256)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
+    if ((e = cudaMalloc(&ctr, 4 * 272 + 16 * 16 * 8 * 8 + 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
     {

@@ -44,10 +44,10 @@ namespace {
 #define TIMER_COUNT(k)
 #endif
 
-constexpr int kConsumerWarps = kTilesPerItem;          // 15
-constexpr int kConsumerThreads = kConsumerWarps * 32;  // 480
+constexpr int kConsumerWarps = kTilesPerItem;          // 7
+constexpr int kConsumerThreads = kConsumerWarps * 32;  // 224
 constexpr int kThreads = kConsumerThreads + 32;        // + 1 producer warp
-constexpr int kStageBytes = kMaxSlots * kChunkBytes;   // 64 KB
+constexpr int kStageBytes = kMaxSlots * kChunkBytes;   // 32 KB
 
 __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -100,9 +100,14 @@ __device__ __forceinline__ void kpair_rect(double (&acc)[4][4][2], uint32_t ra, 
 }
 // The same with all four row fragments active (the usual case: rows come from the denser groups):
 // straight-line code per column pattern, no row guards.
-#define KALL1(c, p) case c: K1(0, p) K1(1, p) K1(2, p) K1(3, p) break;
-#define KALL2(c, p, q) case c: K2(0, p, q) K2(1, p, q) K2(2, p, q) K2(3, p, q) break;
-#define KALL3(c, p, q, r) case c: K3(0, p, q, r) K3(1, p, q, r) K3(2, p, q, r) K3(3, p, q, r) break;
+// (all first-k-step DMMAs, then all second-k-step ones: no accumulator is reused within 28 cycles)
+#define KALL1(c, p) case c: KX(0, p) KX(1, p) KX(2, p) KX(3, p) KY(0, p) KY(1, p) KY(2, p) KY(3, p) break;
+#define KALL2(c, p, q) \
+    case c: KX(0, p) KX(0, q) KX(1, p) KX(1, q) KX(2, p) KX(2, q) KX(3, p) KX(3, q) \
+            KY(0, p) KY(0, q) KY(1, p) KY(1, q) KY(2, p) KY(2, q) KY(3, p) KY(3, q) break;
+#define KALL3(c, p, q, r) \
+    case c: KX(0, p) KX(0, q) KX(0, r) KX(1, p) KX(1, q) KX(1, r) KX(2, p) KX(2, q) KX(2, r) KX(3, p) KX(3, q) KX(3, r) \
+            KY(0, p) KY(0, q) KY(0, r) KY(1, p) KY(1, q) KY(1, r) KY(2, p) KY(2, q) KY(2, r) KY(3, p) KY(3, q) KY(3, r) break;
 __device__ __forceinline__ void kpair_rect_allrows(double (&acc)[4][4][2], uint32_t ca, double2 a0, double2 a1, double2 a2,
                                                    double2 a3, double2 b0, double2 b1, double2 b2, double2 b3) {
     switch (ca) {
@@ -127,16 +132,30 @@ __device__ __forceinline__ void kpair_rect_allrows(double (&acc)[4][4][2], uint3
 #undef KALL2
 #undef KALL3
 // One k-pair of a diagonal tile (row group == column group): fragment pairs i <= j with both active.
-#define KXY_IF(cond, i, j) \
-    if (cond) {            \
-        do { KX(i, j) KY(i, j) } while (never); \
+#define KX_IF(cond, i, j) \
+    if (cond) {           \
+        do { KX(i, j) } while (never); \
+    }
+#define KY_IF(cond, i, j) \
+    if (cond) {           \
+        do { KY(i, j) } while (never); \
     }
 __device__ __forceinline__ void kpair_diag(double (&acc)[4][4][2], uint32_t ra, double2 a0, double2 a1, double2 a2, double2 a3,
                                            double2 b0, double2 b1, double2 b2, double2 b3, int never) {
-    KROW(0, K1(0, 0) KXY_IF(ra & 2u, 0, 1) KXY_IF(ra & 4u, 0, 2) KXY_IF(ra & 8u, 0, 3))
-    KROW(1, K1(1, 1) KXY_IF(ra & 4u, 1, 2) KXY_IF(ra & 8u, 1, 3))
-    KROW(2, K1(2, 2) KXY_IF(ra & 8u, 2, 3))
-    KROW(3, K1(3, 3))
+    if (ra == 0xFu) {   // all ten fragment pairs
+        KX(0, 0) KX(0, 1) KX(0, 2) KX(0, 3) KX(1, 1) KX(1, 2) KX(1, 3) KX(2, 2) KX(2, 3) KX(3, 3)
+        KY(0, 0) KY(0, 1) KY(0, 2) KY(0, 3) KY(1, 1) KY(1, 2) KY(1, 3) KY(2, 2) KY(2, 3) KY(3, 3)
+        return;
+    }
+    // first k-step of every active pair, then the second: no accumulator is reused back to back
+    KROW(0, KX(0, 0) KX_IF(ra & 2u, 0, 1) KX_IF(ra & 4u, 0, 2) KX_IF(ra & 8u, 0, 3))
+    KROW(1, KX(1, 1) KX_IF(ra & 4u, 1, 2) KX_IF(ra & 8u, 1, 3))
+    KROW(2, KX(2, 2) KX_IF(ra & 8u, 2, 3))
+    KROW(3, KX(3, 3))
+    KROW(0, KY(0, 0) KY_IF(ra & 2u, 0, 1) KY_IF(ra & 4u, 0, 2) KY_IF(ra & 8u, 0, 3))
+    KROW(1, KY(1, 1) KY_IF(ra & 4u, 1, 2) KY_IF(ra & 8u, 1, 3))
+    KROW(2, KY(2, 2) KY_IF(ra & 8u, 2, 3))
+    KROW(3, KY(3, 3))
 }
 #undef KROW
 #undef KX
@@ -148,7 +167,8 @@ __device__ __forceinline__ void kpair_diag(double (&acc)[4][4][2], uint32_t ra, 
 #undef KCASE1
 #undef KCASE2
 #undef KCASE3
-#undef KXY_IF
+#undef KX_IF
+#undef KY_IF
 
 // ---- mbarrier / bulk-copy helpers (shared::cta addresses) --------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -348,7 +368,7 @@ GINT_HD inline ContractSmem contract_smem(int nring) {
     return L;
 }
 
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, kCtasPerSm)
 gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -373,11 +393,24 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    // The two CTAs of an SM put their producer warp on different sub-partitions (warp w runs on sub-partition
+    // w % 4), so that the SM's 14 consumer warps spread 3/4/4/3: the first CTA to arrive uses warp 7, the second warp 4.
+    __shared__ int s_parity;
+    if (tid == 0) {
+        unsigned int smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        s_parity = (int)(atomicAdd(P.counter + 1 + (smid & 255u), 1u) & 1u);
+    }
     fence_proxy_async();
     __syncthreads();
+    const int parity = kCtasPerSm == 2 ? s_parity : 0;
+    const int producer_warp = parity ? 4 : kConsumerWarps;
+    // consumer index (which tile of the item): the plan fills tiles[v + 4 r] for virtual sub-partition v (v = 3 holds
+    // one tile fewer); parity 1 swaps sub-partitions 0 and 3
+    const int cidx = parity == 0 ? warp : (warp == 0 ? 3 : (warp == 3 ? 0 : (warp == 7 ? 4 : warp)));
     TIMER_DECL
 
-    if (warp == kConsumerWarps) {
+    if (warp == producer_warp) {
         // ================= producer warp =================
         // Descriptor i+1 is fetched (one bulk copy straight into the slot, completion on its own
         // mbarrier) while the stages of item i are being streamed; the queue index is taken one more
@@ -448,7 +481,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
             TIMER_ADD(0)
             const ItemDesc* cur = &s_desc[ds];
             if (!cur->valid) break;
-            const int sa = cur->item.tiles[warp][0], sb = cur->item.tiles[warp][1];
+            const int sa = cur->item.tiles[cidx][0], sb = cur->item.tiles[cidx][1];
             const bool has_tile = sa != 0xFF;
             const bool diag = sa == sb;
             double acc[4][4][2];
@@ -476,19 +509,28 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
 #else
                 if (has_tile) {
 #endif
-                    // activity nibbles of the stage's k-steps, one byte each; k-pair kp = bytes 2 kp, 2 kp + 1
-                    const uint64_t ma8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sa][s * 8]);
-                    const uint64_t mb8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sb][s * 8]);
-                    const uint32_t ma = (uint32_t)((ma8 | (ma8 >> 8)) & 0x000F000F000F000Full) | (uint32_t)(((ma8 | (ma8 >> 8)) & 0x000F000F000F000Full) >> 28);
-                    const uint32_t mb = (uint32_t)((mb8 | (mb8 >> 8)) & 0x000F000F000F000Full) | (uint32_t)(((mb8 | (mb8 >> 8)) & 0x000F000F000F000Full) >> 28);
+                    // activity nibbles of the stage's k-steps, one byte each; k-pair kp = bytes 2 kp, 2 kp + 1, OR-ed and
+                    // packed: pair 0 -> bits 0-3, pair 1 -> bits 16-19, pair 2 -> bits 4-7, pair 3 -> bits 20-23
+                    uint32_t ma, mb;
+                    if (kStageKsteps == 8) {
+                        const uint64_t ma8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sa][s * 8]);
+                        const uint64_t mb8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sb][s * 8]);
+                        const uint64_t qa = (ma8 | (ma8 >> 8)) & 0x000F000F000F000Full, qb = (mb8 | (mb8 >> 8)) & 0x000F000F000F000Full;
+                        ma = (uint32_t)qa | (uint32_t)(qa >> 28);
+                        mb = (uint32_t)qb | (uint32_t)(qb >> 28);
+                    } else {
+                        const uint32_t ma4 = *reinterpret_cast<const uint32_t*>(&cur->gmask[sa][s * 4]);
+                        const uint32_t mb4 = *reinterpret_cast<const uint32_t*>(&cur->gmask[sb][s * 4]);
+                        ma = (ma4 | (ma4 >> 8)) & 0x000F000Fu;
+                        mb = (mb4 | (mb4 >> 8)) & 0x000F000Fu;
+                    }
                     const unsigned char* stage = s_ring + (size_t)cs * kStageBytes;
                     const double2* pa = reinterpret_cast<const double2*>(stage + sa * kChunkBytes) + lane;
                     const double2* pb = reinterpret_cast<const double2*>(stage + sb * kChunkBytes) + lane;
                     // sign bits of V dV at this lane's four points (k-step ks: bit 4 ks + fk of the stage's 16)
-                    const uint32_t sg = cur->sign[s] >> fk;
+                    const uint32_t sg = (kStagePts == 32 ? cur->sign[s] : (cur->sign[s >> 1] >> ((s & 1) * 16))) >> fk;
 #pragma unroll 1
                     for (int kp = 0; kp < kStagePairs; kp++) {
-                        // packed above: pair 0 -> bits 0-3, pair 1 -> bits 16-19, pair 2 -> bits 4-7, pair 3 -> bits 20-23
 #ifdef GINT_TIMING
                         const uint32_t ra = (P.debug & 8) ? 0xFu : (ma >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
                         const uint32_t ca = (P.debug & 8) ? 0xFu : (mb >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
@@ -588,7 +630,7 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
     }
 #ifdef GINT_TIMING
     if (lane == 0 && blockIdx.x < 16) {
-        long long* out = reinterpret_cast<long long*>(P.counter + 16) + (16 * blockIdx.x + warp) * 8;
+        long long* out = reinterpret_cast<long long*>(P.counter + 272) + (16 * blockIdx.x + warp) * 8;
         for (int k = 0; k < 8; k++) out[k] = tm_[k];
     }
 #endif
@@ -630,7 +672,7 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_
     if (ev) cudaEventRecord(ev[0], stream);
     cudaError_t e = cudaMemsetAsync(H, 0, h_len * sizeof(double), stream);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int), stream);   // work-queue head
+    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 257, stream);   // work-queue head + per-SM arrival counters
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[1], stream);
     if (P.nitems > 0) {
@@ -644,7 +686,7 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_
     }
     if (ev) cudaEventRecord(ev[2], stream);
     if (P.nitems > 0) {
-        const int grid = P.nitems < nsm ? P.nitems : nsm;
+        const int grid = P.nitems < kCtasPerSm * nsm ? P.nitems : kCtasPerSm * nsm;
         gint_vlocal_kernel<<<grid, kThreads, contract_smem_bytes, stream>>>(P, H);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -472,7 +472,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 tcost[(size_t)gi][(size_t)gj] = n;
             }
         std::vector<Proto> protos;
-        const int chunk = 5;   // 5 groups -> a clique of 15 tiles
+        const int chunk = kCliqueGroups;   // 3 groups -> a clique of 6 tiles
         const int nchunk = (ngroup + chunk - 1) / chunk;
         for (int k = 0; k < nchunk; k++) {
             const int k0 = k * chunk, k1 = std::min(ngroup, k0 + chunk);
@@ -537,8 +537,8 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             int used[4] = {0, 0, 0, 0};
             for (size_t t = 0; t < p.tiles.size(); t++) {
                 int q = -1;
-                for (int k = 0; k < 4; k++)   // sub-partition 3 also hosts the producer warp: three consumers there
-                    if (used[k] < (k == 3 ? 3 : 4) && (q < 0 || load[k] < load[q])) q = k;
+                for (int k = 0; k < 4; k++)   // virtual sub-partition 3 also hosts the producer warp: one consumer fewer there
+                    if (used[k] < (k == 3 ? kTilesPerItem / 4 : (kTilesPerItem + 3) / 4) && (q < 0 || load[k] < load[q])) q = k;
                 const int warp = q + 4 * used[q];
                 used[q]++;
                 const double tc = tcost[(size_t)p.tiles[t].first][(size_t)p.tiles[t].second];

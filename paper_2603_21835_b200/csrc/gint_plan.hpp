@@ -15,7 +15,7 @@
 // *rows* of the region's psi matrix, psi = phi sqrt(|V dV|).  Rows are cut into
 // fragments of 8 (one DMMA operand) and groups of 32 (one warp-tile edge).  The
 // upper triangle of the region's  C = psi diag(sign V) psi^T  is cut into 32x32
-// tiles; tiles are packed 15 at a time (one per consumer warp) into *work items*
+// tiles; tiles are packed 7 at a time (one per consumer warp) into *work items*
 // that touch at most kMaxSlots row groups.  The items of a region are consecutive
 // in the work queue; the CTA that takes item q of n evaluates share q of the
 // region's psi (phase 1), writes it to the psi scratch buffer in global memory
@@ -44,8 +44,12 @@ namespace gint {
 constexpr int kMaxOrbPerAtom = 64;
 constexpr int kMaxRegionPoints = 512;          // mesh points of one region
 constexpr int kKstepPts = 4;                   // K of DMMA.8x8x4
-constexpr int kStageKsteps = 8;                // k-steps per pipeline stage
-constexpr int kStagePts = kKstepPts * kStageKsteps;     // 32
+#ifndef GINT_CTAS_PER_SM
+#define GINT_CTAS_PER_SM 1                     // contraction CTAs per SM: 2 x (7 consumer warps + producer) or 1 x (15 + producer)
+#endif
+constexpr int kCtasPerSm = GINT_CTAS_PER_SM;
+constexpr int kStageKsteps = kCtasPerSm == 2 ? 4 : 8;   // k-steps per pipeline stage
+constexpr int kStagePts = kKstepPts * kStageKsteps;     // 16 or 32
 constexpr int kStagePairs = kStageKsteps / 2;           // k-pairs (2x2x2 boxes) per stage
 constexpr int kSlicePts = 32;                  // points of one evaluation task (one lane per point)
 constexpr int kSliceKsteps = kSlicePts / kKstepPts;     // 8
@@ -53,10 +57,11 @@ constexpr int kMaxKsteps = kMaxRegionPoints / kKstepPts;   // 128
 constexpr int kMaxStages = kMaxKsteps / kStageKsteps;      // 32
 constexpr int kGroupRows = 32;                 // rows of one row group = warp-tile edge
 constexpr int kMaxSlots = 8;                   // row groups one work item may touch
-constexpr int kTilesPerItem = 15;              // one 32x32 tile per consumer warp (warp 15 is the producer)
+constexpr int kTilesPerItem = kCtasPerSm == 2 ? 7 : 15;   // one 32x32 tile per consumer warp; a CTA = consumers + 1 producer warp
+constexpr int kCliqueGroups = kCtasPerSm == 2 ? 3 : 5;    // largest c with c (c + 1) / 2 <= kTilesPerItem
 constexpr int kMaxGroups = 40;                 // row groups per region (<= 1280 orbitals listed)
-constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 1024: psi of one (group, stage), fragment order
-constexpr int kChunkBytes = kChunkDoubles * 8;             // 8192
+constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 512: psi of one (group, stage), fragment order
+constexpr int kChunkBytes = kChunkDoubles * 8;             // 4096
 constexpr uint32_t kNoBlock = 0xFFFFFFFFu;
 constexpr uint32_t kPairTransposed = 0x80000000u;
 
@@ -186,7 +191,7 @@ struct Plan {
 };
 
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
-constexpr int kRingStages = 3;          // 3 x 64 KB of psi in flight per SM
+constexpr int kRingStages = 3;          // 3 x 32 KB of psi in flight per CTA, two CTAs per SM
 constexpr size_t kMaxTableSmem = 56 * 1024;   // larger radial tables stay in global memory (L1/L2-cached)
 
 inline uint64_t pack_key(int I, int J, int r1, int r2, int r3) {
