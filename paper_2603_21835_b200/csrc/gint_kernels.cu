@@ -347,9 +347,16 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
         double* psi_region = P.psi + (size_t)__ldg(&reg->psi_chunk0) * kChunkDoubles;
         for (int t = warp; t < ntask; t += kEvalThreads / 32) {
             const uint32_t tk = __ldg(tasks + t);
-            const int slice = (int)(tk >> 16);
-            eval_task(P, tab, entries + (tk & 0xFFFFu), slice, lane, s_off, s_sqrtw,
-                      psi_region + (size_t)(slice * (kSlicePts / kStagePts)) * kChunkDoubles);
+            const Entry* en = entries + (tk & 0xFFFFu);
+            const int s0 = (int)(tk >> 16) * 8;
+            // activity of the run's 8 slices: byte s of the 64 k-step bits starting at slice s0
+            const uint2 km = *reinterpret_cast<const uint2*>(&en->kmask[s0 >> 2]);
+            for (int q = 0; q < 8 && s0 + q < P.nslice; q++) {
+                if ((((q < 4 ? km.x : km.y) >> (8 * (q & 3))) & 0xFFu) == 0u) continue;
+                const int slice = s0 + q;
+                eval_task(P, tab, en, slice, lane, s_off, s_sqrtw,
+                          psi_region + (size_t)(slice * (kSlicePts / kStagePts)) * kChunkDoubles);
+            }
         }
     }
 }

@@ -407,12 +407,19 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             err = "plan tables exceed 2^31 entries";
             return GINT_EUNSUPPORTED;
         }
-        // evaluation tasks: (entry, 32-point slice) pairs with at least one point inside the sphere
-        for (int s = 0; s < nslice; s++)
-            for (int i = 0; i < m; i++) {
-                const Entry& e = P.entries[pos + i];
-                if ((e.kmask[(s * kSliceKsteps) >> 5] >> ((s * kSliceKsteps) & 31)) & 0xFFu) P.etasks.push_back(pack_etask(i, s));
+        // evaluation tasks: (entry, run of up to 8 slices) with at least one point inside the sphere; the kernel
+        // walks the run's active 32-point slices with the entry's data in registers
+        int nactive = 0;
+        for (int i = 0; i < m; i++) {
+            const Entry& e = P.entries[pos + i];
+            for (int h = 0; h * 8 < nslice; h++) {
+                int na = 0;
+                for (int s = h * 8; s < std::min(nslice, h * 8 + 8); s++)
+                    if ((e.kmask[(s * kSliceKsteps) >> 5] >> ((s * kSliceKsteps) & 31)) & 0xFFu) na++;
+                if (na) P.etasks.push_back(pack_etask(i, h));
+                nactive += na;
             }
+        }
         R.ntask = (int32_t)P.etasks.size() - R.task_off;
         // fragment activity: OR of the k-step masks of the entries that own rows of the fragment
         std::vector<std::array<uint32_t, 4>> fmask((size_t)ngroup * 4, std::array<uint32_t, 4>{0, 0, 0, 0});
@@ -588,7 +595,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         R.nitem = (int32_t)ri.items.size();
         if (R.nitem > 0) {
             P.psi_chunks += (int64_t)ngroup * nstage;
-            n_etask += R.ntask;
+            n_etask += nactive;
             region_items.push_back(std::move(ri));
         } else {
             R.ntask = 0;

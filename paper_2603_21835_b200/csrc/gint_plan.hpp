@@ -95,7 +95,7 @@ struct Region {          // 64 bytes
     int32_t nentry;
     int32_t entry0;      // first entry of the region in entries
     int32_t task_off;    // into etasks
-    int32_t ntask;       // evaluation tasks (entry, 32-point slice) with a point inside the sphere
+    int32_t ntask;       // evaluation tasks (entry, run of 8 slices) with a point inside the sphere
     int32_t nitem;       // work items of the region = number of evaluation shares
     int64_t psi_chunk0;  // first 4 KB chunk of the region in the psi scratch: chunk(g, s) = psi_chunk0 + g*nstage + s
     int32_t ngroup;
@@ -103,8 +103,8 @@ struct Region {          // 64 bytes
 };
 static_assert(sizeof(Region) == 64, "Region layout is shared with the device");
 
-// evaluation task word: entry index within the region | slice << 16
-inline uint32_t pack_etask(int e, int slice) { return (uint32_t)e | ((uint32_t)slice << 16); }
+// evaluation task word: entry index within the region | run << 16 (run h = slices 8h .. 8h+7)
+inline uint32_t pack_etask(int e, int run) { return (uint32_t)e | ((uint32_t)run << 16); }
 
 struct WorkItem {        // 128 bytes: 64 of its own + a copy of its region (one fetch instead of two dependent ones)
     int32_t region;
