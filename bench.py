@@ -39,7 +39,7 @@ UNIT = "TFLOP/s"
 
 # DRAM traffic of the integration kernel per launch, from the ncu --set full capture
 # summarised in profiles/ (dram__bytes_read.sum + dram__bytes_write.sum); None = not captured.
-NCU_TRAFFIC_BYTES = {"si512_dzp": 13.608e9 + 1.584e9}   # profiles/r01c_ncu_summary.md, gint_vlocal_kernel
+NCU_TRAFFIC_BYTES = {"si512_dzp": 13.094e9 + 1.565e9}   # profiles/r01d_ncu_summary.md, gint_vlocal_kernel
 
 
 def measured_peaks():
@@ -146,7 +146,7 @@ def main():
     ap.add_argument("--workload", default="si512_dzp")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--ref-atoms", type=int, default=0,
-                    help="row atoms in the oracle sample (default: 128 for the cpu_baseline leg, 32 per step for --impl reference)")
+                    help="row atoms in the oracle sample (default: 256 for the cpu_baseline leg, 32 per step for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -305,7 +305,7 @@ def main():
         "roofline": roofline,
     }
     if not args.no_cpu_baseline and world == 1:
-        na = min(w.natom, args.ref_atoms or 128)
+        na = min(w.natom, args.ref_atoms or 256)
         dt, used, nblk, ntot = oracle_sample(w, na)
         cval = F_pt * na / w.natom / dt * 1e-12
         out["cpu_baseline"] = {
