@@ -191,3 +191,23 @@ def test_large_sampled_blocks(name, nsample):
         B = Hg[off[p]:off[p + 1]].reshape(norb[bj[b]], norb[bi[b]])
         assert np.array_equal(A, B.T)
     assert np.all(np.isfinite(Hg))
+
+
+def test_repeatability_stress():
+    """The contraction kernel is a producer/consumer pipeline (bulk copies, mbarrier rings, dynamic queue) whose
+    timing differs from call to call; 25 calls on the 64-atom workload must agree to rounding (the order of the
+    atomic adds is the only freedom), which a stale or early read of a ring stage would break."""
+    torch = _torch()
+    from paper_2603_21835_b200 import gint_setup, workloads as wl
+    w = wl.make("si64_dzp")
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos)
+    V = torch.from_numpy(w.V).cuda()
+    H0 = ctx.gint_vlocal(V).clone()
+    scale = float(H0.abs().max())
+    H = torch.empty_like(H0)
+    junk = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device="cuda")
+    for i in range(25):
+        if i % 3 == 0:
+            junk.normal_()          # perturb cache state and timing
+        ctx.gint_vlocal(V, H)
+        assert float((H - H0).abs().max()) <= 1e-12 * scale, "call %d differs" % i
