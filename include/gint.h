@@ -113,6 +113,20 @@ int gint_vlocal(gint_ctx *ctx, const double *V_dev, double *H_dev, void *stream)
  * gint_vlocal, copies H back, synchronises.  V_host [N1][N2][N3], H_host [h_len]. */
 int gint_vlocal_host(gint_ctx *ctx, const double *V_host, double *H_host);
 
+/* k-space assembly of the real-space blocks (the next step of the paper's workflow after cal_gint_vl):
+ *
+ *   H_mu,nu(k) = sum_R exp(i k.R) H_mu,nu(R)              -- PAPER.md:92-95 (Sec. 2.1, Eq. 5)
+ *
+ * with k = kfrac[0] b1 + kfrac[1] b2 + kfrac[2] b3, a_i . b_j = 2 pi delta_ij (so k.R = 2 pi kfrac . (R1,R2,R3)).
+ *   H_dev    device pointer, h_len doubles as written by gint_vlocal; read only
+ *   kfrac    HOST pointer, 3 doubles
+ *   Hk_dev   device pointer, [norb_tot][norb_tot] complex numbers as interleaved (re, im) doubles, row-major;
+ *            rows: orbitals of atom I (atoms in input order), columns: orbitals of atom J; OVERWRITTEN
+ * Asynchronous on `stream` (one memset, one kernel).  gint_num_orbitals returns norb_tot and, if `first` is not
+ * NULL, first[natom+1] = the first row/column of every atom (first[natom] = norb_tot). */
+int gint_num_orbitals(const gint_ctx *ctx, int64_t *norb_tot, int64_t *first);
+int gint_fold_k(gint_ctx *ctx, const double *H_dev, const double *kfrac, double *Hk_dev, void *stream);
+
 /* Per-kernel timing on the launch stream.  After gint_set_profiling(ctx, 1) every
  * gint_vlocal call records CUDA events around its kernels on `stream`;
  * gint_get_kernel_ms synchronises on the last call's events and returns durations in

@@ -134,3 +134,25 @@ def vlocal(lattice, ngrid, species, atom_species, atom_pos, V, blocks=None, nthr
     if return_threads:
         return out, (bi, bj, bR, off), rc
     return out, (bi, bj, bR, off)
+
+
+def fold_k(H_flat, blocks, norb_atom, kfrac) -> np.ndarray:
+    """H(k) = sum_R exp(i k.R) H(R)  -- PAPER.md:92-95 (Sec. 2.1, Eq. 5), the plain definition.
+
+    k = kfrac[0] b1 + kfrac[1] b2 + kfrac[2] b3 with a_i . b_j = 2 pi delta_ij, R = n1 a1 + n2 a2 + n3 a3, so
+    k.R = 2 pi (kfrac . n).  Returns the dense complex [norb_tot][norb_tot] matrix; rows are the orbitals of atom I
+    (atoms in input order, orbitals in block order), columns those of atom J.  Pinned by
+    tests/test_oracle_pins.py::test_bloch_sum_dense_gemm_cfg1 (Phi_k^dagger V dV Phi_k through a library GEMM).
+    """
+    bi, bj, bR, off = blocks
+    norb_atom = np.asarray(norb_atom, dtype=np.int64)
+    first = np.concatenate([[0], np.cumsum(norb_atom)])
+    n = int(first[-1])
+    Hk = np.zeros((n, n), dtype=np.complex128)
+    kf = np.asarray(kfrac, dtype=np.float64)
+    for b in range(len(bi)):
+        I, J = int(bi[b]), int(bj[b])
+        ph = np.exp(2j * np.pi * float(kf @ bR[b]))
+        Hk[first[I]:first[I + 1], first[J]:first[J + 1]] += ph * np.asarray(H_flat[off[b]:off[b + 1]]).reshape(
+            int(norb_atom[I]), int(norb_atom[J]))
+    return Hk

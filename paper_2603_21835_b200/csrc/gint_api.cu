@@ -19,6 +19,8 @@ struct gint_ctx {
     int device = -1;
     int nsm = 0;
     std::vector<void*> allocs;
+    gint::FoldPlan fold{};
+    std::vector<int64_t> first_orb;   // [natom+1]
     size_t psi_smem = 0, contract_smem = 0;
     bool profiling = false;
     bool have_events = false;
@@ -116,6 +118,11 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         delete ctx;
         return fail(GINT_ENOMEM, "host allocation failed");
     }
+    {
+        const gint::Plan& PP = ctx->plan;
+        ctx->first_orb.assign(1, 0);
+        for (int a = 0; a < natom; a++) ctx->first_orb.push_back(ctx->first_orb.back() + PP.species[PP.atom_species[a]].norb);
+    }
     if (cuda_device < 0) {   // host-only context
         *out = ctx;
         return GINT_OK;
@@ -152,6 +159,20 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     UP(P.tab_packed, &D.tab)
     UP(P.sp_meta, &D.sp_meta)
     UP(P.sp_real, &D.sp_real)
+    {   // block table for gint_fold_k
+        std::vector<int32_t> run_start, first32(ctx->first_orb.begin(), ctx->first_orb.end());
+        for (size_t b = 0; b < P.blk_i.size(); b++)
+            if (b == 0 || P.blk_i[b] != P.blk_i[b - 1] || P.blk_j[b] != P.blk_j[b - 1]) run_start.push_back((int32_t)b);
+        ctx->fold.nrun = (int32_t)run_start.size();
+        run_start.push_back((int32_t)P.blk_i.size());
+        ctx->fold.norb_tot = (int32_t)ctx->first_orb.back();
+        UP(P.blk_i, &ctx->fold.blk_i)
+        UP(P.blk_j, &ctx->fold.blk_j)
+        UP(P.blk_R, &ctx->fold.blk_R)
+        UP(P.blk_off, &ctx->fold.blk_off)
+        UP(run_start, &ctx->fold.run_start)
+        UP(first32, &ctx->fold.first)
+    }
 #undef UP
     void* ctr = nullptr;   // queue head (+ development timing area)
     if ((e = cudaMalloc(&ctr, 4 * 272 + 16 * 16 * 8 * 8 + 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
@@ -222,6 +243,21 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
                                         (size_t)ctx->plan.blk_off.back(), V_dev, H_dev,
                                         reinterpret_cast<cudaStream_t>(stream), ctx->profiling ? ctx->ev : nullptr);
     if (e != cudaSuccess) return fail_cuda(e, "gint_vlocal launch");
+    return GINT_OK;
+}
+
+int gint_num_orbitals(const gint_ctx* ctx, int64_t* norb_tot, int64_t* first) {
+    if (!ctx) return fail(GINT_EINVAL, "ctx is null");
+    if (norb_tot) *norb_tot = ctx->first_orb.back();
+    if (first) std::memcpy(first, ctx->first_orb.data(), ctx->first_orb.size() * sizeof(int64_t));
+    return GINT_OK;
+}
+
+int gint_fold_k(gint_ctx* ctx, const double* H_dev, const double* kfrac, double* Hk_dev, void* stream) {
+    if (!ctx || !H_dev || !kfrac || !Hk_dev) return fail(GINT_EINVAL, "null argument");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    cudaError_t e = gint::launch_fold(ctx->fold, H_dev, kfrac, Hk_dev, reinterpret_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "gint_fold_k launch");
     return GINT_OK;
 }
 

@@ -37,6 +37,18 @@ struct DevicePlan {
     int32_t never;            // always 0: a branch condition the compiler cannot fold (see DMMA_IF in gint_kernels.cu)
 };
 
+// k-space assembly (gint_fold.cu): the block table as the device needs it
+struct FoldPlan {
+    const int32_t* blk_i;      // [nblk]
+    const int32_t* blk_j;      // [nblk]
+    const int32_t* blk_R;      // [nblk][3]
+    const int64_t* blk_off;    // [nblk+1]
+    const int32_t* run_start;  // [nrun+1]: blocks run_start[r] .. run_start[r+1]-1 share (I, J)
+    const int32_t* first;      // [natom+1]: first orbital of each atom in the dense matrix
+    int32_t nrun, norb_tot;
+};
+cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac, double* Hk, cudaStream_t stream);
+
 size_t psi_kernel_smem(size_t table_bytes);
 size_t contract_kernel_smem(int nring);
 cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool tab_smem);

@@ -498,8 +498,9 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
                 for (int j = 0; j < 4; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
 
             uint32_t todo = cur->item.stage_mask;
+#ifdef GINT_TIMING
             int nvis = 0;
-            (void)nvis;
+#endif
             while (todo) {
                 const int s = __ffs(todo) - 1;
                 todo &= todo - 1;

@@ -211,3 +211,55 @@ def test_repeatability_stress():
             junk.normal_()          # perturb cache state and timing
         ctx.gint_vlocal(V, H)
         assert float((H - H0).abs().max()) <= 1e-12 * scale, "call %d differs" % i
+
+
+@pytest.mark.parametrize("kfrac", [(0.0, 0.0, 0.0), (0.31, -0.17, 0.43), (0.5, 0.25, -0.4)])
+def test_fold_k_against_oracle(cfg1, kfrac):
+    """H(k) = sum_R exp(i k.R) H(R) (Eq. 5) from the GPU blocks against the oracle's folding of the
+    same blocks, element by element; self-image blocks (several R per atom pair) are what cfg1 is for."""
+    torch = _torch()
+    import oracle
+    from helpers import norb_per_atom
+    Hg, ctx = gpu_H(cfg1)
+    Hk = ctx.gint_fold_k(torch.from_numpy(Hg).cuda(), kfrac)
+    torch.cuda.synchronize()
+    ref = oracle.fold_k(Hg, ctx.gint_get_blocks(), norb_per_atom(cfg1), kfrac)
+    n, first = ctx.gint_num_orbitals()
+    assert n == ref.shape[0] and np.array_equal(first, np.concatenate([[0], np.cumsum(norb_per_atom(cfg1))]))
+    got = Hk.cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+    assert np.abs(got - got.conj().T).max() <= 1e-13 * np.abs(ref).max()      # Hermitian: H(R) = H(-R)^T
+
+
+def test_fold_k_cluster_and_large():
+    """Two species with different orbital counts (cluster60, R = 0 only: H(k) is real and k-independent), and the
+    headline size: Gamma point of si512_dzp equals the plain block sum on sampled atom pairs."""
+    torch = _torch()
+    import oracle
+    from helpers import norb_per_atom
+    from paper_2603_21835_b200 import workloads as wl
+    w = wl.make("cluster60")
+    Hg, ctx = gpu_H(w)
+    Hd = torch.from_numpy(Hg).cuda()
+    a = ctx.gint_fold_k(Hd, (0.0, 0.0, 0.0)).cpu().numpy()
+    b = ctx.gint_fold_k(Hd, (0.37, 0.11, -0.29)).cpu().numpy()
+    ref = oracle.fold_k(Hg, ctx.gint_get_blocks(), norb_per_atom(w), (0.0, 0.0, 0.0))
+    assert np.abs(a - ref).max() <= 1e-13 * np.abs(ref).max() and np.array_equal(a, b) and np.all(a.imag == 0)
+    w = wl.make("si512_dzp")
+    Hg, ctx = gpu_H(w)
+    Hk = ctx.gint_fold_k(torch.from_numpy(Hg).cuda(), (0.25, 0.5, -0.125)).cpu().numpy()
+    bi, bj, bR, off = ctx.gint_get_blocks()
+    norb = norb_per_atom(w)
+    first = np.concatenate([[0], np.cumsum(norb)])
+    rng = np.random.default_rng(3)
+    scale = np.abs(Hg).max()
+    for b in rng.choice(len(bi), 200, replace=False):
+        I, J = int(bi[b]), int(bj[b])
+        sel = np.nonzero((bi == I) & (bj == J))[0]
+        ref = sum(np.exp(2j * np.pi * float(np.dot((0.25, 0.5, -0.125), bR[s]))) *
+                  Hg[off[s]:off[s + 1]].reshape(norb[I], norb[J]) for s in sel)
+        assert np.abs(Hk[first[I]:first[I + 1], first[J]:first[J + 1]] - ref).max() <= 1e-13 * scale
+    # an atom pair without any block stays zero
+    has = set(zip(bi.tolist(), bj.tolist()))
+    I, J = next((i, j) for i in range(w.natom) for j in range(w.natom) if (i, j) not in has)
+    assert np.all(Hk[first[I]:first[I + 1], first[J]:first[J + 1]] == 0)

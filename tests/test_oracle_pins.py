@@ -290,6 +290,9 @@ def test_bloch_sum_dense_gemm_cfg1(cfg1, cfg1_oracle, kfrac):
     ref = Phi.conj().T @ (Phi * (w.V.reshape(-1, 1) * dV))
     assert np.abs(Hk - ref).max() <= 1e-13 * np.abs(ref).max()
     assert np.abs(Hk - Hk.conj().T).max() <= 1e-13 * np.abs(ref).max()
+    # the oracle's own k-folding (Eq. 5) is pinned by the same library GEMM
+    Hk2 = oracle.fold_k(H, blocks, norb, kfrac)
+    assert np.abs(Hk2 - ref).max() <= 1e-13 * np.abs(ref).max()
 
 
 def test_gram_matrix_is_psd_and_negative_V_gives_nsd(cfg1):
