@@ -32,6 +32,9 @@ def _load():
         lib.orc_vlocal.restype = ctypes.c_int
         lib.orc_vlocal.argtypes = [c_dp, c_ip, ctypes.c_int, c_dp, c_dp, c_ip, c_ip, c_ip, c_dp, ctypes.c_int, c_ip,
                                    c_dp, c_dp, ctypes.c_int64, c_i32p, c_i32p, c_i32p, c_i64p, c_dp, ctypes.c_int]
+        lib.orc_rho.restype = ctypes.c_int
+        lib.orc_rho.argtypes = [c_dp, c_ip, ctypes.c_int, c_dp, c_dp, c_ip, c_ip, c_ip, c_dp, ctypes.c_int, c_ip, c_dp,
+                                ctypes.c_int64, c_i32p, c_i32p, c_i32p, c_i64p, c_dp, c_dp, ctypes.c_int]
         _lib = lib
     return _lib
 
@@ -156,3 +159,28 @@ def fold_k(H_flat, blocks, norb_atom, kfrac) -> np.ndarray:
         Hk[first[I]:first[I + 1], first[J]:first[J + 1]] += ph * np.asarray(H_flat[off[b]:off[b + 1]]).reshape(
             int(norb_atom[I]), int(norb_atom[J]))
     return Hk
+
+
+def rho(lattice, ngrid, species, atom_species, atom_pos, D_flat, blocks, nthreads: int = 0) -> np.ndarray:
+    """Charge density on the mesh from density-matrix blocks (Eq. 44).
+    `blocks` = (iat, jat, R, offset) as returned by vlocal/enumerate_blocks; D_flat has the H layout."""
+    lib = _load()
+    lattice = np.ascontiguousarray(lattice, dtype=np.float64)
+    ngrid_c = np.ascontiguousarray(ngrid, dtype=np.intc)
+    pos = np.ascontiguousarray(atom_pos, dtype=np.float64)
+    asp = np.ascontiguousarray(atom_species, dtype=np.intc)
+    sp = _SpeciesPack(species)
+    bi = np.ascontiguousarray(blocks[0], dtype=np.int32)
+    bj = np.ascontiguousarray(blocks[1], dtype=np.int32)
+    bR = np.ascontiguousarray(blocks[2], dtype=np.int32).reshape(-1, 3)
+    off = np.ascontiguousarray(blocks[3], dtype=np.int64)
+    D = np.ascontiguousarray(D_flat, dtype=np.float64)
+    assert D.shape[0] == int(off[-1])
+    out = np.zeros(tuple(int(x) for x in ngrid_c), dtype=np.float64)
+    rc = lib.orc_rho(_p(lattice, ctypes.c_double), _p(ngrid_c, ctypes.c_int), *sp.args(), int(pos.shape[0]),
+                     _p(asp, ctypes.c_int), _p(pos, ctypes.c_double), int(bi.shape[0]), _p(bi, ctypes.c_int32),
+                     _p(bj, ctypes.c_int32), _p(bR, ctypes.c_int32), _p(off, ctypes.c_int64), _p(D, ctypes.c_double),
+                     _p(out, ctypes.c_double), int(nthreads))
+    if rc < 0:
+        raise RuntimeError("orc_rho failed: %d" % rc)
+    return out

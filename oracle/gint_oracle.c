@@ -347,3 +347,101 @@ int orc_vlocal(const double *lattice, const int *ngrid, int nspecies, const doub
     free(gstart);
     return err ? -5 : used;
 }
+
+/* ---- public: charge density on the mesh -----------------------------------
+ *   rho(r_g) = sum_{R,R'} sum_{mu,nu} rho_mu,nu(R) phi_mu(r_g - tau_I - R')
+ *                                     phi_nu(r_g - tau_J - R - R')
+ *       -- PAPER.md:384-391 (Sec. 3.3.1, Eq. 44)
+ * written out: for every block (I,J,R) and every UNWRAPPED mesh point n (the
+ * sum over R' is the sum over the unwrapped points that fold onto g = n mod N)
+ * inside both spheres, add D_mu,nu phi_mu(r_n - tau_I) phi_nu(r_n - tau_J - R)
+ * to rho[n mod N].  D holds the listed blocks back to back (same layout as H).
+ * blocks must be grouped by bi.  rho[N1][N2][N3] is overwritten.
+ * Pinned in tests/test_oracle_pins.py by the adjoint identity
+ *   sum_g V(g) rho(g) dV = sum_blocks D : H[V]   (H from orc_vlocal)
+ * and by a brute-force sum on a tiny cell.  Returns threads used or <0.      */
+int orc_rho(const double *lattice, const int *ngrid, int nspecies, const double *sp_rcut, const double *sp_dr,
+            const int *sp_ntab, const int *sp_nrad, const int *sp_l, const double *sp_table, int natom_unused,
+            const int *atom_species, const double *pos, int64_t nblk, const int32_t *bi, const int32_t *bj,
+            const int32_t *bR, const int64_t *d_off, const double *D, double *rho, int nthreads)
+{
+    orc_species sp[16];
+    (void)natom_unused;
+    if (nspecies > 16) return -1;
+    unpack_species(nspecies, sp_rcut, sp_dr, sp_ntab, sp_nrad, sp_l, sp_table, sp);
+    for (int s = 0; s < nspecies; s++)
+        if (sp[s].norb > ORC_MAX_ORB) return -2;
+    double inv[9];
+    double vol = fabs(det3(lattice));
+    if (vol < 1e-300) return -3;
+    inv3(lattice, inv);
+    double blen[3];
+    for (int i = 0; i < 3; i++) blen[i] = sqrt(inv[i] * inv[i] + inv[3 + i] * inv[3 + i] + inv[6 + i] * inv[6 + i]);
+    const int64_t N1 = ngrid[0], N2 = ngrid[1], N3 = ngrid[2];
+    for (int64_t i = 0; i < N1 * N2 * N3; i++) rho[i] = 0.0;
+
+    int64_t ngroup = 0;
+    int64_t *gstart = (int64_t *)malloc(sizeof(int64_t) * (size_t)(nblk + 1));
+    if (!gstart) return -4;
+    for (int64_t b = 0; b < nblk; b++)
+        if (b == 0 || bi[b] != bi[b - 1]) gstart[ngroup++] = b;
+    gstart[ngroup] = nblk;
+
+    int used = 1;
+    int err = 0;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+    }
+#pragma omp parallel for schedule(dynamic, 1)
+#endif
+    for (int64_t g = 0; g < ngroup; g++) {
+        const int I = bi[gstart[g]];
+        const orc_species *sI = &sp[atom_species[I]];
+        const double *tI = pos + 3 * (size_t)I;
+        int lo[3], hi[3];
+        for (int i = 0; i < 3; i++) {
+            double f = tI[0] * inv[i] + tI[1] * inv[3 + i] + tI[2] * inv[6 + i];
+            lo[i] = (int)floor((f - sI->rcut * blen[i]) * (double)ngrid[i]) - 1;
+            hi[i] = (int)ceil((f + sI->rcut * blen[i]) * (double)ngrid[i]) + 1;
+        }
+        double phiI[ORC_MAX_ORB], phiJ[ORC_MAX_ORB];
+        for (int n1 = lo[0]; n1 <= hi[0]; n1++)
+            for (int n2 = lo[1]; n2 <= hi[1]; n2++)
+                for (int n3 = lo[2]; n3 <= hi[2]; n3++) {
+                    double f1 = (double)n1 / (double)N1, f2 = (double)n2 / (double)N2, f3 = (double)n3 / (double)N3;
+                    double r[3], d[3];
+                    for (int c = 0; c < 3; c++) {
+                        r[c] = f1 * lattice[c] + f2 * lattice[3 + c] + f3 * lattice[6 + c];
+                        d[c] = r[c] - tI[c];
+                    }
+                    if (!phi_eval(sI, d, phiI)) continue;
+                    long double acc = 0.0L;
+                    for (int64_t b = gstart[g]; b < gstart[g + 1]; b++) {
+                        const int J = bj[b];
+                        const orc_species *sJ = &sp[atom_species[J]];
+                        for (int c = 0; c < 3; c++)
+                            d[c] = r[c] - (pos[3 * (size_t)J + c] + bR[3 * b] * lattice[c] + bR[3 * b + 1] * lattice[3 + c] +
+                                           bR[3 * b + 2] * lattice[6 + c]);
+                        if (!phi_eval(sJ, d, phiJ)) continue;
+                        const double *Db = D + d_off[b];
+                        for (int mu = 0; mu < sI->norb; mu++) {
+                            double t = 0.0;
+                            for (int nu = 0; nu < sJ->norb; nu++) t += Db[mu * sJ->norb + nu] * phiJ[nu];
+                            acc += (long double)(phiI[mu] * t);
+                        }
+                    }
+                    double *o = rho + (pmod(n1, N1) * N2 + pmod(n2, N2)) * N3 + pmod(n3, N3);
+                    double add = (double)acc;
+#ifdef _OPENMP
+#pragma omp atomic
+#endif
+                    *o += add;
+                }
+    }
+    free(gstart);
+    return err ? -5 : used;
+}

@@ -468,3 +468,87 @@ def test_golden_regression_cfg1(cfg1, cfg1_oracle):
     for I, J, a, b, c, mu, nu, val in lines:
         got = d[(int(I), int(J), int(a), int(b), int(c))][int(mu), int(nu)]
         assert abs(got - float(val)) <= 1e-15 * np.abs(H).max()
+
+
+# ---------------------------------------------------------------------------
+# charge density (Eq. 44): pins of oracle.rho
+# ---------------------------------------------------------------------------
+def test_rho_adjoint_of_vlocal(cfg1, cfg1_oracle):
+    """sum_g V(g) rho[D](g) dV = sum_blocks D : H[V] for ANY D (not symmetric) and ANY V: Eq. 44 is the adjoint of
+    Eq. 45, and H comes from the already pinned orc_vlocal.  A dropped image, a transposed block or a wrong R sign in
+    orc_rho breaks it (cfg1 has self-image blocks and several R per atom pair)."""
+    w = cfg1
+    H0, blocks = cfg1_oracle
+    rng = np.random.default_rng(11)
+    dV = abs(np.linalg.det(w.lattice)) / np.prod(w.ngrid)
+    for trial in range(3):
+        D = rng.normal(size=H0.shape)
+        V = rng.normal(size=w.V.shape)
+        HV, _ = oracle.vlocal(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, V)
+        r = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blocks)
+        lhs, rhs = float((V * r).sum() * dV), float((D * HV).sum())
+        assert abs(lhs - rhs) <= 1e-12 * np.abs(D).sum() * np.abs(HV).max()
+
+
+def test_rho_brute_force_tiny():
+    """Eq. 44 written out with explicit image sums R, R' in {-2..2}^3 on a tiny triclinic cell (numpy loops over the
+    oracle's own phi only): rho(g) = sum_{I,J,R,R'} phi_I(r_g - tau_I - R')^T D(I,J,R) phi_J(r_g - tau_J - R - R')."""
+    w = wl.tiny(seed=9, natom=2, ngrid=(6, 5, 7))
+    H, blocks = oracle.vlocal(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V)
+    bi, bj, bR, off = blocks
+    rng = np.random.default_rng(2)
+    D = rng.normal(size=H.shape)
+    got = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blocks)
+    pts = mesh_points(w.lattice, w.ngrid)
+    norb = norb_per_atom(w)
+    ref = np.zeros(len(pts))
+    rng_img = range(-2, 3)
+    phi_img = {}
+    for I in range(w.natom):
+        for a in rng_img:
+            for b in rng_img:
+                for c in rng_img:
+                    Rv = np.array([a, b, c]) @ w.lattice
+                    phi_img[(I, a, b, c)] = oracle.phi(w.species, int(w.atom_species[I]), pts - w.atom_pos[I] - Rv)
+    for blk in range(len(bi)):
+        I, J = int(bi[blk]), int(bj[blk])
+        Dm = D[off[blk]:off[blk + 1]].reshape(norb[I], norb[J])
+        for a in rng_img:
+            for b in rng_img:
+                for c in rng_img:
+                    key = (J, a + int(bR[blk, 0]), b + int(bR[blk, 1]), c + int(bR[blk, 2]))
+                    if key not in phi_img:
+                        # image outside the explicit window: it must not reach any mesh point of the cell
+                        Rv = np.array(key[1:]) @ w.lattice
+                        assert not np.any(oracle.phi(w.species, int(w.atom_species[J]), pts - w.atom_pos[J] - Rv))
+                        continue
+                    ref += np.einsum("pm,mn,pn->p", phi_img[(I, a, b, c)], Dm, phi_img[key])
+    assert np.abs(got.ravel() - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+def test_rho_of_single_element_and_symmetry(cfg1, cfg1_oracle):
+    """D with one non-zero element gives the product of two orbitals (sum over images); the partner block (J,I,-R)
+    with the transposed matrix gives the same density."""
+    w = cfg1
+    H0, blocks = cfg1_oracle
+    bi, bj, bR, off = blocks
+    norb = norb_per_atom(w)
+    b = int(np.nonzero((bi == 0) & (bj == 3))[0][0])
+    D = np.zeros_like(H0)
+    D[off[b] + 1 * norb[3] + 2] = 1.0            # mu = 1 of atom 0, nu = 2 of atom 3
+    r1 = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blocks)
+    p = int(np.nonzero((bi == 3) & (bj == 0) & np.all(bR == -bR[b], axis=1))[0][0])
+    D2 = np.zeros_like(H0)
+    D2[off[p] + 2 * norb[0] + 1] = 1.0
+    r2 = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D2, blocks)
+    assert np.abs(r1).max() > 0 and np.abs(r1 - r2).max() <= 1e-14 * np.abs(r1).max()
+    pts = mesh_points(w.lattice, w.ngrid)
+    ref = np.zeros(len(pts))
+    for a in range(-2, 3):
+        for b_ in range(-2, 3):
+            for c in range(-2, 3):
+                Rp = np.array([a, b_, c]) @ w.lattice
+                RJ = (np.array([a, b_, c]) + bR[b]) @ w.lattice
+                ref += oracle.phi(w.species, int(w.atom_species[0]), pts - w.atom_pos[0] - Rp)[:, 1] * \
+                    oracle.phi(w.species, int(w.atom_species[3]), pts - w.atom_pos[3] - RJ)[:, 2]
+    assert np.abs(r1.ravel() - ref).max() <= 1e-13 * np.abs(ref).max()
