@@ -113,6 +113,18 @@ int gint_vlocal(gint_ctx *ctx, const double *V_dev, double *H_dev, void *stream)
  * gint_vlocal, copies H back, synchronises.  V_host [N1][N2][N3], H_host [h_len]. */
 int gint_vlocal_host(gint_ctx *ctx, const double *V_host, double *H_host);
 
+/* Charge density on the mesh from density-matrix blocks (the paper's cal_gint_rho):
+ *
+ *   rho(r_g) = sum_{R,R'} sum_{mu,nu} rho_mu,nu(R) phi_mu(r_g - tau_I - R') phi_nu(r_g - tau_J - R - R')
+ *                                                          -- PAPER.md:384-391 (Sec. 3.3.1, Eq. 44)
+ *   D_dev    device pointer, h_len doubles: the blocks rho_mu,nu(I,J,R) in exactly the layout of H (every block of
+ *            the table is used as given; no symmetry of D is assumed); read only
+ *   rho_dev  device pointer, [N1][N2][N3] doubles; OVERWRITTEN
+ * Asynchronous on `stream` (one memset, two kernels; reuses the context's psi scratch, so it must not overlap a
+ * gint_vlocal call on another stream).  First cut: FP64 FMA, not yet on the tensor pipe.  Returns GINT_EUNSUPPORTED
+ * if a region lists more orbitals than fit one stage in shared memory. */
+int gint_rho(gint_ctx *ctx, const double *D_dev, double *rho_dev, void *stream);
+
 /* k-space assembly of the real-space blocks (the next step of the paper's workflow after cal_gint_vl):
  *
  *   H_mu,nu(k) = sum_R exp(i k.R) H_mu,nu(R)              -- PAPER.md:92-95 (Sec. 2.1, Eq. 5)

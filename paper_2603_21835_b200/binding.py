@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgint_b200.so")
 GINT_OK, GINT_EINVAL, GINT_EUNSUPPORTED, GINT_ENOMEM, GINT_ECUDA, GINT_ENODEVICE = 0, -1, -2, -3, -4, -5
 
 EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
-            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
+            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_rho", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
@@ -62,6 +62,8 @@ def _load() -> ctypes.CDLL:
     lib.gint_num_orbitals.argtypes = [vp, P(i64), P(i64)]
     lib.gint_fold_k.restype = ctypes.c_int
     lib.gint_fold_k.argtypes = [vp, vp, P(dbl), vp, vp]
+    lib.gint_rho.restype = ctypes.c_int
+    lib.gint_rho.argtypes = [vp, vp, vp, vp]
     lib.gint_get_stats.restype = ctypes.c_int
     lib.gint_get_stats.argtypes = [vp, P(dbl), i32]
     lib.gint_set_profiling.restype = ctypes.c_int
@@ -162,6 +164,20 @@ class GintContext:
         _check(_lib.gint_vlocal(self._h, ctypes.c_void_p(V_dev.data_ptr()), ctypes.c_void_p(H_dev.data_ptr()),
                                 ctypes.c_void_p(s)), "gint_vlocal")
         return H_dev
+
+    def gint_rho(self, D_dev, rho_dev=None, stream=None):
+        """rho(r_g) of Eq. 44 from density-matrix blocks D_dev (H layout); returns a CUDA float64 tensor [N1][N2][N3]."""
+        import torch
+        if not (D_dev.is_cuda and D_dev.dtype == torch.float64 and D_dev.is_contiguous() and D_dev.numel() == self.h_len):
+            raise ValueError("D_dev must be a contiguous CUDA float64 tensor of h_len elements")
+        if rho_dev is None:
+            rho_dev = torch.empty(self.ngrid, dtype=torch.float64, device=D_dev.device)
+        if not (rho_dev.is_cuda and rho_dev.dtype == torch.float64 and rho_dev.is_contiguous() and tuple(rho_dev.shape) == self.ngrid):
+            raise ValueError("rho_dev must be a contiguous CUDA float64 tensor [N1][N2][N3]")
+        s = torch.cuda.current_stream(D_dev.device).cuda_stream if stream is None else int(stream)
+        _check(_lib.gint_rho(self._h, ctypes.c_void_p(D_dev.data_ptr()), ctypes.c_void_p(rho_dev.data_ptr()),
+                             ctypes.c_void_p(s)), "gint_rho")
+        return rho_dev
 
     def gint_num_orbitals(self):
         """(norb_tot, first[natom+1]) of the dense k-space matrix."""

@@ -21,7 +21,8 @@ struct gint_ctx {
     std::vector<void*> allocs;
     gint::FoldPlan fold{};
     std::vector<int64_t> first_orb;   // [natom+1]
-    size_t psi_smem = 0, contract_smem = 0;
+    size_t psi_smem = 0, contract_smem = 0, rho_smem = 0;
+    bool rho_ok = false;
     bool profiling = false;
     bool have_events = false;
     cudaEvent_t ev[5];
@@ -154,6 +155,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     UP(P.entries, &D.entries)
     UP(P.etasks, &D.etasks)
     UP(P.pair, &D.pair)
+    UP(P.pair_direct, &D.pair_direct)
     UP(P.slot_xyz, &D.slot_xyz)
     UP(P.mirror, &D.mirror)
     UP(P.tab_packed, &D.tab)
@@ -214,6 +216,16 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         release(ctx);
         return fail_cuda(e, "cudaFuncSetAttribute");
     }
+    {   // gint_rho stages one 32-point stage of every row group of a region in shared memory
+        int max_groups = 1;
+        for (const gint::Region& r : P.regions) max_groups = r.ngroup > max_groups ? r.ngroup : max_groups;
+        const size_t need = ((size_t)max_groups * gint::kChunkDoubles + 256) * sizeof(double);
+        ctx->rho_ok = need <= (size_t)prop.sharedMemPerBlockOptin && gint::kStagePts == 32;
+        if (ctx->rho_ok && (e = gint::configure_rho(&ctx->rho_smem, max_groups)) != cudaSuccess) {
+            release(ctx);
+            return fail_cuda(e, "cudaFuncSetAttribute (rho)");
+        }
+    }
     *out = ctx;
     return GINT_OK;
 }
@@ -243,6 +255,18 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
                                         (size_t)ctx->plan.blk_off.back(), V_dev, H_dev,
                                         reinterpret_cast<cudaStream_t>(stream), ctx->profiling ? ctx->ev : nullptr);
     if (e != cudaSuccess) return fail_cuda(e, "gint_vlocal launch");
+    return GINT_OK;
+}
+
+int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* stream) {
+    if (!ctx || !D_dev || !rho_dev) return fail(GINT_EINVAL, "null argument");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    if (!ctx->rho_ok) return fail(GINT_EUNSUPPORTED, "too many orbitals listed for one region for gint_rho; use a smaller bcell");
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    cudaError_t e = gint::launch_psi(ctx->dev, ctx->psi_smem, ctx->plan.tables_in_smem, ctx->nsm, nullptr, st);
+    if (e != cudaSuccess) return fail_cuda(e, "gint_rho psi launch");
+    e = gint::launch_rho_kernel(ctx->dev, ctx->rho_smem, ctx->nsm, D_dev, rho_dev, st);
+    if (e != cudaSuccess) return fail_cuda(e, "gint_rho launch");
     return GINT_OK;
 }
 

@@ -18,6 +18,7 @@ struct DevicePlan {
     const Entry* entries;
     const uint32_t* etasks;   // evaluation tasks: entry within region | slice << 16
     const uint32_t* pair;
+    const uint32_t* pair_direct;   // (entry a, entry b) -> offset of block (I_a, I_b, R_b - R_a) (gint_rho)
     const uint8_t* slot_xyz;  // [nslice*32][4]
     const double* tab;        // packed radial tables, per species [ntab+4][nradp]
     const int32_t* sp_meta;   // per species 12 ints: tab_offset, ntab, nradp, norb, l[8]
@@ -47,6 +48,9 @@ struct FoldPlan {
     const int32_t* first;      // [natom+1]: first orbital of each atom in the dense matrix
     int32_t nrun, norb_tot;
 };
+cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream);
+cudaError_t launch_rho_kernel(const DevicePlan& P, size_t smem, int nsm, const double* D, double* rho, cudaStream_t stream);
+cudaError_t configure_rho(size_t* smem_out, int max_groups);
 cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac, double* Hk, cudaStream_t stream);
 
 size_t psi_kernel_smem(size_t table_bytes);

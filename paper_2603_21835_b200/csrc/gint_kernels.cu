@@ -333,8 +333,8 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
             const uchar4 c = s_xyz[p];
             const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
             double wv = 0.0;
-            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])
-                wv = __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV;
+            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])   // V == nullptr: plain phi (gint_rho)
+                wv = V ? __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV : 1.0;
             s_sqrtw[p] = sqrt(fabs(wv));
             const unsigned int neg = __ballot_sync(0xffffffffu, wv < 0.0);
             if (lane == 0)   // every work item of the region carries the sign bits in its descriptor
@@ -707,6 +707,16 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_
     }
     if (ev) cudaEventRecord(ev[4], stream);
     return e;
+}
+
+cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream) {
+    if (P.nitems <= 0) return cudaSuccess;
+    const int pgrid = P.nwork_regions < 3 * nsm ? P.nwork_regions : 3 * nsm;
+    if (tab_smem)
+        gint_psi_kernel<true><<<pgrid, kEvalThreads, psi_smem, stream>>>(P, V);
+    else
+        gint_psi_kernel<false><<<pgrid, kEvalThreads, psi_smem, stream>>>(P, V);
+    return cudaGetLastError();
 }
 
 // ---- FP64 tensor peak: register-resident DMMA.8x8x4 loop --------------------------------

@@ -440,6 +440,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             }
         // pair table: (row entry a <= column entry b) -> canonical block offset (+ transposed flag)
         P.pair.resize(P.pair.size() + (size_t)m * m, kNoBlock);
+        P.pair_direct.resize(P.pair.size(), kNoBlock);
         for (int a = 0; a < m; a++)
             for (int b = a; b < m; b++) {
                 const Entry& ea = P.entries[pos + a];
@@ -453,6 +454,8 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 uint32_t off = canonical ? lookup(ea.atom, eb.atom, r1, r2, r3) : lookup(eb.atom, ea.atom, -r1, -r2, -r3);
                 if (off != kNoBlock && !canonical) off |= kPairTransposed;
                 P.pair[(size_t)R.pair_off + (size_t)a * m + b] = off;
+                P.pair_direct[(size_t)R.pair_off + (size_t)a * m + b] = lookup(ea.atom, eb.atom, r1, r2, r3);
+                P.pair_direct[(size_t)R.pair_off + (size_t)b * m + a] = lookup(eb.atom, ea.atom, -r1, -r2, -r3);
             }
         // tiles (group gi <= gj) and their cost (DMMAs) per stage
         // the kernel decides per k-pair (2 k-steps, a 2x2x2 box of mesh points): a fragment pair is

@@ -174,6 +174,7 @@ struct Plan {
     std::vector<uint8_t> gmask;
     std::vector<uint32_t> rowinfo;
     std::vector<uint32_t> pair;
+    std::vector<uint32_t> pair_direct;          // same indexing: offset of block (I_a, I_b, R_b - R_a) itself, any order (gint_rho)
     std::vector<WorkItem> items;
     std::vector<ItemDesc> descs;                // one per work item, queue order
     std::vector<uint32_t> etasks;               // evaluation tasks, region-major

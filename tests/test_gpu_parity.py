@@ -263,3 +263,94 @@ def test_fold_k_cluster_and_large():
     has = set(zip(bi.tolist(), bj.tolist()))
     I, J = next((i, j) for i in range(w.natom) for j in range(w.natom) if (i, j) not in has)
     assert np.all(Hk[first[I]:first[I + 1], first[J]:first[J + 1]] == 0)
+
+
+def gpu_rho(w, D, **kw):
+    torch = _torch()
+    from paper_2603_21835_b200 import gint_setup
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=0, **kw)
+    r = ctx.gint_rho(torch.from_numpy(np.ascontiguousarray(D)).cuda())
+    torch.cuda.synchronize()
+    return r.cpu().numpy(), ctx
+
+
+def test_rho_cfg1_and_tiny(cfg1, cfg1_oracle):
+    """Charge density (Eq. 44) against the oracle, element by element, with a random NON-symmetric
+    D: cfg1 (self-image blocks), ragged triclinic meshes, then a gint_vlocal call on the same context (shared psi
+    scratch) still matches."""
+    import oracle
+    from paper_2603_21835_b200 import workloads as wl
+    rng = np.random.default_rng(21)
+    H0, blocks = cfg1_oracle
+    D = rng.normal(size=H0.shape)
+    ref = oracle.rho(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, D, blocks)
+    got, ctx = gpu_rho(cfg1, D)
+    assert np.abs(got - ref).max() <= TOL * np.abs(ref).max()
+    torch = _torch()
+    H = ctx.gint_vlocal(torch.from_numpy(cfg1.V).cuda())
+    assert_parity(H.cpu().numpy(), H0, "vlocal after rho")
+    for seed, ngrid in [(7, (12, 10, 14)), (11, (9, 13, 7))]:
+        w = wl.tiny(seed=seed, ngrid=ngrid)
+        Hr, blk = oracle_H(w)
+        D = rng.normal(size=Hr.shape)
+        ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blk)
+        got, _ = gpu_rho(w, D)
+        assert np.abs(got - ref).max() <= TOL * np.abs(ref).max()
+
+
+def test_rho_cfg2_and_cluster():
+    import oracle
+    from paper_2603_21835_b200 import workloads as wl
+    rng = np.random.default_rng(22)
+    for name in ("si64_dzp", "cluster60"):
+        w = wl.make(name)
+        bi, bj, bR, off = oracle.enumerate_blocks(w.lattice, w.species, w.atom_species, w.atom_pos)
+        D = rng.normal(size=int(off[-1]))
+        ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, (bi, bj, bR, off))
+        got, ctx = gpu_rho(w, D)
+        assert np.array_equal(ctx.gint_get_blocks()[3], off)
+        assert np.abs(got - ref).max() <= TOL * np.abs(ref).max(), name
+
+
+def test_rho_large_sampled_points_and_adjoint():
+    """si512_dzp at full size: 40 sampled mesh points recomputed one by one from Eq. 44 with the oracle's phi (numpy
+    image loops), and the adjoint identity sum_g V rho dV = D : H[V] over the whole mesh (H from gint_vlocal)."""
+    torch = _torch()
+    import oracle
+    from helpers import norb_per_atom
+    from paper_2603_21835_b200 import gint_setup, workloads as wl
+    w = wl.make("si512_dzp")
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos)
+    rng = np.random.default_rng(23)
+    D = rng.normal(size=ctx.h_len)
+    Dd = torch.from_numpy(D).cuda()
+    rho = ctx.gint_rho(Dd)
+    Vd = torch.from_numpy(w.V).cuda()
+    H = ctx.gint_vlocal(Vd)
+    dV = abs(np.linalg.det(w.lattice)) / np.prod(w.ngrid)
+    lhs, rhs = float((Vd * rho).sum()) * dV, float((Dd * H).sum())
+    assert abs(lhs - rhs) <= 1e-10 * float(H.abs().max()) * np.abs(D).sum()
+    rho = rho.cpu().numpy()
+    bi, bj, bR, off = ctx.gint_get_blocks()
+    key = {(int(bi[b]), int(bj[b]), int(bR[b, 0]), int(bR[b, 1]), int(bR[b, 2])): b for b in range(len(bi))}
+    norb = norb_per_atom(w)
+    n = np.array(w.ngrid)
+    scale = np.abs(rho).max()
+    shifts = np.array([[a, b, c] for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)])
+    for g in rng.integers(0, n, size=(40, 3)):
+        r = (g / n) @ w.lattice
+        ents = []      # (atom, image shift R', phi values) of every image that reaches the point
+        for s in shifts:
+            d = r - w.atom_pos - s @ w.lattice
+            for I in np.nonzero(np.einsum("ij,ij->i", d, d) < max(sp.rcut for sp in w.species) ** 2)[0]:
+                ph = oracle.phi(w.species, int(w.atom_species[I]), d[I:I + 1])[0]
+                if np.any(ph):
+                    ents.append((int(I), s, ph))
+        ref = 0.0
+        for I, sa, pa in ents:
+            for J, sb, pb in ents:
+                R = sb - sa
+                b = key.get((I, J, int(R[0]), int(R[1]), int(R[2])))
+                if b is not None:
+                    ref += pa @ D[off[b]:off[b + 1]].reshape(norb[I], norb[J]) @ pb
+        assert abs(rho[tuple(g)] - ref) <= TOL * scale
