@@ -254,7 +254,7 @@ def main():
     e2e_val = F_sym / (e2e_ms * 1e-3) * 1e-12
 
     # ---- next step of the workflow, outside the headline: H(k) = sum_R exp(i k.R) H(R) (Eq. 5) -------------
-    fold = None
+    fold = rho_info = None
     if world == 1:
         ntot = ctx.gint_num_orbitals()[0]
         Hk = torch.empty((ntot, ntot), dtype=torch.complex128, device=dev)
@@ -272,6 +272,19 @@ def main():
         fold = {"ms_per_call": fold_ms, "algorithmic_bytes": fold_bytes, "achieved_gbs": fold_bytes / (fold_ms * 1e-3) * 1e-9,
                 "norb_tot": ntot, "note": "gint_fold_k: H blocks read once, dense complex H(k) written once (memset + kernel)"}
         del Hk
+        # charge density (Eq. 44), first cut
+        Dm = torch.randn(ctx.h_len, dtype=torch.float64, device=dev)
+        rho = ctx.gint_rho(Dm)
+        torch.cuda.synchronize()
+        f0.record()
+        for _ in range(2):
+            ctx.gint_rho(Dm, rho)
+        f1.record()
+        torch.cuda.synchronize()
+        rho_ms = f0.elapsed_time(f1) / 2
+        rho_info = {"ms_per_call": rho_ms, "useful_flops": F_pt, "achieved_tflops": F_pt / (rho_ms * 1e-3) * 1e-12,
+                    "note": "gint_rho first cut (FP64 FMA, ordered entry pairs: F_pt accounting), includes its psi kernel"}
+        del Dm, rho
 
     if rank != 0:
         if world > 1:
@@ -328,6 +341,9 @@ def main():
         fold["peak_gbs"] = peaks["hbm_gbs"]
         fold["frac"] = fold["achieved_gbs"] / peaks["hbm_gbs"]
         out["fold_k"] = fold
+        rho_info["peak_tflops"] = peak
+        rho_info["frac"] = rho_info["achieved_tflops"] / peak
+        out["rho"] = rho_info
     if not args.no_cpu_baseline and world == 1:
         na = min(w.natom, args.ref_atoms or 256)
         dt, used, nblk, ntot = oracle_sample(w, na)

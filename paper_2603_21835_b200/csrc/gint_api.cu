@@ -217,10 +217,13 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         return fail_cuda(e, "cudaFuncSetAttribute");
     }
     {   // gint_rho stages one 32-point stage of every row group of a region in shared memory
-        int max_groups = 1;
-        for (const gint::Region& r : P.regions) max_groups = r.ngroup > max_groups ? r.ngroup : max_groups;
-        const size_t need = ((size_t)max_groups * gint::kChunkDoubles + 256) * sizeof(double);
-        ctx->rho_ok = need <= (size_t)prop.sharedMemPerBlockOptin && gint::kStagePts == 32;
+        int max_groups = 1, max_entries = 0;
+        for (const gint::Region& r : P.regions) {
+            max_groups = r.ngroup > max_groups ? r.ngroup : max_groups;
+            max_entries = r.nentry > max_entries ? r.nentry : max_entries;
+        }
+        const size_t need = ((size_t)max_groups * gint::kGroupRows * 33 + 256 + 8 * 256) * sizeof(double) + 64 * 16 + 64 * 64 * 4;
+        ctx->rho_ok = need <= (size_t)prop.sharedMemPerBlockOptin && gint::kStagePts == 32 && max_entries <= 64;
         if (ctx->rho_ok && (e = gint::configure_rho(&ctx->rho_smem, max_groups)) != cudaSuccess) {
             release(ctx);
             return fail_cuda(e, "cudaFuncSetAttribute (rho)");
@@ -261,7 +264,7 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
 int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* stream) {
     if (!ctx || !D_dev || !rho_dev) return fail(GINT_EINVAL, "null argument");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
-    if (!ctx->rho_ok) return fail(GINT_EUNSUPPORTED, "too many orbitals listed for one region for gint_rho; use a smaller bcell");
+    if (!ctx->rho_ok) return fail(GINT_EUNSUPPORTED, "too many orbitals or atom images listed for one region for gint_rho; use a smaller bcell");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     cudaError_t e = gint::launch_psi(ctx->dev, ctx->psi_smem, ctx->plan.tables_in_smem, ctx->nsm, nullptr, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho psi launch");

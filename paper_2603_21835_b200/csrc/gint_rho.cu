@@ -19,18 +19,16 @@ namespace gint {
 namespace {
 constexpr int kRhoThreads = 256;
 constexpr int kRhoWarps = kRhoThreads / 32;
-static_assert(kStagePts == 32, "gint_rho_kernel assumes 32-point stages (one lane per point)");
+static_assert(kStagePts == 32 && kStagePairs == 4, "gint_rho_kernel assumes 32-point stages (one lane per point)");
 
-// element (row R, point lane) of a (group, stage) chunk in DMMA fragment order (see gint_kernels.cu)
-__device__ __forceinline__ int chunk_index(int R, int lane) {
-    return (R >> 5) * kChunkDoubles + ((((R >> 3) & 3) * kStagePairs + (lane >> 3)) * 32 + (R & 7) * 4 + (lane & 3)) * 2 +
-           ((lane >> 2) & 1);
-}
+constexpr int kMaxEntries = 64;   // entries of a region whose info and pair table are staged in shared memory
+constexpr int kMaxBlock = 256;   // D blocks up to 16 x 16 orbitals are staged per warp in shared memory
+constexpr int kRowLD = 33;   // shared-memory row stride in doubles: conflict-free for the transposing store and the reads
 }  // namespace
 
 __global__ void __launch_bounds__(kRhoThreads) gint_rho_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__ D,
                                                                double* __restrict__ rho) {
-    extern __shared__ __align__(16) double s_phi[];   // [ngroup][1024] + [8 warps][32] partial sums
+    extern __shared__ __align__(16) double s_phi[];   // [ngroup * 32 rows][33] (row = orbital, column = mesh point) + [8 warps][32] partial sums
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nst = P.nstage;
     for (int unit = blockIdx.x; unit < P.nwork_regions * nst; unit += gridDim.x) {
@@ -40,31 +38,92 @@ __global__ void __launch_bounds__(kRhoThreads) gint_rho_kernel(const __grid_cons
         const Entry* entries = P.entries + __ldg(&reg->entry0);
         const uint32_t* pdir = P.pair_direct + __ldg(&reg->pair_off);
         const double* psi = P.psi + ((size_t)__ldg(&reg->psi_chunk0) + st) * kChunkDoubles;
-        double* s_part = s_phi + (size_t)ngroup * kChunkDoubles;
+        double* s_part = s_phi + (size_t)ngroup * kGroupRows * kRowLD;
         __syncthreads();   // previous unit done with shared memory
+        // stage phi of the stage's 32 points, transposed out of the DMMA fragment order (gint_kernels.cu: element
+        // j of a chunk is row 8 i + frow, point (2 kp + kk) 4 + fk with j = (((i 4 + kp) 32 + frow 4 + fk) 2 + kk)
         for (int g = 0; g < ngroup; g++) {
-            const double2* src = reinterpret_cast<const double2*>(psi + (size_t)g * nst * kChunkDoubles);
-            double2* dst = reinterpret_cast<double2*>(s_phi + (size_t)g * kChunkDoubles);
-            for (int i = tid; i < kChunkDoubles / 2; i += kRhoThreads) dst[i] = src[i];
+            const double* src = psi + (size_t)g * nst * kChunkDoubles;
+            for (int j = tid; j < kChunkDoubles; j += kRhoThreads) {
+                const int kk = j & 1, t = j >> 1, fk = t & 3, frow = (t >> 2) & 7, q = t >> 5, kp = q & 3, i = q >> 2;
+                s_phi[(g * kGroupRows + i * 8 + frow) * kRowLD + (2 * kp + kk) * 4 + fk] = src[j];
+            }
         }
+        // the region's entries (active on this stage?, orbitals, first row) and its pair table, once per unit
+        const int ks0 = st * kStageKsteps;   // the stage's 8 k-steps: one byte of the entries' k-step masks
+        int4* s_ent = reinterpret_cast<int4*>(s_part + kRhoWarps * 32 + kRhoWarps * kMaxBlock);
+        uint32_t* s_pdir = reinterpret_cast<uint32_t*>(s_ent + kMaxEntries);
+        for (int i = tid; i < m; i += kRhoThreads)
+            s_ent[i] = make_int4((int)((entries[i].kmask[ks0 >> 5] >> (ks0 & 31)) & 0xFFu), entries[i].norb, entries[i].row0, 0);
+        for (int i = tid; i < m * m; i += kRhoThreads) s_pdir[i] = __ldg(pdir + i);
         __syncthreads();
         double acc = 0.0;
-        const int ks0 = st * kStageKsteps;   // the stage's 8 k-steps: one byte of the entries' k-step masks
-        for (int t = warp; t < m * m; t += kRhoWarps) {
+        double* s_D = s_part + kRhoWarps * 32 + warp * kMaxBlock;   // this warp's copy of the current D block
+        // the warp's pairs, with the next pair's block already in flight (registers) while the current one is used
+        auto pair_offset = [&](int t) -> uint32_t {   // kNoBlock if pair t contributes nothing on this stage
+            if (t >= m * m) return kNoBlock;
             const int a = t / m, b = t - a * m;
-            const Entry* ea = entries + a;
-            const Entry* eb = entries + b;
-            if ((((ea->kmask[ks0 >> 5] >> (ks0 & 31)) & 0xFFu) == 0u) || (((eb->kmask[ks0 >> 5] >> (ks0 & 31)) & 0xFFu) == 0u))
-                continue;   // one of the two orbitals sets vanishes on all 32 points
-            const uint32_t off = __ldg(pdir + t);
-            if (off == kNoBlock) continue;
-            const int nI = ea->norb, nJ = eb->norb, ra = ea->row0, rb = eb->row0;
-            const double* Db = D + off;
-            for (int mu = 0; mu < nI; mu++) {
-                double tsum = 0.0;
-                for (int nu = 0; nu < nJ; nu++) tsum = fma(__ldg(Db + mu * nJ + nu), s_phi[chunk_index(rb + nu, lane)], tsum);
-                acc = fma(s_phi[chunk_index(ra + mu, lane)], tsum, acc);
+            if (s_ent[a].x == 0 || s_ent[b].x == 0) return kNoBlock;
+            return s_pdir[t];
+        };
+        int t = warp;
+        uint32_t off = pair_offset(t);
+        while (t < m * m && off == kNoBlock) { t += kRhoWarps; off = pair_offset(t); }
+        double dreg[kMaxBlock / 32];
+        auto fetch = [&](int tt, uint32_t o) {
+            if (tt >= m * m) return;
+            const int n = s_ent[tt / m].y * s_ent[tt % m].y;
+#pragma unroll
+            for (int k = 0; k < kMaxBlock / 32; k++) dreg[k] = (lane + 32 * k < n) ? __ldg(D + o + lane + 32 * k) : 0.0;
+        };
+        fetch(t, off);
+        while (t < m * m) {
+            const int a = t / m, b = t - a * m;
+            const int nI = s_ent[a].y, nJ = s_ent[b].y, ra = s_ent[a].z, rb = s_ent[b].z;
+            __syncwarp();
+            if (nI <= 16 && nJ <= 16) {   // rows padded to 16 columns: aligned 16-byte broadcast loads
+#pragma unroll
+                for (int k = 0; k < kMaxBlock / 32; k++) {
+                    const int idx = lane + 32 * k;
+                    if (idx < nI * nJ) s_D[(idx / nJ) * 16 + idx % nJ] = dreg[k];
+                }
             }
+            __syncwarp();
+            int tn = t + kRhoWarps;
+            uint32_t offn = pair_offset(tn);
+            while (tn < m * m && offn == kNoBlock) { tn += kRhoWarps; offn = pair_offset(tn); }
+            fetch(tn, offn);
+            if (nI <= 16 && nJ <= 16) {
+                const double* pa = s_phi + ra * kRowLD + lane;
+                const double* pb = s_phi + rb * kRowLD + lane;
+                double vb[16];   // the column orbitals at this lane's point, in registers across the rows
+#pragma unroll
+                for (int nu = 0; nu < 16; nu++) vb[nu] = nu < nJ ? pb[nu * kRowLD] : 0.0;
+                for (int mu = 0; mu < nI; mu++) {
+                    const double2* Dr = reinterpret_cast<const double2*>(s_D + mu * 16);
+                    double t0 = 0.0, t1 = 0.0;
+#pragma unroll
+                    for (int q = 0; q < 8; q++) {
+                        if (2 * q < nJ) {   // columns past nJ hold stale numbers times vb = 0: skipped anyway
+                            const double2 d = Dr[q];
+                            t0 = fma(d.x, vb[2 * q], t0);
+                            if (2 * q + 1 < nJ) t1 = fma(d.y, vb[2 * q + 1], t1);
+                        }
+                    }
+                    acc = fma(pa[mu * kRowLD], t0 + t1, acc);
+                }
+            } else {   // large blocks (more than 16 x 16 orbitals): straight from global memory
+                const double* Db = D + off;
+                const double* pa = s_phi + ra * kRowLD + lane;
+                const double* pb = s_phi + rb * kRowLD + lane;
+                for (int mu = 0; mu < nI; mu++) {
+                    double tsum = 0.0;
+                    for (int nu = 0; nu < nJ; nu++) tsum = fma(__ldg(Db + mu * nJ + nu), pb[nu * kRowLD], tsum);
+                    acc = fma(pa[mu * kRowLD], tsum, acc);
+                }
+            }
+            t = tn;
+            off = offn;
         }
         s_part[warp * 32 + lane] = acc;
         __syncthreads();
@@ -80,7 +139,7 @@ __global__ void __launch_bounds__(kRhoThreads) gint_rho_kernel(const __grid_cons
 }
 
 cudaError_t configure_rho(size_t* smem_out, int max_groups) {
-    const size_t smem = ((size_t)max_groups * kChunkDoubles + kRhoWarps * 32) * sizeof(double);
+    const size_t smem = ((size_t)max_groups * kGroupRows * kRowLD + kRhoWarps * 32 + kRhoWarps * kMaxBlock) * sizeof(double) + kMaxEntries * 16 + kMaxEntries * kMaxEntries * 4;
     *smem_out = smem;
     return cudaFuncSetAttribute(gint_rho_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
 }
