@@ -222,7 +222,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
             max_groups = r.ngroup > max_groups ? r.ngroup : max_groups;
             max_entries = r.nentry > max_entries ? r.nentry : max_entries;
         }
-        const size_t need = ((size_t)max_groups * gint::kGroupRows * 33 + 256 + 8 * 256) * sizeof(double) + 64 * 16 + 64 * 64 * 4;
+        const size_t need = ((size_t)max_groups * gint::kGroupRows * 33 + 512 + 16 * 256) * sizeof(double) + 64 * 16 + 64 * 64 * 4;
         ctx->rho_ok = need <= (size_t)prop.sharedMemPerBlockOptin && gint::kStagePts == 32 && max_entries <= 64;
         if (ctx->rho_ok && (e = gint::configure_rho(&ctx->rho_smem, max_groups)) != cudaSuccess) {
             release(ctx);

@@ -6,7 +6,7 @@
 // In the region picture: rho(p) = sum over ORDERED pairs (a, b) of the region's (atom image) entries of
 // phi_a(p)^T D(I_a, I_b, R_b - R_a) phi_b(p).  phi comes from gint_psi_kernel run with unit weights (the same scratch
 // and fragment layout as gint_vlocal).  One CTA per (region, 32-point stage): the stage's phi of all row groups is
-// staged in shared memory, the 8 warps share the entry pairs (lane = mesh point), partial sums are reduced through
+// staged in shared memory, the 16 warps share the entry pairs (lane = mesh point), partial sums are reduced through
 // shared memory and every mesh point is written once (no atomics).  FP64 FMA, not yet on the tensor pipe.
 #include <cuda_runtime.h>
 
@@ -17,7 +17,7 @@
 namespace gint {
 
 namespace {
-constexpr int kRhoThreads = 256;
+constexpr int kRhoThreads = 512;
 constexpr int kRhoWarps = kRhoThreads / 32;
 static_assert(kStagePts == 32 && kStagePairs == 4, "gint_rho_kernel assumes 32-point stages (one lane per point)");
 
@@ -60,39 +60,50 @@ __global__ void __launch_bounds__(kRhoThreads) gint_rho_kernel(const __grid_cons
         double acc = 0.0;
         double* s_D = s_part + kRhoWarps * 32 + warp * kMaxBlock;   // this warp's copy of the current D block
         // the warp's pairs, with the next pair's block already in flight (registers) while the current one is used
-        auto pair_offset = [&](int t) -> uint32_t {   // kNoBlock if pair t contributes nothing on this stage
-            if (t >= m * m) return kNoBlock;
-            const int a = t / m, b = t - a * m;
-            if (s_ent[a].x == 0 || s_ent[b].x == 0) return kNoBlock;
-            return s_pdir[t];
+        // pairs t = a m + b, t = warp, warp + 16, ...: (a, b) advanced without divisions; the next pair that
+        // contributes on this stage (both entries active, block exists) is looked up in shared memory
+        struct PairIt { int t, a, b; uint32_t off; };
+        auto advance = [&](PairIt& it) {   // to the next contributing pair at or after it.t
+            while (it.t < m * m) {
+                while (it.b >= m) { it.b -= m; it.a++; }
+                if (s_ent[it.a].x != 0 && s_ent[it.b].x != 0) {
+                    it.off = s_pdir[it.t];
+                    if (it.off != kNoBlock) return;
+                }
+                it.t += kRhoWarps;
+                it.b += kRhoWarps;
+            }
+            it.off = kNoBlock;
         };
-        int t = warp;
-        uint32_t off = pair_offset(t);
-        while (t < m * m && off == kNoBlock) { t += kRhoWarps; off = pair_offset(t); }
+        PairIt cur{warp, 0, warp, kNoBlock};
+        advance(cur);
         double dreg[kMaxBlock / 32];
-        auto fetch = [&](int tt, uint32_t o) {
-            if (tt >= m * m) return;
-            const int n = s_ent[tt / m].y * s_ent[tt % m].y;
+        auto fetch = [&](const PairIt& it) {
+            if (it.t >= m * m) return;
+            const uint32_t o = it.off;
+            const int n = s_ent[it.a].y * s_ent[it.b].y;
 #pragma unroll
             for (int k = 0; k < kMaxBlock / 32; k++) dreg[k] = (lane + 32 * k < n) ? __ldg(D + o + lane + 32 * k) : 0.0;
         };
-        fetch(t, off);
-        while (t < m * m) {
-            const int a = t / m, b = t - a * m;
+        fetch(cur);
+        while (cur.t < m * m) {
+            const int a = cur.a, b = cur.b;
+            const uint32_t off = cur.off;
             const int nI = s_ent[a].y, nJ = s_ent[b].y, ra = s_ent[a].z, rb = s_ent[b].z;
             __syncwarp();
             if (nI <= 16 && nJ <= 16) {   // rows padded to 16 columns: aligned 16-byte broadcast loads
 #pragma unroll
+                const float inv_nJ = 1.0f / (float)nJ;
                 for (int k = 0; k < kMaxBlock / 32; k++) {
                     const int idx = lane + 32 * k;
-                    if (idx < nI * nJ) s_D[(idx / nJ) * 16 + idx % nJ] = dreg[k];
+                    const int r = (int)(((float)idx + 0.5f) * inv_nJ);   // idx / nJ for idx < 256, nJ <= 16
+                    if (idx < nI * nJ) s_D[r * 16 + (idx - r * nJ)] = dreg[k];
                 }
             }
             __syncwarp();
-            int tn = t + kRhoWarps;
-            uint32_t offn = pair_offset(tn);
-            while (tn < m * m && offn == kNoBlock) { tn += kRhoWarps; offn = pair_offset(tn); }
-            fetch(tn, offn);
+            PairIt nxt{cur.t + kRhoWarps, cur.a, cur.b + kRhoWarps, kNoBlock};
+            advance(nxt);
+            fetch(nxt);
             if (nI <= 16 && nJ <= 16) {
                 const double* pa = s_phi + ra * kRowLD + lane;
                 const double* pb = s_phi + rb * kRowLD + lane;
@@ -122,8 +133,7 @@ __global__ void __launch_bounds__(kRhoThreads) gint_rho_kernel(const __grid_cons
                     acc = fma(pa[mu * kRowLD], tsum, acc);
                 }
             }
-            t = tn;
-            off = offn;
+            cur = nxt;
         }
         s_part[warp * 32 + lane] = acc;
         __syncthreads();
