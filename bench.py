@@ -282,8 +282,9 @@ def main():
         f1.record()
         torch.cuda.synchronize()
         rho_ms = f0.elapsed_time(f1) / 2
-        rho_info = {"ms_per_call": rho_ms, "useful_flops": F_pt, "achieved_tflops": F_pt / (rho_ms * 1e-3) * 1e-12,
-                    "note": "gint_rho first cut (FP64 FMA, ordered entry pairs: F_pt accounting), includes its psi kernel"}
+        rho_info = {"ms_per_call": rho_ms, "useful_flops": F_sym, "achieved_tflops": F_sym / (rho_ms * 1e-3) * 1e-12,
+                    "note": "gint_rho (Eq. 44) on the tensor pipe: tiles ga <= gb with E = D + D^T folded at gather time, "
+                            "so F_sym accounting as for gint_vlocal; the time includes its psi kernel"}
         del Dm, rho
 
     if rank != 0:

@@ -264,11 +264,13 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
 int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* stream) {
     if (!ctx || !D_dev || !rho_dev) return fail(GINT_EINVAL, "null argument");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
-    if (!ctx->rho_ok) return fail(GINT_EUNSUPPORTED, "too many orbitals or atom images listed for one region for gint_rho; use a smaller bcell");
+    const bool use_dmma = gint::kStagePts == 32 && getenv("GINT_RHO_FMA") == nullptr;
+    if (!use_dmma && !ctx->rho_ok) return fail(GINT_EUNSUPPORTED, "too many orbitals or atom images listed for one region for gint_rho; use a smaller bcell");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     cudaError_t e = gint::launch_psi(ctx->dev, ctx->psi_smem, ctx->plan.tables_in_smem, ctx->nsm, nullptr, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho psi launch");
-    e = gint::launch_rho_kernel(ctx->dev, ctx->rho_smem, ctx->nsm, D_dev, rho_dev, st);
+    e = use_dmma ? gint::launch_rho_dmma(ctx->dev, ctx->contract_smem, ctx->nsm, D_dev, rho_dev, st)
+                 : gint::launch_rho_kernel(ctx->dev, ctx->rho_smem, ctx->nsm, D_dev, rho_dev, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho launch");
     return GINT_OK;
 }

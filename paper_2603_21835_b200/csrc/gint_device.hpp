@@ -49,6 +49,8 @@ struct FoldPlan {
     int32_t nrun, norb_tot;
 };
 cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream);
+cudaError_t launch_rho_dmma(const DevicePlan& P, size_t contract_smem_bytes, int nsm, const double* D, double* rho,
+                            cudaStream_t stream);
 cudaError_t launch_rho_kernel(const DevicePlan& P, size_t smem, int nsm, const double* D, double* rho, cudaStream_t stream);
 cudaError_t configure_rho(size_t* smem_out, int max_groups);
 cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac, double* Hk, cudaStream_t stream);

@@ -9,7 +9,7 @@
 //       lane per mesh point -- and stored to a scratch buffer in DMMA fragment order, together
 //       with the sign bits of V per region.  The V dV weighting of Eq. 45 is thereby folded into
 //       the operand: C = psi diag(sign V) psi^T.
-//   gint_vlocal_kernel  output-stationary contraction (the paper's per-BigGrid dense contraction,
+//   gint_contract_kernel<0>  (gint_vlocal) output-stationary contraction (the paper's per-BigGrid dense contraction,
 //       PAPER.md:380, 413).  One persistent CTA per SM pulls work items from a global queue; a
 //       work item is a set of up to 15 32x32 tiles (one per consumer warp) of the upper triangle
 //       of one region's C.  A producer warp stages the item descriptor and streams the row groups
@@ -375,8 +375,158 @@ GINT_HD inline ContractSmem contract_smem(int nring) {
     return L;
 }
 
+// ---- gint_rho on the tensor pipe (MODE 1 of the contraction kernel) --------------------------------
+//   rho(p) = sum over tiles (ga <= gb) of  Phi_ga(p)^T E Phi_gb(p),   E = D[ga][gb] + D[gb][ga]^T  (ga < gb),
+//                                                                      E = D[ga][ga]               (ga = gb),
+// D[.][.] being the region's density matrix gathered from the blocks (entry a, entry b) -> (I_a, I_b, R_b - R_a)
+// (Eq. 44; no symmetry of D is assumed).  The warp holds E as 4 x 8 A fragments
+// (rows 8 i + lane/4, columns 4 kc + lane%4) in registers for the whole item.  Per k-pair (8 mesh points) it
+// forms T = E Phi_gb as 4 accumulator fragments (rows x 8 points) with the B operand read from the stage
+// (rows of gb are the K dimension, the 8 points the N dimension: conflict-free 8-byte loads in the fragment
+// layout), multiplies by Phi_ga in the accumulator layout, reduces over the rows by shuffles and adds the 8 point
+// values into rho with red.global.add.f64.
+#define RHO_GUARD(cond, body)          \
+    if (cond) {                        \
+        do { body } while (never);     \
+    }
+__device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* __restrict__ D, double* __restrict__ rho,
+                                             uint64_t* s_full, uint64_t* s_empty, uint64_t* s_dfull, uint64_t* s_dempty,
+                                             const ItemDesc* s_desc, const unsigned char* s_ring, int nring, int never,
+                                             int lane, int cidx) {
+    static_assert(kStagePts == 32, "gint_rho needs 32-point stages");
+    const int frow = lane >> 2, fk = lane & 3;
+    uint32_t cs = 0, cph = 0;
+    for (int it = 0;; it++) {
+        const int ds = it % kDescSlots;
+        mbar_wait(smem_u32(s_dfull + ds), ((uint32_t)it / kDescSlots) & 1u);
+        const ItemDesc* cur = &s_desc[ds];
+        if (!cur->valid) break;
+        const int sa = cur->item.tiles[cidx][0], sb = cur->item.tiles[cidx][1];
+        const bool has_tile = sa != 0xFF;
+        const bool diag = sa == sb;
+        // ---- gather the tile of E into A fragments ----
+        double A[4][8];
+        if (has_tile) {
+            const uint32_t* pdir = P.pair_direct + cur->item.reg.pair_off;
+            const int m = cur->item.reg.nentry;
+            uint32_t ci[8];
+#pragma unroll
+            for (int kc = 0; kc < 8; kc++) ci[kc] = cur->rinfo[sb][4 * kc + fk];
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                const uint32_t ri = cur->rinfo[sa][8 * i + frow];
+                const int ea = ri & 0xFFF, mu = (ri >> 12) & 0xFF, nI = ri >> 20;
+#pragma unroll
+                for (int kc = 0; kc < 8; kc++) {
+                    double e = 0.0;
+                    if (ri != kNoBlock && ci[kc] != kNoBlock) {
+                        const int eb = ci[kc] & 0xFFF, nu = (ci[kc] >> 12) & 0xFF, nJ = ci[kc] >> 20;
+                        const uint32_t o1 = __ldg(pdir + ea * m + eb);
+                        if (o1 != kNoBlock) e = __ldg(D + o1 + mu * nJ + nu);
+                        if (!diag) {
+                            const uint32_t o2 = __ldg(pdir + eb * m + ea);
+                            if (o2 != kNoBlock) e += __ldg(D + o2 + nu * nI + mu);
+                        }
+                    }
+                    A[i][kc] = e;
+                }
+            }
+        }
+        const int ox = cur->item.reg.origin[0], oy = cur->item.reg.origin[1], oz = cur->item.reg.origin[2];
+        uint32_t todo = cur->item.stage_mask;
+        while (todo) {
+            const int s = __ffs(todo) - 1;
+            todo &= todo - 1;
+            uint32_t ma = 0, mb = 0;
+            if (has_tile) {
+                const uint64_t ma8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sa][s * 8]);
+                const uint64_t mb8 = *reinterpret_cast<const uint64_t*>(&cur->gmask[sb][s * 8]);
+                const uint64_t qa = (ma8 | (ma8 >> 8)) & 0x000F000F000F000Full, qb = (mb8 | (mb8 >> 8)) & 0x000F000F000F000Full;
+                ma = (uint32_t)qa | (uint32_t)(qa >> 28);
+                mb = (uint32_t)qb | (uint32_t)(qb >> 28);
+            }
+            mbar_wait(smem_u32(s_full + cs), cph);
+            if (has_tile) {
+                const unsigned char* stage = s_ring + (size_t)cs * kStageBytes;
+                const double* chA = reinterpret_cast<const double*>(stage + sa * kChunkBytes);
+                const double* chB = reinterpret_cast<const double*>(stage + sb * kChunkBytes);
+#pragma unroll 1
+                for (int kp = 0; kp < kStagePairs; kp++) {
+                    const uint32_t ra = (ma >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
+                    const uint32_t ca = (mb >> ((kp & 1) * 16 + (kp >> 1) * 4)) & 0xFu;
+                    if (ra == 0u || ca == 0u) continue;
+                    double C[4][2];
+#pragma unroll
+                    for (int i = 0; i < 4; i++) C[i][0] = C[i][1] = 0.0;
+                    // B operand of k-step kc = 2 j + h2: Phi_gb[row 8 j + 4 h2 + lane%4][point lane/4 of the k-pair]
+                    const double* bsrc = chB + ((kp * 32 + fk * 4 + (frow & 3)) * 2 + (frow >> 2));
+                    if ((ra & ca) == 0xFu) {
+#pragma unroll
+                        for (int kc = 0; kc < 8; kc++) {
+                            const double b = bsrc[((kc >> 1) * kStagePairs * 32 + (kc & 1) * 16) * 2];
+#pragma unroll
+                            for (int i = 0; i < 4; i++) dmma8x8x4(C[i][0], C[i][1], A[i][kc], b);
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 4; j++) {
+                            RHO_GUARD(ca & (1u << j), {
+                                const double b0 = bsrc[(j * kStagePairs * 32) * 2];
+                                const double b1 = bsrc[(j * kStagePairs * 32 + 16) * 2];
+#pragma unroll
+                                for (int i = 0; i < 4; i++) {
+                                    RHO_GUARD(ra & (1u << i), {
+                                        dmma8x8x4(C[i][0], C[i][1], A[i][2 * j], b0);
+                                        dmma8x8x4(C[i][0], C[i][1], A[i][2 * j + 1], b1);
+                                    })
+                                }
+                            })
+                        }
+                    }
+                    // C[i][h] = T[row 8 i + lane/4][point 2 (lane%4) + h]: times Phi_ga there, summed over the rows
+                    double p0 = 0.0, p1 = 0.0;
+                    const double* asrc = chA + ((kp * 32 + frow * 4 + ((2 * fk) & 3)) * 2 + (fk >> 1));
+#pragma unroll
+                    for (int i = 0; i < 4; i++) {
+                        if ((ra >> i) & 1u) {
+                            p0 = fma(asrc[(i * kStagePairs * 32) * 2], C[i][0], p0);
+                            p1 = fma(asrc[(i * kStagePairs * 32) * 2 + 2], C[i][1], p1);
+                        }
+                    }
+#pragma unroll
+                    for (int sh = 4; sh < 32; sh <<= 1) {
+                        p0 += __shfl_xor_sync(0xffffffffu, p0, sh);
+                        p1 += __shfl_xor_sync(0xffffffffu, p1, sh);
+                    }
+                    if (frow == 0) {   // lanes 0..3: points 8 kp + 2 fk, + 1 of the stage
+                        const int slot = s * kStagePts + kp * 8 + 2 * fk;
+#pragma unroll
+                        for (int h = 0; h < 2; h++) {
+                            const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[slot + h];
+                            const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
+                            const double v = h ? p1 : p0;
+                            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2] && v != 0.0)
+                                atomicAdd(rho + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3, v);
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(s_empty + cs));
+            if (++cs == (uint32_t)nring) { cs = 0; cph ^= 1u; }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(s_dempty + ds));
+    }
+}
+#undef RHO_GUARD
+
+// MODE 0: gint_vlocal (H += psi diag(sign V) psi^T, Eq. 45).  MODE 1: gint_rho (Eq. 44): the same items, stages and
+// producer; a consumer warp keeps its 32x32 tile of the region's density matrix in registers as the A operand,
+// forms T = E Phi_b on the tensor pipe per 8 points and dots it with Phi_a (see the consumer code below).
+template <int MODE>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm)
-gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H) {
+gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__ Din, double* __restrict__ H) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const ContractSmem L = contract_smem(P.nring);
@@ -479,6 +629,8 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
         }
     } else {
         // ================= consumer warps =================
+        if constexpr (MODE == 0) {
+
         const int frow = lane >> 2, fk = lane & 3;
         uint32_t cs = 0, cph = 0;   // ring slot and phase of the next stage to consume
         for (int it = 0;; it++) {
@@ -635,6 +787,9 @@ gint_vlocal_kernel(const __grid_constant__ DevicePlan P, double* __restrict__ H)
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(s_dempty + ds));   // descriptor (row info, masks) no longer read
         }
+        } else {
+            rho_consumer(P, Din, H, s_full, s_empty, s_dfull, s_dempty, s_desc, s_ring, nring, never, lane, cidx);
+        }
     }
 #ifdef GINT_TIMING
     if (lane == 0 && blockIdx.x < 16) {
@@ -672,7 +827,9 @@ cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool 
     cudaError_t e = tab_smem ? cudaFuncSetAttribute(gint_psi_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psi_smem)
                              : cudaFuncSetAttribute(gint_psi_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psi_smem);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(gint_vlocal_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)contract_smem_bytes);
+    e = cudaFuncSetAttribute(gint_contract_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)contract_smem_bytes);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(gint_contract_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)contract_smem_bytes);
 }
 
 cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
@@ -695,7 +852,7 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_
     if (ev) cudaEventRecord(ev[2], stream);
     if (P.nitems > 0) {
         const int grid = P.nitems < kCtasPerSm * nsm ? P.nitems : kCtasPerSm * nsm;
-        gint_vlocal_kernel<<<grid, kThreads, contract_smem_bytes, stream>>>(P, H);
+        gint_contract_kernel<0><<<grid, kThreads, contract_smem_bytes, stream>>>(P, nullptr, H);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -716,6 +873,19 @@ cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int 
         gint_psi_kernel<true><<<pgrid, kEvalThreads, psi_smem, stream>>>(P, V);
     else
         gint_psi_kernel<false><<<pgrid, kEvalThreads, psi_smem, stream>>>(P, V);
+    return cudaGetLastError();
+}
+
+// gint_rho on the tensor pipe: rho <- 0, queue head <- 0, contraction kernel in MODE 1 (phi must be in the scratch)
+cudaError_t launch_rho_dmma(const DevicePlan& P, size_t contract_smem_bytes, int nsm, const double* D, double* rho,
+                            cudaStream_t stream) {
+    const size_t npts = (size_t)P.ngrid[0] * P.ngrid[1] * P.ngrid[2];
+    cudaError_t e = cudaMemsetAsync(rho, 0, npts * sizeof(double), stream);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 257, stream);
+    if (e != cudaSuccess || P.nitems <= 0) return e;
+    const int grid = P.nitems < kCtasPerSm * nsm ? P.nitems : kCtasPerSm * nsm;
+    gint_contract_kernel<1><<<grid, kThreads, contract_smem_bytes, stream>>>(P, D, rho);
     return cudaGetLastError();
 }
 
