@@ -393,7 +393,7 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
                                              uint64_t* s_full, uint64_t* s_empty, uint64_t* s_dfull, uint64_t* s_dempty,
                                              const ItemDesc* s_desc, const unsigned char* s_ring, int nring, int never,
                                              int lane, int cidx) {
-    static_assert(kStagePts == 32, "gint_rho needs 32-point stages");
+    if (kStagePts != 32) return;   // the 16-point-stage build variant (GINT_CTAS_PER_SM=2) uses the FMA kernel of gint_rho.cu
     const int frow = lane >> 2, fk = lane & 3;
     uint32_t cs = 0, cph = 0;
     for (int it = 0;; it++) {

@@ -19,7 +19,7 @@ namespace gint {
 namespace {
 constexpr int kRhoThreads = 512;
 constexpr int kRhoWarps = kRhoThreads / 32;
-static_assert(kStagePts == 32 && kStagePairs == 4, "gint_rho_kernel assumes 32-point stages (one lane per point)");
+
 
 constexpr int kMaxEntries = 64;   // entries of a region whose info and pair table are staged in shared memory
 constexpr int kMaxBlock = 256;   // D blocks up to 16 x 16 orbitals are staged per warp in shared memory
