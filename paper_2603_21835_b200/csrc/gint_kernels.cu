@@ -416,19 +416,21 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
             for (int i = 0; i < 4; i++) {
                 const uint32_t ri = cur->rinfo[sa][8 * i + frow];
                 const int ea = ri & 0xFFF, mu = (ri >> 12) & 0xFF, nI = ri >> 20;
+                // all pair-table look-ups of the row first, then all block elements (independent loads in flight)
+                uint32_t o1[8], o2[8];
 #pragma unroll
                 for (int kc = 0; kc < 8; kc++) {
-                    double e = 0.0;
-                    if (ri != kNoBlock && ci[kc] != kNoBlock) {
-                        const int eb = ci[kc] & 0xFFF, nu = (ci[kc] >> 12) & 0xFF, nJ = ci[kc] >> 20;
-                        const uint32_t o1 = __ldg(pdir + ea * m + eb);
-                        if (o1 != kNoBlock) e = __ldg(D + o1 + mu * nJ + nu);
-                        if (!diag) {
-                            const uint32_t o2 = __ldg(pdir + eb * m + ea);
-                            if (o2 != kNoBlock) e += __ldg(D + o2 + nu * nI + mu);
-                        }
-                    }
-                    A[i][kc] = e;
+                    const bool ok = ri != kNoBlock && ci[kc] != kNoBlock;
+                    const int eb = ci[kc] & 0xFFF;
+                    o1[kc] = ok ? __ldg(pdir + ea * m + eb) : kNoBlock;
+                    o2[kc] = (ok && !diag) ? __ldg(pdir + eb * m + ea) : kNoBlock;
+                }
+#pragma unroll
+                for (int kc = 0; kc < 8; kc++) {
+                    const int nu = (ci[kc] >> 12) & 0xFF, nJ = ci[kc] >> 20;
+                    const double e1 = o1[kc] != kNoBlock ? __ldg(D + o1[kc] + mu * nJ + nu) : 0.0;
+                    const double e2 = o2[kc] != kNoBlock ? __ldg(D + o2[kc] + nu * nI + mu) : 0.0;
+                    A[i][kc] = e1 + e2;
                 }
             }
         }
