@@ -92,8 +92,8 @@ __global__ void __launch_bounds__(kRhoThreads) gint_rho_kernel(const __grid_cons
             const int nI = s_ent[a].y, nJ = s_ent[b].y, ra = s_ent[a].z, rb = s_ent[b].z;
             __syncwarp();
             if (nI <= 16 && nJ <= 16) {   // rows padded to 16 columns: aligned 16-byte broadcast loads
-#pragma unroll
                 const float inv_nJ = 1.0f / (float)nJ;
+#pragma unroll
                 for (int k = 0; k < kMaxBlock / 32; k++) {
                     const int idx = lane + 32 * k;
                     const int r = (int)(((float)idx + 0.5f) * inv_nJ);   // idx / nJ for idx < 256, nJ <= 16
