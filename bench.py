@@ -12,7 +12,7 @@ H blocks; mirror kernel) over the whole mesh.  Prints ONE JSON line (rank 0).
   ms_per_step      ms per gint_vlocal call (CUDA events, L2 flushed between calls)
   e2e              same metric through gint_vlocal_host: pinned HOST V in, HOST H out,
                    both copies inside the timed region
-  roofline         the dominant kernel (gint_vlocal_kernel, the contraction) alone: achieved
+  roofline         the dominant kernel (gint_contract_kernel<0>, the contraction of gint_vlocal) alone: achieved
                    TFLOP/s (F_sym / its event-timed duration) over the FP64 tensor (DMMA.8x8x4)
                    peak measured live; the psi kernel's HBM figures ride along
   cpu_baseline     the CPU oracle, as it stands, on a bounded sample of the same workload
@@ -39,7 +39,7 @@ UNIT = "TFLOP/s"
 
 # DRAM traffic of the integration kernel per launch, from the ncu --set full capture
 # summarised in profiles/ (dram__bytes_read.sum + dram__bytes_write.sum); None = not captured.
-NCU_TRAFFIC_BYTES = {"si512_dzp": 13.094e9 + 1.565e9}   # profiles/r01d_ncu_summary.md, gint_vlocal_kernel
+NCU_TRAFFIC_BYTES = {"si512_dzp": 13.094e9 + 1.565e9}   # profiles/r01d_ncu_summary.md (the kernel was still named gint_vlocal_kernel there)
 
 
 def measured_peaks():
@@ -305,7 +305,7 @@ def main():
     roofline = {
         "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
         "traffic": NCU_TRAFFIC_BYTES.get(w.name),
-        "kernel": "gint_vlocal_kernel", "kernel_ms": main_ms, "mirror_kernel_ms": mirror_ms,
+        "kernel": "gint_contract_kernel<0>", "kernel_ms": main_ms, "mirror_kernel_ms": mirror_ms,
         "kernel_share_of_step": main_ms / ms_per_step,
         "psi_kernel": {"kernel": "gint_psi_kernel", "kernel_ms": psi_ms, "share_of_step": psi_ms / ms_per_step,
                        "bound": "hbm", "algorithmic_bytes": psi_bytes,
