@@ -354,3 +354,19 @@ def test_rho_large_sampled_points_and_adjoint():
                 if b is not None:
                     ref += pa @ D[off[b]:off[b + 1]].reshape(norb[I], norb[J]) @ pb
         assert abs(rho[tuple(g)] - ref) <= TOL * scale
+
+
+def test_rho_fma_fallback_matches_tensor_path(cfg1, cfg1_oracle, monkeypatch):
+    """The FP64-FMA kernel of csrc/gint_rho.cu (GINT_RHO_FMA=1, read at call time) and the tensor-pipe path give the
+    same density to rounding, and both match the oracle."""
+    import oracle
+    rng = np.random.default_rng(31)
+    H0, blocks = cfg1_oracle
+    D = rng.normal(size=H0.shape)
+    ref = oracle.rho(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, D, blocks)
+    a, _ = gpu_rho(cfg1, D)
+    monkeypatch.setenv("GINT_RHO_FMA", "1")
+    b, _ = gpu_rho(cfg1, D)
+    scale = np.abs(ref).max()
+    assert np.abs(a - ref).max() <= TOL * scale and np.abs(b - ref).max() <= TOL * scale
+    assert np.abs(a - b).max() <= 1e-12 * scale
