@@ -494,21 +494,18 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
                             p1 = fma(asrc[(i * kStagePairs * 32) * 2 + 2], C[i][1], p1);
                         }
                     }
-#pragma unroll
-                    for (int sh = 4; sh < 32; sh <<= 1) {
-                        p0 += __shfl_xor_sync(0xffffffffu, p0, sh);
-                        p1 += __shfl_xor_sync(0xffffffffu, p1, sh);
-                    }
-                    if (frow == 0) {   // lanes 0..3: points 8 kp + 2 fk, + 1 of the stage
-                        const int slot = s * kStagePts + kp * 8 + 2 * fk;
-#pragma unroll
-                        for (int h = 0; h < 2; h++) {
-                            const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[slot + h];
-                            const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
-                            const double v = h ? p1 : p0;
-                            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2] && v != 0.0)
-                                atomicAdd(rho + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3, v);
-                        }
+                    // sum over the 8 row lanes (lane/4): lanes with even lane/4 end up with the first point's total,
+                    // odd ones with the second's (one exchange), then two plain butterfly steps
+                    const bool odd = (frow & 1) != 0;
+                    double keep = odd ? p1 : p0;
+                    keep += __shfl_xor_sync(0xffffffffu, odd ? p0 : p1, 4);
+                    keep += __shfl_xor_sync(0xffffffffu, keep, 8);
+                    keep += __shfl_xor_sync(0xffffffffu, keep, 16);
+                    if (frow < 2) {   // lanes 0..7: point 8 kp + 2 fk + lane/4 of the stage
+                        const uchar4 c = reinterpret_cast<const uchar4*>(P.slot_xyz)[s * kStagePts + kp * 8 + 2 * fk + frow];
+                        const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
+                        if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2] && keep != 0.0)
+                            atomicAdd(rho + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3, keep);
                     }
                 }
             }
