@@ -98,6 +98,36 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def useful_flops(w):
+    """F_pt = sum_g 2 n(g)^2 and F_sym = sum_g n(g)(n(g)+1), n(g) = orbitals non-zero at mesh point g (all atom
+    images counted), counted here with a k-d tree over the atom images -- no library call, so
+    that the oracle arm (--impl reference) runs with the product .so absent."""
+    from scipy.spatial import cKDTree
+    n1, n2, n3 = (int(x) for x in w.ngrid)
+    f = np.stack(np.meshgrid(np.arange(n1) / n1, np.arange(n2) / n2, np.arange(n3) / n3, indexing="ij"), axis=-1)
+    pts = f.reshape(-1, 3) @ w.lattice
+    inv = np.linalg.inv(w.lattice)
+    norb = np.zeros(pts.shape[0], dtype=np.int64)
+    for s_id, sp in enumerate(w.species):
+        atoms = w.atom_pos[np.asarray(w.atom_species) == s_id]
+        if atoms.shape[0] == 0:
+            continue
+        reach = np.ceil(sp.rcut * np.linalg.norm(inv, axis=0)).astype(int) + 1      # images that can reach the cell
+        fa = atoms @ inv
+        lo, hi = np.floor(fa.min(0)).astype(int), np.floor(fa.max(0)).astype(int)
+        sh = np.array([[a, b, c] for a in range(-hi[0] - reach[0], -lo[0] + reach[0] + 1)
+                       for b in range(-hi[1] - reach[1], -lo[1] + reach[1] + 1)
+                       for c in range(-hi[2] - reach[2], -lo[2] + reach[2] + 1)])
+        img = (atoms[None, :, :] + (sh @ w.lattice)[:, None, :]).reshape(-1, 3)
+        c = img @ inv                                                               # keep images near the cell only
+        pad = sp.rcut * np.linalg.norm(inv, axis=0) + 1e-9
+        img = img[np.all((c > -pad) & (c < 1.0 + pad), axis=1)]
+        cnt = cKDTree(img).query_ball_point(pts, sp.rcut * (1.0 - 1e-15), return_length=True, workers=-1)
+        norb += sp.norb * np.asarray(cnt, dtype=np.int64)
+    nn = norb.astype(np.float64)
+    return float(np.sum(2.0 * nn * nn)), float(np.sum(nn * (nn + 1.0)))
+
+
 def oracle_sample(w, natoms_sample, nthreads=0):
     """Time the CPU oracle on all blocks of the first `natoms_sample` row atoms."""
     import oracle
@@ -155,10 +185,8 @@ def main():
     w = workloads.make(args.workload)
 
     if args.impl == "reference":
-        # host-only plan just for the flop count of the workload (no CUDA call is made)
-        from paper_2603_21835_b200 import gint_setup
-        st = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1).gint_get_stats()
-        run_reference(args, w, st["F_pt"])
+        # the oracle arm loads oracle/ and the seeded input generator only: no product library, no CUDA
+        run_reference(args, w, useful_flops(w)[0])
         return
 
     import torch

@@ -1,4 +1,4 @@
-"""CPU oracle for gint_vlocal -- TEST INFRASTRUCTURE ONLY.
+"""CPU oracle for gint_vlocal / gint_rho / gint_fvl / gint_fold_k -- TEST INFRASTRUCTURE ONLY.
 
 Thin ctypes binding of oracle/gint_oracle.c (which holds all the arithmetic and
 cites the paper).  Only tests/, __graft_entry__.smoke() and bench.py's
@@ -35,6 +35,12 @@ def _load():
         lib.orc_rho.restype = ctypes.c_int
         lib.orc_rho.argtypes = [c_dp, c_ip, ctypes.c_int, c_dp, c_dp, c_ip, c_ip, c_ip, c_dp, ctypes.c_int, c_ip, c_dp,
                                 ctypes.c_int64, c_i32p, c_i32p, c_i32p, c_i64p, c_dp, c_dp, ctypes.c_int]
+        lib.orc_phi_grad.restype = ctypes.c_int
+        lib.orc_phi_grad.argtypes = [ctypes.c_int, c_dp, c_dp, c_ip, c_ip, c_ip, c_dp, ctypes.c_int, ctypes.c_int, c_dp,
+                                     c_dp, c_dp]
+        lib.orc_fvl.restype = ctypes.c_int
+        lib.orc_fvl.argtypes = [c_dp, c_ip, ctypes.c_int, c_dp, c_dp, c_ip, c_ip, c_ip, c_dp, ctypes.c_int, c_ip, c_dp,
+                                c_dp, ctypes.c_int64, c_i32p, c_i32p, c_i32p, c_i64p, c_dp, c_dp, ctypes.c_int]
         _lib = lib
     return _lib
 
@@ -184,3 +190,45 @@ def rho(lattice, ngrid, species, atom_species, atom_pos, D_flat, blocks, nthread
     if rc < 0:
         raise RuntimeError("orc_rho failed: %d" % rc)
     return out
+
+
+def phi_grad(species: Sequence, which: int, d: np.ndarray):
+    """(phi[npts][norb], grad[npts][norb][3]) of species `which` at displacements d: Eq. 1 and its gradient with the
+    radial derivative taken from the same cubic Lagrange interpolant (readings #19, #20)."""
+    lib = _load()
+    sp = _SpeciesPack(species)
+    d = np.ascontiguousarray(np.asarray(d, dtype=np.float64).reshape(-1, 3))
+    n = int(sp.norb[which])
+    ph = np.empty((d.shape[0], n), dtype=np.float64)
+    gr = np.empty((d.shape[0], n, 3), dtype=np.float64)
+    rc = lib.orc_phi_grad(*sp.args(), int(which), int(d.shape[0]), _p(d, ctypes.c_double), _p(ph, ctypes.c_double),
+                          _p(gr, ctypes.c_double))
+    if rc < 0:
+        raise RuntimeError("orc_phi_grad failed: %d" % rc)
+    return ph, gr
+
+
+def fvl(lattice, ngrid, species, atom_species, atom_pos, V, D_flat, blocks, nthreads: int = 0) -> np.ndarray:
+    """Local Pulay force F[natom][3] (Eq. 46; reading #18):
+    F_K = - sum_blocks D(I,J,R) : dH(I,J,R)/dtau_K at fixed V.  `blocks` = (iat, jat, R, offset), D_flat in the H layout."""
+    lib = _load()
+    lattice = np.ascontiguousarray(lattice, dtype=np.float64)
+    ngrid_c = np.ascontiguousarray(ngrid, dtype=np.intc)
+    pos = np.ascontiguousarray(atom_pos, dtype=np.float64)
+    asp = np.ascontiguousarray(atom_species, dtype=np.intc)
+    V = np.ascontiguousarray(V, dtype=np.float64)
+    sp = _SpeciesPack(species)
+    bi = np.ascontiguousarray(blocks[0], dtype=np.int32)
+    bj = np.ascontiguousarray(blocks[1], dtype=np.int32)
+    bR = np.ascontiguousarray(blocks[2], dtype=np.int32).reshape(-1, 3)
+    off = np.ascontiguousarray(blocks[3], dtype=np.int64)
+    D = np.ascontiguousarray(D_flat, dtype=np.float64)
+    assert D.shape[0] == int(off[-1]) and V.shape == tuple(int(x) for x in ngrid_c)
+    F = np.zeros((pos.shape[0], 3), dtype=np.float64)
+    rc = lib.orc_fvl(_p(lattice, ctypes.c_double), _p(ngrid_c, ctypes.c_int), *sp.args(), int(pos.shape[0]),
+                     _p(asp, ctypes.c_int), _p(pos, ctypes.c_double), _p(V, ctypes.c_double), int(bi.shape[0]),
+                     _p(bi, ctypes.c_int32), _p(bj, ctypes.c_int32), _p(bR, ctypes.c_int32), _p(off, ctypes.c_int64),
+                     _p(D, ctypes.c_double), _p(F, ctypes.c_double), int(nthreads))
+    if rc < 0:
+        raise RuntimeError("orc_fvl failed: %d" % rc)
+    return F

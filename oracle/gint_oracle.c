@@ -445,3 +445,221 @@ int orc_rho(const double *lattice, const int *ngrid, int nspecies, const double 
     free(gstart);
     return err ? -5 : used;
 }
+
+/* ==== local Pulay force (the paper's cal_gint_fvl) ===========================================
+ *
+ *   F_I = - sum_R sum_{mu,nu} rho_{nu mu}(R) sum_g [ d phi_mu(r_g - tau_I)/d tau_I  V(r_g) phi_nu(r_g - tau_J - R)
+ *                                                   + phi_mu(r_g - tau_I) V(r_g) d phi_nu(r_g - tau_J - R)/d tau_I ] dV
+ *       -- PAPER.md:400-411 (Sec. 3.3.1, Eq. 46); general form PAPER.md:262-266 (Eq. 30): "The derivatives of the
+ *          NAOs are computed analytically for the angular part (real spherical harmonics) and numerically for the
+ *          radial part."
+ *
+ * Readings:
+ *   #18 The density-matrix coefficient of the orbital pair (mu on atom I in cell 0, nu on atom J in cell R) is the
+ *       block element D(I,J,R)[mu][nu] -- the same coefficient that Eq. 44 calls rho_{mu nu}(R) and Eq. 46 calls
+ *       rho_{nu mu}(R) (with Eq. 29, E = sum_R sum_{mu nu} rho_{nu mu}(R) H_{mu nu}(R)).  Hence
+ *           F_K = - sum_blocks sum_{mu nu} D(I,J,R)[mu][nu] * d H(I,J,R)[mu][nu] / d tau_K   at fixed V and D,
+ *       the derivative acting on phi_mu when K = I and on phi_nu when K = J (both when I = J).  With
+ *       d phi(r - tau)/d tau = -grad phi(r - tau):
+ *           F_I += dV sum_n V[n mod N] sum_{mu nu} D[mu][nu] grad phi_mu(r_n - tau_I) phi_nu(r_n - tau_J - R)
+ *           F_J += dV sum_n V[n mod N] sum_{mu nu} D[mu][nu] phi_mu(r_n - tau_I) grad phi_nu(r_n - tau_J - R)
+ *       (all-space sum over unwrapped mesh points n, reading #1).
+ *   #19 Radial derivative: the derivative of the SAME cubic Lagrange interpolant that defines f (reading #4),
+ *       f'(r) = (1/dr) sum_j T[k+j] L_j'(t); angular part analytic.  With phi = f(r) P(d/r), P the homogeneous
+ *       polynomial of degree l behind Y_lm:  grad phi = f' rhat P + (f / r) (gradP(rhat) - l P rhat).
+ *   #20 At r < 1e-12 (reading #6) the limit for f ~ r^l is used: grad phi = c_1 f'(0) e_m for l = 1, 0 otherwise.
+ *       Outside the cutoff (r >= rcut) grad phi = 0.
+ */
+
+/* derivative of the interpolant with respect to r */
+static double radial_interp_deriv(const double *T, double r, double dr)
+{
+    double s = r / dr;
+    int k = (int)floor(s);
+    double t = s - (double)k;
+    /* d/dt of L0..L3 of radial_interp */
+    double D0 = -((2.0 - t) * (3.0 - t) + (1.0 - t) * (3.0 - t) + (1.0 - t) * (2.0 - t)) / 6.0;
+    double D1 = ((2.0 - t) * (3.0 - t) - t * (3.0 - t) - t * (2.0 - t)) / 2.0;
+    double D2 = -((1.0 - t) * (3.0 - t) - t * (3.0 - t) - t * (1.0 - t)) / 2.0;
+    double D3 = ((1.0 - t) * (2.0 - t) - t * (2.0 - t) - t * (1.0 - t)) / 6.0;
+    return (T[k] * D0 + T[k + 1] * D1 + T[k + 2] * D2 + T[k + 3] * D3) / dr;
+}
+
+/* homogeneous polynomials P_lm(x,y,z) with Y_lm(rhat) = P_lm(rhat), and their Cartesian gradients (reading #7) */
+static int ylm_poly_grad(int l, double x, double y, double z, double *P, double (*G)[3])
+{
+    const double pi = 3.14159265358979323846;
+    if (l == 0) {
+        P[0] = 0.5 * sqrt(1.0 / pi);
+        G[0][0] = G[0][1] = G[0][2] = 0.0;
+        return 1;
+    }
+    if (l == 1) {
+        double c = sqrt(3.0 / (4.0 * pi));
+        P[0] = c * y; G[0][0] = 0.0; G[0][1] = c;   G[0][2] = 0.0;
+        P[1] = c * z; G[1][0] = 0.0; G[1][1] = 0.0; G[1][2] = c;
+        P[2] = c * x; G[2][0] = c;   G[2][1] = 0.0; G[2][2] = 0.0;
+        return 3;
+    }
+    if (l == 2) {
+        double c1 = 0.5 * sqrt(15.0 / pi), c2 = 0.25 * sqrt(5.0 / pi), c3 = 0.25 * sqrt(15.0 / pi);
+        P[0] = c1 * x * y;                         G[0][0] = c1 * y;        G[0][1] = c1 * x;        G[0][2] = 0.0;
+        P[1] = c1 * y * z;                         G[1][0] = 0.0;           G[1][1] = c1 * z;        G[1][2] = c1 * y;
+        P[2] = c2 * (2.0 * z * z - x * x - y * y); G[2][0] = -2.0 * c2 * x; G[2][1] = -2.0 * c2 * y; G[2][2] = 4.0 * c2 * z;
+        P[3] = c1 * x * z;                         G[3][0] = c1 * z;        G[3][1] = 0.0;           G[3][2] = c1 * x;
+        P[4] = c3 * (x * x - y * y);               G[4][0] = 2.0 * c3 * x;  G[4][1] = -2.0 * c3 * y; G[4][2] = 0.0;
+        return 5;
+    }
+    return -1;
+}
+
+/* phi and grad phi for all orbitals of one species at displacement d; returns 0 outside the cutoff */
+static int phi_grad_eval(const orc_species *sp, const double d[3], double *phi, double (*grad)[3])
+{
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    int o = 0;
+    if (!(r < sp->rcut)) {
+        for (int i = 0; i < sp->norb; i++) phi[i] = grad[i][0] = grad[i][1] = grad[i][2] = 0.0;
+        return 0;
+    }
+    double u[3] = {0.0, 0.0, 0.0};
+    if (r >= 1e-12) {
+        u[0] = d[0] / r;
+        u[1] = d[1] / r;
+        u[2] = d[2] / r;
+    }
+    for (int k = 0; k < sp->nrad; k++) {
+        const double *T = sp->table + (size_t)k * sp->ntab;
+        const int l = sp->l[k];
+        double f = radial_interp(T, r, sp->dr), fp = radial_interp_deriv(T, r, sp->dr);
+        double P[7], G[7][3];
+        int nm = ylm_poly_grad(l, u[0], u[1], u[2], P, G);
+        for (int m = 0; m < nm; m++, o++) {
+            if (r < 1e-12) { /* reading #20 */
+                phi[o] = (l == 0) ? f * P[m] : 0.0;
+                for (int c = 0; c < 3; c++) grad[o][c] = (l == 1) ? fp * G[m][c] : 0.0;
+            } else {
+                phi[o] = f * P[m];
+                for (int c = 0; c < 3; c++)
+                    grad[o][c] = fp * u[c] * P[m] + (f / r) * (G[m][c] - (double)l * P[m] * u[c]);
+            }
+        }
+    }
+    return 1;
+}
+
+/* public: orbital gradients at given displacements (used by the pins) */
+int orc_phi_grad(int nspecies, const double *sp_rcut, const double *sp_dr, const int *sp_ntab, const int *sp_nrad,
+                 const int *sp_l, const double *sp_table, int species, int npts, const double *d /* [npts][3] */,
+                 double *phi /* [npts][norb] */, double *grad /* [npts][norb][3] */)
+{
+    orc_species sp[16];
+    if (nspecies > 16 || species < 0 || species >= nspecies) return -1;
+    unpack_species(nspecies, sp_rcut, sp_dr, sp_ntab, sp_nrad, sp_l, sp_table, sp);
+    if (sp[species].norb > ORC_MAX_ORB) return -2;
+    for (int p = 0; p < npts; p++)
+        phi_grad_eval(&sp[species], d + 3 * (size_t)p, phi + (size_t)p * sp[species].norb,
+                      (double(*)[3])(grad + (size_t)p * sp[species].norb * 3));
+    return sp[species].norb;
+}
+
+/* public: forces F[natom][3] (overwritten) from density-matrix blocks D (H layout), Eq. 46 as read above.
+ * blocks grouped by bi.  Returns threads used or <0. */
+int orc_fvl(const double *lattice, const int *ngrid, int nspecies, const double *sp_rcut, const double *sp_dr,
+            const int *sp_ntab, const int *sp_nrad, const int *sp_l, const double *sp_table, int natom,
+            const int *atom_species, const double *pos, const double *V, int64_t nblk, const int32_t *bi,
+            const int32_t *bj, const int32_t *bR, const int64_t *d_off, const double *D, double *F, int nthreads)
+{
+    orc_species sp[16];
+    if (nspecies > 16) return -1;
+    unpack_species(nspecies, sp_rcut, sp_dr, sp_ntab, sp_nrad, sp_l, sp_table, sp);
+    for (int s = 0; s < nspecies; s++)
+        if (sp[s].norb > ORC_MAX_ORB) return -2;
+    double inv[9];
+    double vol = fabs(det3(lattice));
+    if (vol < 1e-300) return -3;
+    inv3(lattice, inv);
+    double blen[3];
+    for (int i = 0; i < 3; i++) blen[i] = sqrt(inv[i] * inv[i] + inv[3 + i] * inv[3 + i] + inv[6 + i] * inv[6 + i]);
+    const int64_t N1 = ngrid[0], N2 = ngrid[1], N3 = ngrid[2];
+    const double dV = vol / ((double)N1 * (double)N2 * (double)N3);
+    long double *Facc = (long double *)calloc((size_t)natom * 3, sizeof(long double));
+    int64_t *gstart = (int64_t *)malloc(sizeof(int64_t) * (size_t)(nblk + 1));
+    if (!Facc || !gstart) {
+        free(Facc);
+        free(gstart);
+        return -4;
+    }
+    int64_t ngroup = 0;
+    for (int64_t b = 0; b < nblk; b++)
+        if (b == 0 || bi[b] != bi[b - 1]) gstart[ngroup++] = b;
+    gstart[ngroup] = nblk;
+
+    int used = 1;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+    }
+#pragma omp parallel for schedule(dynamic, 1)
+#endif
+    for (int64_t g = 0; g < ngroup; g++) {
+        const int I = bi[gstart[g]];
+        const orc_species *sI = &sp[atom_species[I]];
+        const double *tI = pos + 3 * (size_t)I;
+        int lo[3], hi[3];
+        for (int i = 0; i < 3; i++) {
+            double f = tI[0] * inv[i] + tI[1] * inv[3 + i] + tI[2] * inv[6 + i];
+            lo[i] = (int)floor((f - sI->rcut * blen[i]) * (double)ngrid[i]) - 1;
+            hi[i] = (int)ceil((f + sI->rcut * blen[i]) * (double)ngrid[i]) + 1;
+        }
+        double phiI[ORC_MAX_ORB], gI[ORC_MAX_ORB][3], phiJ[ORC_MAX_ORB], gJ[ORC_MAX_ORB][3];
+        for (int n1 = lo[0]; n1 <= hi[0]; n1++)
+            for (int n2 = lo[1]; n2 <= hi[1]; n2++)
+                for (int n3 = lo[2]; n3 <= hi[2]; n3++) {
+                    double f1 = (double)n1 / (double)N1, f2 = (double)n2 / (double)N2, f3 = (double)n3 / (double)N3;
+                    double r[3], d[3];
+                    for (int c = 0; c < 3; c++) {
+                        r[c] = f1 * lattice[c] + f2 * lattice[3 + c] + f3 * lattice[6 + c];
+                        d[c] = r[c] - tI[c];
+                    }
+                    if (!phi_grad_eval(sI, d, phiI, gI)) continue;
+                    const double v = V[(pmod(n1, N1) * N2 + pmod(n2, N2)) * N3 + pmod(n3, N3)];
+                    for (int64_t b = gstart[g]; b < gstart[g + 1]; b++) {
+                        const int J = bj[b];
+                        const orc_species *sJ = &sp[atom_species[J]];
+                        for (int c = 0; c < 3; c++)
+                            d[c] = r[c] - (pos[3 * (size_t)J + c] + bR[3 * b] * lattice[c] + bR[3 * b + 1] * lattice[3 + c] +
+                                           bR[3 * b + 2] * lattice[6 + c]);
+                        if (!phi_grad_eval(sJ, d, phiJ, gJ)) continue;
+                        const double *Db = D + d_off[b];
+                        double fI[3] = {0.0, 0.0, 0.0}, fJ[3] = {0.0, 0.0, 0.0};
+                        for (int mu = 0; mu < sI->norb; mu++)
+                            for (int nu = 0; nu < sJ->norb; nu++) {
+                                const double dmn = Db[mu * sJ->norb + nu];
+                                for (int c = 0; c < 3; c++) {
+                                    fI[c] += dmn * gI[mu][c] * phiJ[nu];
+                                    fJ[c] += dmn * phiI[mu] * gJ[nu][c];
+                                }
+                            }
+                        for (int c = 0; c < 3; c++) {
+                            long double aI = (long double)(v * fI[c]), aJ = (long double)(v * fJ[c]);
+#ifdef _OPENMP
+#pragma omp atomic
+#endif
+                            Facc[3 * (size_t)I + c] += aI;
+#ifdef _OPENMP
+#pragma omp atomic
+#endif
+                            Facc[3 * (size_t)J + c] += aJ;
+                        }
+                    }
+                }
+    }
+    for (int i = 0; i < 3 * natom; i++) F[i] = (double)(Facc[i] * (long double)dV);
+    free(Facc);
+    free(gstart);
+    return used;
+}

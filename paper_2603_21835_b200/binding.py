@@ -23,7 +23,8 @@ EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
-              "regions", "ksteps_full", "ksteps_partial", "dmma_in_partial_ksteps", "stage_visits", "dmma_max_sched_item", "dmma_max_sched_stage", "dmma_max_warp_stage", "s23")
+              "regions", "ksteps_full", "ksteps_partial", "dmma_in_partial_ksteps", "stage_visits", "dmma_max_sched_item", "dmma_max_sched_stage", "dmma_max_warp_stage", "bcell1", "bcell2", "bcell3",
+              "s26", "s27", "s28", "s29", "s30", "s31")
 
 
 class GintError(RuntimeError):
@@ -123,8 +124,8 @@ class GintContext:
         return iat[:n], jat[:n], R[:n], off
 
     def gint_get_stats(self) -> dict:
-        s = np.zeros(24, dtype=np.float64)
-        n = _check(_lib.gint_get_stats(self._h, _ptr(s, ctypes.c_double), 24), "gint_get_stats")
+        s = np.zeros(32, dtype=np.float64)
+        n = _check(_lib.gint_get_stats(self._h, _ptr(s, ctypes.c_double), 32), "gint_get_stats")
         return {STAT_NAMES[i]: float(s[i]) for i in range(n)}
 
     def gint_set_profiling(self, on: bool = True):

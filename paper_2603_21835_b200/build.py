@@ -9,8 +9,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgint_b200.so")
-SOURCES = ["gint_api.cu", "gint_kernels.cu", "gint_fold.cu", "gint_rho.cu", "gint_plan.cpp"]
-HEADERS = ["gint_device.hpp", "gint_plan.hpp", os.path.join("..", "..", "include", "gint.h")]
+SOURCES = ["gint_api.cu", "gint_kernels.cu", "gint_fold.cu", "gint_plan.cpp"]
+HEADERS = ["gint_device.hpp", "gint_plan.hpp", "gint_kstep_dispatch.inc", os.path.join("..", "..", "include", "gint.h")]
 
 
 def _stale() -> bool:
@@ -27,7 +27,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
            "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "-cudart", "static",
            "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    cmd[1:1] = os.environ.get("GINT_BUILD_FLAGS", "").split()
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")

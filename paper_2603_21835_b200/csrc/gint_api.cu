@@ -21,8 +21,7 @@ struct gint_ctx {
     std::vector<void*> allocs;
     gint::FoldPlan fold{};
     std::vector<int64_t> first_orb;   // [natom+1]
-    size_t psi_smem = 0, contract_smem = 0, rho_smem = 0;
-    bool rho_ok = false;
+    size_t psi_smem = 0, contract_smem = 0;
     bool profiling = false;
     bool have_events = false;
     cudaEvent_t ev[5];
@@ -40,8 +39,23 @@ int fail(int code, const std::string& msg) {
 }
 int fail_cuda(cudaError_t e, const char* where) {
     g_last_error = std::string(where) + ": " + cudaGetErrorString(e);
-    return GINT_ECUDA;
+    return e == cudaErrorMemoryAllocation ? GINT_ENOMEM : GINT_ECUDA;
 }
+
+// Every device entry point runs on the context's device, whatever device is current in the calling thread, and
+// leaves the caller's current device as it found it.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int device) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+    }
+    ~DeviceGuard() {
+        int now = -1;
+        if (prev >= 0 && cudaGetDevice(&now) == cudaSuccess && now != prev) cudaSetDevice(prev);
+    }
+};
 
 template <typename T>
 cudaError_t upload(gint_ctx* ctx, const std::vector<T>& host, const T** dev_out) {
@@ -57,20 +71,7 @@ cudaError_t upload(gint_ctx* ctx, const std::vector<T>& host, const T** dev_out)
 
 void release(gint_ctx* ctx) {
     if (ctx->device >= 0) {
-        cudaSetDevice(ctx->device);
-#ifdef GINT_TIMING
-        if (ctx->dev.counter) {
-            std::vector<long long> tm(16 * 16 * 8);
-            cudaDeviceSynchronize();
-            cudaMemcpy(tm.data(), ctx->dev.counter + 272, tm.size() * 8, cudaMemcpyDeviceToHost);
-            fprintf(stderr, "[timing] cta 3, per warp (ms): descwait fullwait contract flush | warp 15 = producer: emptywait\n");
-            for (int w = 0; w < 8; w++) {
-                const long long* v = &tm[(16 * 3 + w) * 8];
-                fprintf(stderr, "   warp %2d (sched %d): %7.3f %7.3f %7.3f %7.3f   items %lld  wait@stage0 %7.3f @1-3 %7.3f\n", w, w & 3, v[0] / 1.965e6,
-                        (v[3] == 0 ? v[1] : v[3]) / 1.965e6, v[4] / 1.965e6, v[5] / 1.965e6, v[6], v[1] / 1.965e6, v[2] / 1.965e6);
-            }
-        }
-#endif
+        DeviceGuard guard(ctx->device);
         for (void* p : ctx->allocs) cudaFree(p);
         if (ctx->have_events)
             for (int i = 0; i < 5; i++) cudaEventDestroy(ctx->ev[i]);
@@ -128,7 +129,8 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         *out = ctx;
         return GINT_OK;
     }
-    cudaError_t e = cudaSetDevice(cuda_device);
+    DeviceGuard guard(cuda_device);
+    cudaError_t e = guard.err;
     if (e != cudaSuccess) { delete ctx; return fail_cuda(e, "cudaSetDevice"); }
     ctx->device = cuda_device;
     cudaDeviceProp prop;
@@ -176,8 +178,8 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         UP(first32, &ctx->fold.first)
     }
 #undef UP
-    void* ctr = nullptr;   // queue head (+ development timing area)
-    if ((e = cudaMalloc(&ctr, 4 * 272 + 16 * 16 * 8 * 8 + 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
+    void* ctr = nullptr;   // work-queue head
+    if ((e = cudaMalloc(&ctr, 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
     {
@@ -203,31 +205,15 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     D.nregions = (int32_t)P.regions.size();
     D.nring = P.nring;
     D.never = 0;
-    D.debug = 0;
-#ifdef GINT_TIMING
-    if (const char* dbg = getenv("GINT_DEBUG")) D.debug = atoi(dbg);
-#endif
     D.nitems = (int32_t)P.items.size();
     D.nmirror = (int32_t)P.mirror.size();
     D.tab_doubles = (int32_t)P.tab_packed.size();
-    ctx->psi_smem = gint::psi_kernel_smem(P.tables_in_smem ? P.tab_packed.size() * sizeof(double) : 0);
+    D.nspecies = (int32_t)P.species.size();
+    ctx->psi_smem = gint::psi_kernel_smem(P.tables_in_smem ? P.tab_packed.size() * sizeof(double) : 0, (int)P.species.size());
     ctx->contract_smem = gint::contract_kernel_smem(P.nring);
     if ((e = gint::configure_kernels(ctx->psi_smem, ctx->contract_smem, P.tables_in_smem)) != cudaSuccess) {
         release(ctx);
         return fail_cuda(e, "cudaFuncSetAttribute");
-    }
-    {   // gint_rho stages one 32-point stage of every row group of a region in shared memory
-        int max_groups = 1, max_entries = 0;
-        for (const gint::Region& r : P.regions) {
-            max_groups = r.ngroup > max_groups ? r.ngroup : max_groups;
-            max_entries = r.nentry > max_entries ? r.nentry : max_entries;
-        }
-        const size_t need = ((size_t)max_groups * gint::kGroupRows * 33 + 512 + 16 * 256) * sizeof(double) + 64 * 16 + 64 * 64 * 4;
-        ctx->rho_ok = need <= (size_t)prop.sharedMemPerBlockOptin && gint::kStagePts == 32 && max_entries <= 64;
-        if (ctx->rho_ok && (e = gint::configure_rho(&ctx->rho_smem, max_groups)) != cudaSuccess) {
-            release(ctx);
-            return fail_cuda(e, "cudaFuncSetAttribute (rho)");
-        }
     }
     *out = ctx;
     return GINT_OK;
@@ -254,6 +240,8 @@ int gint_get_blocks(const gint_ctx* ctx, int32_t* iat, int32_t* jat, int32_t* R,
 int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream) {
     if (!ctx || !V_dev || !H_dev) return fail(GINT_EINVAL, "null argument");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaError_t e = gint::launch_vlocal(ctx->dev, ctx->psi_smem, ctx->contract_smem, ctx->plan.tables_in_smem, ctx->nsm,
                                         (size_t)ctx->plan.blk_off.back(), V_dev, H_dev,
                                         reinterpret_cast<cudaStream_t>(stream), ctx->profiling ? ctx->ev : nullptr);
@@ -264,13 +252,12 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
 int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* stream) {
     if (!ctx || !D_dev || !rho_dev) return fail(GINT_EINVAL, "null argument");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
-    const bool use_dmma = gint::kStagePts == 32 && getenv("GINT_RHO_FMA") == nullptr;
-    if (!use_dmma && !ctx->rho_ok) return fail(GINT_EUNSUPPORTED, "too many orbitals or atom images listed for one region for gint_rho; use a smaller bcell");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     cudaError_t e = gint::launch_psi(ctx->dev, ctx->psi_smem, ctx->plan.tables_in_smem, ctx->nsm, nullptr, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho psi launch");
-    e = use_dmma ? gint::launch_rho_dmma(ctx->dev, ctx->contract_smem, ctx->nsm, D_dev, rho_dev, st)
-                 : gint::launch_rho_kernel(ctx->dev, ctx->rho_smem, ctx->nsm, D_dev, rho_dev, st);
+    e = gint::launch_rho_dmma(ctx->dev, ctx->contract_smem, ctx->nsm, D_dev, rho_dev, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho launch");
     return GINT_OK;
 }
@@ -285,6 +272,8 @@ int gint_num_orbitals(const gint_ctx* ctx, int64_t* norb_tot, int64_t* first) {
 int gint_fold_k(gint_ctx* ctx, const double* H_dev, const double* kfrac, double* Hk_dev, void* stream) {
     if (!ctx || !H_dev || !kfrac || !Hk_dev) return fail(GINT_EINVAL, "null argument");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaError_t e = gint::launch_fold(ctx->fold, H_dev, kfrac, Hk_dev, reinterpret_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, "gint_fold_k launch");
     return GINT_OK;
@@ -293,7 +282,8 @@ int gint_fold_k(gint_ctx* ctx, const double* H_dev, const double* kfrac, double*
 int gint_vlocal_host(gint_ctx* ctx, const double* V_host, double* H_host) {
     if (!ctx || !V_host || !H_host) return fail(GINT_EINVAL, "null argument");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
-    cudaError_t e = cudaSetDevice(ctx->device);
+    DeviceGuard guard(ctx->device);
+    cudaError_t e = guard.err;
     if (e != cudaSuccess) return fail_cuda(e, "cudaSetDevice");
     const size_t nV = (size_t)ctx->plan.ngrid[0] * ctx->plan.ngrid[1] * ctx->plan.ngrid[2];
     const size_t nH = (size_t)ctx->plan.blk_off.back();
@@ -314,8 +304,9 @@ int gint_vlocal_host(gint_ctx* ctx, const double* V_host, double* H_host) {
 int gint_set_profiling(gint_ctx* ctx, int32_t on) {
     if (!ctx) return fail(GINT_EINVAL, "ctx is null");
     if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     if (on && !ctx->have_events) {
-        cudaSetDevice(ctx->device);
         for (int i = 0; i < 5; i++) {
             cudaError_t e = cudaEventCreate(&ctx->ev[i]);
             if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
@@ -329,6 +320,8 @@ int gint_set_profiling(gint_ctx* ctx, int32_t on) {
 int gint_get_kernel_ms(gint_ctx* ctx, double* ms) {
     if (!ctx || !ms) return fail(GINT_EINVAL, "null argument");
     if (!ctx->profiling || !ctx->have_events) return fail(GINT_EINVAL, "profiling is off");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaError_t e = cudaEventSynchronize(ctx->ev[4]);
     if (e != cudaSuccess) return fail_cuda(e, "cudaEventSynchronize");
     float a = 0, b = 0, c = 0, d = 0;
@@ -345,7 +338,7 @@ int gint_get_kernel_ms(gint_ctx* ctx, double* ms) {
 
 int gint_get_stats(const gint_ctx* ctx, double* stats, int32_t n) {
     if (!ctx || !stats) return fail(GINT_EINVAL, "null argument");
-    const int m = n < 24 ? n : 24;
+    const int m = n < 32 ? n : 32;
     for (int i = 0; i < m; i++) stats[i] = ctx->plan.stats[i];
     return m;
 }
@@ -364,7 +357,8 @@ int gint_get_cell_lists(const gint_ctx* ctx, int64_t* ncell, int64_t* nentry, in
 
 int gint_measure_fp64_peak(int32_t cuda_device, double seconds, double* tflops) {
     if (!tflops || cuda_device < 0) return fail(GINT_EINVAL, "bad argument");
-    cudaError_t e = cudaSetDevice(cuda_device);
+    DeviceGuard guard(cuda_device);
+    cudaError_t e = guard.err;
     if (e != cudaSuccess) return fail_cuda(e, "cudaSetDevice");
     cudaDeviceProp prop;
     if ((e = cudaGetDeviceProperties(&prop, cuda_device)) != cudaSuccess) return fail_cuda(e, "cudaGetDeviceProperties");

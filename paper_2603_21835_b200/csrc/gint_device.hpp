@@ -1,5 +1,5 @@
 // gint_device.hpp -- kernel parameter block and launchers shared by gint_api.cu and gint_kernels.cu.
-// The plan structures (Entry, Region, WorkItem, ItemDesc, MirrorItem, SmemLayout) are plain
+// The plan structures (Entry, Region, WorkItem, ItemDesc, MirrorItem, PairWord) are plain
 // C++ and come from gint_plan.hpp; the device reads them exactly as the host wrote them.
 #pragma once
 #include <cuda_runtime.h>
@@ -16,15 +16,15 @@ struct DevicePlan {
     ItemDesc* descs;          // one per work item, queue order; sign bits filled in by gint_psi_kernel
     const Region* regions;
     const Entry* entries;
-    const uint32_t* etasks;   // evaluation tasks: entry within region | slice << 16
-    const uint32_t* pair;
+    const uint32_t* etasks;   // evaluation tasks: entry within region | run of 8 stages << 16
+    const PairWord* pair;     // (entry a <= entry b) -> where C[mu of a][nu of b] goes in H (gint_vlocal flush)
     const uint32_t* pair_direct;   // (entry a, entry b) -> offset of block (I_a, I_b, R_b - R_a) (gint_rho)
     const uint8_t* slot_xyz;  // [nslice*32][4]
     const double* tab;        // packed radial tables, per species [ntab+4][nradp]
     const int32_t* sp_meta;   // per species 12 ints: tab_offset, ntab, nradp, norb, l[8]
     const double* sp_real;    // per species: rcut^2, 1/dr
     const MirrorItem* mirror;
-    double* psi;              // scratch: psi_chunks x 512 doubles, zero-filled once at setup
+    double* psi;              // scratch: psi_chunks x 1024 doubles, zero-filled once at setup
     unsigned int* counter;    // work-queue head, reset before every launch
     const int32_t* work_regions;   // indices of the regions that own work items
     double estep[9];          // mesh step vectors a_d / N_d (rows)
@@ -33,9 +33,9 @@ struct DevicePlan {
     int32_t nks_pad, nslice, nstage;
     int32_t nitems, nmirror, nregions, nwork_regions;
     int32_t tab_doubles;
+    int32_t nspecies;
     int32_t nring;
-    int32_t debug;            // development builds (GINT_TIMING) only: 1 skip contraction, 2 skip evaluation, 4 skip flush
-    int32_t never;            // always 0: a branch condition the compiler cannot fold (see DMMA_IF in gint_kernels.cu)
+    int32_t never;            // always 0: a branch condition the compiler cannot fold (see KROW in gint_kernels.cu)
 };
 
 // k-space assembly (gint_fold.cu): the block table as the device needs it
@@ -51,11 +51,9 @@ struct FoldPlan {
 cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream);
 cudaError_t launch_rho_dmma(const DevicePlan& P, size_t contract_smem_bytes, int nsm, const double* D, double* rho,
                             cudaStream_t stream);
-cudaError_t launch_rho_kernel(const DevicePlan& P, size_t smem, int nsm, const double* D, double* rho, cudaStream_t stream);
-cudaError_t configure_rho(size_t* smem_out, int max_groups);
 cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac, double* Hk, cudaStream_t stream);
 
-size_t psi_kernel_smem(size_t table_bytes);
+size_t psi_kernel_smem(size_t table_bytes, int nspecies);
 size_t contract_kernel_smem(int nring);
 cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool tab_smem);
 // ev: nullptr, or 5 events recorded at call start / before psi / before contraction / after it / after mirror

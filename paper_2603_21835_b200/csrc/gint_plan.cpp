@@ -85,11 +85,9 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         for (int c = 0; c < 3; c++)
             if (!std::isfinite(atom_pos[3 * a + c])) { err = "atom position not finite"; return GINT_EINVAL; }
     }
-    int64_t bprod = 1;
     for (int d = 0; d < 3; d++) {
         P.ngrid[d] = ngrid[d];
         int b = (bcell && bcell[d] > 0) ? bcell[d] : 0;
-        bprod *= (b > 0 ? b : 1);
         if (b == 0) {   // default: the largest of 8, 6, 4 that divides N (8 with a ragged last region otherwise)
             b = 8;
             for (int c : {8, 6, 4})
@@ -100,7 +98,10 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         P.ncell[d] = (ngrid[d] + b - 1) / b;
         for (int c = 0; c < 3; c++) P.estep[3 * d + c] = lattice[3 * d + c] / (double)ngrid[d];
     }
-    if (bprod > kMaxRegionPoints || (int64_t)P.bcell[0] * P.bcell[1] * P.bcell[2] > kMaxRegionPoints) { err = "region (bcell) larger than 512 mesh points"; return GINT_EUNSUPPORTED; }
+    // checked after clamping to the mesh: at most 512 points per region, every edge <= 255 (point offsets are bytes)
+    if ((int64_t)P.bcell[0] * P.bcell[1] * P.bcell[2] > kMaxRegionPoints) { err = "region (bcell) larger than 512 mesh points"; return GINT_EUNSUPPORTED; }
+    for (int d = 0; d < 3; d++)
+        if (P.bcell[d] > 255) { err = "region (bcell) edge longer than 255 mesh points"; return GINT_EUNSUPPORTED; }
     P.dV = vol / ((double)ngrid[0] * (double)ngrid[1] * (double)ngrid[2]);
 
     double inv[9];
@@ -144,7 +145,8 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                     }
         }
     const int64_t nblk = (int64_t)P.blk_i.size();
-    if (P.blk_off.back() >= (int64_t)kNoBlock) { err = "H buffer exceeds 2^32 doubles"; return GINT_EUNSUPPORTED; }
+    // block offsets are stored in 32 bits (kNoBlock = 2^32 - 1 marks "no such block"): H below 32 GiB
+    if (P.blk_off.back() >= (int64_t)kNoBlock) { err = "H buffer exceeds 2^32 - 1 doubles"; return GINT_EUNSUPPORTED; }
 
     // ---- hash (I,J,R) -> offset; mirror lists ---------------------------------
     uint32_t hsize = 16;
@@ -216,9 +218,6 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     }
     P.tables_in_smem = P.tab_packed.size() * sizeof(double) <= kMaxTableSmem;
     P.nring = kRingStages;
-#ifdef GINT_TIMING
-    if (const char* e = getenv("GINT_NRING")) P.nring = std::min(P.nring, atoi(e));
-#endif
     P.smem_bytes = 256 + smem_align((size_t)kDescSlots * sizeof(ItemDesc)) + (size_t)P.nring * kMaxSlots * kChunkBytes;
 
     // ---- point order inside a region: k-steps of 4 points, slices of 8 k-steps -----------------
@@ -439,7 +438,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 gm[(size_t)g * nks_pad + ks] = b;
             }
         // pair table: (row entry a <= column entry b) -> canonical block offset (+ transposed flag)
-        P.pair.resize(P.pair.size() + (size_t)m * m, kNoBlock);
+        P.pair.resize(P.pair.size() + (size_t)m * m, PairWord{kNoBlock, 0, 0});
         P.pair_direct.resize(P.pair.size(), kNoBlock);
         for (int a = 0; a < m; a++)
             for (int b = a; b < m; b++) {
@@ -451,25 +450,28 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 const bool zeroR = (r1 == 0 && r2 == 0 && r3 == 0);
                 const bool posR = (r1 > 0) || (r1 == 0 && (r2 > 0 || (r2 == 0 && r3 > 0)));
                 const bool canonical = (ea.atom < eb.atom) || (ea.atom == eb.atom && (zeroR || posR));
-                uint32_t off = canonical ? lookup(ea.atom, eb.atom, r1, r2, r3) : lookup(eb.atom, ea.atom, -r1, -r2, -r3);
-                if (off != kNoBlock && !canonical) off |= kPairTransposed;
-                P.pair[(size_t)R.pair_off + (size_t)a * m + b] = off;
+                PairWord pw;
+                pw.off = canonical ? lookup(ea.atom, eb.atom, r1, r2, r3) : lookup(eb.atom, ea.atom, -r1, -r2, -r3);
+                pw.smu = (uint16_t)(canonical ? eb.norb : 1);
+                pw.snu = (uint16_t)(canonical ? 1 : ea.norb);
+                P.pair[(size_t)R.pair_off + (size_t)a * m + b] = pw;
                 P.pair_direct[(size_t)R.pair_off + (size_t)a * m + b] = lookup(ea.atom, eb.atom, r1, r2, r3);
                 P.pair_direct[(size_t)R.pair_off + (size_t)b * m + a] = lookup(eb.atom, ea.atom, -r1, -r2, -r3);
             }
         // tiles (group gi <= gj) and their cost (DMMAs) per stage
-        // the kernel decides per k-pair (2 k-steps, a 2x2x2 box of mesh points): a fragment pair is
-        // executed for both k-steps if either holds an in-sphere point of both fragments' rows
+        // the kernel decides per k-step (4 mesh points): a fragment pair is executed if the k-step holds an
+        // in-sphere point of both fragments' rows
+        auto kstep_cost = [&](int gi, int gj, int ks) {
+            const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
+            if (gi != gj) return __builtin_popcount(ra) * __builtin_popcount(ca);
+            int n = 0;
+            for (int i = 0; i < 4; i++)
+                if ((ra >> i) & 1u) n += __builtin_popcount(ca >> i);
+            return n;
+        };
         auto tile_stage_cost = [&](int gi, int gj, int st) {
             int n = 0;
-            for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks += 2) {
-                const unsigned ra = gm[(size_t)gi * nks_pad + ks] | gm[(size_t)gi * nks_pad + ks + 1];
-                const unsigned ca = gm[(size_t)gj * nks_pad + ks] | gm[(size_t)gj * nks_pad + ks + 1];
-                if (gi != gj) n += 2 * __builtin_popcount(ra) * __builtin_popcount(ca);
-                else
-                    for (int i = 0; i < 4; i++)
-                        if ((ra >> i) & 1u) n += 2 * __builtin_popcount(ca >> i);
-            }
+            for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) n += kstep_cost(gi, gj, ks);
             return n;
         };
         struct Proto { std::vector<std::pair<int, int>> tiles; std::vector<int> groups; };
@@ -556,20 +558,29 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 w.tiles[warp][0] = (uint8_t)slot_of(p.tiles[t].first);
                 w.tiles[warp][1] = (uint8_t)slot_of(p.tiles[t].second);
                 exec_dmma += tc;
-                for (int ks = 0; ks < nks_pad; ks += 2) {
+                for (int ks = 0; ks < nks_pad; ks++) {
                     const int gi = p.tiles[t].first, gj = p.tiles[t].second;
-                    const unsigned ra = gm[(size_t)gi * nks_pad + ks] | gm[(size_t)gi * nks_pad + ks + 1];
-                    const unsigned ca = gm[(size_t)gj * nks_pad + ks] | gm[(size_t)gj * nks_pad + ks + 1];
-                    int nd = 0;
-                    if (gi != gj) nd = 2 * __builtin_popcount(ra) * __builtin_popcount(ca);
-                    else
-                        for (int i = 0; i < 4; i++)
-                            if ((ra >> i) & 1u) nd += 2 * __builtin_popcount(ca >> i);
-                    if (gi != gj && nd == 32) ks_full += 1;
+                    const int nd = kstep_cost(gi, gj, ks);
+                    if (gi != gj && nd == 16) ks_full += 1;
                     else if (nd > 0) { ks_part += 1; dmma_part += nd; }
                 }
                 for (int st = 0; st < nstage; st++)
                     if (tile_stage_cost(p.tiles[t].first, p.tiles[t].second, st) > 0) w.stage_mask |= 1u << st;
+                for (int st = 0; st < nstage; st++) {   // development statistics: how uniform are the masks within a stage
+                    const int gi = p.tiles[t].first, gj = p.tiles[t].second;
+                    const int c = tile_stage_cost(gi, gj, st);
+                    if (!c) continue;
+                    bool uniform = true, allact = true; int first = -1;
+                    for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) {
+                        const int key = gm[(size_t)gi * nks_pad + ks] | (gm[(size_t)gj * nks_pad + ks] << 4);
+                        if (kstep_cost(gi, gj, ks) == 0) { allact = false; continue; }
+                        if (first < 0) first = key; else if (key != first) uniform = false;
+                    }
+                    if (c == (gi == gj ? 80 : 128)) P.stats[26] += c;
+                    if (uniform && allact) P.stats[27] += c;
+                    if (uniform) P.stats[28] += c;
+                    P.stats[29] += 1;
+                }
             }
             ri.cost += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
             bal_item += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
@@ -626,14 +637,18 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         const Region& R = d.item.reg;
         for (int q = 0; q < d.item.nslot; q++) {
             const int g = d.item.slot_group[q];
-            std::memcpy(d.gmask[q], &P.gmask[(size_t)R.gmask_off + (size_t)g * nks_pad], (size_t)nks_pad);
+            const uint8_t* gmq = &P.gmask[(size_t)R.gmask_off + (size_t)g * nks_pad];
+            for (int st = 0; st < nstage; st++) {
+                uint32_t wd = 0;
+                for (int ks = 0; ks < kStageKsteps; ks++) wd |= (uint32_t)(gmq[st * kStageKsteps + ks] & 0xFu) << (4 * ks);
+                d.gm32[q][st] = wd;
+            }
             std::memcpy(d.rinfo[q], &P.rowinfo[(size_t)R.rowinfo_off + (size_t)g * kGroupRows], sizeof(uint32_t) * kGroupRows);
         }
         for (int st = 0; st < nstage; st++) {
             uint32_t a = 0;
             for (int q = 0; q < d.item.nslot; q++)
-                for (int ks = 0; ks < kStageKsteps; ks++)
-                    if (d.gmask[q][st * kStageKsteps + ks]) a |= 1u << q;
+                if (d.gm32[q][st]) a |= 1u << q;
             d.act[st] = (uint8_t)a;
         }
         d.valid = 1;
@@ -667,6 +682,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[20] = bal_item;    // sum over items of the heaviest scheduler's DMMAs (perfect overlap inside an item)
     P.stats[21] = bal_stage;   // same if the warps moved through the stages in lockstep
     P.stats[22] = bal_warp;    // sum over (item, stage) of the heaviest single warp's DMMAs
+    for (int d = 0; d < 3; d++) P.stats[23 + d] = (double)P.bcell[d];
     return GINT_OK;
 }
 

@@ -7,20 +7,19 @@
 // -- PAPER.md:380 (Sec. 3.3.1), Fig. 2 at PAPER.md:368.
 //
 // A *region* is this build's BigGrid: a box of up to 512 mesh points.  Its points
-// are ordered into k-steps of 4 points (the K of one DMMA.8x8x4), stages of 4
-// k-steps (16 points, one shared-memory pipeline stage of the contraction) and
-// evaluation slices of 2 stages (32 points, one lane per point).  Every (atom
-// image, region) pair whose sphere holds a point of the region is an *entry*;
-// entries are sorted densest first and their orbitals are packed into consecutive
-// *rows* of the region's psi matrix, psi = phi sqrt(|V dV|).  Rows are cut into
-// fragments of 8 (one DMMA operand) and groups of 32 (one warp-tile edge).  The
-// upper triangle of the region's  C = psi diag(sign V) psi^T  is cut into 32x32
-// tiles; tiles are packed 7 at a time (one per consumer warp) into *work items*
-// that touch at most kMaxSlots row groups.  The items of a region are consecutive
-// in the work queue; the CTA that takes item q of n evaluates share q of the
-// region's psi (phase 1), writes it to the psi scratch buffer in global memory
-// (L2-resident between the sibling CTAs) and later streams the groups its tiles
-// need back through shared memory with bulk copies (phase 2).
+// are ordered into k-steps of 4 points (2x2x1, the K of one DMMA.8x8x4) and stages
+// of 8 k-steps (32 points: one shared-memory pipeline stage of the contraction and
+// one evaluation slice of the psi kernel, one lane per point).  Every (atom image,
+// region) pair whose sphere holds a point of the region is an *entry*; entries are
+// sorted densest first and their orbitals are packed into consecutive *rows* of the
+// region's psi matrix, psi = phi sqrt(|V dV|).  Rows are cut into fragments of 8
+// (one DMMA operand) and groups of 32 (one warp-tile edge).  The upper triangle of
+// the region's  C = psi diag(sign V) psi^T  is cut into 32x32 tiles; tiles are
+// packed kTilesPerItem at a time (one per consumer warp) into *work items* that
+// touch at most kMaxSlots row groups.  gint_psi_kernel writes psi of every region
+// once into the scratch buffer (chunks of one (group, stage): [k-step 8][row 32]
+// [point 4] doubles = 8 KB); gint_contract_kernel streams the chunks an item needs
+// through a shared-memory ring with bulk copies.
 //
 // Output of the plan (plain arrays, uploaded verbatim by gint_api.cu):
 //   * block table (I,J,R) sorted, offsets, mirror list
@@ -44,26 +43,20 @@ namespace gint {
 constexpr int kMaxOrbPerAtom = 64;
 constexpr int kMaxRegionPoints = 512;          // mesh points of one region
 constexpr int kKstepPts = 4;                   // K of DMMA.8x8x4
-#ifndef GINT_CTAS_PER_SM
-#define GINT_CTAS_PER_SM 1                     // contraction CTAs per SM: 2 x (7 consumer warps + producer) or 1 x (15 + producer)
-#endif
-constexpr int kCtasPerSm = GINT_CTAS_PER_SM;
-constexpr int kStageKsteps = kCtasPerSm == 2 ? 4 : 8;   // k-steps per pipeline stage
-constexpr int kStagePts = kKstepPts * kStageKsteps;     // 16 or 32
-constexpr int kStagePairs = kStageKsteps / 2;           // k-pairs (2x2x2 boxes) per stage
-constexpr int kSlicePts = 32;                  // points of one evaluation task (one lane per point)
-constexpr int kSliceKsteps = kSlicePts / kKstepPts;     // 8
+constexpr int kStageKsteps = 8;                // k-steps per pipeline stage
+constexpr int kStagePts = kKstepPts * kStageKsteps;     // 32: one stage = one evaluation slice (one lane per point)
+constexpr int kSlicePts = kStagePts;
+constexpr int kSliceKsteps = kStageKsteps;
 constexpr int kMaxKsteps = kMaxRegionPoints / kKstepPts;   // 128
-constexpr int kMaxStages = kMaxKsteps / kStageKsteps;      // 32
+constexpr int kMaxStages = kMaxKsteps / kStageKsteps;      // 16
 constexpr int kGroupRows = 32;                 // rows of one row group = warp-tile edge
 constexpr int kMaxSlots = 8;                   // row groups one work item may touch
-constexpr int kTilesPerItem = kCtasPerSm == 2 ? 7 : 15;   // one 32x32 tile per consumer warp; a CTA = consumers + 1 producer warp
-constexpr int kCliqueGroups = kCtasPerSm == 2 ? 3 : 5;    // largest c with c (c + 1) / 2 <= kTilesPerItem
+constexpr int kTilesPerItem = 15;              // one 32x32 tile per consumer warp; a CTA = 15 consumer warps + 1 producer warp
+constexpr int kCliqueGroups = 5;               // largest c with c (c + 1) / 2 <= kTilesPerItem
 constexpr int kMaxGroups = 40;                 // row groups per region (<= 1280 orbitals listed)
-constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 512: psi of one (group, stage), fragment order
-constexpr int kChunkBytes = kChunkDoubles * 8;             // 4096
+constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 1024: psi of one (group, stage), [k-step][row][point]
+constexpr int kChunkBytes = kChunkDoubles * 8;             // 8192
 constexpr uint32_t kNoBlock = 0xFFFFFFFFu;
-constexpr uint32_t kPairTransposed = 0x80000000u;
 
 struct SpeciesHost {
     double rcut = 0, dr = 0;
@@ -97,20 +90,20 @@ struct Region {          // 64 bytes
     int32_t task_off;    // into etasks
     int32_t ntask;       // evaluation tasks (entry, run of 8 slices) with a point inside the sphere
     int32_t nitem;       // work items of the region = number of evaluation shares
-    int64_t psi_chunk0;  // first 4 KB chunk of the region in the psi scratch: chunk(g, s) = psi_chunk0 + g*nstage + s
+    int64_t psi_chunk0;  // first 8 KB chunk of the region in the psi scratch: chunk(g, s) = psi_chunk0 + g*nstage + s
     int32_t ngroup;
     int32_t item0;       // first work item of the region in queue order (its nitem items are consecutive)
 };
 static_assert(sizeof(Region) == 64, "Region layout is shared with the device");
 
-// evaluation task word: entry index within the region | run << 16 (run h = slices 8h .. 8h+7)
+// evaluation task word: entry index within the region | run << 16 (run h = stages 8h .. 8h+7)
 inline uint32_t pack_etask(int e, int run) { return (uint32_t)e | ((uint32_t)run << 16); }
 
 struct WorkItem {        // 128 bytes: 64 of its own + a copy of its region (one fetch instead of two dependent ones)
     int32_t region;
     int16_t share;       // index of the item within its region: evaluates tasks t = share (mod nitem)
     int16_t ntile;
-    uint32_t stage_mask; // bit s: stage s (16 points) holds work for this item
+    uint32_t stage_mask; // bit s: stage s (32 points) holds work for this item
     uint8_t tiles[16][2];              // per consumer warp: (slot of row group, slot of column group), 0xFF = no tile
     uint8_t slot_group[kMaxSlots];     // region row group held by each slot
     int32_t nslot;
@@ -124,6 +117,15 @@ struct MirrorItem {   // dst block (I,J,R) <- transpose of src block (J,I,-R); s
     int32_t nI, nJ;
 };
 
+// Pair-table entry (row entry a <= column entry b of a region): where element (mu of a, nu of b) of the region's
+// C goes in H: off + mu * smu + nu * snu.  (smu, snu) = (n_b, 1) if the block (I_a, I_b, R_b - R_a) is canonical,
+// (1, n_a) if it is the transpose of the canonical block (I_b, I_a, R_a - R_b).  off = kNoBlock: no such block.
+struct PairWord {
+    uint32_t off;
+    uint16_t smu, snu;
+};
+static_assert(sizeof(PairWord) == 8, "PairWord layout is shared with the device");
+
 // rowinfo word: entry index within the region | mu << 12 | norb << 20; kNoBlock for padding rows
 inline uint32_t pack_rowinfo(int e, int mu, int norb) { return (uint32_t)e | ((uint32_t)mu << 12) | ((uint32_t)norb << 20); }
 
@@ -134,14 +136,15 @@ constexpr int kDescSlots = 3;           // item descriptors in flight in the con
 // memory by the contraction kernel's producer warp with one bulk copy.
 struct ItemDesc {
     WorkItem item;                                  // 128 (item.reg = its region)
-    uint8_t gmask[kMaxSlots][kMaxKsteps];           // 1024: fragment activity nibbles of the item's slots
-    uint32_t sign[kMaxRegionPoints / 32];           // 64: bit p = sign bit of V dV at point slot p
-    uint8_t act[32];                                // per stage (<= 32): bit q = slot q has an active k-step in the stage
+    uint32_t gm32[kMaxSlots][kMaxStages];           // 512: per (slot, stage): nibble ks = fragments of the slot's group
+                                                    //      with an in-sphere point in k-step ks of the stage
+    uint32_t sign[kMaxStages];                      // 64: bit p = sign bit of V dV at point p of the stage
+    uint8_t act[32];                                // per stage: bit q = slot q has an active k-step in the stage
     uint32_t rinfo[kMaxSlots][kGroupRows];          // 1024: row info words of the item's slots (flush)
     int32_t valid;                                  // 0 = queue exhausted
     int32_t pad[7];
 };
-static_assert(kSlicePts % kStagePts == 0 && kStageKsteps % 2 == 0 && kStageKsteps <= 8, "stage geometry");
+static_assert(kStageKsteps == 8 && kStagePts == 32, "one stage = 8 k-steps = one 32-bit mask word = one lane per point");
 static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
 struct Plan {
@@ -173,26 +176,26 @@ struct Plan {
     std::vector<Entry> entries;                 // region-major, densest first inside a region
     std::vector<uint8_t> gmask;
     std::vector<uint32_t> rowinfo;
-    std::vector<uint32_t> pair;
+    std::vector<PairWord> pair;                 // [nentry][nentry] per region, a <= b filled
     std::vector<uint32_t> pair_direct;          // same indexing: offset of block (I_a, I_b, R_b - R_a) itself, any order (gint_rho)
     std::vector<WorkItem> items;
     std::vector<ItemDesc> descs;                // one per work item, queue order
     std::vector<uint32_t> etasks;               // evaluation tasks, region-major
-    int64_t psi_chunks = 0;                     // 4 KB chunks of the psi scratch buffer
+    int64_t psi_chunks = 0;                     // 8 KB chunks of the psi scratch buffer
     // packed radial tables for the device: per species [ntab+4][nradp] (node-major, nradp = nrad rounded up
     // to even, every function pre-multiplied by its Y_lm constant, four zero nodes appended)
     std::vector<double> tab_packed;
     std::vector<int32_t> sp_meta;               // per species: tab_offset, ntab, nradp, norb, l[0..7] (12 ints)
     std::vector<double> sp_real;                // per species: rcut^2, 1/dr
     // statistics
-    double stats[24] = {0};
+    double stats[32] = {0};
     size_t smem_bytes = 0;
     bool tables_in_smem = true;
     int nring = 0;                              // pipeline stages of the psi ring in shared memory
 };
 
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
-constexpr int kRingStages = 3;          // 3 x 32 KB of psi in flight per CTA, two CTAs per SM
+constexpr int kRingStages = 3;          // 3 x 64 KB of psi in flight per CTA
 constexpr size_t kMaxTableSmem = 56 * 1024;   // larger radial tables stay in global memory (L1/L2-cached)
 
 inline uint64_t pack_key(int I, int J, int r1, int r2, int r3) {

@@ -165,3 +165,41 @@ def test_error_codes():
         setup(atom_pos=pos)
     assert e.value.code == binding.GINT_EINVAL
     assert binding._strerror(binding.GINT_ECUDA) == "CUDA error"
+
+
+def test_bench_flop_count_matches_the_plan(cfg1):
+    """bench.py counts the useful flops itself (k-d tree over atom images) so that its oracle arm needs no product
+    library; the count equals the plan's own statistics on a cubic cell with self-images, a triclinic cell and the
+    two-species cluster."""
+    import sys
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2603_21835_b200 import gint_setup
+    for w in (cfg1, wl.tiny(seed=7), wl.tiny(seed=11, ngrid=(9, 13, 7)), wl.make("cluster60")):
+        st = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1).gint_get_stats()
+        fpt, fsym = bench.useful_flops(w)
+        assert fpt == st["F_pt"] and fsym == st["F_sym"], w.name
+
+
+def test_reference_arm_runs_without_the_product_library(tmp_path):
+    """`bench.py --impl reference` must load oracle/ only: run it with the product .so masked (an import hook that
+    fails on the binding) and check the JSON line."""
+    import json
+    import subprocess
+    import sys
+    hook = tmp_path / "sitecustomize.py"
+    hook.write_text(
+        "import sys, importlib.abc\n"
+        "class _Block(importlib.abc.MetaPathFinder):\n"
+        "    def find_spec(self, name, path, target=None):\n"
+        "        if name == 'paper_2603_21835_b200.binding':\n"
+        "            raise ImportError('product library masked for this test')\n"
+        "sys.meta_path.insert(0, _Block())\n")
+    env = dict(os.environ, PYTHONPATH=str(tmp_path) + os.pathsep + os.environ.get("PYTHONPATH", ""))
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "si8_sz",
+                          "--steps", "1", "--warmup", "0", "--ref-atoms", "2"], env=env, capture_output=True, text=True,
+                         timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+    assert line["e2e"]["h2d_bytes_per_step"] == 0

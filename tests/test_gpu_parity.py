@@ -163,26 +163,19 @@ def test_cfg2_full():
     assert_parity(Hg, Hr, "si64_dzp")
 
 
-@pytest.mark.parametrize("name,nsample", [("si216_dzp", 300), ("si512_dzp", 400)])
-def test_large_sampled_blocks(name, nsample):
-    """Full-size configs in the launch configuration bench.py times: sampled blocks are
-    computed one by one by the oracle; global properties checked on everything."""
+@pytest.mark.parametrize("name", ["si216_dzp", "si512_dzp"])
+def test_large_full_output(name):
+    """Full-size configs in the launch configuration bench.py times (default big cells, whole work queue, the
+    multi-GB psi scratch): EVERY element of H against the oracle at the 1e-10 bar, plus exact transpose symmetry."""
     from paper_2603_21835_b200 import workloads as wl
     from helpers import norb_per_atom
     w = wl.make(name)
     Hg, ctx = gpu_H(w)
-    bi, bj, bR, off = ctx.gint_get_blocks()
+    Hr, blocks = oracle_H(w)
+    assert_blocks_equal(ctx, blocks)
+    assert_parity(Hg, Hr, name)
+    bi, bj, bR, off = blocks
     rng = np.random.default_rng(42)
-    sel = np.sort(rng.choice(len(bi), nsample, replace=False))
-    onsite = np.nonzero((bi == bj) & np.all(bR == 0, axis=1))[0][:8]
-    sel = np.unique(np.concatenate([sel, onsite]))
-    Hs, (si, sj, sR, soff) = oracle_H(w, blocks=(bi[sel], bj[sel], bR[sel]))
-    scale = np.abs(Hs).max()
-    worst = 0.0
-    for n, b in enumerate(sel):
-        worst = max(worst, np.abs(Hg[off[b]:off[b + 1]] - Hs[soff[n]:soff[n + 1]]).max())
-    assert worst <= TOL * scale, "sampled blocks: %.3e vs scale %.3e" % (worst, scale)
-    # property valid at any size: exact transpose symmetry between partner blocks
     norb = norb_per_atom(w)
     key = {(int(bi[b]), int(bj[b]), int(bR[b, 0]), int(bR[b, 1]), int(bR[b, 2])): b for b in range(len(bi))}
     for b in rng.choice(len(bi), 2000, replace=False):
@@ -190,7 +183,59 @@ def test_large_sampled_blocks(name, nsample):
         A = Hg[off[b]:off[b + 1]].reshape(norb[bi[b]], norb[bj[b]])
         B = Hg[off[p]:off[p + 1]].reshape(norb[bj[b]], norb[bi[b]])
         assert np.array_equal(A, B.T)
-    assert np.all(np.isfinite(Hg))
+
+
+def _sharded_cases():
+    from paper_2603_21835_b200 import workloads as wl
+    return [("si8_sz", lambda: wl.make("si8_sz")), ("tiny_ragged", lambda: wl.tiny(seed=7, ngrid=(12, 10, 14))),
+            ("tiny_9_13_7", lambda: wl.tiny(seed=11, ngrid=(9, 13, 7))), ("si64_dzp", lambda: wl.make("si64_dzp"))]
+
+
+@pytest.mark.parametrize("nranks", [2, 3])
+@pytest.mark.parametrize("case", [0, 1, 2, 3])
+def test_sharded_kernel_path_sums_to_oracle(case, nranks):
+    """The multi-GPU path on the one GPU there is: one context per rank with
+    gint_options.rank/nranks, every rank's gint_vlocal and gint_rho run on cuda:0, the partial H / rho buffers summed
+    (what the all-reduce does) and compared with the oracle; gint_fold_k on the summed H.  The tiny cases have fewer
+    cell layers along a1 than ranks, so some rank owns no work at all (its H must be all zeros)."""
+    torch = _torch()
+    import oracle
+    from helpers import norb_per_atom
+    from paper_2603_21835_b200 import gint_setup
+    name, mk = _sharded_cases()[case]
+    w = mk()
+    Hr, blocks = oracle_H(w)
+    rng = np.random.default_rng(100 + case)
+    D = rng.normal(size=Hr.shape)
+    rho_ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blocks)
+    Vd = torch.from_numpy(w.V).cuda()
+    Dd = torch.from_numpy(D).cuda()
+    Hsum = torch.zeros(Hr.shape[0], dtype=torch.float64, device="cuda")
+    rsum = torch.zeros(tuple(int(x) for x in w.ngrid), dtype=torch.float64, device="cuda")
+    fsum, empty_ranks, ctx = 0.0, 0, None
+    for r in range(nranks):
+        ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=0, rank=r, nranks=nranks)
+        assert_blocks_equal(ctx, blocks)
+        st = ctx.gint_get_stats()
+        fsum += st["F_sym"]
+        Hp = ctx.gint_vlocal(Vd)
+        rp = ctx.gint_rho(Dd)
+        if st["items"] == 0:
+            empty_ranks += 1
+            assert float(Hp.abs().max()) == 0.0 and float(rp.abs().max()) == 0.0
+        Hsum += Hp
+        rsum += rp
+    torch.cuda.synchronize()
+    full = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1).gint_get_stats()
+    assert fsum == full["F_sym"]
+    if name.startswith("tiny") and nranks == 3:
+        assert empty_ranks >= 1
+    assert_parity(Hsum.cpu().numpy(), Hr, "%s sharded x%d" % (name, nranks))
+    assert np.abs(rsum.cpu().numpy() - rho_ref).max() <= TOL * np.abs(rho_ref).max()
+    kf = (0.31, -0.17, 0.43)
+    Hk = ctx.gint_fold_k(Hsum, kf).cpu().numpy()
+    ref = oracle.fold_k(Hr, blocks, norb_per_atom(w), kf)
+    assert np.abs(Hk - ref).max() <= 1e-10 * np.abs(ref).max()
 
 
 def test_repeatability_stress():
@@ -312,12 +357,11 @@ def test_rho_cfg2_and_cluster():
         assert np.abs(got - ref).max() <= TOL * np.abs(ref).max(), name
 
 
-def test_rho_large_sampled_points_and_adjoint():
-    """si512_dzp at full size: 40 sampled mesh points recomputed one by one from Eq. 44 with the oracle's phi (numpy
-    image loops), and the adjoint identity sum_g V rho dV = D : H[V] over the whole mesh (H from gint_vlocal)."""
+def test_rho_large_full_mesh():
+    """si512_dzp at full size: every mesh point of rho against the oracle at the 1e-10 bar (random NON-symmetric D),
+    and the adjoint identity sum_g V rho dV = D : H[V] with H from gint_vlocal on the same context."""
     torch = _torch()
     import oracle
-    from helpers import norb_per_atom
     from paper_2603_21835_b200 import gint_setup, workloads as wl
     w = wl.make("si512_dzp")
     ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos)
@@ -329,44 +373,9 @@ def test_rho_large_sampled_points_and_adjoint():
     H = ctx.gint_vlocal(Vd)
     dV = abs(np.linalg.det(w.lattice)) / np.prod(w.ngrid)
     lhs, rhs = float((Vd * rho).sum()) * dV, float((Dd * H).sum())
-    assert abs(lhs - rhs) <= 1e-10 * float(H.abs().max()) * np.abs(D).sum()
-    rho = rho.cpu().numpy()
-    bi, bj, bR, off = ctx.gint_get_blocks()
-    key = {(int(bi[b]), int(bj[b]), int(bR[b, 0]), int(bR[b, 1]), int(bR[b, 2])): b for b in range(len(bi))}
-    norb = norb_per_atom(w)
-    n = np.array(w.ngrid)
-    scale = np.abs(rho).max()
-    shifts = np.array([[a, b, c] for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)])
-    for g in rng.integers(0, n, size=(40, 3)):
-        r = (g / n) @ w.lattice
-        ents = []      # (atom, image shift R', phi values) of every image that reaches the point
-        for s in shifts:
-            d = r - w.atom_pos - s @ w.lattice
-            for I in np.nonzero(np.einsum("ij,ij->i", d, d) < max(sp.rcut for sp in w.species) ** 2)[0]:
-                ph = oracle.phi(w.species, int(w.atom_species[I]), d[I:I + 1])[0]
-                if np.any(ph):
-                    ents.append((int(I), s, ph))
-        ref = 0.0
-        for I, sa, pa in ents:
-            for J, sb, pb in ents:
-                R = sb - sa
-                b = key.get((I, J, int(R[0]), int(R[1]), int(R[2])))
-                if b is not None:
-                    ref += pa @ D[off[b]:off[b + 1]].reshape(norb[I], norb[J]) @ pb
-        assert abs(rho[tuple(g)] - ref) <= TOL * scale
-
-
-def test_rho_fma_fallback_matches_tensor_path(cfg1, cfg1_oracle, monkeypatch):
-    """The FP64-FMA kernel of csrc/gint_rho.cu (GINT_RHO_FMA=1, read at call time) and the tensor-pipe path give the
-    same density to rounding, and both match the oracle."""
-    import oracle
-    rng = np.random.default_rng(31)
-    H0, blocks = cfg1_oracle
-    D = rng.normal(size=H0.shape)
-    ref = oracle.rho(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, D, blocks)
-    a, _ = gpu_rho(cfg1, D)
-    monkeypatch.setenv("GINT_RHO_FMA", "1")
-    b, _ = gpu_rho(cfg1, D)
-    scale = np.abs(ref).max()
-    assert np.abs(a - ref).max() <= TOL * scale and np.abs(b - ref).max() <= TOL * scale
-    assert np.abs(a - b).max() <= 1e-12 * scale
+    # both sides are sums of ~1e7 terms of size <= max|H| max|D|: 1e-10 of the largest partial sum
+    assert abs(lhs - rhs) <= 1e-10 * float((Dd * H).abs().sum())
+    ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, ctx.gint_get_blocks())
+    got = rho.cpu().numpy()
+    assert np.all(np.isfinite(got))
+    assert np.abs(got - ref).max() <= TOL * np.abs(ref).max()
