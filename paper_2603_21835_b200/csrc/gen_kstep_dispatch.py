@@ -51,13 +51,90 @@ def diag():
     return out
 
 
+def run_block(name, tblname, key, a_frags, b_frags, pairs, diag):
+    """One pattern of a RUN of consecutive k-steps (1 KB apart in the chunks): software-pipelined loop over two
+    register sets (ping-pong, no copies) -- the operands of the next k-step are loaded (predicated on there being
+    one) before the DMMAs of the current one are issued, so a single warp can keep the FP64 tensor pipe busy by
+    itself, with the fewest instructions around the DMMAs.  Operands: %0..%31 accumulators, %32 / %33 shared-memory
+    byte addresses of the lane's A / B element of the first k-step, %34 number of k-steps, %35 pattern."""
+    L = name + str(key)
+    o = ['"%s:\\n\\t"' % L]
+
+    def lds(pred, dst_prefix, off):
+        out = []
+        for i in a_frags:
+            out.append('"%sld.shared.f64 %sa%d, [pa+%d];\\n\\t"' % (pred, dst_prefix, i, 256 * i + off))
+        for j in b_frags:
+            out.append('"%sld.shared.f64 %sb%d, [pb+%d];\\n\\t"' % (pred, dst_prefix, j, 256 * j + off))
+        return out
+
+    def mmas(prefix):
+        out = []
+        for (i, j) in pairs:
+            c0, c1 = (4 * i + j) * 2, (4 * i + j) * 2 + 1
+            bop = ("%sa%d" % (prefix, j)) if diag else ("%sb%d" % (prefix, j))
+            out.append('"mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%%%d,%%%d}, {%sa%d}, {%s}, {%%%d,%%%d};\\n\\t"' % (c0, c1, prefix, i, bop, c0, c1))
+        return out
+
+    def advance(nbytes):
+        out = ['"add.u32 pa, pa, %d;\\n\\t"' % nbytes]
+        if b_frags:
+            out.append('"add.u32 pb, pb, %d;\\n\\t"' % nbytes)
+        return out
+
+    o += lds("", "", 0)
+    o.append('"%sL:\\n\\t"' % L)
+    o.append('"setp.gt.u32 p, n, 1;\\n\\t"')
+    o += lds("@p ", "n", 1024)
+    o += mmas("")
+    o.append('"@!p bra.uni %sDONE;\\n\\t"' % name)
+    o.append('"setp.gt.u32 p, n, 2;\\n\\t"')
+    o += lds("@p ", "", 2048)
+    o += mmas("n")
+    o += advance(2048)
+    o.append('"sub.u32 n, n, 2;\\n\\t"')
+    o.append('"@p bra.uni %sL;\\n\\t"' % L)
+    o.append('"bra.uni %sDONE;\\n\\t"' % name)
+    return o
+
+
+RUN_HEAD = ['"{\\n\\t"', '".reg .f64 a<4>, b<4>, na<4>, nb<4>;\\n\\t"', '".reg .pred p;\\n\\t"', '".reg .u32 pa, pb, n;\\n\\t"',
+            '"mov.u32 pa, %32;\\n\\t"', '"mov.u32 pb, %33;\\n\\t"', '"mov.u32 n, %34;\\n\\t"']
+
+
+def rect_runs():
+    """off-diagonal tile, all four row fragments active (97 % of the off-diagonal DMMAs): pattern = column mask ca"""
+    out = list(RUN_HEAD)
+    labels = ", ".join("RR%d" % k if k else "RRDONE" for k in range(16))
+    out += ['"RRTBL: .branchtargets %s;\\n\\t"' % labels, '"brx.idx.uni %35, RRTBL;\\n\\t"']
+    for ca in range(1, 16):
+        cols = [j for j in range(4) if (ca >> j) & 1]
+        out += run_block("RR", "RRTBL", ca, [0, 1, 2, 3], cols, [(i, j) for i in range(4) for j in cols], False)
+    out.append('"RRDONE:\\n\\t}\\n"')
+    return out
+
+
+def diag_runs():
+    """diagonal tile (row group == column group, so B = A): pattern = fragment mask ra, pairs i <= j"""
+    out = list(RUN_HEAD)
+    labels = ", ".join("DR%d" % k if k else "DRDONE" for k in range(16))
+    out += ['"DRTBL: .branchtargets %s;\\n\\t"' % labels, '"brx.idx.uni %35, DRTBL;\\n\\t"']
+    for ra in range(1, 16):
+        fr = [i for i in range(4) if (ra >> i) & 1]
+        out += run_block("DR", "DRTBL", ra, fr, [], [(i, j) for i in fr for j in fr if i <= j], True)
+    out.append('"DRDONE:\\n\\t}\\n"')
+    return out
+
+
 def main():
     here = os.path.dirname(os.path.abspath(__file__))
     with open(os.path.join(here, "gint_kstep_dispatch.inc"), "w") as f:
         f.write("// GENERATED by gen_kstep_dispatch.py -- do not edit.  Inline-PTX bodies of the k-step dispatch\n")
         f.write("// (brx.idx jump table over the fragment-activity patterns; see gint_kernels.cu).\n")
         f.write("#define GINT_KSTEP_RECT_ASM \\\n    " + " \\\n    ".join(rect()) + "\n\n")
-        f.write("#define GINT_KSTEP_DIAG_ASM \\\n    " + " \\\n    ".join(diag()) + "\n")
+        f.write("#define GINT_KSTEP_DIAG_ASM \\\n    " + " \\\n    ".join(diag()) + "\n\n")
+        f.write("#define GINT_RUN_RECT_ASM \\\n    " + " \\\n    ".join(rect_runs()) + "\n\n")
+        f.write("#define GINT_RUN_DIAG_ASM \\\n    " + " \\\n    ".join(diag_runs()) + "\n")
 
 
 if __name__ == "__main__":

@@ -148,11 +148,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         release(ctx);                                                  \
         return fail_cuda(e, "upload " #vec);                           \
     }
-    {
-        const gint::ItemDesc* dd = nullptr;
-        if ((e = upload(ctx, P.descs, &dd)) != cudaSuccess) { release(ctx); return fail_cuda(e, "upload descs"); }
-        D.descs = const_cast<gint::ItemDesc*>(dd);
-    }
+    UP(P.descs, &D.descs)
     UP(P.regions, &D.regions)
     UP(P.entries, &D.entries)
     UP(P.etasks, &D.etasks)
@@ -178,14 +174,16 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         UP(first32, &ctx->fold.first)
     }
 #undef UP
-    void* ctr = nullptr;   // work-queue head
-    if ((e = cudaMalloc(&ctr, 64)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
+    void* ctr = nullptr;   // work-queue head, shift of the potential, partial (min, max) of V
+    if ((e = cudaMalloc(&ctr, 128 + 2 * 512 * sizeof(double))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
     ctx->allocs.push_back(ctr);
     D.counter = reinterpret_cast<unsigned int*>(ctr);
+    D.shift = reinterpret_cast<gint::ShiftDev*>(reinterpret_cast<unsigned char*>(ctr) + 64);
+    D.vpart = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(ctr) + 128);
     {
         std::vector<int32_t> work;
         for (size_t r = 0; r < P.regions.size(); r++)
-            if (P.regions[r].nitem > 0) work.push_back((int32_t)r);
+            if (P.regions[r].ntile > 0) work.push_back((int32_t)r);
         D.nwork_regions = (int32_t)work.size();
         if ((e = upload(ctx, work, &D.work_regions)) != cudaSuccess) { release(ctx); return fail_cuda(e, "upload work_regions"); }
     }
@@ -205,7 +203,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     D.nregions = (int32_t)P.regions.size();
     D.nring = P.nring;
     D.never = 0;
-    D.nitems = (int32_t)P.items.size();
+    D.nitems = (int32_t)P.descs.size();
     D.nmirror = (int32_t)P.mirror.size();
     D.tab_doubles = (int32_t)P.tab_packed.size();
     D.nspecies = (int32_t)P.species.size();
@@ -214,6 +212,22 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
     if ((e = gint::configure_kernels(ctx->psi_smem, ctx->contract_smem, P.tables_in_smem)) != cudaSuccess) {
         release(ctx);
         return fail_cuda(e, "cudaFuncSetAttribute");
+    }
+    {   // S = grid overlap blocks (Eq. 45 with V = 1): the per-call shift of the potential needs them (gint_hinit_kernel)
+        const size_t nH = (size_t)P.blk_off.back(), nV = (size_t)P.ngrid[0] * P.ngrid[1] * P.ngrid[2];
+        void *Sd = nullptr, *ones = nullptr;
+        if ((e = cudaMalloc(&Sd, (nH ? nH : 1) * sizeof(double))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc S"); }
+        ctx->allocs.push_back(Sd);
+        D.S = reinterpret_cast<const double*>(Sd);
+        if ((e = cudaMalloc(&ones, nV * sizeof(double))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc V=1"); }
+        std::vector<double> one(nV, 1.0);
+        e = cudaMemcpy(ones, one.data(), nV * sizeof(double), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess)
+            e = gint::launch_vlocal(D, ctx->psi_smem, ctx->contract_smem, P.tables_in_smem, ctx->nsm, nH,
+                                    reinterpret_cast<const double*>(ones), reinterpret_cast<double*>(Sd), true, nullptr, nullptr);
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        cudaFree(ones);
+        if (e != cudaSuccess) { release(ctx); return fail_cuda(e, "grid overlap S"); }
     }
     *out = ctx;
     return GINT_OK;
@@ -243,7 +257,7 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
     DeviceGuard guard(ctx->device);
     if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaError_t e = gint::launch_vlocal(ctx->dev, ctx->psi_smem, ctx->contract_smem, ctx->plan.tables_in_smem, ctx->nsm,
-                                        (size_t)ctx->plan.blk_off.back(), V_dev, H_dev,
+                                        (size_t)ctx->plan.blk_off.back(), V_dev, H_dev, false,
                                         reinterpret_cast<cudaStream_t>(stream), ctx->profiling ? ctx->ev : nullptr);
     if (e != cudaSuccess) return fail_cuda(e, "gint_vlocal launch");
     return GINT_OK;

@@ -11,9 +11,16 @@
 
 namespace gint {
 
+// Shift of the potential chosen per gint_vlocal call (gint_hinit_kernel): H = c S - C (neg = 1) or c S + C (neg = 0),
+// C = sum_g phi |V - c| phi dV.
+struct ShiftDev {
+    double c;
+    uint32_t neg, pad;
+};
+
 // Kernel parameter block (passed by value as a __grid_constant__).
 struct DevicePlan {
-    ItemDesc* descs;          // one per work item, queue order; sign bits filled in by gint_psi_kernel
+    const ItemDesc* descs;    // one per work item, queue order
     const Region* regions;
     const Entry* entries;
     const uint32_t* etasks;   // evaluation tasks: entry within region | run of 8 stages << 16
@@ -24,6 +31,9 @@ struct DevicePlan {
     const int32_t* sp_meta;   // per species 12 ints: tab_offset, ntab, nradp, norb, l[8]
     const double* sp_real;    // per species: rcut^2, 1/dr
     const MirrorItem* mirror;
+    const double* S;          // grid overlap blocks (Eq. 45 with V = 1), H layout; built once at setup
+    ShiftDev* shift;          // this call's shift of the potential
+    double* vpart;            // per-block (min, max) of V
     double* psi;              // scratch: psi_chunks x 1024 doubles, zero-filled once at setup
     unsigned int* counter;    // work-queue head, reset before every launch
     const int32_t* work_regions;   // indices of the regions that own work items
@@ -57,8 +67,9 @@ size_t psi_kernel_smem(size_t table_bytes, int nspecies);
 size_t contract_kernel_smem(int nring);
 cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool tab_smem);
 // ev: nullptr, or 5 events recorded at call start / before psi / before contraction / after it / after mirror
+// raw: integrate a non-negative V without the shift (builds S at setup)
 cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
-                          size_t h_len, const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev);
+                          size_t h_len, const double* V, double* H, bool raw, cudaStream_t stream, cudaEvent_t* ev);
 cudaError_t measure_dmma_peak(double seconds, int nsm, double* tflops);
 
 }  // namespace gint

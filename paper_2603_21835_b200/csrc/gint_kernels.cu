@@ -4,22 +4,26 @@
 //
 // Two kernels per call, both behind gint_vlocal (plus a tiny mirror kernel):
 //
-//   gint_psi_kernel     psi = phi sqrt(|V dV|) for every (atom image, mesh point) pair listed by
+//   gint_vrange_kernel / gint_hinit_kernel   range of V, then H <- c S with S the grid overlap (Eq. 45 with
+//       V = 1, computed once at setup) and c = max V (or min V, whichever is smaller in magnitude): the rest of
+//       the call integrates the one-signed potential u = |V - c| >= 0,  H = c S -/+ sum_g phi u phi dV,  so that
+//       the weight can be split evenly over the two operands of a SYMMETRIC product (no per-point sign).
+//   gint_psi_kernel     psi = phi sqrt(u dV) for every (atom image, mesh point) pair listed by
 //       the plan, evaluated exactly once -- Eq. 1: 4-point Lagrange radial table x real Y_lm, one
-//       lane per mesh point -- and stored to a scratch buffer as chunks [k-step][row][point] of one
-//       (row group, 32-point stage), together with the sign bits of V per region.  The V dV
-//       weighting of Eq. 45 is thereby folded into the operand: C = psi diag(sign V) psi^T.
+//       lane per mesh point -- and stored to a scratch buffer as chunks [k-step][row pair][point][parity] of
+//       one (row group, 32-point stage).  The V dV weighting of Eq. 45 is thereby folded into the operand:
+//       C = psi psi^T.
 //   gint_contract_kernel<0>  (gint_vlocal) output-stationary contraction (the paper's per-BigGrid dense
 //       contraction).  One persistent CTA per SM pulls work items from a global
 //       queue; a work item is a set of up to 15 32x32 tiles (one per consumer warp) of the upper
-//       triangle of one region's C.  A producer warp stages the item descriptor and streams the row
+//       triangle of a region's C (small left-over tile sets of several regions share an item).  A producer warp stages the item descriptor and streams the row
 //       groups the tiles need through a ring of shared-memory stages (32 points each) with
 //       cp.async.bulk + mbarrier, running ahead across item boundaries; the 15 consumer warps keep
 //       their tile in registers and issue mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has no FP64
 //       kind).  (fragment, k-step) pairs that hold no in-sphere point are skipped by warp-uniform
 //       branches on host-built activity nibbles (a predicated-off DMMA still costs its 16 pipe
-//       cycles); the operands of the next active k-step are loaded while the DMMAs of the current
-//       one issue (two register sets, ping-pong).  After the last stage the warp adds its tile into
+//       cycles) -- one indexed jump per k-step into straight-line code for its fragment pattern.
+//       After the last stage the warp adds its tile into
 //       the canonical H blocks with red.global.add.f64 (once per item, not once per BigGrid).
 //   gint_contract_kernel<1>  (gint_rho, Eq. 44): same items, stages and producer;
 //       see rho_consumer.
@@ -68,7 +72,7 @@ __device__ __forceinline__ void load_kstep(Frag8& o, const double* __restrict__ 
     o.b3 = pb[off + 96];
 }
 __device__ __forceinline__ int frag_lane_offset(int lane) { return ((lane >> 3) << 3) + ((lane & 3) << 1) + ((lane >> 2) & 1); }
-__device__ __forceinline__ double flip_sign(double v, uint32_t x) {
+__device__ __forceinline__ double flip_sign(double v, uint32_t x) {   // x = 0 or 0x80000000
     return __hiloint2double(__double2hiint(v) ^ (int)x, __double2loint(v));
 }
 
@@ -92,29 +96,27 @@ __device__ __forceinline__ void kstep_rect(double (&acc)[4][4][2], const Frag8& 
 __device__ __forceinline__ void kstep_diag(double (&acc)[4][4][2], const Frag8& o, uint32_t key) {
     asm volatile(GINT_KSTEP_DIAG_ASM KSTEP_OPERANDS);
 }
+// A RUN of n consecutive k-steps with one pattern (the activity of a fragment along a stage is an interval, so
+// patterns persist: 3.7 k-steps per run on the Si workloads): one jump per run into a software-pipelined loop that
+// loads the next k-step's operands before the DMMAs of the current one are issued -- a single warp keeps the tensor
+// pipe busy by itself.  pa / pb: shared-memory byte addresses of this lane's element of fragment 0 of the first
+// k-step (k-steps are 1 KB apart, fragments 256 B).
+#define KRUN_OPERANDS                                                                                            \
+    : KACC_ROW(0), KACC_ROW(1), KACC_ROW(2), KACC_ROW(3)                                                         \
+    : "r"(pa), "r"(pb), "r"(n), "r"(key)
+// off-diagonal tile with all four row fragments active; key = column mask ca
+__device__ __forceinline__ void run_rect(double (&acc)[4][4][2], uint32_t pa, uint32_t pb, uint32_t n, uint32_t key) {
+    asm volatile(GINT_RUN_RECT_ASM KRUN_OPERANDS);
+}
+// diagonal tile (B = A, pairs i <= j); key = fragment mask ra
+__device__ __forceinline__ void run_diag(double (&acc)[4][4][2], uint32_t pa, uint32_t n, uint32_t key) {
+    const uint32_t pb = pa;
+    asm volatile(GINT_RUN_DIAG_ASM KRUN_OPERANDS);
+}
+#undef KRUN_OPERANDS
 #undef KACC
 #undef KACC_ROW
 #undef KSTEP_OPERANDS
-#define KX(i, j) dmma8x8x4(acc[i][j][0], acc[i][j][1], o.a##i, o.b##j);
-#define KC15(i) KX(i, 0) KX(i, 1) KX(i, 2) KX(i, 3)
-// sign of V dV onto the B operand (x = sign bit of this lane's point, already in bit 31)
-__device__ __forceinline__ void sign_b(Frag8& o, uint32_t x) {
-    o.b0 = flip_sign(o.b0, x);
-    o.b1 = flip_sign(o.b1, x);
-    o.b2 = flip_sign(o.b2, x);
-    o.b3 = flip_sign(o.b3, x);
-}
-// all 16 (10 on the diagonal) fragment pairs of one k-step
-__device__ __forceinline__ void kstep_full(double (&acc)[4][4][2], const Frag8& o, bool diag) {
-    if (!diag) {
-        KC15(0) KC15(1) KC15(2) KC15(3)
-    } else {
-        KX(0, 0) KX(0, 1) KX(0, 2) KX(0, 3) KX(1, 1) KX(1, 2) KX(1, 3) KX(2, 2) KX(2, 3) KX(3, 3)
-    }
-}
-#undef KX
-#undef KC15
-
 // ---- mbarrier / bulk-copy helpers (shared::cta addresses) --------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -236,7 +238,7 @@ __device__ __forceinline__ void eval_task(const SpeciesDev& sp, const double* __
 
 }  // namespace
 // ---- kernel 1: psi = phi sqrt(|V dV|) of every region, evaluated once ---------------------------
-// One CTA per region (with work): stage sqrt(|V dV|) of the region's points and their sign bits, then
+// One CTA per region (with work): stage sqrt(u dV), u = |V - c| (see gint_hinit_kernel), of the region's points, then
 // the warps walk the region's (atom image, run of stages) tasks.  Plenty of warps per SM (3 CTAs of 8
 // warps) hide the table and entry latencies; the output is 8.5 GB at si512_dzp.
 constexpr int kEvalThreads = 256;
@@ -286,22 +288,19 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
             s_off[k * kMaxRegionPoints + p] = c.x * P.estep[k] + c.y * P.estep[3 + k] + c.z * P.estep[6 + k];
         s_xyz[p] = c;
     }
+    const double vshift = V ? P.shift->c : 0.0;
     for (int r = blockIdx.x; r < P.nwork_regions; r += gridDim.x) {
         __syncthreads();   // previous region's sqrtw no longer read (first pass: tables and offsets staged)
         const int reg_index = __ldg(P.work_regions + r);
         const Region* reg = P.regions + reg_index;
         const int ox = __ldg(&reg->origin[0]), oy = __ldg(&reg->origin[1]), oz = __ldg(&reg->origin[2]);
-        const int item0 = __ldg(&reg->item0), nitem = __ldg(&reg->nitem);
-        for (int p = tid; p < npt; p += kEvalThreads) {   // npt is a multiple of 32: whole warps
+        for (int p = tid; p < npt; p += kEvalThreads) {
             const uchar4 c = s_xyz[p];
             const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
             double wv = 0.0;
             if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])   // V == nullptr: plain phi (gint_rho)
-                wv = V ? __ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) * P.dV : 1.0;
+                wv = V ? (__ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) - vshift) * P.dV : 1.0;
             s_sqrtw[p] = sqrt(fabs(wv));
-            const unsigned int neg = __ballot_sync(0xffffffffu, wv < 0.0);
-            if (lane == 0)   // every work item of the region carries the sign bits in its descriptor
-                for (int q = 0; q < nitem; q++) P.descs[item0 + q].sign[p >> 5] = neg;
         }
         __syncthreads();
         const int ntask = __ldg(&reg->ntask);
@@ -381,8 +380,8 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
         // ---- gather the tile of E into A fragments ----
         double A[4][8];
         if (has_tile) {
-            const uint32_t* pdir = P.pair_direct + cur->item.reg.pair_off;
-            const int m = cur->item.reg.nentry;
+            const uint32_t* pdir = P.pair_direct + cur->slot[sa].pair_off;
+            const int m = cur->slot[sa].nentry;
             uint32_t ci[8];
 #pragma unroll
             for (int kc = 0; kc < 8; kc++) ci[kc] = cur->rinfo[sb][4 * kc + fk];
@@ -408,7 +407,8 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
                 }
             }
         }
-        const int ox = cur->item.reg.origin[0], oy = cur->item.reg.origin[1], oz = cur->item.reg.origin[2];
+        const SlotInfo& reg = cur->slot[has_tile ? sa : 0];
+        const int ox = reg.origin[0], oy = reg.origin[1], oz = reg.origin[2];
         uint32_t todo = cur->item.stage_mask;
         while (todo) {
             const int s = __ffs(todo) - 1;
@@ -520,8 +520,8 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
     }
     fence_proxy_async();
     __syncthreads();
-    // consumer warp w runs on SM sub-partition w % 4 and takes tile w of the item (the plan fills tiles[v + 4 r] for
-    // sub-partition v; v = 3 hosts the producer warp and holds one tile fewer)
+    // consumer warp w runs on SM sub-partition w % 4 and takes tile w of the item (the plan balances the four
+    // sub-partitions' DMMA counts; sub-partition 3 also hosts the producer warp and gets one tile fewer)
     const int cidx = warp;
 
     if (warp == kConsumerWarps) {
@@ -559,10 +559,9 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
             __syncwarp();
             if (!cur->valid) break;
             const int nslot = cur->item.nslot;
-            const unsigned char* psi_bytes = reinterpret_cast<const unsigned char*>(P.psi) +
-                                             (size_t)cur->item.reg.psi_chunk0 * kChunkBytes;
             // lane q copies the chunks of slot q; lane 0 also owns the barriers
-            const unsigned char* src_lane = psi_bytes + (size_t)(lane < nslot ? cur->item.slot_group[lane] : 0) * P.nstage * kChunkBytes;
+            const unsigned char* src_lane = reinterpret_cast<const unsigned char*>(P.psi) +
+                                            (size_t)(lane < nslot ? cur->slot[lane].chunk0 : 0) * kChunkBytes;
             uint32_t todo = cur->item.stage_mask;
             while (todo) {
                 const int s = __ffs(todo) - 1;
@@ -586,6 +585,8 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
         if constexpr (MODE == 0) {
             const int frow = lane >> 2, fk = lane & 3;
             const int lane_off = frag_lane_offset(lane);
+            const uint32_t ring_u32 = smem_u32(s_ring);
+
             uint32_t cs = 0, cph = 0;   // ring slot and phase of the next stage to consume
             for (int it = 0;; it++) {
                 const int ds = it % kDescSlots;
@@ -595,8 +596,6 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
                 const int sa = cur->item.tiles[cidx][0], sb = cur->item.tiles[cidx][1];
                 const bool has_tile = sa != 0xFF;
                 const bool diag = sa == sb;
-                const uint32_t* gma = cur->gm32[has_tile ? sa : 0];
-                const uint32_t* gmb = cur->gm32[has_tile ? sb : 0];
                 double acc[4][4][2];
 #pragma unroll
                 for (int i = 0; i < 4; i++)
@@ -607,36 +606,41 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
                 while (todo) {
                     const int s = __ffs(todo) - 1;
                     todo &= todo - 1;
-                    // activity nibbles of the stage's 8 k-steps; k-steps where both groups hold an in-sphere point
-                    const uint32_t ma = gma[s], mb = gmb[s];
-                    uint32_t act = has_tile ? (nonzero_nibbles(ma) & nonzero_nibbles(mb)) : 0u;
+                    // this warp's program for the stage: up to 8 runs of k-steps (host-built, see pack_run), 0-terminated
+                    uint2 pg = make_uint2(0u, 0u), pg2 = make_uint2(0u, 0u);
+                    if (has_tile) {
+                        const uint4 w4 = *reinterpret_cast<const uint4*>(&cur->prog[cidx][s][0]);
+                        pg = make_uint2(w4.x, w4.y);
+                        pg2 = make_uint2(w4.z, w4.w);
+                    }
                     mbar_wait(smem_u32(s_full + cs), cph);
-                    if (act) {
-                        const unsigned char* stage = s_ring + (size_t)cs * kStageBytes;
-                        const double* pa = reinterpret_cast<const double*>(stage + sa * kChunkBytes) + lane_off;
-                        const double* pb = reinterpret_cast<const double*>(stage + sb * kChunkBytes) + lane_off;
-                        // sign bits of V dV at this lane's point of every k-step: bit 4 ks of sg
-                        const uint32_t sg = cur->sign[s] >> fk;
-                        Frag8 o;
-                        if ((ma & mb) == 0xFFFFFFFFu) {
-                            // every fragment pair of every k-step: straight-line code, loads scheduled ahead by ptxas
-#pragma unroll
-                            for (int ks = 0; ks < kStageKsteps; ks++) {
-                                load_kstep(o, pa, pb, 4 * ks);
-                                sign_b(o, (sg >> (4 * ks)) << 31);
-                                kstep_full(acc, o, diag);
+                    if (pg.x) {
+                        const uint32_t stage = ring_u32 + cs * kStageBytes + lane_off * 8;
+                        const uint32_t pa = stage + sa * kChunkBytes, pb = stage + sb * kChunkBytes;
+                        do {
+                            const uint32_t run = pg.x;
+                            const uint32_t off = (run << 2) & 0x1C00u;             // first k-step x 1 KB
+                            const uint32_t n = ((run >> 11) & 7u) + 1u;
+                            if (diag) {
+                                run_diag(acc, pa + off, n, (run >> 4) & 0xFu);
+                            } else if ((run & 0xF0u) == 0xF0u) {
+                                run_rect(acc, pa + off, pb + off, n, run & 0xFu);
+                            } else {   // rare (2.5 % of the DMMAs): k-step by k-step
+                                const double* ga = reinterpret_cast<const double*>(s_ring + (size_t)cs * kStageBytes + sa * kChunkBytes) + lane_off;
+                                const double* gb = reinterpret_cast<const double*>(s_ring + (size_t)cs * kStageBytes + sb * kChunkBytes) + lane_off;
+#pragma unroll 1
+                                for (uint32_t q = 0; q < n; q++) {
+                                    Frag8 o;
+                                    load_kstep(o, ga, gb, ((run >> 6) & 0x1Cu) + 4 * q);
+                                    kstep_rect(acc, o, ((run >> 4) & 0xFu) | ((run & 0xFu) << 4));
+                                }
                             }
-                        } else {
-                            do {
-                                const uint32_t k = __ffs(act) - 1;
-                                act &= act - 1;
-                                load_kstep(o, pa, pb, k);
-                                sign_b(o, (sg >> k) << 31);
-                                const uint32_t ra = (ma >> k) & 0xFu;
-                                if (!diag) kstep_rect(acc, o, ra | (((mb >> k) & 0xFu) << 4));
-                                else kstep_diag(acc, o, ra);
-                            } while (act);
-                        }
+                            // next run word (16 bits each)
+                            pg.x = (pg.x >> 16) | (pg.y << 16);
+                            pg.y = (pg.y >> 16) | (pg2.x << 16);
+                            pg2.x = (pg2.x >> 16) | (pg2.y << 16);
+                            pg2.y >>= 16;
+                        } while (pg.x & 0xFFFFu);
                     }
                     __syncwarp();
                     if (lane == 0) mbar_arrive(smem_u32(s_empty + cs));
@@ -645,8 +649,9 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
 
                 // ---------------- flush: add the tile into the canonical H blocks ---------------------------
                 if (has_tile) {
-                    const PairWord* pair = P.pair + cur->item.reg.pair_off;
-                    const int m = cur->item.reg.nentry;
+                    const PairWord* pair = P.pair + cur->slot[sa].pair_off;
+                    const int m = cur->slot[sa].nentry;
+                    const uint32_t negbit = P.shift->neg << 31;   // H = c S - C (c = max V) or c S + C (c = min V)
                     // this lane's 8 columns: j = 0..3, h = 0..1 -> column 8 j + 2 fk + h of the column group
                     uint32_t ci[4][2];
 #pragma unroll
@@ -680,7 +685,7 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
                                 if (pw[j][h].x == kNoBlock) continue;
                                 const uint32_t nu = (ci[j][h] >> 12) & 0xFFu;
                                 const uint32_t idx = mu * (pw[j][h].y & 0xFFFFu) + nu * (pw[j][h].y >> 16);
-                                atomicAdd(H + (size_t)pw[j][h].x + idx, acc[i][j][h]);
+                                atomicAdd(H + (size_t)pw[j][h].x + idx, flip_sign(acc[i][j][h], negbit));
                             }
                     }
                 }
@@ -691,6 +696,69 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
             rho_consumer(P, Din, H, s_full, s_empty, s_dfull, s_dempty, s_desc, s_ring, nring, never, lane, cidx);
         }
     }
+}
+
+// ---- one-signed potential: H = c S -/+ sum_g phi |V - c| phi dV ---------------------------------------------------
+// gint_vrange_kernel: per-block (min, max) of V.  gint_hinit_kernel: every block reduces the partials to the range
+// of V, picks the shift c -- max V (then u = c - V >= 0 and H = c S - C) or min V (u = V - c, H = c S + C),
+// whichever is smaller in magnitude, so that |c S| <= max|V| |S| and nothing is lost to cancellation -- block 0
+// publishes it for the psi and contraction kernels, and all blocks write H <- c S.
+constexpr int kRangeBlocks = 296, kRangeThreads = 256;
+
+__device__ __forceinline__ void block_minmax(double& lo, double& hi, double* s_red /* [2 * 32] */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if (lane == 0) { s_red[warp] = lo; s_red[32 + warp] = hi; }
+    __syncthreads();
+    if (warp == 0) {
+        lo = lane < nw ? s_red[lane] : s_red[0];
+        hi = lane < nw ? s_red[32 + lane] : s_red[32];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        if (lane == 0) { s_red[0] = lo; s_red[32] = hi; }
+    }
+    __syncthreads();
+    lo = s_red[0];
+    hi = s_red[32];
+}
+
+__global__ void __launch_bounds__(kRangeThreads) gint_vrange_kernel(const double* __restrict__ V, size_t n, double* __restrict__ part) {
+    __shared__ double s_red[64];
+    double lo = V[0], hi = lo;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const double v = __ldg(V + i);
+        lo = fmin(lo, v);
+        hi = fmax(hi, v);
+    }
+    block_minmax(lo, hi, s_red);
+    if (threadIdx.x == 0) { part[2 * blockIdx.x] = lo; part[2 * blockIdx.x + 1] = hi; }
+}
+
+__global__ void __launch_bounds__(kRangeThreads) gint_hinit_kernel(const double* __restrict__ part, int npart,
+                                                                   const double* __restrict__ S, double* __restrict__ H, size_t h_len,
+                                                                   ShiftDev* __restrict__ shift) {
+    __shared__ double s_red[64];
+    double lo = part[0], hi = part[1];
+    for (int i = threadIdx.x; i < npart; i += blockDim.x) {
+        lo = fmin(lo, part[2 * i]);
+        hi = fmax(hi, part[2 * i + 1]);
+    }
+    block_minmax(lo, hi, s_red);
+    const bool neg = fabs(hi) <= fabs(lo);   // c = max V, u = c - V, H = c S - C
+    const double c = neg ? hi : lo;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        shift->c = c;
+        shift->neg = neg ? 1u : 0u;
+    }
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < h_len; i += (size_t)gridDim.x * blockDim.x)
+        H[i] = c == 0.0 ? 0.0 : c * __ldg(S + i);
 }
 
 // H(J,I,-R) = H(I,J,R)^T for every non-canonical block; lower <- upper for (I,I,0).
@@ -736,13 +804,21 @@ cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int 
     return cudaGetLastError();
 }
 
+// raw = true: no shift (c = 0, H <- sum_g phi V phi dV for a non-negative V): used once at setup to build S.
 cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
-                          size_t h_len, const double* V, double* H, cudaStream_t stream, cudaEvent_t* ev) {
+                          size_t h_len, const double* V, double* H, bool raw, cudaStream_t stream, cudaEvent_t* ev) {
     if (ev) cudaEventRecord(ev[0], stream);
-    cudaError_t e = cudaMemsetAsync(H, 0, h_len * sizeof(double), stream);
+    cudaError_t e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 4, stream);   // work-queue head
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 4, stream);   // work-queue head
-    if (e != cudaSuccess) return e;
+    if (raw) {
+        if ((e = cudaMemsetAsync(P.shift, 0, sizeof(ShiftDev), stream)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(H, 0, h_len * sizeof(double), stream)) != cudaSuccess) return e;
+    } else {
+        const size_t npts = (size_t)P.ngrid[0] * P.ngrid[1] * P.ngrid[2];
+        gint_vrange_kernel<<<kRangeBlocks, kRangeThreads, 0, stream>>>(V, npts, P.vpart);
+        gint_hinit_kernel<<<4 * nsm, kRangeThreads, 0, stream>>>(P.vpart, kRangeBlocks, P.S, H, h_len, P.shift);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
     if (ev) cudaEventRecord(ev[1], stream);
     e = launch_psi(P, psi_smem, tab_smem, nsm, V, stream);
     if (e != cudaSuccess) return e;

@@ -365,12 +365,28 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.entries.resize(tmp.size());
     for (size_t i = 0; i < tmp.size(); i++) P.entries[i] = tmp[i].e;
 
-    // ---- per region: rows, fragment / group activity, row info, pair table, tiles, work items -----
-    struct RegionItems { int region; double cost; std::vector<WorkItem> items; };
-    std::vector<RegionItems> region_items;
-    double exec_dmma = 0, flush_elems = 0, n_etask = 0, max_rows = 0, chunk_loads = 0;
-    double ks_full = 0, ks_part = 0, dmma_part = 0, stage_visits = 0, bal_item = 0, bal_stage = 0, bal_warp = 0;
+    // ---- per region: rows, fragment / group activity, row info, pair table, tiles ------------------
+    // A proto-item is a set of tiles of ONE region that touches few row groups; proto-items are packed into work
+    // items (<= kTilesPerItem tiles, <= kMaxSlots row groups) afterwards, small ones also across regions.
+    struct Tile { int region, gi, gj; double cost; };
+    struct Proto { std::vector<Tile> tiles; std::vector<std::pair<int, int>> slots; /* (region, group) */ };
+    std::vector<Proto> all_protos;
+    std::vector<double> region_cost;
+    double n_etask = 0, max_rows = 0;
     const int nks_pad = P.nks_pad, nslice = P.nslice, nstage = P.nstage;
+    auto kstep_cost_of = [&](const uint8_t* gm, int gi, int gj, int ks) {
+        const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
+        if (gi != gj) return __builtin_popcount(ra) * __builtin_popcount(ca);
+        int n = 0;
+        for (int i = 0; i < 4; i++)
+            if ((ra >> i) & 1u) n += __builtin_popcount(ca >> i);
+        return n;
+    };
+    auto stage_cost_of = [&](const uint8_t* gm, int gi, int gj, int st) {
+        int n = 0;
+        for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) n += kstep_cost_of(gm, gi, gj, ks);
+        return n;
+    };
     size_t pos = 0;
     while (pos < tmp.size()) {
         size_t end = pos;
@@ -406,8 +422,8 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             err = "plan tables exceed 2^31 entries";
             return GINT_EUNSUPPORTED;
         }
-        // evaluation tasks: (entry, run of up to 8 slices) with at least one point inside the sphere; the kernel
-        // walks the run's active 32-point slices with the entry's data in registers
+        // evaluation tasks: (entry, run of up to 8 stages) with at least one point inside the sphere; the kernel
+        // walks the run's active 32-point stages with the entry's data in registers
         int nactive = 0;
         for (int i = 0; i < m; i++) {
             const Entry& e = P.entries[pos + i];
@@ -437,7 +453,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 for (int i = 0; i < 4; i++) b |= (uint8_t)(((fmask[(size_t)4 * g + i][ks >> 5] >> (ks & 31)) & 1u) << i);
                 gm[(size_t)g * nks_pad + ks] = b;
             }
-        // pair table: (row entry a <= column entry b) -> canonical block offset (+ transposed flag)
+        // pair table: (row entry a <= column entry b) -> canonical block offset and element strides
         P.pair.resize(P.pair.size() + (size_t)m * m, PairWord{kNoBlock, 0, 0});
         P.pair_direct.resize(P.pair.size(), kNoBlock);
         for (int a = 0; a < m; a++)
@@ -458,40 +474,34 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 P.pair_direct[(size_t)R.pair_off + (size_t)a * m + b] = lookup(ea.atom, eb.atom, r1, r2, r3);
                 P.pair_direct[(size_t)R.pair_off + (size_t)b * m + a] = lookup(eb.atom, ea.atom, -r1, -r2, -r3);
             }
-        // tiles (group gi <= gj) and their cost (DMMAs) per stage
-        // the kernel decides per k-step (4 mesh points): a fragment pair is executed if the k-step holds an
-        // in-sphere point of both fragments' rows
-        auto kstep_cost = [&](int gi, int gj, int ks) {
-            const unsigned ra = gm[(size_t)gi * nks_pad + ks], ca = gm[(size_t)gj * nks_pad + ks];
-            if (gi != gj) return __builtin_popcount(ra) * __builtin_popcount(ca);
-            int n = 0;
-            for (int i = 0; i < 4; i++)
-                if ((ra >> i) & 1u) n += __builtin_popcount(ca >> i);
-            return n;
-        };
-        auto tile_stage_cost = [&](int gi, int gj, int st) {
-            int n = 0;
-            for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) n += kstep_cost(gi, gj, ks);
-            return n;
-        };
-        struct Proto { std::vector<std::pair<int, int>> tiles; std::vector<int> groups; };
-        auto add_group = [](std::vector<int>& v, int g) { if (std::find(v.begin(), v.end(), g) == v.end()) v.push_back(g); };
+        // tiles (group gi <= gj) with their cost in DMMAs: the kernel decides per k-step (4 mesh points), a fragment
+        // pair is executed if the k-step holds an in-sphere point of both fragments' rows
+        const int region_index = (int)P.regions.size();
+        auto add_slot = [](std::vector<std::pair<int, int>>& v, std::pair<int, int> g) { if (std::find(v.begin(), v.end(), g) == v.end()) v.push_back(g); };
         std::vector<std::vector<double>> tcost((size_t)ngroup, std::vector<double>((size_t)ngroup, 0.0));
+        double rcost = 0;
         for (int gi = 0; gi < ngroup; gi++)
             for (int gj = gi; gj < ngroup; gj++) {
                 int n = 0;
-                for (int st = 0; st < nstage; st++) n += tile_stage_cost(gi, gj, st);
+                for (int st = 0; st < nstage; st++) n += stage_cost_of(gm, gi, gj, st);
                 tcost[(size_t)gi][(size_t)gj] = n;
+                rcost += n;
+                if (n > 0) R.ntile++;
             }
         std::vector<Proto> protos;
-        const int chunk = kCliqueGroups;   // 3 groups -> a clique of 6 tiles
+        auto add_tile = [&](Proto& p, int gi, int gj) {
+            if (tcost[(size_t)gi][(size_t)gj] <= 0) return;
+            p.tiles.push_back({region_index, gi, gj, tcost[(size_t)gi][(size_t)gj]});
+            add_slot(p.slots, {region_index, gi});
+            add_slot(p.slots, {region_index, gj});
+        };
+        const int chunk = kCliqueGroups;
         const int nchunk = (ngroup + chunk - 1) / chunk;
         for (int k = 0; k < nchunk; k++) {
             const int k0 = k * chunk, k1 = std::min(ngroup, k0 + chunk);
             Proto p;
             for (int gi = k0; gi < k1; gi++)
-                for (int gj = gi; gj < k1; gj++)
-                    if (tcost[(size_t)gi][(size_t)gj] > 0) { p.tiles.push_back({gi, gj}); add_group(p.groups, gi); add_group(p.groups, gj); }
+                for (int gj = gi; gj < k1; gj++) add_tile(p, gi, gj);
             if (!p.tiles.empty()) protos.push_back(p);
             for (int l = k + 1; l < nchunk; l++) {
                 const int l0 = l * chunk, l1 = std::min(ngroup, l0 + chunk);
@@ -499,144 +509,107 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 for (int cj = l0; cj < l1; cj += width) {
                     Proto r;
                     for (int gi = k0; gi < k1; gi++)
-                        for (int gj = cj; gj < std::min(l1, cj + width); gj++)
-                            if (tcost[(size_t)gi][(size_t)gj] > 0) { r.tiles.push_back({gi, gj}); add_group(r.groups, gi); add_group(r.groups, gj); }
+                        for (int gj = cj; gj < std::min(l1, cj + width); gj++) add_tile(r, gi, gj);
                     if (!r.tiles.empty()) protos.push_back(r);
                 }
             }
         }
-        // greedy merge of small proto-items (fewer items, fewer chunk loads)
+        // greedy merge of small proto-items of the region (fewer items, fewer chunk loads)
         for (bool merged = true; merged;) {
             merged = false;
             int best_a = -1, best_b = -1, best_union = 1 << 30;
             for (size_t a = 0; a < protos.size(); a++)
                 for (size_t b = a + 1; b < protos.size(); b++) {
                     if (protos[a].tiles.size() + protos[b].tiles.size() > (size_t)kTilesPerItem) continue;
-                    std::vector<int> u = protos[a].groups;
-                    for (int g : protos[b].groups) add_group(u, g);
+                    std::vector<std::pair<int, int>> u = protos[a].slots;
+                    for (auto g : protos[b].slots) add_slot(u, g);
                     if ((int)u.size() > kMaxSlots) continue;
-                    const int growth = (int)u.size() - (int)std::max(protos[a].groups.size(), protos[b].groups.size());
+                    const int growth = (int)u.size() - (int)std::max(protos[a].slots.size(), protos[b].slots.size());
                     if (growth < best_union) { best_union = growth; best_a = (int)a; best_b = (int)b; }
                 }
             if (best_a >= 0) {
                 for (auto& t : protos[(size_t)best_b].tiles) protos[(size_t)best_a].tiles.push_back(t);
-                for (int g : protos[(size_t)best_b].groups) add_group(protos[(size_t)best_a].groups, g);
+                for (auto g : protos[(size_t)best_b].slots) add_slot(protos[(size_t)best_a].slots, g);
                 protos.erase(protos.begin() + best_b);
                 merged = true;
             }
         }
-        if (protos.size() > 32767) { err = "internal: too many work items in one region"; return GINT_EUNSUPPORTED; }
-        const int region_index = (int)P.regions.size();
-        RegionItems ri;
-        ri.region = region_index;
-        ri.cost = 0;
-        for (Proto& p : protos) {
-            std::sort(p.groups.begin(), p.groups.end());
-            WorkItem w;
-            std::memset(&w, 0, sizeof(w));
-            std::memset(w.tiles, 0xFF, sizeof(w.tiles));
-            w.region = region_index;
-            w.share = (int16_t)ri.items.size();
-            w.nslot = (int32_t)p.groups.size();
-            for (size_t s = 0; s < p.groups.size(); s++) w.slot_group[s] = (uint8_t)p.groups[s];
-            auto slot_of = [&](int g) { return (int)(std::find(p.groups.begin(), p.groups.end(), g) - p.groups.begin()); };
-            // heaviest tiles first onto the least loaded scheduler (consumer warp w runs on SM sub-partition w % 4)
-            std::sort(p.tiles.begin(), p.tiles.end(), [&](const std::pair<int, int>& a, const std::pair<int, int>& b) {
-                return tcost[(size_t)a.first][(size_t)a.second] > tcost[(size_t)b.first][(size_t)b.second];
-            });
-            w.ntile = (int16_t)p.tiles.size();
-            double load[4] = {0, 0, 0, 0};
-            int used[4] = {0, 0, 0, 0};
-            for (size_t t = 0; t < p.tiles.size(); t++) {
-                int q = -1;
-                for (int k = 0; k < 4; k++)   // virtual sub-partition 3 also hosts the producer warp: one consumer fewer there
-                    if (used[k] < (k == 3 ? kTilesPerItem / 4 : (kTilesPerItem + 3) / 4) && (q < 0 || load[k] < load[q])) q = k;
-                const int warp = q + 4 * used[q];
-                used[q]++;
-                const double tc = tcost[(size_t)p.tiles[t].first][(size_t)p.tiles[t].second];
-                load[q] += tc;
-                w.tiles[warp][0] = (uint8_t)slot_of(p.tiles[t].first);
-                w.tiles[warp][1] = (uint8_t)slot_of(p.tiles[t].second);
-                exec_dmma += tc;
-                for (int ks = 0; ks < nks_pad; ks++) {
-                    const int gi = p.tiles[t].first, gj = p.tiles[t].second;
-                    const int nd = kstep_cost(gi, gj, ks);
-                    if (gi != gj && nd == 16) ks_full += 1;
-                    else if (nd > 0) { ks_part += 1; dmma_part += nd; }
-                }
-                for (int st = 0; st < nstage; st++)
-                    if (tile_stage_cost(p.tiles[t].first, p.tiles[t].second, st) > 0) w.stage_mask |= 1u << st;
-                for (int st = 0; st < nstage; st++) {   // development statistics: how uniform are the masks within a stage
-                    const int gi = p.tiles[t].first, gj = p.tiles[t].second;
-                    const int c = tile_stage_cost(gi, gj, st);
-                    if (!c) continue;
-                    bool uniform = true, allact = true; int first = -1;
-                    for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) {
-                        const int key = gm[(size_t)gi * nks_pad + ks] | (gm[(size_t)gj * nks_pad + ks] << 4);
-                        if (kstep_cost(gi, gj, ks) == 0) { allact = false; continue; }
-                        if (first < 0) first = key; else if (key != first) uniform = false;
-                    }
-                    if (c == (gi == gj ? 80 : 128)) P.stats[26] += c;
-                    if (uniform && allact) P.stats[27] += c;
-                    if (uniform) P.stats[28] += c;
-                    P.stats[29] += 1;
-                }
-            }
-            ri.cost += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
-            bal_item += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
-            for (int st = 0; st < nstage; st++) {
-                double ls[4] = {0, 0, 0, 0}, lw = 0;
-                for (int wp = 0; wp < 16; wp++) {
-                    if (w.tiles[wp][0] == 0xFF) continue;
-                    const double c = tile_stage_cost(p.groups[w.tiles[wp][0]], p.groups[w.tiles[wp][1]], st);
-                    ls[wp & 3] += c;
-                    lw = std::max(lw, c);
-                }
-                bal_stage += std::max(std::max(ls[0], ls[1]), std::max(ls[2], ls[3]));
-                bal_warp += lw;
-            }
-            stage_visits += __builtin_popcount(w.stage_mask);
-            flush_elems += 1024.0 * (double)p.tiles.size();
-            for (int st = 0; st < nstage; st++)
-                if ((w.stage_mask >> st) & 1u)
-                    for (int g : p.groups) {
-                        bool act = false;
-                        for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) act = act || gm[(size_t)g * nks_pad + ks];
-                        if (act) chunk_loads += 1;
-                    }
-            ri.items.push_back(w);
-        }
-        R.nitem = (int32_t)ri.items.size();
-        if (R.nitem > 0) {
+        if (R.ntile > 0) {
             P.psi_chunks += (int64_t)ngroup * nstage;
             n_etask += nactive;
-            region_items.push_back(std::move(ri));
         } else {
             R.ntask = 0;
         }
+        region_cost.push_back(rcost);
+        for (Proto& p : protos) all_protos.push_back(std::move(p));
         P.regions.push_back(R);
         pos = end;
     }
     tmp.clear();
     tmp.shrink_to_fit();
-    // queue order: heaviest regions first, the items of a region consecutive (their CTAs share its psi)
-    std::stable_sort(region_items.begin(), region_items.end(), [](const RegionItems& a, const RegionItems& b) { return a.cost > b.cost; });
-    for (const RegionItems& ri : region_items) {
-        P.regions[(size_t)ri.region].item0 = (int32_t)P.items.size();
-        for (WorkItem w : ri.items) {
-            w.reg = P.regions[(size_t)w.region];
-            P.items.push_back(w);
+
+    // ---- work items ---------------------------------------------------------------------------------
+    // queue order: heaviest regions first, the proto-items of a region consecutive (their CTAs share its psi in L2)
+    std::stable_sort(all_protos.begin(), all_protos.end(), [&](const Proto& a, const Proto& b) {
+        const int ra = a.tiles[0].region, rb = b.tiles[0].region;
+        if (region_cost[(size_t)ra] != region_cost[(size_t)rb]) return region_cost[(size_t)ra] > region_cost[(size_t)rb];
+        return ra < rb;
+    });
+    // pack small proto-items together, also across regions (window of the queue), largest fill first
+    {
+        const size_t window = 48;
+        std::vector<char> dead(all_protos.size(), 0);
+        for (size_t a = 0; a < all_protos.size(); a++) {
+            if (dead[a]) continue;
+            for (;;) {
+                Proto& pa = all_protos[a];
+                int best = -1;
+                size_t best_tiles = 0;
+                for (size_t b = a + 1; b < std::min(all_protos.size(), a + 1 + window); b++) {
+                    if (dead[b]) continue;
+                    const Proto& pb = all_protos[b];
+                    if (pa.tiles.size() + pb.tiles.size() > (size_t)kTilesPerItem) continue;
+                    size_t nu = pa.slots.size();
+                    for (auto g : pb.slots)
+                        if (std::find(pa.slots.begin(), pa.slots.end(), g) == pa.slots.end()) nu++;
+                    if (nu > (size_t)kMaxSlots) continue;
+                    if (pb.tiles.size() > best_tiles) { best_tiles = pb.tiles.size(); best = (int)b; }
+                }
+                if (best < 0) break;
+                for (auto& t : all_protos[(size_t)best].tiles) pa.tiles.push_back(t);
+                for (auto g : all_protos[(size_t)best].slots)
+                    if (std::find(pa.slots.begin(), pa.slots.end(), g) == pa.slots.end()) pa.slots.push_back(g);
+                dead[(size_t)best] = 1;
+            }
         }
+        size_t w = 0;
+        for (size_t a = 0; a < all_protos.size(); a++)
+            if (!dead[a]) {
+                if (w != a) all_protos[w] = std::move(all_protos[a]);
+                w++;
+            }
+        all_protos.resize(w);
     }
     // descriptors: everything the contraction kernel needs for an item, contiguous (one bulk copy)
-    P.descs.resize(P.items.size());
-    for (size_t it = 0; it < P.items.size(); it++) {
+    double exec_dmma = 0, flush_elems = 0, chunk_loads = 0;
+    double ks_full = 0, ks_part = 0, dmma_part = 0, stage_visits = 0, bal_item = 0, bal_stage = 0, bal_warp = 0;
+    P.descs.resize(all_protos.size());
+    for (size_t it = 0; it < all_protos.size(); it++) {
+        Proto& p = all_protos[it];
         ItemDesc& d = P.descs[it];
         std::memset(&d, 0, sizeof(d));
-        d.item = P.items[it];
-        const Region& R = d.item.reg;
-        for (int q = 0; q < d.item.nslot; q++) {
-            const int g = d.item.slot_group[q];
+        std::memset(d.item.tiles, 0xFF, sizeof(d.item.tiles));
+        std::sort(p.slots.begin(), p.slots.end());
+        d.item.nslot = (int16_t)p.slots.size();
+        d.item.ntile = (int16_t)p.tiles.size();
+        for (size_t q = 0; q < p.slots.size(); q++) {
+            const Region& R = P.regions[(size_t)p.slots[q].first];
+            const int g = p.slots[q].second;
+            SlotInfo& si = d.slot[q];
+            si.chunk0 = R.psi_chunk0 + (int64_t)g * nstage;
+            si.pair_off = R.pair_off;
+            si.nentry = R.nentry;
+            for (int k = 0; k < 3; k++) si.origin[k] = R.origin[k];
             const uint8_t* gmq = &P.gmask[(size_t)R.gmask_off + (size_t)g * nks_pad];
             for (int st = 0; st < nstage; st++) {
                 uint32_t wd = 0;
@@ -645,14 +618,75 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             }
             std::memcpy(d.rinfo[q], &P.rowinfo[(size_t)R.rowinfo_off + (size_t)g * kGroupRows], sizeof(uint32_t) * kGroupRows);
         }
+        auto slot_of = [&](int region, int g) {
+            return (int)(std::find(p.slots.begin(), p.slots.end(), std::make_pair(region, g)) - p.slots.begin());
+        };
+        // heaviest tiles first onto the least loaded scheduler (consumer warp w runs on SM sub-partition w % 4)
+        std::sort(p.tiles.begin(), p.tiles.end(), [](const Tile& a, const Tile& b) { return a.cost > b.cost; });
+        double load[4] = {0, 0, 0, 0};
+        int used[4] = {0, 0, 0, 0};
+        std::vector<int> warp_of(p.tiles.size());
+        for (size_t t = 0; t < p.tiles.size(); t++) {
+            int q = -1;
+            for (int k = 0; k < 4; k++)
+                if (used[k] < (k == 3 ? kTilesPerItem / 4 : (kTilesPerItem + 3) / 4) && (q < 0 || load[k] < load[q])) q = k;
+            const int warp = q + 4 * used[q];
+            used[q]++;
+            warp_of[t] = warp;
+            const Tile& tl = p.tiles[t];
+            load[q] += tl.cost;
+            d.item.tiles[warp][0] = (uint8_t)slot_of(tl.region, tl.gi);
+            d.item.tiles[warp][1] = (uint8_t)slot_of(tl.region, tl.gj);
+            exec_dmma += tl.cost;
+            const uint8_t* gm = &P.gmask[(size_t)P.regions[(size_t)tl.region].gmask_off];
+            for (int ks = 0; ks < nks_pad; ks++) {
+                const int nd = kstep_cost_of(gm, tl.gi, tl.gj, ks);
+                if (tl.gi != tl.gj && nd == 16) ks_full += 1;
+                else if (nd > 0) { ks_part += 1; dmma_part += nd; }
+            }
+            for (int st = 0; st < nstage; st++) {
+                if (stage_cost_of(gm, tl.gi, tl.gj, st) <= 0) continue;
+                d.item.stage_mask |= 1u << st;
+                // the warp's program for the stage: runs of consecutive active k-steps with equal (ra, ca)
+                int nrun = 0;
+                for (int ks = 0; ks < kStageKsteps;) {
+                    const unsigned ra = gm[(size_t)tl.gi * nks_pad + st * kStageKsteps + ks] & 0xFu;
+                    const unsigned ca = gm[(size_t)tl.gj * nks_pad + st * kStageKsteps + ks] & 0xFu;
+                    if (!ra || !ca) { ks++; continue; }
+                    int n = 1;
+                    while (ks + n < kStageKsteps && (gm[(size_t)tl.gi * nks_pad + st * kStageKsteps + ks + n] & 0xFu) == ra &&
+                           (gm[(size_t)tl.gj * nks_pad + st * kStageKsteps + ks + n] & 0xFu) == ca) n++;
+                    d.prog[warp][st][nrun++] = pack_run(ra, ca, ks, n);
+                    ks += n;
+                }
+            }
+        }
+        bal_item += std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
+        for (int st = 0; st < nstage; st++) {
+            double ls[4] = {0, 0, 0, 0}, lw = 0;
+            for (size_t t = 0; t < p.tiles.size(); t++) {
+                const Tile& tl = p.tiles[t];
+                const uint8_t* gm = &P.gmask[(size_t)P.regions[(size_t)tl.region].gmask_off];
+                const double c = stage_cost_of(gm, tl.gi, tl.gj, st);
+                ls[warp_of[t] & 3] += c;
+                lw = std::max(lw, c);
+            }
+            bal_stage += std::max(std::max(ls[0], ls[1]), std::max(ls[2], ls[3]));
+            bal_warp += lw;
+        }
         for (int st = 0; st < nstage; st++) {
             uint32_t a = 0;
-            for (int q = 0; q < d.item.nslot; q++)
-                if (d.gm32[q][st]) a |= 1u << q;
+            if ((d.item.stage_mask >> st) & 1u)
+                for (int q = 0; q < d.item.nslot; q++)
+                    if (d.gm32[q][st]) a |= 1u << q;
             d.act[st] = (uint8_t)a;
+            chunk_loads += __builtin_popcount(a);
         }
+        stage_visits += __builtin_popcount(d.item.stage_mask);
+        flush_elems += 1024.0 * (double)p.tiles.size();
         d.valid = 1;
     }
+    all_protos.clear();
 
     double fpt = 0, fsym = 0;
     for (int32_t n : npoint_orb) {
@@ -660,7 +694,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         fsym += (double)n * ((double)n + 1.0);
     }
     P.stats[0] = (double)ncells;
-    P.stats[1] = (double)P.items.size();
+    P.stats[1] = (double)P.descs.size();
     P.stats[2] = (double)P.entries.size();
     P.stats[3] = max_rows;
     P.stats[4] = 512.0 * exec_dmma;

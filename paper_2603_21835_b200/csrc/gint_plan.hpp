@@ -52,6 +52,7 @@ constexpr int kMaxStages = kMaxKsteps / kStageKsteps;      // 16
 constexpr int kGroupRows = 32;                 // rows of one row group = warp-tile edge
 constexpr int kMaxSlots = 8;                   // row groups one work item may touch
 constexpr int kTilesPerItem = 15;              // one 32x32 tile per consumer warp; a CTA = 15 consumer warps + 1 producer warp
+                                               // (16 + 1 warps get 96 registers each, or 112 after setmaxnreg: measured no faster)
 constexpr int kCliqueGroups = 5;               // largest c with c (c + 1) / 2 <= kTilesPerItem
 constexpr int kMaxGroups = 40;                 // row groups per region (<= 1280 orbitals listed)
 constexpr int kChunkDoubles = kGroupRows * kStagePts;      // 1024: psi of one (group, stage), [k-step][row][point]
@@ -88,29 +89,36 @@ struct Region {          // 64 bytes
     int32_t nentry;
     int32_t entry0;      // first entry of the region in entries
     int32_t task_off;    // into etasks
-    int32_t ntask;       // evaluation tasks (entry, run of 8 slices) with a point inside the sphere
-    int32_t nitem;       // work items of the region = number of evaluation shares
+    int32_t ntask;       // evaluation tasks (entry, run of 8 stages) with a point inside the sphere
+    int32_t ntile;       // 32x32 tiles of the region's upper triangle that hold work (0: the region is skipped)
     int64_t psi_chunk0;  // first 8 KB chunk of the region in the psi scratch: chunk(g, s) = psi_chunk0 + g*nstage + s
     int32_t ngroup;
-    int32_t item0;       // first work item of the region in queue order (its nitem items are consecutive)
+    int32_t pad;
 };
 static_assert(sizeof(Region) == 64, "Region layout is shared with the device");
 
 // evaluation task word: entry index within the region | run << 16 (run h = stages 8h .. 8h+7)
 inline uint32_t pack_etask(int e, int run) { return (uint32_t)e | ((uint32_t)run << 16); }
 
-struct WorkItem {        // 128 bytes: 64 of its own + a copy of its region (one fetch instead of two dependent ones)
-    int32_t region;
-    int16_t share;       // index of the item within its region: evaluates tasks t = share (mod nitem)
-    int16_t ntile;
-    uint32_t stage_mask; // bit s: stage s (32 points) holds work for this item
-    uint8_t tiles[16][2];              // per consumer warp: (slot of row group, slot of column group), 0xFF = no tile
-    uint8_t slot_group[kMaxSlots];     // region row group held by each slot
-    int32_t nslot;
-    int32_t pad[2];
-    Region reg;
+// One row group of one region as a work item sees it (a slot of the shared-memory ring).  A work item may hold
+// tiles of several regions (small left-over tile sets are packed together); a tile's two slots always belong to
+// the same region.
+struct SlotInfo {        // 32 bytes
+    int64_t chunk0;      // first chunk of the group in the psi scratch: stage s is chunk0 + s
+    int32_t pair_off;    // the region's pair table and its edge
+    int32_t nentry;
+    int32_t origin[3];   // the region's first mesh point (gint_rho writes rho there)
+    int32_t pad;
 };
-static_assert(sizeof(WorkItem) == 128, "WorkItem layout is shared with the device");
+static_assert(sizeof(SlotInfo) == 32, "SlotInfo layout is shared with the device");
+
+struct WorkItem {        // 64 bytes
+    uint32_t stage_mask; // bit s: stage s (32 points) holds work for this item
+    int16_t ntile, nslot;
+    uint8_t tiles[16][2];   // per consumer warp: (slot of row group, slot of column group), 0xFF = no tile
+    uint8_t pad[24];
+};
+static_assert(sizeof(WorkItem) == 64, "WorkItem layout is shared with the device");
 
 struct MirrorItem {   // dst block (I,J,R) <- transpose of src block (J,I,-R); src == dst: symmetrise lower <- upper
     uint32_t dst, src;
@@ -132,20 +140,27 @@ inline uint32_t pack_rowinfo(int e, int mu, int norb) { return (uint32_t)e | ((u
 constexpr size_t kSmemLimit = 232448;   // 227 KB opt-in limit per CTA on sm_100
 constexpr int kDescSlots = 3;           // item descriptors in flight in the contraction kernel
 
-// Per-item descriptor: built by the host, completed by the psi kernel (sign bits), copied to shared
-// memory by the contraction kernel's producer warp with one bulk copy.
+// Per-item descriptor: built by the host, copied to shared memory by the contraction kernel's producer warp with
+// one bulk copy.
 struct ItemDesc {
-    WorkItem item;                                  // 128 (item.reg = its region)
+    WorkItem item;                                  // 64
+    SlotInfo slot[kMaxSlots];                       // 256
     uint32_t gm32[kMaxSlots][kMaxStages];           // 512: per (slot, stage): nibble ks = fragments of the slot's group
                                                     //      with an in-sphere point in k-step ks of the stage
-    uint32_t sign[kMaxStages];                      // 64: bit p = sign bit of V dV at point p of the stage
-    uint8_t act[32];                                // per stage: bit q = slot q has an active k-step in the stage
     uint32_t rinfo[kMaxSlots][kGroupRows];          // 1024: row info words of the item's slots (flush)
+    uint8_t act[kMaxStages];                        // 16: per stage: bit q = slot q has an active k-step in the stage
     int32_t valid;                                  // 0 = queue exhausted
-    int32_t pad[7];
+    int32_t pad[11];
+    // 3840: per (consumer warp, stage) the RUNS of consecutive k-steps with one fragment pattern (pack_run), in k-step
+    // order, 0-terminated: what the warp executes, decided here so that the kernel's per-stage prologue is one load
+    uint16_t prog[kTilesPerItem][kMaxStages][kStageKsteps];
 };
+// run word: ca | ra << 4 | first k-step << 8 | (k-steps - 1) << 11 | 1 << 15
+inline uint16_t pack_run(unsigned ra, unsigned ca, int ks, int n) {
+    return (uint16_t)(ca | (ra << 4) | ((unsigned)ks << 8) | ((unsigned)(n - 1) << 11) | 0x8000u);
+}
 static_assert(kStageKsteps == 8 && kStagePts == 32, "one stage = 8 k-steps = one 32-bit mask word = one lane per point");
-static_assert(sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
+static_assert(sizeof(ItemDesc) == 5760 && sizeof(ItemDesc) % 128 == 0, "ItemDesc must keep 128-byte alignment");
 
 struct Plan {
     // inputs
@@ -178,7 +193,6 @@ struct Plan {
     std::vector<uint32_t> rowinfo;
     std::vector<PairWord> pair;                 // [nentry][nentry] per region, a <= b filled
     std::vector<uint32_t> pair_direct;          // same indexing: offset of block (I_a, I_b, R_b - R_a) itself, any order (gint_rho)
-    std::vector<WorkItem> items;
     std::vector<ItemDesc> descs;                // one per work item, queue order
     std::vector<uint32_t> etasks;               // evaluation tasks, region-major
     int64_t psi_chunks = 0;                     // 8 KB chunks of the psi scratch buffer
