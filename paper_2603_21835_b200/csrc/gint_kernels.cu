@@ -673,8 +673,9 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
 #pragma unroll
                             for (int h = 0; h < 2; h++) {
                                 // diagonal tile: fragments i > j were never computed (zero), i == j needs row <= column
-                                const bool ok = ci[j][h] != kNoBlock && acc[i][j][h] != 0.0 &&
-                                                !(diag && i == j && frow > 2 * fk + h);
+                                // zero test on the bits: an FP64 compare would take a slot of the pipe the DMMAs run on
+                                const bool nz = (((uint32_t)__double2hiint(acc[i][j][h]) << 1) | (uint32_t)__double2loint(acc[i][j][h])) != 0u;
+                                const bool ok = ci[j][h] != kNoBlock && nz && !(diag && i == j && frow > 2 * fk + h);
                                 pw[j][h] = ok ? __ldg(reinterpret_cast<const uint2*>(prow + (ci[j][h] & 0xFFFu)))
                                               : make_uint2(kNoBlock, 0u);
                             }
