@@ -24,7 +24,7 @@ EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
               "regions", "ksteps_full", "ksteps_partial", "dmma_in_partial_ksteps", "stage_visits", "dmma_max_sched_item", "dmma_max_sched_stage", "dmma_max_warp_stage", "bcell1", "bcell2", "bcell3",
-              "s26", "s27", "s28", "s29", "s30", "s31")
+              "dmma_diag_runs", "dmma_rect_runs", "dmma_other_runs", "runs", "s30", "s31")
 
 
 class GintError(RuntimeError):
