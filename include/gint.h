@@ -120,10 +120,29 @@ int gint_vlocal_host(gint_ctx *ctx, const double *V_host, double *H_host);
  *   D_dev    device pointer, h_len doubles: the blocks rho_mu,nu(I,J,R) in exactly the layout of H (every block of
  *            the table is used as given; no symmetry of D is assumed); read only
  *   rho_dev  device pointer, [N1][N2][N3] doubles; OVERWRITTEN
- * Asynchronous on `stream` (one memset, two kernels; reuses the context's psi scratch, so it must not overlap a
- * gint_vlocal call on another stream).  First cut: FP64 FMA, not yet on the tensor pipe.  Returns GINT_EUNSUPPORTED
- * if a region lists more orbitals than fit one stage in shared memory. */
+ * Asynchronous on `stream` (two memsets, the psi kernel with unit weights and the contraction kernel in its density
+ * mode, FP64 tensor pipe).  All calls on one context share its scratch buffers and work queue: they must be
+ * stream-ordered with each other (same stream, or ordered by events).
+ * With nranks > 1 rho holds this rank's partial sum. */
 int gint_rho(gint_ctx *ctx, const double *D_dev, double *rho_dev, void *stream);
+
+/* Local Pulay force (the paper's cal_gint_fvl):
+ *
+ *   F_I = - sum_R sum_{mu,nu} rho_nu,mu(R) sum_g [ d phi_mu(r_g - tau_I)/d tau_I  V(r_g) phi_nu(r_g - tau_J - R)
+ *                                                + phi_mu(r_g - tau_I) V(r_g) d phi_nu(r_g - tau_J - R)/d tau_I ] dV
+ *                                                          -- PAPER.md:400-411 (Sec. 3.3.1, Eq. 46)
+ * read as F_K = - sum_blocks sum_{mu,nu} D(I,J,R)[mu][nu] dH(I,J,R)[mu][nu]/d tau_K at fixed V and D (the derivative
+ * acts on phi_mu for K = I and on phi_nu for K = J), all-space mesh sum as for gint_vlocal.  Radial derivative: the
+ * derivative of the same cubic Lagrange interpolant that defines the radial function ("numerically for the radial
+ * part"), angular part analytic.  At r < 1e-12: grad phi = f'(0) c_1 e_m for l = 1, 0 otherwise.
+ *   V_dev   device pointer, [N1][N2][N3] doubles; read only
+ *   D_dev   device pointer, h_len doubles: density-matrix blocks in the layout of H (no symmetry assumed); read only
+ *   F_dev   device pointer, [natom][3] doubles (Hartree / bohr, Cartesian); OVERWRITTEN
+ * Asynchronous on `stream`: psi kernel (unit weights), E = D + D^T gather, T = E Phi on the FP64 tensor pipe, force
+ * kernel.  The first call allocates two more scratch buffers (8 (32 ngroup)^2 bytes per region and one as large as
+ * the psi scratch) and may return GINT_ENOMEM; later calls allocate nothing.  Same stream-ordering rule as gint_rho.
+ * With nranks > 1 F holds this rank's partial sum. */
+int gint_fvl(gint_ctx *ctx, const double *V_dev, const double *D_dev, double *F_dev, void *stream);
 
 /* k-space assembly of the real-space blocks (the next step of the paper's workflow after cal_gint_vl):
  *

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgint_b200.so")
 GINT_OK, GINT_EINVAL, GINT_EUNSUPPORTED, GINT_ENOMEM, GINT_ECUDA, GINT_ENODEVICE = 0, -1, -2, -3, -4, -5
 
 EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
-            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_rho", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
+            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_rho", "gint_fvl", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
@@ -65,6 +65,8 @@ def _load() -> ctypes.CDLL:
     lib.gint_fold_k.argtypes = [vp, vp, P(dbl), vp, vp]
     lib.gint_rho.restype = ctypes.c_int
     lib.gint_rho.argtypes = [vp, vp, vp, vp]
+    lib.gint_fvl.restype = ctypes.c_int
+    lib.gint_fvl.argtypes = [vp, vp, vp, vp, vp]
     lib.gint_get_stats.restype = ctypes.c_int
     lib.gint_get_stats.argtypes = [vp, P(dbl), i32]
     lib.gint_set_profiling.restype = ctypes.c_int
@@ -179,6 +181,22 @@ class GintContext:
         _check(_lib.gint_rho(self._h, ctypes.c_void_p(D_dev.data_ptr()), ctypes.c_void_p(rho_dev.data_ptr()),
                              ctypes.c_void_p(s)), "gint_rho")
         return rho_dev
+
+    def gint_fvl(self, V_dev, D_dev, F_dev=None, stream=None):
+        """Local Pulay force of Eq. 46 from V and density-matrix blocks D_dev (H layout); returns a CUDA float64 tensor [natom][3]."""
+        import torch
+        if not (V_dev.is_cuda and V_dev.dtype == torch.float64 and V_dev.is_contiguous() and tuple(V_dev.shape) == self.ngrid):
+            raise ValueError("V_dev must be a contiguous CUDA float64 tensor [N1][N2][N3]")
+        if not (D_dev.is_cuda and D_dev.dtype == torch.float64 and D_dev.is_contiguous() and D_dev.numel() == self.h_len):
+            raise ValueError("D_dev must be a contiguous CUDA float64 tensor of h_len elements")
+        if F_dev is None:
+            F_dev = torch.empty((self.natom, 3), dtype=torch.float64, device=V_dev.device)
+        if not (F_dev.is_cuda and F_dev.dtype == torch.float64 and F_dev.is_contiguous() and tuple(F_dev.shape) == (self.natom, 3)):
+            raise ValueError("F_dev must be a contiguous CUDA float64 tensor [natom][3]")
+        s = torch.cuda.current_stream(V_dev.device).cuda_stream if stream is None else int(stream)
+        _check(_lib.gint_fvl(self._h, ctypes.c_void_p(V_dev.data_ptr()), ctypes.c_void_p(D_dev.data_ptr()),
+                             ctypes.c_void_p(F_dev.data_ptr()), ctypes.c_void_p(s)), "gint_fvl")
+        return F_dev
 
     def gint_num_orbitals(self):
         """(norb_tot, first[natom+1]) of the dense k-space matrix."""

@@ -25,6 +25,9 @@ struct gint_ctx {
     bool profiling = false;
     bool have_events = false;
     cudaEvent_t ev[5];
+    gint::FvlPlan fvl{};           // built at the first gint_fvl call
+    bool have_fvl = false;
+    size_t force_smem = 0;
     double* V_scratch = nullptr;   // gint_vlocal_host only
     double* H_scratch = nullptr;
 };
@@ -273,6 +276,60 @@ int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* stream) 
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho psi launch");
     e = gint::launch_rho_dmma(ctx->dev, ctx->contract_smem, ctx->nsm, D_dev, rho_dev, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho launch");
+    return GINT_OK;
+}
+
+// scratch buffers and tables of gint_fvl, allocated when it is first called (E: 8 (32 ngroup)^2 bytes per region,
+// T: as large as the psi scratch)
+static int fvl_init(gint_ctx* ctx) {
+    const gint::Plan& P = ctx->plan;
+    gint::FvlPlan& F = ctx->fvl;
+    std::vector<int64_t> e0(P.regions.size(), 0);
+    std::vector<int4> tasks;
+    int64_t echunks = 0;
+    for (size_t r = 0; r < P.regions.size(); r++) {
+        const gint::Region& R = P.regions[r];
+        if (R.ntile <= 0) continue;
+        e0[r] = echunks;
+        echunks += (int64_t)R.ngroup * R.ngroup;
+        for (int rq = 0; rq * 4 < R.ngroup; rq++)
+            for (int sq = 0; sq * 4 < P.nstage; sq++) tasks.push_back(make_int4((int)r, rq, sq, 0));
+    }
+    cudaError_t e;
+    if ((e = upload(ctx, P.gmask, &F.gmask)) != cudaSuccess) return fail_cuda(e, "upload gmask");
+    if ((e = upload(ctx, P.rowinfo, &F.rowinfo)) != cudaSuccess) return fail_cuda(e, "upload rowinfo");
+    if ((e = upload(ctx, e0, &F.e_chunk0)) != cudaSuccess) return fail_cuda(e, "upload e_chunk0");
+    if ((e = upload(ctx, tasks, &F.tg_tasks)) != cudaSuccess) return fail_cuda(e, "upload tgemm tasks");
+    void *es = nullptr, *ts = nullptr;
+    if ((e = cudaMalloc(&es, echunks ? (size_t)echunks * gint::kChunkBytes : 16)) != cudaSuccess) return fail_cuda(e, "cudaMalloc E scratch");
+    ctx->allocs.push_back(es);
+    if ((e = cudaMalloc(&ts, P.psi_chunks ? (size_t)P.psi_chunks * gint::kChunkBytes : 16)) != cudaSuccess) return fail_cuda(e, "cudaMalloc T scratch");
+    ctx->allocs.push_back(ts);
+    F.escratch = reinterpret_cast<double*>(es);
+    F.tscratch = reinterpret_cast<double*>(ts);
+    F.ntg = (int32_t)tasks.size();
+    F.nks_pad = P.nks_pad;
+    ctx->force_smem = gint::force_kernel_smem(P.tables_in_smem ? P.tab_packed.size() * sizeof(double) : 0, (int)P.species.size());
+    if ((e = gint::configure_fvl(ctx->force_smem, P.tables_in_smem)) != cudaSuccess) return fail_cuda(e, "cudaFuncSetAttribute (fvl)");
+    ctx->have_fvl = true;
+    return GINT_OK;
+}
+
+int gint_fvl(gint_ctx* ctx, const double* V_dev, const double* D_dev, double* F_dev, void* stream) {
+    if (!ctx || !V_dev || !D_dev || !F_dev) return fail(GINT_EINVAL, "null argument");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
+    if (!ctx->have_fvl) {
+        const int rc = fvl_init(ctx);
+        if (rc != GINT_OK) return rc;
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    cudaError_t e = gint::launch_psi(ctx->dev, ctx->psi_smem, ctx->plan.tables_in_smem, ctx->nsm, nullptr, st);
+    if (e != cudaSuccess) return fail_cuda(e, "gint_fvl psi launch");
+    e = gint::launch_fvl(ctx->dev, ctx->fvl, ctx->force_smem, ctx->plan.tables_in_smem, ctx->nsm, (int)ctx->plan.atom_species.size(),
+                         V_dev, D_dev, F_dev, st, nullptr);
+    if (e != cudaSuccess) return fail_cuda(e, "gint_fvl launch");
     return GINT_OK;
 }
 

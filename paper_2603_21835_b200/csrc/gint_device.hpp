@@ -58,6 +58,20 @@ struct FoldPlan {
     const int32_t* first;      // [natom+1]: first orbital of each atom in the dense matrix
     int32_t nrun, norb_tot;
 };
+// local Pulay force (gint_fvl.cu): what its kernels need beyond DevicePlan; built at the first gint_fvl call
+struct FvlPlan {
+    const uint8_t* gmask;      // per region [ngroup][nks_pad]: fragment activity nibble per k-step (Region::gmask_off)
+    const uint32_t* rowinfo;   // per region [ngroup * 32]: entry | mu << 12 | norb << 20 (Region::rowinfo_off)
+    const int64_t* e_chunk0;   // per region: first 8 KB chunk of its E = D + D^T in escratch ([ga][gb] sub-blocks)
+    const int4* tg_tasks;      // CTA tasks of gint_tgemm_kernel: (region, row quad, stage quad, 0)
+    double* escratch;
+    double* tscratch;          // T = E Phi, psi chunk layout (same chunk indices as the psi scratch)
+    int32_t ntg, nks_pad;
+};
+size_t force_kernel_smem(size_t table_bytes, int nspecies);
+cudaError_t configure_fvl(size_t force_smem, bool tab_smem);
+cudaError_t launch_fvl(const DevicePlan& P, const FvlPlan& F, size_t force_smem, bool tab_smem, int nsm, int natom,
+                       const double* V, const double* D, double* Fout, cudaStream_t stream, cudaEvent_t* ev);
 cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream);
 cudaError_t launch_rho_dmma(const DevicePlan& P, size_t contract_smem_bytes, int nsm, const double* D, double* rho,
                             cudaStream_t stream);

@@ -379,3 +379,100 @@ def test_rho_large_full_mesh():
     got = rho.cpu().numpy()
     assert np.all(np.isfinite(got))
     assert np.abs(got - ref).max() <= TOL * np.abs(ref).max()
+
+
+# ---- gint_fvl: local Pulay force (Eq. 46) ------------------------------------------------------
+def gpu_fvl(w, D, **kw):
+    torch = _torch()
+    from paper_2603_21835_b200 import gint_setup
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, **kw)
+    F = ctx.gint_fvl(torch.from_numpy(np.ascontiguousarray(w.V)).cuda(), torch.from_numpy(np.ascontiguousarray(D)).cuda())
+    torch.cuda.synchronize()
+    return F.cpu().numpy(), ctx
+
+
+def assert_force_parity(got, ref, what):
+    assert np.all(np.isfinite(got)), what
+    err = np.abs(got - ref).max()
+    assert err <= TOL * np.abs(ref).max(), "%s: max|dF| %.3e vs max|F| %.3e" % (what, err, np.abs(ref).max())
+
+
+def test_fvl_cfg1_and_tiny(cfg1, cfg1_oracle):
+    """Force of Eq. 46 against the oracle with a random NON-symmetric D: cfg1 (self-image blocks), ragged triclinic
+    meshes (s, p, d shells), an atom on a mesh point (r = 0 rule), then gint_vlocal and gint_rho on the same context
+    still match (shared scratch)."""
+    import oracle
+    from paper_2603_21835_b200 import workloads as wl
+    rng = np.random.default_rng(31)
+    H0, blocks = cfg1_oracle
+    D = rng.normal(size=H0.shape)
+    ref = oracle.fvl(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cfg1.V, D, blocks)
+    got, ctx = gpu_fvl(cfg1, D)
+    assert_force_parity(got, ref, "cfg1")
+    torch = _torch()
+    H = ctx.gint_vlocal(torch.from_numpy(cfg1.V).cuda())
+    assert_parity(H.cpu().numpy(), H0, "vlocal after fvl")
+    rho_ref = oracle.rho(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, D, blocks)
+    rho = ctx.gint_rho(torch.from_numpy(D).cuda()).cpu().numpy()
+    assert np.abs(rho - rho_ref).max() <= TOL * np.abs(rho_ref).max()
+    got2 = ctx.gint_fvl(torch.from_numpy(cfg1.V).cuda(), torch.from_numpy(D).cuda()).cpu().numpy()
+    assert_force_parity(got2, ref, "cfg1, second call")
+    for seed, ngrid in [(7, (12, 10, 14)), (11, (9, 13, 7))]:
+        w = wl.tiny(seed=seed, ngrid=ngrid)
+        Hr, blk = oracle_H(w)
+        D = rng.normal(size=Hr.shape)
+        ref = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blk)
+        got, _ = gpu_fvl(w, D)
+        assert_force_parity(got, ref, "tiny %d" % seed)
+    # an atom exactly on a mesh point
+    w = wl.tiny(seed=5, ngrid=(12, 12, 12))
+    pos = np.array(w.atom_pos, dtype=np.float64)
+    pos[0] = (np.array([3, 4, 5]) / 12.0) @ np.asarray(w.lattice)
+    w.atom_pos = pos
+    Hr, blk = oracle_H(w)
+    D = rng.normal(size=Hr.shape)
+    ref = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blk)
+    got, _ = gpu_fvl(w, D)
+    assert_force_parity(got, ref, "atom on a mesh point")
+
+
+def test_fvl_cfg2_and_cluster():
+    import oracle
+    from paper_2603_21835_b200 import workloads as wl
+    rng = np.random.default_rng(32)
+    for name in ("si64_dzp", "cluster60"):
+        w = wl.make(name)
+        blocks = oracle.enumerate_blocks(w.lattice, w.species, w.atom_species, w.atom_pos)
+        D = rng.normal(size=int(blocks[3][-1]))
+        ref = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blocks)
+        got, _ = gpu_fvl(w, D)
+        assert_force_parity(got, ref, name)
+
+
+def test_fvl_sharded_sums_to_oracle(cfg1, cfg1_oracle):
+    """nranks = 2, 3 on one GPU: the partial forces of the ranks sum to the oracle's."""
+    import oracle
+    rng = np.random.default_rng(33)
+    H0, blocks = cfg1_oracle
+    D = rng.normal(size=H0.shape)
+    ref = oracle.fvl(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cfg1.V, D, blocks)
+    for nranks in (2, 3):
+        tot = np.zeros_like(ref)
+        for rank in range(nranks):
+            got, _ = gpu_fvl(cfg1, D, rank=rank, nranks=nranks)
+            tot += got
+        assert_force_parity(tot, ref, "nranks %d" % nranks)
+
+
+def test_fvl_large_full():
+    """si512_dzp at full size: all 512 x 3 force components against the oracle at the 1e-10 bar."""
+    import oracle
+    from paper_2603_21835_b200 import workloads as wl
+    w = wl.make("si512_dzp")
+    rng = np.random.default_rng(34)
+    blocks = oracle.enumerate_blocks(w.lattice, w.species, w.atom_species, w.atom_pos)
+    D = rng.normal(size=int(blocks[3][-1]))
+    got, ctx = gpu_fvl(w, D)
+    assert np.array_equal(ctx.gint_get_blocks()[3], blocks[3])
+    ref = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blocks)
+    assert_force_parity(got, ref, "si512_dzp")
