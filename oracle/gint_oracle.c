@@ -87,6 +87,21 @@ static int ylm_real(int l, double x, double y, double z, double *out)
         out[4] = c3 * (x * x - y * y);
         return 5;
     }
+    if (l == 3) { /* reading #7 extended: real f harmonics, m = -3..3, Cartesian forms on the unit sphere */
+        double a = 0.25 * sqrt(35.0 / (2.0 * pi)); /* m = -3, +3 */
+        double b = 0.5 * sqrt(105.0 / pi);         /* m = -2 */
+        double c = 0.25 * sqrt(21.0 / (2.0 * pi)); /* m = -1, +1 */
+        double d = 0.25 * sqrt(7.0 / pi);          /* m = 0 */
+        double e = 0.25 * sqrt(105.0 / pi);        /* m = +2 */
+        out[0] = a * y * (3.0 * x * x - y * y);
+        out[1] = b * x * y * z;
+        out[2] = c * y * (5.0 * z * z - 1.0);
+        out[3] = d * z * (5.0 * z * z - 3.0);
+        out[4] = c * x * (5.0 * z * z - 1.0);
+        out[5] = e * z * (x * x - y * y);
+        out[6] = a * x * (x * x - 3.0 * y * y);
+        return 7;
+    }
     return -1;
 }
 
@@ -121,7 +136,7 @@ static int phi_eval(const orc_species *sp, const double d[3], double *out)
     }
     for (int k = 0; k < sp->nrad; k++) {
         double f = radial_interp(sp->table + (size_t)k * sp->ntab, r, sp->dr);
-        double Y[5];
+        double Y[7];
         int nm = ylm_real(sp->l[k], x, y, z, Y);
         if (sp->l[k] > 0 && r < 1e-12) /* reading #6: l>0 -> 0 at the nucleus */
             for (int m = 0; m < nm; m++) Y[m] = 0.0;
@@ -509,6 +524,26 @@ static int ylm_poly_grad(int l, double x, double y, double z, double *P, double 
         P[3] = c1 * x * z;                         G[3][0] = c1 * z;        G[3][1] = 0.0;           G[3][2] = c1 * x;
         P[4] = c3 * (x * x - y * y);               G[4][0] = 2.0 * c3 * x;  G[4][1] = -2.0 * c3 * y; G[4][2] = 0.0;
         return 5;
+    }
+    if (l == 3) { /* homogeneous cubic forms of the f harmonics (r^2 = x^2 + y^2 + z^2 put back) and their gradients */
+        double a = 0.25 * sqrt(35.0 / (2.0 * pi)), b = 0.5 * sqrt(105.0 / pi), c = 0.25 * sqrt(21.0 / (2.0 * pi));
+        double d = 0.25 * sqrt(7.0 / pi), e = 0.25 * sqrt(105.0 / pi);
+        double q = 4.0 * z * z - x * x - y * y; /* 5 z^2 - r^2 */
+        P[0] = a * y * (3.0 * x * x - y * y);
+        G[0][0] = a * 6.0 * x * y; G[0][1] = a * (3.0 * x * x - 3.0 * y * y); G[0][2] = 0.0;
+        P[1] = b * x * y * z;
+        G[1][0] = b * y * z; G[1][1] = b * x * z; G[1][2] = b * x * y;
+        P[2] = c * y * q;
+        G[2][0] = c * (-2.0 * x * y); G[2][1] = c * (q - 2.0 * y * y); G[2][2] = c * 8.0 * y * z;
+        P[3] = d * z * (2.0 * z * z - 3.0 * x * x - 3.0 * y * y); /* z (5 z^2 - 3 r^2) */
+        G[3][0] = d * (-6.0 * x * z); G[3][1] = d * (-6.0 * y * z); G[3][2] = d * (6.0 * z * z - 3.0 * x * x - 3.0 * y * y);
+        P[4] = c * x * q;
+        G[4][0] = c * (q - 2.0 * x * x); G[4][1] = c * (-2.0 * x * y); G[4][2] = c * 8.0 * x * z;
+        P[5] = e * z * (x * x - y * y);
+        G[5][0] = e * 2.0 * x * z; G[5][1] = -e * 2.0 * y * z; G[5][2] = e * (x * x - y * y);
+        P[6] = a * x * (x * x - 3.0 * y * y);
+        G[6][0] = a * (3.0 * x * x - 3.0 * y * y); G[6][1] = -a * 6.0 * x * y; G[6][2] = 0.0;
+        return 7;
     }
     return -1;
 }

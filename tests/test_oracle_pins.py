@@ -712,3 +712,97 @@ def test_fvl_shift_atoms_roll_V_and_linearity(cfg1, cfg1_oracle):
     Fa = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, 2.0 * w.V - 0.5 * V2, D, blocks)
     Fb = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, V2, D, blocks)
     assert np.abs(Fa - (2.0 * F - 0.5 * Fb)).max() <= 1e-12 * np.abs(F).max()
+
+
+# ---- l = 3 (f shells, reading #7 extended) --------------------------------------------------
+def test_real_ylm_against_scipy_up_to_l3():
+    """Every real Y_lm of the oracle, l = 0..3, against SciPy's complex harmonics (a library routine): with SciPy's
+    Condon-Shortley Y_l^m, the real harmonic WITHOUT that phase is sqrt(2) (-1)^m Re Y_l^m (m > 0),
+    sqrt(2) (-1)^m Im Y_l^|m| (m < 0), Y_l^0 (m = 0), in the order m = -l..l.  A wrong constant, sign, m-order or a
+    swapped Cartesian factor in any of the 16 functions fails."""
+    from scipy.special import sph_harm_y
+    sp = unit_table_species([0, 1, 2, 3])
+    rng = np.random.default_rng(41)
+    d = rng.normal(size=(300, 3))
+    d *= (rng.uniform(0.1, 1.9, size=300) / np.linalg.norm(d, axis=1))[:, None]
+    Y = oracle.phi([sp], 0, d)
+    assert Y.shape[1] == 16
+    r = np.linalg.norm(d, axis=1)
+    theta, phi = np.arccos(d[:, 2] / r), np.arctan2(d[:, 1], d[:, 0])
+    col = 0
+    for l in range(4):
+        for m in range(-l, l + 1):
+            y = sph_harm_y(l, abs(m), theta, phi)
+            ref = y.real if m == 0 else math.sqrt(2) * (-1) ** m * (y.real if m > 0 else y.imag)
+            assert np.abs(Y[:, col] - ref).max() < 1e-14, (l, m)
+            col += 1
+
+
+def test_f_shell_unsold_orthonormality_and_nucleus():
+    sp = unit_table_species([3, 0, 3])
+    rng = np.random.default_rng(42)
+    d = rng.normal(size=(400, 3))
+    d *= (rng.uniform(0.1, 1.9, size=400) / np.linalg.norm(d, axis=1))[:, None]
+    Y = oracle.phi([sp], 0, d)
+    assert Y.shape[1] == 7 + 1 + 7
+    assert np.abs((Y[:, :7] ** 2).sum(1) - 7 / (4 * math.pi)).max() < 1e-14        # Unsold
+    assert np.abs(Y[:, 8:] - Y[:, :7]).max() == 0.0
+    sp = unit_table_species([0, 1, 2, 3])
+    nth, nph = 12, 24
+    x, wth = np.polynomial.legendre.leggauss(nth)
+    ph = 2 * math.pi * np.arange(nph) / nph
+    st = np.sqrt(1 - x * x)
+    q = np.stack([np.outer(st, np.cos(ph)), np.outer(st, np.sin(ph)), np.outer(x, np.ones(nph))], axis=-1).reshape(-1, 3)
+    wq = np.outer(wth, np.full(nph, 2 * math.pi / nph)).reshape(-1)
+    Yq = oracle.phi([sp], 0, q * 1.3)
+    assert np.abs(Yq.T @ (Yq * wq[:, None]) - np.eye(16)).max() < 1e-13
+    v = oracle.phi([sp], 0, np.zeros((1, 3)))[0]
+    assert v[0] != 0.0 and np.all(v[1:] == 0.0)                                   # reading #6
+
+
+def test_f_shell_gradient_matches_finite_differences():
+    """grad phi of an f shell (homogeneous cubic forms and their gradients, reading #19) against central differences
+    of oracle.phi, whose l = 3 values are pinned against SciPy above."""
+    sp = wl.make_species("f", 4.0, [(3, 0.6), (0, 0.8), (3, 1.0)], dr=0.01)
+    rng = np.random.default_rng(43)
+    u = rng.normal(size=(200, 3))
+    u /= np.linalg.norm(u, axis=1)[:, None]
+    r = (rng.integers(5, 380, size=200) + rng.uniform(0.3, 0.7, size=200)) * 0.01
+    d = u * r[:, None]
+    ph, gr = oracle.phi_grad([sp], 0, d)
+    assert np.abs(ph - oracle.phi([sp], 0, d)).max() <= 1e-15 * np.abs(ph).max()
+    h = 2e-5
+    for c in range(3):
+        e = np.zeros(3)
+        e[c] = h
+        fd = (oracle.phi([sp], 0, d + e) - oracle.phi([sp], 0, d - e)) / (2 * h)
+        assert np.abs(gr[:, :, c] - fd).max() <= 2e-8 * max(1.0, np.abs(gr).max())
+    _, g0 = oracle.phi_grad([sp], 0, np.zeros((1, 3)))
+    assert np.all(g0[0, :7] == 0.0) and np.all(g0[0, 8:] == 0.0)                   # reading #20: only l = 1 survives
+
+
+def test_f_shell_brute_force_and_force_fd():
+    """Whole pipeline with an f shell on a triclinic cell: H blocks against the dense enlarged-window sum, and the
+    force against Richardson-extrapolated central differences of the energy D : H[V] (as for l <= 2 above)."""
+    w = wl.tiny(seed=13, natom=2, ngrid=(10, 9, 11), shells=((0, 0.7), (3, 0.6)), rcut=3.0)
+    H, blocks = run_oracle(w)
+    d = block_dict(H, blocks, norb_per_atom(w))
+    scale = np.abs(H).max()
+    keys = list(d.keys())
+    for k in keys[::max(1, len(keys) // 10)]:
+        ref = brute_force_block(w, k[0], k[1], k[2:])
+        assert np.abs(d[k] - ref).max() <= 1e-13 * scale, k
+    rng = np.random.default_rng(44)
+    D = rng.normal(size=H.shape)
+    F = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blocks)
+    fs = np.abs(F).max()
+    for K in range(w.natom):
+        for c in range(3):
+            est = []
+            for h in (4e-3, 2e-3):
+                pp, pm = w.atom_pos.copy(), w.atom_pos.copy()
+                pp[K, c] += h
+                pm[K, c] -= h
+                est.append(-(_energy(w, D, blocks, pp) - _energy(w, D, blocks, pm)) / (2 * h))
+            rich = (4 * est[1] - est[0]) / 3
+            assert abs(rich - F[K, c]) <= 2e-6 * fs, (K, c, rich, F[K, c])
