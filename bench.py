@@ -37,9 +37,18 @@ sys.path.insert(0, ROOT)
 METRIC = "gint_vlocal FP64 TFLOP/s (useful flops F_sym per H build; ms/call in ms_per_step, % of roofline in roofline.frac)"
 UNIT = "TFLOP/s"
 
-# DRAM traffic of the integration kernel per launch, from the ncu --set full capture
-# summarised in profiles/ (dram__bytes_read.sum + dram__bytes_write.sum); None = not captured.
-NCU_TRAFFIC_BYTES = {"si512_dzp": 13.094e9 + 1.565e9}   # profiles/r01d_ncu_summary.md (the kernel was still named gint_vlocal_kernel there)
+
+
+def ncu_traffic(workload):
+    """DRAM traffic of the contraction kernel per launch (dram__bytes_read.sum + dram__bytes_write.sum of the latest
+    ncu --set full capture), read from profiles/ncu_traffic.json at run time; None if no capture is recorded."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        with open(p) as f:
+            rec = json.load(f).get(workload)
+        return None if rec is None else float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"])
+    except (OSError, ValueError, KeyError):
+        return None
 
 
 def measured_peaks():
@@ -282,7 +291,7 @@ def main():
     e2e_val = F_sym / (e2e_ms * 1e-3) * 1e-12
 
     # ---- next step of the workflow, outside the headline: H(k) = sum_R exp(i k.R) H(R) (Eq. 5) -------------
-    fold = rho_info = None
+    fold = rho_info = fvl_info = None
     if world == 1:
         ntot = ctx.gint_num_orbitals()[0]
         Hk = torch.empty((ntot, ntot), dtype=torch.complex128, device=dev)
@@ -313,7 +322,19 @@ def main():
         rho_info = {"ms_per_call": rho_ms, "useful_flops": F_sym, "achieved_tflops": F_sym / (rho_ms * 1e-3) * 1e-12,
                     "note": "gint_rho (Eq. 44) on the tensor pipe: tiles ga <= gb with E = D + D^T folded at gather time, "
                             "so F_sym accounting as for gint_vlocal; the time includes its psi kernel"}
-        del Dm, rho
+        # local Pulay force (Eq. 46)
+        Fv = ctx.gint_fvl(V, Dm)
+        torch.cuda.synchronize()
+        f0.record()
+        for _ in range(2):
+            ctx.gint_fvl(V, Dm, Fv)
+        f1.record()
+        torch.cuda.synchronize()
+        fvl_ms = f0.elapsed_time(f1) / 2
+        fvl_info = {"ms_per_call": fvl_ms, "useful_flops": F_pt, "achieved_tflops": F_pt / (fvl_ms * 1e-3) * 1e-12,
+                    "note": "gint_fvl (Eq. 46): psi kernel + E = D + D^T gather + T = E Phi (DMMA, dense inside active "
+                            "(row group, stage) pairs) + force kernel; T needs every (row, column) pair, so F_pt accounting"}
+        del Dm, rho, Fv
 
     if rank != 0:
         if world > 1:
@@ -332,11 +353,11 @@ def main():
     hbm_bytes = 8.0 * float(np.prod(w.ngrid)) + 8.0 * ctx.h_len
     roofline = {
         "bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-        "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+        "traffic": ncu_traffic(w.name),
         "kernel": "gint_contract_kernel<0>", "kernel_ms": main_ms, "mirror_kernel_ms": mirror_ms,
         "kernel_share_of_step": main_ms / ms_per_step,
         "psi_kernel": {"kernel": "gint_psi_kernel", "kernel_ms": psi_ms, "share_of_step": psi_ms / ms_per_step,
-                       "bound": "hbm", "algorithmic_bytes": psi_bytes,
+                       "bound": "hbm", "implementation_bytes": psi_bytes,
                        "achieved_gbs": psi_bytes / (psi_ms * 1e-3) * 1e-9, "peak_gbs": peaks["hbm_gbs"],
                        "frac": psi_bytes / (psi_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"],
                        "note": "writes psi = phi sqrt(|V dV|) once per listed (atom image, point) pair: "
@@ -351,11 +372,12 @@ def main():
     }
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "ms_per_step": ms_per_step, "ms_median": float(np.median(step_ms)), "ms_min": float(step_ms.min()),
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "natom": w.natom, "norb": w.norb_total, "ngrid": [int(x) for x in w.ngrid],
                    "nblocks": ctx.nblocks, "h_doubles": ctx.h_len,
-                   "bcell": [next(c for c in (8, 6, 4, int(n)) if int(n) % c == 0) for n in w.ngrid],
+                   "bcell": [int(st["bcell1"]), int(st["bcell2"]), int(st["bcell3"])],
                    "psi_scratch_bytes": st["psi_scratch_bytes"],
                    "l2": "flushed between timed iterations (256 MB write)", "parallelism": "cells sharded x%d" % world,
                    "input_sha256": w.sha256()[:16], "setup_s": setup_s, "wall_s_timed_region": wall},
@@ -373,6 +395,9 @@ def main():
         rho_info["peak_tflops"] = peak
         rho_info["frac"] = rho_info["achieved_tflops"] / peak
         out["rho"] = rho_info
+        fvl_info["peak_tflops"] = peak
+        fvl_info["frac"] = fvl_info["achieved_tflops"] / peak
+        out["fvl"] = fvl_info
     if not args.no_cpu_baseline and world == 1:
         na = min(w.natom, args.ref_atoms or 256)
         dt, used, nblk, ntot = oracle_sample(w, na)

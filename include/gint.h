@@ -21,10 +21,12 @@
  *   - The sum over g runs over all space with V periodic on the mesh.
  *   - Radial part: 4-point (cubic) Lagrange interpolation of the table on the
  *     forward stencil k..k+3, k = floor(r/dr); phi = 0 iff r >= rcut.
- *   - Real Y_lm, l <= 2, no Condon-Shortley phase, with (x,y,z) = r/|r|:
+ *   - Real Y_lm, l <= 3, no Condon-Shortley phase, with (x,y,z) = r/|r|:
  *       l=0: 1/(2 sqrt(pi));   l=1: sqrt(3/4pi) * {y, z, x};
  *       l=2: {1/2 sqrt(15/pi) xy, 1/2 sqrt(15/pi) yz, 1/4 sqrt(5/pi) (3z^2-1),
- *             1/2 sqrt(15/pi) xz, 1/4 sqrt(15/pi) (x^2-y^2)}.
+ *             1/2 sqrt(15/pi) xz, 1/4 sqrt(15/pi) (x^2-y^2)};
+ *       l=3: {1/4 sqrt(35/2pi) y(3x^2-y^2), 1/2 sqrt(105/pi) xyz, 1/4 sqrt(21/2pi) y(5z^2-1), 1/4 sqrt(7/pi) z(5z^2-3),
+ *             1/4 sqrt(21/2pi) x(5z^2-1), 1/4 sqrt(105/pi) z(x^2-y^2), 1/4 sqrt(35/2pi) x(x^2-3y^2)}.
  *     For |r| < 1e-12 bohr the l>0 components are 0.
  *   - Orbital order inside an atom: radial functions in the order given, each
  *     followed by its 2l+1 m-components in the order above.
@@ -50,7 +52,7 @@ extern "C" {
 
 #define GINT_OK 0
 #define GINT_EINVAL (-1)       /* null pointer, bad shape, non-positive size, table too short, singular lattice */
-#define GINT_EUNSUPPORTED (-2) /* l > 2, too many orbitals per atom, H too large for 32-bit block offsets */
+#define GINT_EUNSUPPORTED (-2) /* l > 3, too many orbitals per atom, H too large for 32-bit block offsets */
 #define GINT_ENOMEM (-3)       /* host or device allocation failed */
 #define GINT_ECUDA (-4)        /* CUDA runtime error; text via gint_last_error() */
 #define GINT_ENODEVICE (-5)    /* call needs a device but the context was created host-only (cuda_device < 0) */

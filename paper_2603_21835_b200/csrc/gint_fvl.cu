@@ -312,6 +312,18 @@ gint_force_kernel(const __grid_constant__ DevicePlan P, const __grid_constant__ 
                         const double ty = tval(), tz = tval(), tx = tval();
                         const double A = fma(ty, y, fma(tz, z, tx * x)) * (fd - qq);
                         gx = fma(A, x, fma(qq, tx, gx)); gy = fma(A, y, fma(qq, ty, gy)); gz = fma(A, z, fma(qq, tz, gz));
+                    } else if (l == 3) {
+                        // homogeneous cubic forms (table carries 1/2 sqrt(105/pi)) and their gradients
+                        const double qq = fv * rinv;
+                        const double ca = 0.20412414523193151, cc = 0.15811388300841897, cd = 0.12909944487358055;
+                        const double u0 = tval() * ca, u1 = tval(), u2 = tval() * cc, u3 = tval() * cd, u4 = tval() * cc, u5 = tval() * 0.5, u6 = tval() * ca;
+                        const double x2 = x * x, y2 = y * y, z2 = z * z, h = 4.0 * z2 - x2 - y2;
+                        const double A = (u0 * y * (3.0 * x2 - y2) + u1 * x * y * z + u2 * y * h + u3 * z * (2.0 * z2 - 3.0 * x2 - 3.0 * y2) +
+                                          u4 * x * h + u5 * z * (x2 - y2) + u6 * x * (x2 - 3.0 * y2)) * (fd - 3.0 * qq);
+                        const double bx = u0 * 6.0 * x * y + u1 * y * z - 2.0 * u2 * x * y - 6.0 * u3 * x * z + u4 * (h - 2.0 * x2) + 2.0 * u5 * x * z + 3.0 * u6 * (x2 - y2);
+                        const double by = 3.0 * u0 * (x2 - y2) + u1 * x * z + u2 * (h - 2.0 * y2) - 6.0 * u3 * y * z - 2.0 * u4 * x * y - 2.0 * u5 * y * z - 6.0 * u6 * x * y;
+                        const double bz = u1 * x * y + 8.0 * u2 * y * z + u3 * (6.0 * z2 - 3.0 * x2 - 3.0 * y2) + 8.0 * u4 * x * z + u5 * (x2 - y2);
+                        gx = fma(A, x, fma(qq, bx, gx)); gy = fma(A, y, fma(qq, by, gy)); gz = fma(A, z, fma(qq, bz, gz));
                     } else {
                         const double qq = fv * rinv;
                         const double c2 = 0.28867513459481288;

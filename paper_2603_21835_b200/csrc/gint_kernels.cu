@@ -214,13 +214,23 @@ __device__ __forceinline__ void eval_task(const SpeciesDev& sp, const double* __
             put(fv * y);
             put(fv * z);
             put(fv * x);
-        } else {
+        } else if (l == 2) {
             // table carries 1/2 sqrt(15/pi); ratios: 1/4 sqrt(5/pi) / that = 1/(2 sqrt 3), 1/4 sqrt(15/pi) / that = 1/2
             put(fv * (x * y));
             put(fv * (y * z));
             put(fv * (fma(3.0 * z, z, -lnz) * 0.28867513459481288));
             put(fv * (x * z));
             put(fv * (fma(x, x, -(y * y)) * 0.5));
+        } else {
+            // l = 3, m = -3..3; table carries 1/2 sqrt(105/pi); ratios 1/(2 sqrt 6), 1/(2 sqrt 10), 1/(2 sqrt 15), 1/2
+            const double x2 = x * x, y2 = y * y, q = fma(5.0 * z, z, -lnz);
+            put(fv * (0.20412414523193151 * y * fma(3.0, x2, -y2)));
+            put(fv * (x * y * z));
+            put(fv * (0.15811388300841897 * y * q));
+            put(fv * (0.12909944487358055 * z * fma(5.0 * z, z, -3.0 * lnz)));
+            put(fv * (0.15811388300841897 * x * q));
+            put(fv * (0.5 * z * (x2 - y2)));
+            put(fv * (0.20412414523193151 * x * fma(-3.0, y2, x2)));
         }
     };
     for (int f = 0; f < nradp; f += 2) {

@@ -70,7 +70,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         sp.norb = 0;
         for (int k = 0; k < sp.nrad; k++) {
             if (sp.l[k] < 0) { err = "negative l"; return GINT_EINVAL; }
-            if (sp.l[k] > 2) { err = "l > 2 not supported"; return GINT_EUNSUPPORTED; }
+            if (sp.l[k] > 3) { err = "l > 3 not supported"; return GINT_EUNSUPPORTED; }
             sp.norb += 2 * sp.l[k] + 1;
         }
         if (sp.norb > kMaxOrbPerAtom) { err = "too many orbitals per atom"; return GINT_EUNSUPPORTED; }
@@ -192,11 +192,11 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     }
 
     // ---- packed radial tables: node-major [ntab+4][nradp], pre-multiplied by the Y_lm constant -------
-    // l=0: 1/(2 sqrt(pi)); l=1: sqrt(3/4pi); l=2: 1/2 sqrt(15/pi) (the kernel applies the two remaining
-    // l=2 ratios to the angular polynomials).  Four zero nodes follow the table: the stencil of a point
+    // l=0: 1/(2 sqrt(pi)); l=1: sqrt(3/4pi); l=2: 1/2 sqrt(15/pi); l=3: 1/2 sqrt(105/pi) (the kernels apply the
+    // remaining l=2 and l=3 ratios to the angular polynomials).  Four zero nodes follow the table: the stencil of a point
     // outside the sphere is redirected there, so phi == 0 exactly for r >= rcut.
     {
-        const double ylm_c[3] = {0.28209479177387814, 0.48860251190291992, 1.0925484305920792};
+        const double ylm_c[4] = {0.28209479177387814, 0.48860251190291992, 1.0925484305920792, 2.8906114210352295};
         size_t off = 0;
         for (int s = 0; s < nspecies; s++) {
             SpeciesHost& sp = P.species[s];

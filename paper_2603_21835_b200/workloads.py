@@ -132,6 +132,16 @@ def species_dzp(name: str, rcut: float, a1: float, a2: float) -> Species:
     return make_species(name, rcut, [(0, a1), (0, a2), (1, a1), (1, a2), (2, a1)])
 
 
+def species_tzdp(name: str, rcut: float, a1: float, a2: float, a3: float) -> Species:
+    """3s 3p 2d = 22 orbitals, the basis of the paper's performance runs."""
+    return make_species(name, rcut, [(0, a1), (0, a2), (0, a3), (1, a1), (1, a2), (1, a3), (2, a1), (2, a2)])
+
+
+def species_dzpf(name: str, rcut: float, a1: float, a2: float) -> Species:
+    """2s 2p 1d 1f = 20 orbitals: exercises l = 3 (the paper's larger basis sets carry f shells)."""
+    return make_species(name, rcut, [(0, a1), (0, a2), (1, a1), (1, a2), (2, a1), (3, a1)])
+
+
 def species_2s1p(name: str, rcut: float, a1: float, a2: float) -> Species:
     """H-like 2s 1p = 5 orbitals; the single p shell uses zeta-1's alpha."""
     return make_species(name, rcut, [(0, a1), (0, a2), (1, a1)])
@@ -217,7 +227,11 @@ def si_like(nrep: int, seed: int, basis: str, disp: float, ngrid: int, name: str
     lattice = np.eye(3) * a
     ideal = diamond_supercell(nrep)
     pos = ideal + rng.uniform(-disp, disp, size=ideal.shape)   # draw 1: displacements [natom][3]
-    sp = species_sz(6.0) if basis == "SZ" else species_dzp("Si-DZP", 8.0, 0.3, 0.9)
+    sp = {"SZ": lambda: species_sz(6.0),
+          "DZP": lambda: species_dzp("Si-DZP", 8.0, 0.3, 0.9),
+          "TZDP": lambda: species_tzdp("Si-TZDP", 8.0, 0.3, 0.6, 1.2),
+          "DZP10": lambda: species_dzp("Si-DZP-rc10", 10.0, 0.3, 0.9),
+          "DZPF": lambda: species_dzpf("Si-DZPF", 6.0, 0.5, 1.0)}[basis]()
     ng = np.array([ngrid] * 3, dtype=np.int32)
     V = gaussian_wells(lattice, ng, pos, np.full(pos.shape[0], -2.0))
     V = V + fourier_noise(lattice, ng, rng)                     # draw 2: Fourier coefficients
@@ -253,10 +267,13 @@ def cluster60(seed: int = 4, ngrid: int = 160, box: float = 40.0) -> Workload:
 
 
 CONFIGS = ("si8_sz", "si64_dzp", "si216_dzp", "si512_dzp", "cluster60")
+# second workloads: the paper's own basis (TZDP 3s3p2d = 22 orbitals, rc = 8 a.u.),
+# its validation cutoff (rc = 10 a.u.) and an f shell; same cells, meshes, seeds and V recipe
+EXTRA_CONFIGS = ("si8_dzpf", "si64_tzdp", "si64_dzp_rc10", "si512_tzdp", "si512_dzp_rc10")
 
 
 def make(name: str) -> Workload:
-    """The five BASELINE.json configs, by name (see CONFIGS)."""
+    """The five BASELINE.json configs (CONFIGS) and the second workloads (EXTRA_CONFIGS), by name."""
     if name == "si8_sz":
         return si_like(1, 0, "SZ", 0.05, 36, name)
     if name == "si64_dzp":
@@ -267,6 +284,16 @@ def make(name: str) -> Workload:
         return si_like(4, 3, "DZP", 0.1, 144, name)
     if name == "cluster60":
         return cluster60()
+    if name == "si8_dzpf":
+        return si_like(1, 0, "DZPF", 0.05, 36, name)
+    if name == "si64_tzdp":
+        return si_like(2, 1, "TZDP", 0.1, 72, name)
+    if name == "si64_dzp_rc10":
+        return si_like(2, 1, "DZP10", 0.1, 72, name)
+    if name == "si512_tzdp":
+        return si_like(4, 3, "TZDP", 0.1, 144, name)
+    if name == "si512_dzp_rc10":
+        return si_like(4, 3, "DZP10", 0.1, 144, name)
     raise KeyError(name)
 
 
