@@ -61,7 +61,7 @@ typedef struct gint_ctx gint_ctx; /* opaque; owns all host and device metadata *
 
 /* One atomic species: nrad tabulated radial functions f(r), node k at r = k*dr.
  * Requirements: dr > 0, rcut > 0, ntab*dr >= rcut + 3*dr (the forward stencil may
- * read three nodes past floor(rcut/dr)); 0 <= l[k] <= 2; sum(2l+1) <= 64.
+ * read three nodes past floor(rcut/dr)); 0 <= l[k] <= 3; nrad <= 8; sum(2l+1) <= 64.
  * The arrays are copied during gint_setup and not retained. */
 typedef struct {
     double rcut;         /* phi == 0 for r >= rcut (bohr)                          */
@@ -91,6 +91,15 @@ typedef struct {
 int gint_setup(gint_ctx **out, const double *lattice, const int32_t *ngrid, int32_t nspecies,
                const gint_species *species, int32_t natom, const int32_t *atom_species, const double *atom_pos,
                int32_t cuda_device, const gint_options *opt);
+
+/* New atom positions for an existing context (Ehrenfest dynamics moves the nuclei every step, PAPER.md:220-222,
+ * Eq. 42 at PAPER.md:326): rebuilds the big-cell lists, the block table and the work items for atom_pos
+ * ([natom][3] Cartesian, bohr, host pointer; species, lattice, mesh, big-cell size and rank stay as given to
+ * gint_setup) and replaces the context's device tables and scratch buffers.  The BLOCK TABLE MAY CHANGE (pairs move
+ * in and out of range): query gint_num_blocks / gint_get_blocks again and size H, D accordingly.  Synchronises the
+ * device first (calls in flight read the old tables).  On a plan error (GINT_EINVAL / GINT_EUNSUPPORTED) the context
+ * is unchanged; on a CUDA error afterwards it is only good for gint_destroy. */
+int gint_update_positions(gint_ctx *ctx, const double *atom_pos);
 
 /* Number of H blocks and length of the H buffer in doubles. */
 int gint_num_blocks(const gint_ctx *ctx, int64_t *nblocks, int64_t *h_len);

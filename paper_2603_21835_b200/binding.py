@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libgint_b200.so")
 
 GINT_OK, GINT_EINVAL, GINT_EUNSUPPORTED, GINT_ENOMEM, GINT_ECUDA, GINT_ENODEVICE = 0, -1, -2, -3, -4, -5
 
-EXPORTED = ("gint_setup", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
+EXPORTED = ("gint_setup", "gint_update_positions", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
             "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_rho", "gint_fvl", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
@@ -51,6 +51,8 @@ def _load() -> ctypes.CDLL:
     P = ctypes.POINTER
     lib.gint_setup.restype = ctypes.c_int
     lib.gint_setup.argtypes = [P(vp), P(dbl), P(i32), i32, P(_Species), i32, P(i32), P(dbl), i32, P(_Options)]
+    lib.gint_update_positions.restype = ctypes.c_int
+    lib.gint_update_positions.argtypes = [vp, P(dbl)]
     lib.gint_num_blocks.restype = ctypes.c_int
     lib.gint_num_blocks.argtypes = [vp, P(i64), P(i64)]
     lib.gint_get_blocks.restype = ctypes.c_int
@@ -110,6 +112,16 @@ class GintContext:
         self._h = ctypes.c_void_p(handle)
         self.natom = int(natom)
         self.ngrid = tuple(int(x) for x in ngrid)
+        nb, hl = ctypes.c_int64(), ctypes.c_int64()
+        _check(_lib.gint_num_blocks(self._h, ctypes.byref(nb), ctypes.byref(hl)), "gint_num_blocks")
+        self.nblocks, self.h_len = int(nb.value), int(hl.value)
+
+    def gint_update_positions(self, atom_pos):
+        """Rebuild the context for new atom positions [natom][3]; nblocks / h_len are refreshed (the block table may change)."""
+        pos = np.ascontiguousarray(atom_pos, dtype=np.float64).reshape(-1, 3)
+        if pos.shape[0] != self.natom:
+            raise ValueError("atom_pos must be [natom][3]")
+        _check(_lib.gint_update_positions(self._h, _ptr(pos, ctypes.c_double)), "gint_update_positions")
         nb, hl = ctypes.c_int64(), ctypes.c_int64()
         _check(_lib.gint_num_blocks(self._h, ctypes.byref(nb), ctypes.byref(hl)), "gint_num_blocks")
         self.nblocks, self.h_len = int(nb.value), int(hl.value)

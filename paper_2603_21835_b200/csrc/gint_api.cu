@@ -84,6 +84,123 @@ void release(gint_ctx* ctx) {
     delete ctx;
 }
 
+// Device side of a context: upload the plan, allocate the scratch buffers, build the grid overlap S.  On failure the
+// caller releases the context (everything allocated so far is in ctx->allocs).
+int device_init(gint_ctx* ctx) {
+    const int natom = (int)ctx->plan.atom_species.size();
+    (void)natom;
+    DeviceGuard guard(ctx->device);
+    cudaError_t e = guard.err;
+    if (e != cudaSuccess) return fail_cuda(e, "cudaSetDevice");
+    const int cuda_device = ctx->device;
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, cuda_device);
+    if (e != cudaSuccess) { return fail_cuda(e, "cudaGetDeviceProperties"); }
+    ctx->nsm = prop.multiProcessorCount;
+    if (ctx->plan.smem_bytes > (size_t)prop.sharedMemPerBlockOptin) {
+        return fail(GINT_EUNSUPPORTED, "device offers too little shared memory per block");
+    }
+    gint::Plan& P = ctx->plan;
+    gint::DevicePlan& D = ctx->dev;
+#define UP(vec, ptr)                                                   \
+    if ((e = upload(ctx, vec, ptr)) != cudaSuccess) {                  \
+        return fail_cuda(e, "upload " #vec);                           \
+    }
+    UP(P.descs, &D.descs)
+    UP(P.regions, &D.regions)
+    UP(P.entries, &D.entries)
+    UP(P.etasks, &D.etasks)
+    UP(P.pair, &D.pair)
+    UP(P.pair_direct, &D.pair_direct)
+    UP(P.slot_xyz, &D.slot_xyz)
+    UP(P.mirror, &D.mirror)
+    UP(P.tab_packed, &D.tab)
+    UP(P.sp_meta, &D.sp_meta)
+    UP(P.sp_real, &D.sp_real)
+    {   // block table for gint_fold_k
+        std::vector<int32_t> run_start, first32(ctx->first_orb.begin(), ctx->first_orb.end());
+        for (size_t b = 0; b < P.blk_i.size(); b++)
+            if (b == 0 || P.blk_i[b] != P.blk_i[b - 1] || P.blk_j[b] != P.blk_j[b - 1]) run_start.push_back((int32_t)b);
+        ctx->fold.nrun = (int32_t)run_start.size();
+        run_start.push_back((int32_t)P.blk_i.size());
+        ctx->fold.norb_tot = (int32_t)ctx->first_orb.back();
+        UP(P.blk_i, &ctx->fold.blk_i)
+        UP(P.blk_j, &ctx->fold.blk_j)
+        UP(P.blk_R, &ctx->fold.blk_R)
+        UP(P.blk_off, &ctx->fold.blk_off)
+        UP(run_start, &ctx->fold.run_start)
+        UP(first32, &ctx->fold.first)
+    }
+#undef UP
+    void* ctr = nullptr;   // work-queue head, shift of the potential, partial (min, max) of V
+    if ((e = cudaMalloc(&ctr, 128 + 2 * 512 * sizeof(double))) != cudaSuccess) { return fail_cuda(e, "cudaMalloc counter"); }
+    ctx->allocs.push_back(ctr);
+    D.counter = reinterpret_cast<unsigned int*>(ctr);
+    D.shift = reinterpret_cast<gint::ShiftDev*>(reinterpret_cast<unsigned char*>(ctr) + 64);
+    D.vpart = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(ctr) + 128);
+    {
+        std::vector<int32_t> work;
+        for (size_t r = 0; r < P.regions.size(); r++)
+            if (P.regions[r].ntile > 0) work.push_back((int32_t)r);
+        D.nwork_regions = (int32_t)work.size();
+        if ((e = upload(ctx, work, &D.work_regions)) != cudaSuccess) { return fail_cuda(e, "upload work_regions"); }
+    }
+    // psi scratch: zero-filled once; rows and slices that no evaluation task writes stay zero for good
+    void* psi = nullptr;
+    const size_t psi_bytes = (size_t)P.psi_chunks * gint::kChunkBytes;
+    if ((e = cudaMalloc(&psi, psi_bytes ? psi_bytes : 16)) != cudaSuccess) { return fail_cuda(e, "cudaMalloc psi scratch"); }
+    ctx->allocs.push_back(psi);
+    if (psi_bytes && (e = cudaMemset(psi, 0, psi_bytes)) != cudaSuccess) { return fail_cuda(e, "cudaMemset psi scratch"); }
+    D.psi = reinterpret_cast<double*>(psi);
+    std::memcpy(D.estep, P.estep, sizeof(D.estep));
+    D.dV = P.dV;
+    for (int d = 0; d < 3; d++) D.ngrid[d] = P.ngrid[d];
+    D.nks_pad = P.nks_pad;
+    D.nslice = P.nslice;
+    D.nstage = P.nstage;
+    D.nregions = (int32_t)P.regions.size();
+    D.nring = P.nring;
+    D.never = 0;
+    D.nitems = (int32_t)P.descs.size();
+    D.nmirror = (int32_t)P.mirror.size();
+    D.tab_doubles = (int32_t)P.tab_packed.size();
+    D.nspecies = (int32_t)P.species.size();
+    ctx->psi_smem = gint::psi_kernel_smem(P.tables_in_smem ? P.tab_packed.size() * sizeof(double) : 0, (int)P.species.size());
+    ctx->contract_smem = gint::contract_kernel_smem(P.nring);
+    if ((e = gint::configure_kernels(ctx->psi_smem, ctx->contract_smem, P.tables_in_smem)) != cudaSuccess) {
+        return fail_cuda(e, "cudaFuncSetAttribute");
+    }
+    {   // S = grid overlap blocks (Eq. 45 with V = 1): the per-call shift of the potential needs them (gint_hinit_kernel)
+        const size_t nH = (size_t)P.blk_off.back(), nV = (size_t)P.ngrid[0] * P.ngrid[1] * P.ngrid[2];
+        void *Sd = nullptr, *ones = nullptr;
+        if ((e = cudaMalloc(&Sd, (nH ? nH : 1) * sizeof(double))) != cudaSuccess) { return fail_cuda(e, "cudaMalloc S"); }
+        ctx->allocs.push_back(Sd);
+        D.S = reinterpret_cast<const double*>(Sd);
+        if ((e = cudaMalloc(&ones, nV * sizeof(double))) != cudaSuccess) { return fail_cuda(e, "cudaMalloc V=1"); }
+        std::vector<double> one(nV, 1.0);
+        e = cudaMemcpy(ones, one.data(), nV * sizeof(double), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess)
+            e = gint::launch_vlocal(D, ctx->psi_smem, ctx->contract_smem, P.tables_in_smem, ctx->nsm, nH,
+                                    reinterpret_cast<const double*>(ones), reinterpret_cast<double*>(Sd), true, nullptr, nullptr);
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        cudaFree(ones);
+        if (e != cudaSuccess) { return fail_cuda(e, "grid overlap S"); }
+    }
+    return GINT_OK;
+}
+
+// frees what device_init allocated (the context keeps its events and host-call scratch)
+void device_release_arrays(gint_ctx* ctx) {
+    DeviceGuard guard(ctx->device);
+    for (void* p : ctx->allocs) cudaFree(p);
+    ctx->allocs.clear();
+    ctx->have_fvl = false;
+    ctx->fvl = gint::FvlPlan{};
+    ctx->fold = gint::FoldPlan{};
+    ctx->dev = gint::DevicePlan{};
+    if (ctx->H_scratch) { cudaFree(ctx->H_scratch); ctx->H_scratch = nullptr; }
+}
+
 }  // namespace
 
 extern "C" {
@@ -132,108 +249,47 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         *out = ctx;
         return GINT_OK;
     }
-    DeviceGuard guard(cuda_device);
-    cudaError_t e = guard.err;
-    if (e != cudaSuccess) { delete ctx; return fail_cuda(e, "cudaSetDevice"); }
     ctx->device = cuda_device;
-    cudaDeviceProp prop;
-    e = cudaGetDeviceProperties(&prop, cuda_device);
-    if (e != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaGetDeviceProperties"); }
-    ctx->nsm = prop.multiProcessorCount;
-    if (ctx->plan.smem_bytes > (size_t)prop.sharedMemPerBlockOptin) {
+    const int rc = device_init(ctx);
+    if (rc != GINT_OK) {
         release(ctx);
-        return fail(GINT_EUNSUPPORTED, "device offers too little shared memory per block");
-    }
-    gint::Plan& P = ctx->plan;
-    gint::DevicePlan& D = ctx->dev;
-#define UP(vec, ptr)                                                   \
-    if ((e = upload(ctx, vec, ptr)) != cudaSuccess) {                  \
-        release(ctx);                                                  \
-        return fail_cuda(e, "upload " #vec);                           \
-    }
-    UP(P.descs, &D.descs)
-    UP(P.regions, &D.regions)
-    UP(P.entries, &D.entries)
-    UP(P.etasks, &D.etasks)
-    UP(P.pair, &D.pair)
-    UP(P.pair_direct, &D.pair_direct)
-    UP(P.slot_xyz, &D.slot_xyz)
-    UP(P.mirror, &D.mirror)
-    UP(P.tab_packed, &D.tab)
-    UP(P.sp_meta, &D.sp_meta)
-    UP(P.sp_real, &D.sp_real)
-    {   // block table for gint_fold_k
-        std::vector<int32_t> run_start, first32(ctx->first_orb.begin(), ctx->first_orb.end());
-        for (size_t b = 0; b < P.blk_i.size(); b++)
-            if (b == 0 || P.blk_i[b] != P.blk_i[b - 1] || P.blk_j[b] != P.blk_j[b - 1]) run_start.push_back((int32_t)b);
-        ctx->fold.nrun = (int32_t)run_start.size();
-        run_start.push_back((int32_t)P.blk_i.size());
-        ctx->fold.norb_tot = (int32_t)ctx->first_orb.back();
-        UP(P.blk_i, &ctx->fold.blk_i)
-        UP(P.blk_j, &ctx->fold.blk_j)
-        UP(P.blk_R, &ctx->fold.blk_R)
-        UP(P.blk_off, &ctx->fold.blk_off)
-        UP(run_start, &ctx->fold.run_start)
-        UP(first32, &ctx->fold.first)
-    }
-#undef UP
-    void* ctr = nullptr;   // work-queue head, shift of the potential, partial (min, max) of V
-    if ((e = cudaMalloc(&ctr, 128 + 2 * 512 * sizeof(double))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc counter"); }
-    ctx->allocs.push_back(ctr);
-    D.counter = reinterpret_cast<unsigned int*>(ctr);
-    D.shift = reinterpret_cast<gint::ShiftDev*>(reinterpret_cast<unsigned char*>(ctr) + 64);
-    D.vpart = reinterpret_cast<double*>(reinterpret_cast<unsigned char*>(ctr) + 128);
-    {
-        std::vector<int32_t> work;
-        for (size_t r = 0; r < P.regions.size(); r++)
-            if (P.regions[r].ntile > 0) work.push_back((int32_t)r);
-        D.nwork_regions = (int32_t)work.size();
-        if ((e = upload(ctx, work, &D.work_regions)) != cudaSuccess) { release(ctx); return fail_cuda(e, "upload work_regions"); }
-    }
-    // psi scratch: zero-filled once; rows and slices that no evaluation task writes stay zero for good
-    void* psi = nullptr;
-    const size_t psi_bytes = (size_t)P.psi_chunks * gint::kChunkBytes;
-    if ((e = cudaMalloc(&psi, psi_bytes ? psi_bytes : 16)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc psi scratch"); }
-    ctx->allocs.push_back(psi);
-    if (psi_bytes && (e = cudaMemset(psi, 0, psi_bytes)) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMemset psi scratch"); }
-    D.psi = reinterpret_cast<double*>(psi);
-    std::memcpy(D.estep, P.estep, sizeof(D.estep));
-    D.dV = P.dV;
-    for (int d = 0; d < 3; d++) D.ngrid[d] = P.ngrid[d];
-    D.nks_pad = P.nks_pad;
-    D.nslice = P.nslice;
-    D.nstage = P.nstage;
-    D.nregions = (int32_t)P.regions.size();
-    D.nring = P.nring;
-    D.never = 0;
-    D.nitems = (int32_t)P.descs.size();
-    D.nmirror = (int32_t)P.mirror.size();
-    D.tab_doubles = (int32_t)P.tab_packed.size();
-    D.nspecies = (int32_t)P.species.size();
-    ctx->psi_smem = gint::psi_kernel_smem(P.tables_in_smem ? P.tab_packed.size() * sizeof(double) : 0, (int)P.species.size());
-    ctx->contract_smem = gint::contract_kernel_smem(P.nring);
-    if ((e = gint::configure_kernels(ctx->psi_smem, ctx->contract_smem, P.tables_in_smem)) != cudaSuccess) {
-        release(ctx);
-        return fail_cuda(e, "cudaFuncSetAttribute");
-    }
-    {   // S = grid overlap blocks (Eq. 45 with V = 1): the per-call shift of the potential needs them (gint_hinit_kernel)
-        const size_t nH = (size_t)P.blk_off.back(), nV = (size_t)P.ngrid[0] * P.ngrid[1] * P.ngrid[2];
-        void *Sd = nullptr, *ones = nullptr;
-        if ((e = cudaMalloc(&Sd, (nH ? nH : 1) * sizeof(double))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc S"); }
-        ctx->allocs.push_back(Sd);
-        D.S = reinterpret_cast<const double*>(Sd);
-        if ((e = cudaMalloc(&ones, nV * sizeof(double))) != cudaSuccess) { release(ctx); return fail_cuda(e, "cudaMalloc V=1"); }
-        std::vector<double> one(nV, 1.0);
-        e = cudaMemcpy(ones, one.data(), nV * sizeof(double), cudaMemcpyHostToDevice);
-        if (e == cudaSuccess)
-            e = gint::launch_vlocal(D, ctx->psi_smem, ctx->contract_smem, P.tables_in_smem, ctx->nsm, nH,
-                                    reinterpret_cast<const double*>(ones), reinterpret_cast<double*>(Sd), true, nullptr, nullptr);
-        if (e == cudaSuccess) e = cudaDeviceSynchronize();
-        cudaFree(ones);
-        if (e != cudaSuccess) { release(ctx); return fail_cuda(e, "grid overlap S"); }
+        return rc;
     }
     *out = ctx;
     return GINT_OK;
+}
+
+int gint_update_positions(gint_ctx* ctx, const double* atom_pos) {
+    if (!ctx || !atom_pos) return fail(GINT_EINVAL, "null argument");
+    const gint::Plan& old = ctx->plan;
+    const int natom = (int)old.atom_species.size();
+    gint_ctx* fresh = new (std::nothrow) gint_ctx;
+    if (!fresh) return fail(GINT_ENOMEM, "host allocation failed");
+    try {
+        std::string err;
+        std::vector<int32_t> asp(old.atom_species.begin(), old.atom_species.end());
+        const int32_t ng[3] = {old.ngrid[0], old.ngrid[1], old.ngrid[2]};
+        const int32_t bc[3] = {old.bcell[0], old.bcell[1], old.bcell[2]};
+        const int rc = gint::build_plan(fresh->plan, old.lattice, ng, (int)old.species.size(), old.species.data(), natom,
+                                        asp.data(), atom_pos, bc, old.rank, old.nranks, err);
+        if (rc != GINT_OK) {
+            delete fresh;
+            return fail(rc, err);   // the context is unchanged
+        }
+    } catch (const std::bad_alloc&) {
+        delete fresh;
+        return fail(GINT_ENOMEM, "host allocation failed");
+    }
+    std::swap(ctx->plan, fresh->plan);
+    delete fresh;
+    if (ctx->device < 0) return GINT_OK;
+    {
+        DeviceGuard guard(ctx->device);
+        if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
+        cudaDeviceSynchronize();   // calls in flight still read the old tables
+    }
+    device_release_arrays(ctx);
+    return device_init(ctx);
 }
 
 int gint_num_blocks(const gint_ctx* ctx, int64_t* nblocks, int64_t* h_len) {

@@ -6,7 +6,9 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <atomic>
 #include <numeric>
+#include <thread>
 
 #include "../../include/gint.h"
 
@@ -37,7 +39,31 @@ inline int64_t floordiv(int64_t a, int64_t b) {
     return (r != 0 && ((r < 0) != (b < 0))) ? q - 1 : q;
 }
 
-inline size_t align16(size_t x) { return (x + 15) & ~size_t(15); }
+// f(i, thread) for i in [0, n), indices handed out in blocks of `grain` to hardware_concurrency() threads (at most 32)
+template <class F>
+void parallel_for(size_t n, size_t grain, F f) {
+    unsigned nt = std::thread::hardware_concurrency();
+    if (const char* env = std::getenv("GINT_SETUP_THREADS")) nt = (unsigned)std::atoi(env);
+    nt = std::max(1u, std::min(nt, 32u));
+    if ((size_t)nt * grain > n) nt = (unsigned)std::max<size_t>(1, n / std::max<size_t>(1, grain));
+    if (nt <= 1) {
+        for (size_t i = 0; i < n; i++) f(i, 0u);
+        return;
+    }
+    std::atomic<size_t> next{0};
+    auto body = [&](unsigned t) {
+        for (;;) {
+            const size_t b = next.fetch_add(grain);
+            if (b >= n) break;
+            for (size_t i = b; i < std::min(n, b + grain); i++) f(i, t);
+        }
+    };
+    std::vector<std::thread> th;
+    for (unsigned t = 1; t < nt; t++) th.emplace_back(body, t);
+    body(0);
+    for (auto& x : th) x.join();
+}
+constexpr unsigned kMaxThreads = 32;
 
 }  // namespace
 
@@ -112,38 +138,47 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     // ---- block table (sorted by I, J, R1, R2, R3) ---------------------------
     auto norb_of = [&](int a) { return P.species[P.atom_species[a]].norb; };
     auto rc_of = [&](int a) { return P.species[P.atom_species[a]].rcut; };
-    P.blk_off.push_back(0);
-    for (int I = 0; I < natom; I++)
-        for (int J = 0; J < natom; J++) {
-            double dc[3], f[3];
-            for (int c = 0; c < 3; c++) dc[c] = atom_pos[3 * I + c] - atom_pos[3 * J + c];
-            const double reach = rc_of(I) + rc_of(J);
-            int lo[3], hi[3];
-            for (int d = 0; d < 3; d++) {
-                f[d] = dc[0] * inv[d] + dc[1] * inv[3 + d] + dc[2] * inv[6 + d];
-                lo[d] = (int)std::floor(f[d] - reach * blen[d]) - 1;
-                hi[d] = (int)std::ceil(f[d] + reach * blen[d]) + 1;
-            }
-            for (int r1 = lo[0]; r1 <= hi[0]; r1++)
-                for (int r2 = lo[1]; r2 <= hi[1]; r2++)
-                    for (int r3 = lo[2]; r3 <= hi[2]; r3++) {
-                        double v[3];
-                        for (int c = 0; c < 3; c++)
-                            v[c] = r1 * lattice[c] + r2 * lattice[3 + c] + r3 * lattice[6 + c] - dc[c];
-                        if (std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) < reach) {
-                            if (std::abs(r1) > 127 || std::abs(r2) > 127 || std::abs(r3) > 127) {
-                                err = "lattice image index beyond +-127";
-                                return GINT_EUNSUPPORTED;
+    {
+        struct Blk { int32_t J, r1, r2, r3; };
+        std::vector<std::vector<Blk>> per_atom((size_t)natom);
+        std::atomic<int> bad{0};
+        parallel_for((size_t)natom, 4, [&](size_t Is, unsigned) {
+            const int I = (int)Is;
+            for (int J = 0; J < natom; J++) {
+                double dc[3], f[3];
+                for (int c = 0; c < 3; c++) dc[c] = atom_pos[3 * I + c] - atom_pos[3 * J + c];
+                const double reach = rc_of(I) + rc_of(J);
+                int lo[3], hi[3];
+                for (int d = 0; d < 3; d++) {
+                    f[d] = dc[0] * inv[d] + dc[1] * inv[3 + d] + dc[2] * inv[6 + d];
+                    lo[d] = (int)std::floor(f[d] - reach * blen[d]) - 1;
+                    hi[d] = (int)std::ceil(f[d] + reach * blen[d]) + 1;
+                }
+                for (int r1 = lo[0]; r1 <= hi[0]; r1++)
+                    for (int r2 = lo[1]; r2 <= hi[1]; r2++)
+                        for (int r3 = lo[2]; r3 <= hi[2]; r3++) {
+                            double v[3];
+                            for (int c = 0; c < 3; c++)
+                                v[c] = r1 * lattice[c] + r2 * lattice[3 + c] + r3 * lattice[6 + c] - dc[c];
+                            if (std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]) < reach) {
+                                if (std::abs(r1) > 127 || std::abs(r2) > 127 || std::abs(r3) > 127) { bad = 1; continue; }
+                                per_atom[Is].push_back({J, r1, r2, r3});
                             }
-                            P.blk_i.push_back(I);
-                            P.blk_j.push_back(J);
-                            P.blk_R.push_back(r1);
-                            P.blk_R.push_back(r2);
-                            P.blk_R.push_back(r3);
-                            P.blk_off.push_back(P.blk_off.back() + (int64_t)norb_of(I) * norb_of(J));
                         }
-                    }
-        }
+            }
+        });
+        if (bad) { err = "lattice image index beyond +-127"; return GINT_EUNSUPPORTED; }
+        P.blk_off.push_back(0);
+        for (int I = 0; I < natom; I++)
+            for (const Blk& b : per_atom[(size_t)I]) {
+                P.blk_i.push_back(I);
+                P.blk_j.push_back(b.J);
+                P.blk_R.push_back(b.r1);
+                P.blk_R.push_back(b.r2);
+                P.blk_R.push_back(b.r3);
+                P.blk_off.push_back(P.blk_off.back() + (int64_t)norb_of(I) * norb_of(b.J));
+            }
+    }
     const int64_t nblk = (int64_t)P.blk_i.size();
     // block offsets are stored in 32 bits (kNoBlock = 2^32 - 1 marks "no such block"): H below 32 GiB
     if (P.blk_off.back() >= (int64_t)kNoBlock) { err = "H buffer exceeds 2^32 - 1 doubles"; return GINT_EUNSUPPORTED; }
@@ -261,10 +296,15 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         }
     struct Tmp { int64_t cell; int npop; Entry e; };
     std::vector<Tmp> tmp;
-    tmp.reserve((size_t)natom * 256);
     std::vector<int32_t> npoint_orb((size_t)ngrid[0] * ngrid[1] * ngrid[2], 0);
     double n_insphere = 0;
-    for (int I = 0; I < natom; I++) {
+    std::vector<std::vector<Tmp>> tmp_thread(kMaxThreads);
+    std::vector<double> insphere_thread(kMaxThreads, 0.0);
+    std::atomic<int> bad_image{0};
+    parallel_for((size_t)natom, 2, [&](size_t Is, unsigned tid) {
+        const int I = (int)Is;
+        std::vector<Tmp>& tmp = tmp_thread[tid];
+        double& n_insphere = insphere_thread[tid];
         const int sp_id = P.atom_species[I];
         const double rc = P.species[sp_id].rcut, rc2 = rc * rc;
         const int norb = P.species[sp_id].norb;
@@ -290,7 +330,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 for (auto& qc3 : rng[2]) {
                     const int q[3] = {qc1.first, qc2.first, qc3.first};
                     const int c[3] = {qc1.second, qc2.second, qc3.second};
-                    if (std::abs(q[0]) > 127 || std::abs(q[1]) > 127 || std::abs(q[2]) > 127) { err = "image index beyond +-127"; return GINT_EUNSUPPORTED; }
+                    if (std::abs(q[0]) > 127 || std::abs(q[1]) > 127 || std::abs(q[2]) > 127) { bad_image = 1; continue; }
                     Entry e;
                     std::memset(&e, 0, sizeof(e));
                     const int o[3] = {c[0] * bx, c[1] * by, c[2] * bz};
@@ -318,7 +358,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                             const int ks = s / kKstepPts;
                             e.kmask[ks >> 5] |= 1u << (ks & 31);
                             npin++;
-                            npoint_orb[((size_t)(o[0] + ix) * ngrid[1] + (o[1] + iy)) * ngrid[2] + (o[2] + iz)] += norb;
+                            __atomic_fetch_add(&npoint_orb[((size_t)(o[0] + ix) * ngrid[1] + (o[1] + iy)) * ngrid[2] + (o[2] + iz)], norb, __ATOMIC_RELAXED);
                         }
                     }
                     if (!npin) continue;
@@ -331,6 +371,12 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                     tmp.push_back({((int64_t)c[0] * P.ncell[1] + c[1]) * P.ncell[2] + c[2], npop, e});
                 }
         }
+    });
+    if (bad_image) { err = "image index beyond +-127"; return GINT_EUNSUPPORTED; }
+    for (unsigned t = 0; t < kMaxThreads; t++) {
+        tmp.insert(tmp.end(), tmp_thread[t].begin(), tmp_thread[t].end());
+        n_insphere += insphere_thread[t];
+        std::vector<Tmp>().swap(tmp_thread[t]);
     }
     auto rkey = [](const Entry& e) { return (uint32_t)(e.Rpack & 0xFFFFFF); };
     // query lists: per region sorted by (atom, R)
@@ -412,41 +458,66 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) n += kstep_cost_of(gm, gi, gj, ks);
         return n;
     };
-    size_t pos = 0;
-    while (pos < tmp.size()) {
-        size_t end = pos;
-        while (end < tmp.size() && tmp[end].cell == tmp[pos].cell) end++;
-        const int64_t c = tmp[pos].cell;
-        const int m = (int)(end - pos);
-        if (m > 4095) { err = "more than 4095 atom images touch one region"; return GINT_EUNSUPPORTED; }
-        Region R;
-        std::memset(&R, 0, sizeof(R));
-        const int c3 = (int)(c % P.ncell[2]), c2 = (int)((c / P.ncell[2]) % P.ncell[1]), c1 = (int)(c / ((int64_t)P.ncell[1] * P.ncell[2]));
-        R.origin[0] = c1 * bx;
-        R.origin[1] = c2 * by;
-        R.origin[2] = c3 * bz;
-        int rows = 0;
-        for (int i = 0; i < m; i++) {
-            P.entries[pos + i].row0 = rows;
-            rows += P.entries[pos + i].norb;
+    // prepass (serial, cheap): region boundaries in the entry list, rows, offsets into the shared tables
+    struct Span { size_t pos, end; };
+    std::vector<Span> spans;
+    {
+        const int task_runs = (nslice + 7) / 8;
+        size_t gm_off = 0, ri_off = 0, pr_off = 0, tk_off = 0;
+        for (size_t pos = 0; pos < tmp.size();) {
+            size_t end = pos;
+            while (end < tmp.size() && tmp[end].cell == tmp[pos].cell) end++;
+            const int64_t c = tmp[pos].cell;
+            const int m = (int)(end - pos);
+            if (m > 4095) { err = "more than 4095 atom images touch one region"; return GINT_EUNSUPPORTED; }
+            Region R;
+            std::memset(&R, 0, sizeof(R));
+            const int c3 = (int)(c % P.ncell[2]), c2 = (int)((c / P.ncell[2]) % P.ncell[1]), c1 = (int)(c / ((int64_t)P.ncell[1] * P.ncell[2]));
+            R.origin[0] = c1 * bx;
+            R.origin[1] = c2 * by;
+            R.origin[2] = c3 * bz;
+            int rows = 0;
+            for (int i = 0; i < m; i++) {
+                P.entries[pos + i].row0 = rows;
+                rows += P.entries[pos + i].norb;
+            }
+            const int nfrag = (rows + 7) / 8, ngroup = (nfrag + 3) / 4;
+            if (ngroup > kMaxGroups) { err = "too many orbitals listed for one region; use a smaller bcell"; return GINT_EUNSUPPORTED; }
+            max_rows = std::max(max_rows, (double)rows);
+            R.nrow = rows;
+            R.nentry = m;
+            R.entry0 = (int32_t)pos;
+            R.ngroup = ngroup;
+            R.gmask_off = (int32_t)gm_off;
+            R.rowinfo_off = (int32_t)ri_off;
+            R.pair_off = (int32_t)pr_off;
+            R.task_off = (int32_t)tk_off;      // room for every (entry, run); only the active ones are listed
+            gm_off += (size_t)ngroup * nks_pad;
+            ri_off += (size_t)ngroup * kGroupRows;
+            pr_off += (size_t)m * m;
+            tk_off += (size_t)m * task_runs;
+            if (gm_off > 0x7FFFFFFFu || pr_off > 0x7FFFFFFFu || tk_off > 0x7FFFFFFFu) {
+                err = "plan tables exceed 2^31 entries";
+                return GINT_EUNSUPPORTED;
+            }
+            P.regions.push_back(R);
+            spans.push_back({pos, end});
+            pos = end;
         }
-        const int nfrag = (rows + 7) / 8, ngroup = (nfrag + 3) / 4;
-        if (ngroup > kMaxGroups) { err = "too many orbitals listed for one region; use a smaller bcell"; return GINT_EUNSUPPORTED; }
-        max_rows = std::max(max_rows, (double)rows);
-        R.nrow = rows;
-        R.nentry = m;
-        R.entry0 = (int32_t)pos;
-        R.ngroup = ngroup;
-        R.gmask_off = (int32_t)P.gmask.size();
-        R.rowinfo_off = (int32_t)P.rowinfo.size();
-        R.pair_off = (int32_t)P.pair.size();
-        R.task_off = (int32_t)P.etasks.size();
-        R.psi_chunk0 = P.psi_chunks;
-        if (P.gmask.size() + (size_t)ngroup * nks_pad > 0x7FFFFFFFu || P.pair.size() + (size_t)m * m > 0x7FFFFFFFu ||
-            P.etasks.size() + (size_t)m * nslice > 0x7FFFFFFFu) {
-            err = "plan tables exceed 2^31 entries";
-            return GINT_EUNSUPPORTED;
-        }
+        P.gmask.assign(gm_off, 0);
+        P.rowinfo.assign(ri_off, kNoBlock);
+        P.pair.assign(pr_off, PairWord{kNoBlock, 0, 0});
+        P.pair_direct.assign(pr_off, kNoBlock);
+        P.etasks.assign(tk_off, 0u);
+    }
+    const size_t nreg = P.regions.size();
+    std::vector<std::vector<Proto>> region_protos(nreg);
+    std::vector<int> region_active(nreg, 0);
+    region_cost.assign(nreg, 0.0);
+    parallel_for(nreg, 8, [&](size_t rix, unsigned) {
+        Region& R = P.regions[rix];
+        const size_t pos = spans[rix].pos;
+        const int m = R.nentry, ngroup = R.ngroup;
         // evaluation tasks: (entry, run of up to 8 stages) with at least one point inside the sphere; the kernel
         // walks the run's active 32-point stages with the entry's data in registers
         int nactive = 0;
@@ -456,21 +527,18 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 int na = 0;
                 for (int s = h * 8; s < std::min(nslice, h * 8 + 8); s++)
                     if ((e.kmask[(s * kSliceKsteps) >> 5] >> ((s * kSliceKsteps) & 31)) & 0xFFu) na++;
-                if (na) P.etasks.push_back(pack_etask(i, h));
+                if (na) P.etasks[(size_t)R.task_off + (size_t)(R.ntask++)] = pack_etask(i, h);
                 nactive += na;
             }
         }
-        R.ntask = (int32_t)P.etasks.size() - R.task_off;
         // fragment activity: OR of the k-step masks of the entries that own rows of the fragment
         std::vector<std::array<uint32_t, 4>> fmask((size_t)ngroup * 4, std::array<uint32_t, 4>{0, 0, 0, 0});
-        P.rowinfo.resize(P.rowinfo.size() + (size_t)ngroup * kGroupRows, kNoBlock);
         for (int i = 0; i < m; i++) {
             const Entry& e = P.entries[pos + i];
             for (int mu = 0; mu < e.norb; mu++) P.rowinfo[(size_t)R.rowinfo_off + e.row0 + mu] = pack_rowinfo(i, mu, e.norb);
             for (int f = e.row0 / 8; f <= (e.row0 + e.norb - 1) / 8; f++)
                 for (int k = 0; k < 4; k++) fmask[(size_t)f][k] |= e.kmask[k];
         }
-        P.gmask.resize(P.gmask.size() + (size_t)ngroup * nks_pad, 0);
         uint8_t* gm = &P.gmask[(size_t)R.gmask_off];
         for (int g = 0; g < ngroup; g++)
             for (int ks = 0; ks < nks_pad; ks++) {
@@ -479,8 +547,6 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 gm[(size_t)g * nks_pad + ks] = b;
             }
         // pair table: (row entry a <= column entry b) -> canonical block offset and element strides
-        P.pair.resize(P.pair.size() + (size_t)m * m, PairWord{kNoBlock, 0, 0});
-        P.pair_direct.resize(P.pair.size(), kNoBlock);
         for (int a = 0; a < m; a++)
             for (int b = a; b < m; b++) {
                 const Entry& ea = P.entries[pos + a];
@@ -501,7 +567,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             }
         // tiles (group gi <= gj) with their cost in DMMAs: the kernel decides per k-step (4 mesh points), a fragment
         // pair is executed if the k-step holds an in-sphere point of both fragments' rows
-        const int region_index = (int)P.regions.size();
+        const int region_index = (int)rix;
         auto add_slot = [](std::vector<std::pair<int, int>>& v, std::pair<int, int> g) { if (std::find(v.begin(), v.end(), g) == v.end()) v.push_back(g); };
         std::vector<std::vector<double>> tcost((size_t)ngroup, std::vector<double>((size_t)ngroup, 0.0));
         double rcost = 0;
@@ -559,16 +625,19 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 merged = true;
             }
         }
+        if (R.ntile > 0) region_active[rix] = nactive;
+        else R.ntask = 0;
+        region_cost[rix] = rcost;
+        region_protos[rix] = std::move(protos);
+    });
+    for (size_t rix = 0; rix < nreg; rix++) {   // psi scratch chunks in region order; proto-items in region order
+        Region& R = P.regions[rix];
+        R.psi_chunk0 = P.psi_chunks;
         if (R.ntile > 0) {
-            P.psi_chunks += (int64_t)ngroup * nstage;
-            n_etask += nactive;
-        } else {
-            R.ntask = 0;
+            P.psi_chunks += (int64_t)R.ngroup * nstage;
+            n_etask += region_active[rix];
         }
-        region_cost.push_back(rcost);
-        for (Proto& p : protos) all_protos.push_back(std::move(p));
-        P.regions.push_back(R);
-        pos = end;
+        for (Proto& p : region_protos[rix]) all_protos.push_back(std::move(p));
     }
     tmp.clear();
     tmp.shrink_to_fit();
@@ -620,7 +689,13 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     double dmma_diag = 0, dmma_rect = 0, dmma_slow = 0, nruns = 0;
     double ks_full = 0, ks_part = 0, dmma_part = 0, stage_visits = 0, bal_item = 0, bal_stage = 0, bal_warp = 0;
     P.descs.resize(all_protos.size());
-    for (size_t it = 0; it < all_protos.size(); it++) {
+    struct Acc { double v[14] = {0}; };
+    std::vector<Acc> accs(kMaxThreads);
+    parallel_for(all_protos.size(), 16, [&](size_t it, unsigned tid) {
+        double* av = accs[tid].v;
+        double &exec_dmma = av[0], &flush_elems = av[1], &chunk_loads = av[2], &dmma_diag = av[3], &dmma_rect = av[4],
+               &dmma_slow = av[5], &nruns = av[6], &ks_full = av[7], &ks_part = av[8], &dmma_part = av[9],
+               &stage_visits = av[10], &bal_item = av[11], &bal_stage = av[12], &bal_warp = av[13];
         Proto& p = all_protos[it];
         ItemDesc& d = P.descs[it];
         std::memset(&d, 0, sizeof(d));
@@ -775,6 +850,11 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         stage_visits += __builtin_popcount(d.item.stage_mask);
         flush_elems += 1024.0 * (double)p.tiles.size();
         d.valid = 1;
+    });
+    for (const Acc& a : accs) {
+        exec_dmma += a.v[0]; flush_elems += a.v[1]; chunk_loads += a.v[2]; dmma_diag += a.v[3]; dmma_rect += a.v[4];
+        dmma_slow += a.v[5]; nruns += a.v[6]; ks_full += a.v[7]; ks_part += a.v[8]; dmma_part += a.v[9];
+        stage_visits += a.v[10]; bal_item += a.v[11]; bal_stage += a.v[12]; bal_warp += a.v[13];
     }
     all_protos.clear();
 

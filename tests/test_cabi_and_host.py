@@ -152,9 +152,9 @@ def test_error_codes():
     with pytest.raises(binding.GintError) as e:
         setup(species=[short])
     assert e.value.code == binding.GINT_EINVAL
-    f_shell = wl.Species("f", sp.rcut, sp.dr, np.array([3], dtype=np.int32), sp.table[:1].copy())
+    g_shell = wl.Species("g", sp.rcut, sp.dr, np.array([4], dtype=np.int32), sp.table[:1].copy())
     with pytest.raises(binding.GintError) as e:
-        setup(species=[f_shell])
+        setup(species=[g_shell])
     assert e.value.code == binding.GINT_EUNSUPPORTED
     with pytest.raises(binding.GintError) as e:
         setup(bcell=(16, 8, 8))
@@ -203,3 +203,32 @@ def test_reference_arm_runs_without_the_product_library(tmp_path):
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_update_positions_equals_fresh_setup(cfg1):
+    """gint_update_positions (moving nuclei): a host-only context moved to new
+    positions holds the same block table, cell lists and plan statistics as a context set up there, whatever the
+    number of setup threads; a bad position leaves the context unchanged."""
+    import os
+    from paper_2603_21835_b200 import gint_setup
+    rng = np.random.default_rng(61)
+    pos2 = cfg1.atom_pos + rng.uniform(-0.6, 0.6, size=cfg1.atom_pos.shape)
+    ctx = gint_setup(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cuda_device=-1)
+    nb0 = ctx.nblocks
+    ctx.gint_update_positions(pos2)
+    os.environ["GINT_SETUP_THREADS"] = "1"
+    try:
+        ref = gint_setup(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, pos2, cuda_device=-1)
+    finally:
+        del os.environ["GINT_SETUP_THREADS"]
+    assert ctx.nblocks == ref.nblocks and ctx.h_len == ref.h_len and ctx.nblocks != nb0
+    for a, b in zip(ctx.gint_get_blocks(), ref.gint_get_blocks()):
+        assert np.array_equal(a, b)
+    for a, b in zip(ctx.gint_get_cell_lists(), ref.gint_get_cell_lists()):
+        assert np.array_equal(a, b)
+    assert ctx.gint_get_stats() == ref.gint_get_stats()
+    bad = pos2.copy()
+    bad[0, 0] = np.nan
+    with pytest.raises(Exception):
+        ctx.gint_update_positions(bad)
+    assert ctx.gint_get_stats() == ref.gint_get_stats()

@@ -476,3 +476,54 @@ def test_fvl_large_full():
     assert np.array_equal(ctx.gint_get_blocks()[3], blocks[3])
     ref = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blocks)
     assert_force_parity(got, ref, "si512_dzp")
+
+
+# ---- second workloads: f shell, the paper's TZDP basis, rc = 10 ------------------------------
+@pytest.mark.parametrize("name", ["si8_dzpf", "si64_tzdp", "si64_dzp_rc10"])
+def test_second_workloads_all_three_calls(name):
+    """gint_vlocal, gint_rho and gint_fvl element by element against the oracle on: an f shell (l = 3, 20 orbitals),
+    TZDP 3s3p2d = 22 orbitals per atom (the basis of the paper's performance runs) and rc = 10 a.u.
+    (its validation cutoff)."""
+    torch = _torch()
+    import oracle
+    from paper_2603_21835_b200 import gint_setup, workloads as wl
+    w = wl.make(name)
+    Hr, blocks = oracle_H(w)
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos)
+    assert np.array_equal(ctx.gint_get_blocks()[3], blocks[3])
+    Vd = torch.from_numpy(w.V).cuda()
+    assert_parity(ctx.gint_vlocal(Vd).cpu().numpy(), Hr, name)
+    rng = np.random.default_rng(51)
+    D = rng.normal(size=Hr.shape)
+    Dd = torch.from_numpy(D).cuda()
+    ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blocks)
+    got = ctx.gint_rho(Dd).cpu().numpy()
+    assert np.abs(got - ref).max() <= TOL * np.abs(ref).max(), name + " rho"
+    Fr = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blocks)
+    assert_force_parity(ctx.gint_fvl(Vd, Dd).cpu().numpy(), Fr, name + " fvl")
+
+
+def test_update_positions_on_device(cfg1):
+    """Moving the atoms (velocity-Verlet step of Ehrenfest dynamics): after gint_update_positions all
+    three calls match the oracle at the new geometry, and moving back reproduces the first H bit for bit."""
+    torch = _torch()
+    import oracle
+    from paper_2603_21835_b200 import gint_setup
+    w = cfg1
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos)
+    Vd = torch.from_numpy(w.V).cuda()
+    H0 = ctx.gint_vlocal(Vd).cpu().numpy()
+    rng = np.random.default_rng(62)
+    pos2 = w.atom_pos + rng.uniform(-0.5, 0.5, size=w.atom_pos.shape)
+    ctx.gint_update_positions(pos2)
+    Hr, blocks = oracle.vlocal(w.lattice, w.ngrid, w.species, w.atom_species, pos2, w.V)
+    assert np.array_equal(ctx.gint_get_blocks()[3], blocks[3])
+    assert_parity(ctx.gint_vlocal(Vd).cpu().numpy(), Hr, "moved atoms")
+    D = rng.normal(size=Hr.shape)
+    Dd = torch.from_numpy(D).cuda()
+    ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, pos2, D, blocks)
+    assert np.abs(ctx.gint_rho(Dd).cpu().numpy() - ref).max() <= TOL * np.abs(ref).max()
+    Fr = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, pos2, w.V, D, blocks)
+    assert_force_parity(ctx.gint_fvl(Vd, Dd).cpu().numpy(), Fr, "moved atoms")
+    ctx.gint_update_positions(w.atom_pos)
+    assert np.array_equal(ctx.gint_vlocal(Vd).cpu().numpy(), H0)
