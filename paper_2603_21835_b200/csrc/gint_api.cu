@@ -88,7 +88,6 @@ void release(gint_ctx* ctx) {
 // caller releases the context (everything allocated so far is in ctx->allocs).
 int device_init(gint_ctx* ctx) {
     const int natom = (int)ctx->plan.atom_species.size();
-    (void)natom;
     DeviceGuard guard(ctx->device);
     cudaError_t e = guard.err;
     if (e != cudaSuccess) return fail_cuda(e, "cudaSetDevice");
@@ -130,6 +129,20 @@ int device_init(gint_ctx* ctx) {
         UP(P.blk_off, &ctx->fold.blk_off)
         UP(run_start, &ctx->fold.run_start)
         UP(first32, &ctx->fold.first)
+        std::vector<int32_t> row_run0((size_t)natom + 1, 0), col_atom;
+        for (int r = 0; r < ctx->fold.nrun; r++) row_run0[(size_t)P.blk_i[(size_t)run_start[(size_t)r]] + 1]++;
+        for (int a = 0; a < natom; a++) {
+            row_run0[(size_t)a + 1] += row_run0[(size_t)a];
+            col_atom.insert(col_atom.end(), (size_t)(first32[(size_t)a + 1] - first32[(size_t)a]), a);
+        }
+        UP(row_run0, &ctx->fold.row_run0)
+        UP(col_atom, &ctx->fold.col_atom)
+        void* ph = nullptr;
+        if ((e = cudaMalloc(&ph, (P.blk_i.size() + 1) * sizeof(double2))) != cudaSuccess) return fail_cuda(e, "cudaMalloc fold phases");
+        ctx->allocs.push_back(ph);
+        ctx->fold.phase = reinterpret_cast<double2*>(ph);
+        ctx->fold.nblk = (int32_t)P.blk_i.size();
+        ctx->fold.natom = natom;
     }
 #undef UP
     void* ctr = nullptr;   // work-queue head, shift of the potential, partial (min, max) of V

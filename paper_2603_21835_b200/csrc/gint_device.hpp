@@ -56,7 +56,10 @@ struct FoldPlan {
     const int64_t* blk_off;    // [nblk+1]
     const int32_t* run_start;  // [nrun+1]: blocks run_start[r] .. run_start[r+1]-1 share (I, J)
     const int32_t* first;      // [natom+1]: first orbital of each atom in the dense matrix
-    int32_t nrun, norb_tot;
+    const int32_t* row_run0;   // [natom+1]: first run of each row atom
+    const int32_t* col_atom;   // [norb_tot]: atom of each column of the dense matrix
+    double2* phase;            // [nblk] scratch: exp(2 pi i kfrac . R) of every block, rewritten by each call
+    int32_t nrun, norb_tot, nblk, natom;
 };
 // local Pulay force (gint_fvl.cu): what its kernels need beyond DevicePlan; built at the first gint_fvl call
 struct FvlPlan {

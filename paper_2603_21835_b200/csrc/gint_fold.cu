@@ -3,9 +3,11 @@
 //   H_mu,nu(k) = sum_R exp(i k.R) H_mu,nu(R)                      (Sec. 2.1, Eq. 5)
 //
 // with k = kfrac . (b1, b2, b3), a_i . b_j = 2 pi delta_ij, so k.R = 2 pi kfrac . (R1, R2, R3).  The block table is
-// sorted by (I, J, R), so the blocks of an atom pair are consecutive: one warp owns a pair, sums its images in
-// registers and writes each element of the dense matrix once (no atomics).  Pairs without a block stay zero from the
-// memset.  The kernel is HBM-bound: it reads H once and writes the touched part of H(k) once.
+// sorted by (I, J, R), so the blocks of an atom pair are consecutive (a "run").  Single pass, every element of the
+// dense matrix written exactly once, zeros included (no memset): one CTA per row atom I sweeps the n_I rows of the
+// dense matrix, consecutive threads on consecutive columns (coalesced 16-byte stores); a column's atom J comes from a
+// table, the run (I, J) from a binary search in the row's run list (shared memory), the phases exp(2 pi i kfrac . R)
+// of all blocks from a small kernel run first.  HBM-bound: H read once, H(k) written once.
 #include <cuda_runtime.h>
 
 #include <cstdint>
@@ -14,40 +16,73 @@
 
 namespace gint {
 
-__global__ void __launch_bounds__(256) gint_fold_kernel(const FoldPlan F, const double* __restrict__ H, double k1, double k2,
-                                                        double k3, double2* __restrict__ Hk) {
-    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (w >= F.nrun) return;
-    const int b0 = F.run_start[w], b1 = F.run_start[w + 1];
-    const int I = F.blk_i[b0], J = F.blk_j[b0];
-    const int r0 = F.first[I], c0 = F.first[J];
-    const int nI = F.first[I + 1] - r0, nJ = F.first[J + 1] - c0;
-    const int n = nI * nJ;
-    for (int idx = lane; idx < n; idx += 32) {
-        double re = 0.0, im = 0.0;
-        for (int b = b0; b < b1; b++) {
-            const double x = k1 * F.blk_R[3 * b] + k2 * F.blk_R[3 * b + 1] + k3 * F.blk_R[3 * b + 2];
-            double s, c;
-            sincospi(2.0 * x, &s, &c);
-            const double h = H[F.blk_off[b] + idx];
-            re = fma(c, h, re);
-            im = fma(s, h, im);
+__global__ void __launch_bounds__(256) gint_fold_phase_kernel(const FoldPlan F, double k1, double k2, double k3) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= F.nblk) return;
+    const double x = k1 * F.blk_R[3 * b] + k2 * F.blk_R[3 * b + 1] + k3 * F.blk_R[3 * b + 2];
+    double s, c;
+    sincospi(2.0 * x, &s, &c);
+    F.phase[b] = make_double2(c, s);
+}
+
+constexpr int kFoldRunsSmem = 4096;   // run list of a row atom kept in shared memory up to this length
+constexpr int kFoldCols = 4;          // columns per thread: a CTA covers 1024 consecutive columns of one row atom
+
+__global__ void __launch_bounds__(256) gint_fold_kernel(const FoldPlan F, const double* __restrict__ H, double2* __restrict__ Hk) {
+    __shared__ int32_t s_runJ[kFoldRunsSmem];
+    const int I = blockIdx.y;
+    const int run0 = F.row_run0[I], nrun = F.row_run0[I + 1] - run0;
+    const int r0 = F.first[I], nI = F.first[I + 1] - r0;
+    const bool in_smem = nrun <= kFoldRunsSmem;
+    if (in_smem)
+        for (int i = threadIdx.x; i < nrun; i += blockDim.x) s_runJ[i] = F.blk_j[F.run_start[run0 + i]];
+    __syncthreads();
+    // this thread's columns: the run (I, J) of each is looked up once and reused for the n_I rows
+    int b0[kFoldCols], b1[kFoldCols], e0[kFoldCols], nJ[kFoldCols];
+#pragma unroll
+    for (int q = 0; q < kFoldCols; q++) {
+        const int c = (blockIdx.x * kFoldCols + q) * 256 + threadIdx.x;
+        b0[q] = b1[q] = e0[q] = nJ[q] = 0;
+        if (c >= F.norb_tot) continue;
+        const int J = __ldg(F.col_atom + c);
+        int lo = 0, hi = nrun;   // first run of the row with atom >= J
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const int Jm = in_smem ? s_runJ[mid] : __ldg(F.blk_j + __ldg(F.run_start + run0 + mid));
+            if (Jm < J) lo = mid + 1;
+            else hi = mid;
         }
-        const int mu = idx / nJ, nu = idx - mu * nJ;
-        Hk[(size_t)(r0 + mu) * F.norb_tot + (c0 + nu)] = make_double2(re, im);
+        if (lo < nrun && (in_smem ? s_runJ[lo] : __ldg(F.blk_j + __ldg(F.run_start + run0 + lo))) == J) {
+            const int c0 = __ldg(F.first + J);
+            nJ[q] = __ldg(F.first + J + 1) - c0;
+            e0[q] = c - c0;
+            b0[q] = __ldg(F.run_start + run0 + lo);
+            b1[q] = __ldg(F.run_start + run0 + lo + 1);
+        }
+    }
+    for (int mu = 0; mu < nI; mu++) {
+#pragma unroll
+        for (int q = 0; q < kFoldCols; q++) {
+            const int c = (blockIdx.x * kFoldCols + q) * 256 + threadIdx.x;
+            if (c >= F.norb_tot) continue;
+            double re = 0.0, im = 0.0;
+            for (int b = b0[q]; b < b1[q]; b++) {
+                const double2 ph = F.phase[b];
+                const double h = __ldg(H + __ldg(F.blk_off + b) + mu * nJ[q] + e0[q]);
+                re = fma(ph.x, h, re);
+                im = fma(ph.y, h, im);
+            }
+            Hk[(size_t)(r0 + mu) * F.norb_tot + c] = make_double2(re, im);
+        }
     }
 }
 
 cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac, double* Hk, cudaStream_t stream) {
-    cudaError_t e = cudaMemsetAsync(Hk, 0, sizeof(double) * 2 * (size_t)F.norb_tot * F.norb_tot, stream);
-    if (e != cudaSuccess) return e;
-    if (F.nrun > 0) {
-        const int wpb = 256 / 32;
-        gint_fold_kernel<<<(F.nrun + wpb - 1) / wpb, 256, 0, stream>>>(F, H, kfrac[0], kfrac[1], kfrac[2],
-                                                                        reinterpret_cast<double2*>(Hk));
-        e = cudaGetLastError();
-    }
-    return e;
+    if (F.natom <= 0) return cudaSuccess;
+    if (F.nblk > 0) gint_fold_phase_kernel<<<(F.nblk + 255) / 256, 256, 0, stream>>>(F, kfrac[0], kfrac[1], kfrac[2]);
+    const dim3 grid((unsigned)((F.norb_tot + kFoldCols * 256 - 1) / (kFoldCols * 256)), (unsigned)F.natom);
+    gint_fold_kernel<<<grid, 256, 0, stream>>>(F, H, reinterpret_cast<double2*>(Hk));
+    return cudaGetLastError();
 }
 
 }  // namespace gint

@@ -231,7 +231,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     // remaining l=2 and l=3 ratios to the angular polynomials).  Four zero nodes follow the table: the stencil of a point
     // outside the sphere is redirected there, so phi == 0 exactly for r >= rcut.
     {
-        const double ylm_c[4] = {0.28209479177387814, 0.48860251190291992, 1.0925484305920792, 2.8906114210352295};
+        const double ylm_c[4] = {0.28209479177387814, 0.48860251190291992, 1.0925484305920792, 2.890611442640554};
         size_t off = 0;
         for (int s = 0; s < nspecies; s++) {
             SpeciesHost& sp = P.species[s];
@@ -732,10 +732,17 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         const size_t nt = p.tiles.size();
         std::vector<int> warp_of(nt), sched(nt);
         std::vector<std::array<int, kMaxStages>> sc(nt);
+        std::vector<std::array<uint8_t, kMaxKsteps>> kcost(nt);   // DMMAs per (tile, k-step)
         for (size_t t = 0; t < nt; t++) {
             const Tile& tl = p.tiles[t];
             const uint8_t* gm = &P.gmask[(size_t)P.regions[(size_t)tl.region].gmask_off];
-            for (int st = 0; st < kMaxStages; st++) sc[t][st] = st < nstage ? stage_cost_of(gm, tl.gi, tl.gj, st) : 0;
+            for (int ks = 0; ks < nks_pad; ks++) kcost[t][ks] = (uint8_t)kstep_cost_of(gm, tl.gi, tl.gj, ks);
+            for (int st = 0; st < kMaxStages; st++) {
+                int n = 0;
+                if (st < nstage)
+                    for (int ks = st * kStageKsteps; ks < (st + 1) * kStageKsteps; ks++) n += kcost[t][ks];
+                sc[t][st] = n;
+            }
         }
         {
             // the producer warp shares sub-partition 3, which therefore gets one tile fewer
@@ -762,7 +769,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 for (int st = 0; st < nstage; st++) { L[from][st] -= sc[t][st]; L[to][st] += sc[t][st]; }
             };
             long cur = objective();
-            for (int pass = 0, improved = 1; improved && pass < 8; pass++) {
+            for (int pass = 0, improved = 1; improved && pass < 2; pass++) {
                 improved = 0;
                 for (size_t t = 0; t < nt; t++)
                     for (int q = 0; q < 4; q++) {
@@ -797,12 +804,12 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
             exec_dmma += tl.cost;
             const uint8_t* gm = &P.gmask[(size_t)P.regions[(size_t)tl.region].gmask_off];
             for (int ks = 0; ks < nks_pad; ks++) {
-                const int nd = kstep_cost_of(gm, tl.gi, tl.gj, ks);
+                const int nd = kcost[t][ks];
                 if (tl.gi != tl.gj && nd == 16) ks_full += 1;
                 else if (nd > 0) { ks_part += 1; dmma_part += nd; }
             }
             for (int st = 0; st < nstage; st++) {
-                if (stage_cost_of(gm, tl.gi, tl.gj, st) <= 0) continue;
+                if (sc[t][st] <= 0) continue;
                 d.item.stage_mask |= 1u << st;
                 // the warp's program for the stage: runs of consecutive active k-steps with equal (ra, ca)
                 int nrun = 0;
@@ -816,7 +823,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                     d.prog[warp][st][nrun++] = pack_run(ra, ca, ks, n);
                     {   // DMMAs by code path of the contraction kernel
                         int nd = 0;
-                        for (int q = 0; q < n; q++) nd += kstep_cost_of(gm, tl.gi, tl.gj, st * kStageKsteps + ks + q);
+                        for (int q = 0; q < n; q++) nd += kcost[t][st * kStageKsteps + ks + q];
                         if (tl.gi == tl.gj) dmma_diag += nd;
                         else if (ra == 0xFu) dmma_rect += nd;
                         else dmma_slow += nd;
@@ -830,9 +837,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         for (int st = 0; st < nstage; st++) {
             double ls[4] = {0, 0, 0, 0}, lw = 0;
             for (size_t t = 0; t < p.tiles.size(); t++) {
-                const Tile& tl = p.tiles[t];
-                const uint8_t* gm = &P.gmask[(size_t)P.regions[(size_t)tl.region].gmask_off];
-                const double c = stage_cost_of(gm, tl.gi, tl.gj, st);
+                const double c = sc[t][st];
                 ls[warp_of[t] & 3] += c;
                 lw = std::max(lw, c);
             }

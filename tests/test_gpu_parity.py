@@ -66,7 +66,7 @@ def test_tiny_triclinic_ragged(seed, ngrid):
     assert_parity(Hg, Hr, "tiny seed %d" % seed)
 
 
-@pytest.mark.parametrize("bcell", [(4, 4, 4), (2, 2, 2), (1, 1, 4), (3, 2, 4), (4, 4, 2), (2, 8, 4)])
+@pytest.mark.parametrize("bcell", [(4, 4, 4), (2, 2, 2), (1, 1, 4), (3, 2, 4), (4, 4, 2), (2, 8, 4), (1, 1, 36), (1, 1, 300)])
 def test_big_cell_shapes(cfg1, cfg1_oracle, bcell):
     Hr, _ = cfg1_oracle
     Hg, _ = gpu_H(cfg1, bcell=bcell)
@@ -505,7 +505,8 @@ def test_second_workloads_all_three_calls(name):
 
 def test_update_positions_on_device(cfg1):
     """Moving the atoms (velocity-Verlet step of Ehrenfest dynamics): after gint_update_positions all
-    three calls match the oracle at the new geometry, and moving back reproduces the first H bit for bit."""
+    three calls match the oracle at the new geometry, and moving back reproduces the first H (to the rounding of the
+    atomics' order)."""
     torch = _torch()
     import oracle
     from paper_2603_21835_b200 import gint_setup
@@ -526,4 +527,4 @@ def test_update_positions_on_device(cfg1):
     Fr = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, pos2, w.V, D, blocks)
     assert_force_parity(ctx.gint_fvl(Vd, Dd).cpu().numpy(), Fr, "moved atoms")
     ctx.gint_update_positions(w.atom_pos)
-    assert np.array_equal(ctx.gint_vlocal(Vd).cpu().numpy(), H0)
+    assert np.abs(ctx.gint_vlocal(Vd).cpu().numpy() - H0).max() <= 1e-13 * np.abs(H0).max()
