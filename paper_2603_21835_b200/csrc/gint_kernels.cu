@@ -43,7 +43,6 @@ namespace {
 constexpr int kConsumerWarps = kTilesPerItem;          // 15
 constexpr int kConsumerThreads = kConsumerWarps * 32;
 constexpr int kThreads = kConsumerThreads + 32;        // + 1 producer warp
-constexpr int kStageBytes = kMaxSlots * kChunkBytes;   // 64 KB
 constexpr int kKstepDoubles = kGroupRows * kKstepPts;  // 128: one k-step of a chunk, [row 32][point 4]
 
 __device__ __forceinline__ void dmma8x8x4(double& c0, double& c1, double a, double b) {
@@ -347,7 +346,7 @@ GINT_HD inline ContractSmem contract_smem(int nring) {
     uint32_t o = 0;
     L.bar = o;   o += 256;   // mbarriers: full[8], empty[8], desc_full[4], desc_empty[4]
     L.desc = o;  o += smem_align((size_t)kDescSlots * sizeof(ItemDesc));
-    L.ring = o;  o += (uint32_t)nring * kStageBytes;
+    L.ring = o;  o += (uint32_t)nring * kChunkBytes;
     L.total = o;
     return L;
 }
@@ -378,7 +377,7 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
                                              const ItemDesc* s_desc, const unsigned char* s_ring, int nring, int never,
                                              int lane, int cidx) {
     const int frow = lane >> 2, fk = lane & 3;
-    uint32_t cs = 0, cph = 0;
+    uint32_t cseq = 0, cpos = 0;   // as in the gint_vlocal consumer
     for (int it = 0;; it++) {
         const int ds = it % kDescSlots;
         mbar_wait(smem_u32(s_dfull + ds), ((uint32_t)it / kDescSlots) & 1u);
@@ -430,11 +429,14 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
                 ma |= ma >> 4;
                 mb |= mb >> 4;
             }
-            mbar_wait(smem_u32(s_full + cs), cph);
+            const uint32_t act = cur->act[s];
+            mbar_wait(smem_u32(s_full + (cseq & 7u)), (cseq >> 3) & 1u);
             if (has_tile) {
-                const unsigned char* stage = s_ring + (size_t)cs * kStageBytes;
-                const double* chA = reinterpret_cast<const double*>(stage + sa * kChunkBytes);
-                const double* chB = reinterpret_cast<const double*>(stage + sb * kChunkBytes);
+                uint32_t ca = cpos + (uint32_t)__popc(act & ((1u << sa) - 1u)), cb = cpos + (uint32_t)__popc(act & ((1u << sb) - 1u));
+                if (ca >= (uint32_t)nring) ca -= (uint32_t)nring;
+                if (cb >= (uint32_t)nring) cb -= (uint32_t)nring;
+                const double* chA = reinterpret_cast<const double*>(s_ring + (size_t)ca * kChunkBytes);
+                const double* chB = reinterpret_cast<const double*>(s_ring + (size_t)cb * kChunkBytes);
 #pragma unroll 1
                 for (int kp = 0; kp < kStageKsteps / 2; kp++) {
                     const uint32_t ra = (ma >> (8 * kp)) & 0xFu;
@@ -489,8 +491,10 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(s_empty + cs));
-            if (++cs == (uint32_t)nring) { cs = 0; cph ^= 1u; }
+            if (lane == 0) mbar_arrive(smem_u32(s_empty + (cseq & 7u)));
+            cseq++;
+            cpos += (uint32_t)__popc(act);
+            if (cpos >= (uint32_t)nring) cpos -= (uint32_t)nring;
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(s_dempty + ds));
@@ -513,12 +517,12 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
     uint64_t* s_dfull = s_full + 16;                                          // [4] descriptor staged
     uint64_t* s_dempty = s_full + 20;                                         // [4] descriptor released
     ItemDesc* s_desc = reinterpret_cast<ItemDesc*>(smem_raw + L.desc);        // [kDescSlots]
-    unsigned char* s_ring = smem_raw + L.ring;                                // [nring][slot][8 KB]
+    unsigned char* s_ring = smem_raw + L.ring;                                // [nring] chunk buffers of 8 KB
     const int nring = P.nring;
     const int never = P.never;   // always 0; see KROW
 
     if (tid == 0) {
-        for (int i = 0; i < nring; i++) {
+        for (int i = 0; i < kRingMaxStages; i++) {
             mbar_init(smem_u32(s_full + i), 1);
             mbar_init(smem_u32(s_empty + i), kConsumerWarps);
         }
@@ -539,7 +543,10 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
         // Descriptor i+1 is fetched (one bulk copy straight into the slot, completion on its own
         // mbarrier) while the stages of item i are being streamed; the queue index is taken one more
         // item ahead so that the atomic's latency is off the critical path as well.
-        uint32_t rs = 0, rph = 0;   // ring slot and phase of the next stage to fill
+        // The ring is a circle of nring 8 KB chunk buffers; a stage takes as many consecutive buffers as it has active
+        // chunks (5.9 on average, not 8), so more stages are in flight and a warp that is ahead waits less often.
+        // Stage number seq uses the barrier pair seq % 8.  All lanes keep the same bookkeeping.
+        uint32_t seq = 0, tail = 0, head = 0, inflight = 0, cnt_word = 0;   // cnt_word: 4 bits per barrier pair = chunks held
         auto fetch_desc = [&](int i, unsigned int it) {   // lane 0: item index it -> descriptor slot i % 3
             const int ds = i % kDescSlots;
             mbar_wait(smem_u32(s_dempty + ds), (((uint32_t)i / kDescSlots) & 1u) ^ 1u);
@@ -577,17 +584,28 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
                 const int s = __ffs(todo) - 1;
                 todo &= todo - 1;
                 const uint32_t act = cur->act[s];
-                const uint32_t bar = smem_u32(s_full + rs);
+                const uint32_t c = (uint32_t)__popc(act);
+                while (inflight + c > (uint32_t)nring || seq - tail >= (uint32_t)kRingMaxStages) {   // oldest stage released?
+                    mbar_wait(smem_u32(s_empty + (tail & 7u)), (tail >> 3) & 1u);
+                    inflight -= (cnt_word >> (4u * (tail & 7u))) & 15u;
+                    tail++;
+                }
+                const uint32_t slot = seq & 7u, bar = smem_u32(s_full + slot);
                 if (lane == 0) {
-                    mbar_wait(smem_u32(s_empty + rs), rph ^ 1u);
-                    if (act) mbar_arrive_expect_tx(bar, (uint32_t)__popc(act) * kChunkBytes);
+                    if (act) mbar_arrive_expect_tx(bar, c * kChunkBytes);
                     else mbar_arrive(bar);
                 }
                 __syncwarp();
-                if ((act >> lane) & 1u)
-                    bulk_g2s(smem_u32(s_ring + (size_t)rs * kStageBytes) + lane * kChunkBytes,
-                             src_lane + (size_t)s * kChunkBytes, kChunkBytes, bar);
-                if (++rs == (uint32_t)nring) { rs = 0; rph ^= 1u; }
+                if ((act >> lane) & 1u) {
+                    uint32_t pos = head + (uint32_t)__popc(act & ((1u << lane) - 1u));
+                    if (pos >= (uint32_t)nring) pos -= (uint32_t)nring;
+                    bulk_g2s(smem_u32(s_ring) + pos * kChunkBytes, src_lane + (size_t)s * kChunkBytes, kChunkBytes, bar);
+                }
+                cnt_word = (cnt_word & ~(15u << (4u * slot))) | (c << (4u * slot));
+                head += c;
+                if (head >= (uint32_t)nring) head -= (uint32_t)nring;
+                inflight += c;
+                seq++;
             }
         }
     } else {
@@ -597,7 +615,7 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
             const int lane_off = frag_lane_offset(lane);
             const uint32_t ring_u32 = smem_u32(s_ring);
 
-            uint32_t cs = 0, cph = 0;   // ring slot and phase of the next stage to consume
+            uint32_t cseq = 0, cpos = 0;   // number of the next stage to consume and its first chunk buffer in the ring
             for (int it = 0;; it++) {
                 const int ds = it % kDescSlots;
                 mbar_wait(smem_u32(s_dfull + ds), ((uint32_t)it / kDescSlots) & 1u);
@@ -623,10 +641,14 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
                         pg = make_uint2(w4.x, w4.y);
                         pg2 = make_uint2(w4.z, w4.w);
                     }
-                    mbar_wait(smem_u32(s_full + cs), cph);
+                    const uint32_t act = cur->act[s];
+                    mbar_wait(smem_u32(s_full + (cseq & 7u)), (cseq >> 3) & 1u);
                     if (pg.x) {
-                        const uint32_t stage = ring_u32 + cs * kStageBytes + lane_off * 8;
-                        const uint32_t pa = stage + sa * kChunkBytes, pb = stage + sb * kChunkBytes;
+                        // the stage's active chunks sit in consecutive ring buffers from cpos on, in slot order
+                        uint32_t ca = cpos + (uint32_t)__popc(act & ((1u << sa) - 1u)), cb = cpos + (uint32_t)__popc(act & ((1u << sb) - 1u));
+                        if (ca >= (uint32_t)nring) ca -= (uint32_t)nring;
+                        if (cb >= (uint32_t)nring) cb -= (uint32_t)nring;
+                        const uint32_t pa = ring_u32 + ca * kChunkBytes + lane_off * 8, pb = ring_u32 + cb * kChunkBytes + lane_off * 8;
                         do {
                             const uint32_t run = pg.x;
                             const uint32_t off = (run << 2) & 0x1C00u;             // first k-step x 1 KB
@@ -636,8 +658,8 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
                             } else if ((run & 0xF0u) == 0xF0u) {
                                 run_rect(acc, pa + off, pb + off, n, run & 0xFu);
                             } else {   // rare (2.5 % of the DMMAs): k-step by k-step
-                                const double* ga = reinterpret_cast<const double*>(s_ring + (size_t)cs * kStageBytes + sa * kChunkBytes) + lane_off;
-                                const double* gb = reinterpret_cast<const double*>(s_ring + (size_t)cs * kStageBytes + sb * kChunkBytes) + lane_off;
+                                const double* ga = reinterpret_cast<const double*>(s_ring + (size_t)ca * kChunkBytes) + lane_off;
+                                const double* gb = reinterpret_cast<const double*>(s_ring + (size_t)cb * kChunkBytes) + lane_off;
 #pragma unroll 1
                                 for (uint32_t q = 0; q < n; q++) {
                                     Frag8 o;
@@ -653,8 +675,10 @@ gint_contract_kernel(const __grid_constant__ DevicePlan P, const double* __restr
                         } while (pg.x & 0xFFFFu);
                     }
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(smem_u32(s_empty + cs));
-                    if (++cs == (uint32_t)nring) { cs = 0; cph ^= 1u; }
+                    if (lane == 0) mbar_arrive(smem_u32(s_empty + (cseq & 7u)));
+                    cseq++;
+                    cpos += (uint32_t)__popc(act);
+                    if (cpos >= (uint32_t)nring) cpos -= (uint32_t)nring;
                 }
 
                 // ---------------- flush: add the tile into the canonical H blocks ---------------------------

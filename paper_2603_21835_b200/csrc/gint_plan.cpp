@@ -252,8 +252,8 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         }
     }
     P.tables_in_smem = P.tab_packed.size() * sizeof(double) <= kMaxTableSmem;
-    P.nring = kRingStages;
-    P.smem_bytes = 256 + smem_align((size_t)kDescSlots * sizeof(ItemDesc)) + (size_t)P.nring * kMaxSlots * kChunkBytes;
+    P.nring = kRingChunks;
+    P.smem_bytes = 256 + smem_align((size_t)kDescSlots * sizeof(ItemDesc)) + (size_t)P.nring * kChunkBytes;
 
     // ---- point order inside a region: k-steps of 4 points, slices of 8 k-steps -----------------
     const int bx = P.bcell[0], by = P.bcell[1], bz = P.bcell[2];

@@ -205,11 +205,12 @@ struct Plan {
     double stats[32] = {0};
     size_t smem_bytes = 0;
     bool tables_in_smem = true;
-    int nring = 0;                              // pipeline stages of the psi ring in shared memory
+    int nring = 0;                              // 8 KB chunk buffers of the psi ring in shared memory
 };
 
 GINT_HD inline uint32_t smem_align(size_t x) { return (uint32_t)((x + 127) & ~size_t(127)); }
-constexpr int kRingStages = 3;          // 3 x 64 KB of psi in flight per CTA
+constexpr int kRingChunks = 26;         // 26 x 8 KB of psi in flight per CTA: stages occupy only their active chunks
+constexpr int kRingMaxStages = 8;       // stages in flight (one full / empty mbarrier pair each)
 constexpr size_t kMaxTableSmem = 56 * 1024;   // larger radial tables stay in global memory (L1/L2-cached)
 
 inline uint64_t pack_key(int I, int J, int r1, int r2, int r3) {
