@@ -251,6 +251,7 @@ __device__ __forceinline__ void eval_task(const SpeciesDev& sp, const double* __
 // the warps walk the region's (atom image, run of stages) tasks.  Plenty of warps per SM (3 CTAs of 8
 // warps) hide the table and entry latencies; the output is 8.5 GB at si512_dzp.
 constexpr int kEvalThreads = 256;
+constexpr int kEvalCtasPerSm = 2;
 
 struct EvalSmem {
     uint32_t off, xyz, sqrtw, spec, tab, total;
@@ -260,7 +261,7 @@ GINT_HD inline EvalSmem eval_smem(size_t table_bytes, int nspecies) {
     uint32_t o = 0;
     L.off = o;   o += 3 * kMaxRegionPoints * 8;
     L.xyz = o;   o += kMaxRegionPoints * 4;
-    L.sqrtw = o; o += kMaxRegionPoints * 8;
+    L.sqrtw = o; o += 2 * kMaxRegionPoints * 8;   // two regions (double buffer)
     L.spec = o;  o += smem_align((size_t)nspecies * sizeof(SpeciesDev));
     L.tab = o;   o += smem_align(table_bytes);
     L.total = o;
@@ -268,14 +269,14 @@ GINT_HD inline EvalSmem eval_smem(size_t table_bytes, int nspecies) {
 }
 
 template <bool TAB_SMEM>
-__global__ void __launch_bounds__(kEvalThreads, 3)
+__global__ void __launch_bounds__(kEvalThreads, kEvalCtasPerSm)
 gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__ V) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const EvalSmem L = eval_smem(TAB_SMEM ? (size_t)P.tab_doubles * sizeof(double) : 0, P.nspecies);
     double* s_off = reinterpret_cast<double*>(smem_raw + L.off);
     uchar4* s_xyz = reinterpret_cast<uchar4*>(smem_raw + L.xyz);
-    double* s_sqrtw = reinterpret_cast<double*>(smem_raw + L.sqrtw);
+    double* s_sqrtw2 = reinterpret_cast<double*>(smem_raw + L.sqrtw);
     double* s_tab = reinterpret_cast<double*>(smem_raw + L.tab);
     SpeciesDev* s_spec = reinterpret_cast<SpeciesDev*>(smem_raw + L.spec);
     if (TAB_SMEM) {
@@ -298,34 +299,67 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
         s_xyz[p] = c;
     }
     const double vshift = V ? P.shift->c : 0.0;
-    for (int r = blockIdx.x; r < P.nwork_regions; r += gridDim.x) {
-        __syncthreads();   // previous region's sqrtw no longer read (first pass: tables and offsets staged)
-        const int reg_index = __ldg(P.work_regions + r);
-        const Region* reg = P.regions + reg_index;
+    // sqrt(u dV) of a region's points, two points per thread; the values of the NEXT region are fetched (work list ->
+    // region origin -> V: three dependent global loads) while the tasks of the current one run, into the other buffer
+    auto fetch_w = [&](int r, double (&w)[kMaxRegionPoints / kEvalThreads]) {
+        const Region* reg = P.regions + __ldg(P.work_regions + r);
         const int ox = __ldg(&reg->origin[0]), oy = __ldg(&reg->origin[1]), oz = __ldg(&reg->origin[2]);
-        for (int p = tid; p < npt; p += kEvalThreads) {
-            const uchar4 c = s_xyz[p];
-            const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
-            double wv = 0.0;
-            if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])   // V == nullptr: plain phi (gint_rho)
-                wv = V ? (__ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) - vshift) * P.dV : 1.0;
-            s_sqrtw[p] = sqrt(fabs(wv));
+#pragma unroll
+        for (int k = 0; k < kMaxRegionPoints / kEvalThreads; k++) {
+            const int p = tid + k * kEvalThreads;
+            w[k] = 0.0;
+            if (p < npt) {
+                const uchar4 c = s_xyz[p];
+                const int g1 = ox + c.x, g2 = oy + c.y, g3 = oz + c.z;
+                if (c.w && g1 < P.ngrid[0] && g2 < P.ngrid[1] && g3 < P.ngrid[2])   // V == nullptr: plain phi (gint_rho)
+                    w[k] = V ? (__ldg(V + ((size_t)g1 * P.ngrid[1] + g2) * P.ngrid[2] + g3) - vshift) * P.dV : 1.0;
+            }
         }
-        __syncthreads();
+    };
+    auto store_w = [&](double* dst, const double (&w)[kMaxRegionPoints / kEvalThreads]) {
+#pragma unroll
+        for (int k = 0; k < kMaxRegionPoints / kEvalThreads; k++) {
+            const int p = tid + k * kEvalThreads;
+            if (p < npt) dst[p] = sqrt(fabs(w[k]));
+        }
+    };
+    __syncthreads();   // s_xyz, tables and species staged
+    double wnext[kMaxRegionPoints / kEvalThreads];
+    int buf = 0;
+    if ((int)blockIdx.x < P.nwork_regions) {
+        fetch_w(blockIdx.x, wnext);
+        store_w(s_sqrtw2, wnext);
+    }
+    __syncthreads();
+    for (int r = blockIdx.x; r < P.nwork_regions; r += gridDim.x) {
+        const double* s_sqrtw = s_sqrtw2 + buf * kMaxRegionPoints;
+        const bool more = r + (int)gridDim.x < P.nwork_regions;
+        if (more) fetch_w(r + gridDim.x, wnext);
+        const Region* reg = P.regions + __ldg(P.work_regions + r);
         const int ntask = __ldg(&reg->ntask);
         const uint32_t* tasks = P.etasks + __ldg(&reg->task_off);
         const Entry* entries = P.entries + __ldg(&reg->entry0);
         double* psi_region = P.psi + (size_t)__ldg(&reg->psi_chunk0) * kChunkDoubles;
         const int gstride = P.nstage * kChunkDoubles;
-        for (int t = warp; t < ntask; t += kEvalThreads / 32) {
+        // the entry of a task (position, species, first row, activity of the run's 8 stages: byte s of the 64 k-step
+        // bits starting at stage s0) is fetched one task ahead: two dependent global loads hidden behind an evaluation
+        struct TaskRegs { double relx, rely, relz; int rp, row0, s0; uint2 km; };
+        auto fetch_task = [&](int t, TaskRegs& tr) {
             const uint32_t tk = __ldg(tasks + t);
             const Entry* en = entries + (tk & 0xFFFFu);
-            const int s0 = (int)(tk >> 16) * 8;
-            // the entry, once per task: position, species, first row, activity of the run's 8 stages (byte s of the
-            // 64 k-step bits starting at stage s0)
-            const double relx = __ldg(&en->rel[0]), rely = __ldg(&en->rel[1]), relz = __ldg(&en->rel[2]);
-            const int spi = (__ldg(&en->Rpack) >> 24) & 0x7F, row0 = __ldg(&en->row0);
-            const uint2 km = __ldg(reinterpret_cast<const uint2*>(&en->kmask[s0 >> 2]));
+            tr.s0 = (int)(tk >> 16) * 8;
+            tr.relx = __ldg(&en->rel[0]); tr.rely = __ldg(&en->rel[1]); tr.relz = __ldg(&en->rel[2]);
+            tr.rp = __ldg(&en->Rpack); tr.row0 = __ldg(&en->row0);
+            tr.km = __ldg(reinterpret_cast<const uint2*>(&en->kmask[tr.s0 >> 2]));
+        };
+        TaskRegs nxt;
+        if (warp < ntask) fetch_task(warp, nxt);
+        for (int t = warp; t < ntask; t += kEvalThreads / 32) {
+            const TaskRegs cur = nxt;
+            if (t + kEvalThreads / 32 < ntask) fetch_task(t + kEvalThreads / 32, nxt);
+            const double relx = cur.relx, rely = cur.rely, relz = cur.relz;
+            const int spi = (cur.rp >> 24) & 0x7F, row0 = cur.row0, s0 = cur.s0;
+            const uint2 km = cur.km;
             const SpeciesDev& sp = s_spec[spi];
             for (int q = 0; q < 8 && s0 + q < P.nstage; q++) {
                 if ((((q < 4 ? km.x : km.y) >> (8 * (q & 3))) & 0xFFu) == 0u) continue;
@@ -334,6 +368,9 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
                           psi_region + (size_t)stage * kChunkDoubles);
             }
         }
+        if (more) store_w(s_sqrtw2 + (buf ^ 1) * kMaxRegionPoints, wnext);
+        buf ^= 1;
+        __syncthreads();   // next region's weights visible; this region's no longer read
     }
 }
 
@@ -831,7 +868,7 @@ cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool 
 
 cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream) {
     if (P.nitems <= 0) return cudaSuccess;
-    const int pgrid = P.nwork_regions < 3 * nsm ? P.nwork_regions : 3 * nsm;
+    const int pgrid = P.nwork_regions < kEvalCtasPerSm * nsm ? P.nwork_regions : kEvalCtasPerSm * nsm;
     if (tab_smem)
         gint_psi_kernel<true><<<pgrid, kEvalThreads, psi_smem, stream>>>(P, V);
     else
