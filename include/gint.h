@@ -74,7 +74,8 @@ typedef struct {
 
 /* Tuning / sharding options; pass NULL for the defaults. */
 typedef struct {
-    int32_t bcell[3]; /* big-cell edge in mesh points ("BigGrid"); 0 -> 4.  Need not divide N. */
+    int32_t bcell[3]; /* big-cell edge in mesh points ("BigGrid"); 0 -> the largest of 8, 6, 4 that
+                         divides N (8 otherwise).  Need not divide N; clamped to N; product <= 512, edge <= 255. */
     int32_t rank;     /* this process' share of the big cells: cells with                                   */
     int32_t nranks;   /*   (cell index along a1) % nranks == rank are integrated; 0/1 -> all (single GPU)  */
 } gint_options;
@@ -189,8 +190,10 @@ int gint_get_kernel_ms(gint_ctx *ctx, double *ms /* [4] */);
  * stats[9] F_sym = sum_g n(g) (n(g)+1) (useful flops when H(R)=H(-R)^T is exploited)
  * stats[10] in-sphere (atom image, point) pairs   stats[11] (atom image, point) pairs evaluated per call
  * stats[12] psi scratch buffer (bytes, device)    stats[13] psi bytes streamed back from L2 per call
- * stats[14] shared-memory ring stages             stats[15] non-empty regions
- * Returns the number of entries written (<= n, at most 16). */
+ * stats[14] 8 KB chunk buffers of the shared-memory ring    stats[15] non-empty regions
+ * stats[16..22] k-step / balance statistics of the plan, stats[23..25] big-cell edge actually used,
+ * stats[26..29] DMMAs by code path of the contraction kernel (diagonal runs, all-row runs, other) and number of runs
+ * Returns the number of entries written (<= n, at most 32). */
 int gint_get_stats(const gint_ctx *ctx, double *stats, int32_t n);
 
 /* Copy out the per-cell lists (host logic tests).  cell_start[ncell+1] indexes

@@ -540,7 +540,7 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
 #undef RHO_ROW
 #undef RHO_GUARD
 
-// MODE 0: gint_vlocal (H += psi diag(sign V) psi^T, Eq. 45).  MODE 1: gint_rho (Eq. 44): the same items, stages and
+// MODE 0: gint_vlocal (H -/+= psi psi^T, Eq. 45 with the one-signed potential).  MODE 1: gint_rho (Eq. 44): the same items, stages and
 // producer; a consumer warp keeps its 32x32 tile of the region's density matrix in registers as the A operand,
 // forms T = E Phi_b on the tensor pipe per 8 points and dots it with Phi_a (rho_consumer above).
 template <int MODE>

@@ -10,15 +10,15 @@
 // are ordered into k-steps of 4 points (2x2x1, the K of one DMMA.8x8x4) and stages
 // of 8 k-steps (32 points: one shared-memory pipeline stage of the contraction and
 // one evaluation slice of the psi kernel, one lane per point).  Every (atom image,
-// region) pair whose sphere holds a point of the region is an *entry*; entries are
-// sorted densest first and their orbitals are packed into consecutive *rows* of the
-// region's psi matrix, psi = phi sqrt(|V dV|).  Rows are cut into fragments of 8
+// region) pair whose sphere holds a point of the region is an *entry*; entries that
+// cover the whole region come first, the others in a chain of similar coverage, and
+// their orbitals are packed into consecutive *rows* of the region's psi matrix.  Rows are cut into fragments of 8
 // (one DMMA operand) and groups of 32 (one warp-tile edge).  The upper triangle of
-// the region's  C = psi diag(sign V) psi^T  is cut into 32x32 tiles; tiles are
+// the region's  C = psi psi^T  (psi = phi sqrt(|V - c| dV), see gint_kernels.cu)  is cut into 32x32 tiles; tiles are
 // packed kTilesPerItem at a time (one per consumer warp) into *work items* that
 // touch at most kMaxSlots row groups.  gint_psi_kernel writes psi of every region
-// once into the scratch buffer (chunks of one (group, stage): [k-step 8][row 32]
-// [point 4] doubles = 8 KB); gint_contract_kernel streams the chunks an item needs
+// once into the scratch buffer (chunks of one (group, stage): [k-step 8][row pair 16]
+// [point 4][row parity 2] doubles = 8 KB); gint_contract_kernel streams the chunks an item needs
 // through a shared-memory ring with bulk copies.
 //
 // Output of the plan (plain arrays, uploaded verbatim by gint_api.cu):
