@@ -638,9 +638,24 @@ int orc_fvl(const double *lattice, const int *ngrid, int nspecies, const double 
 #pragma omp single
         used = omp_get_num_threads();
     }
+#endif
+    /* one private accumulator array per thread, summed at the end: the terms and their long double accumulation are
+     * unchanged; only the contended atomic updates of long doubles (lock-based, 6 per (point, block)) are gone */
+    long double *Fthr = (long double *)calloc((size_t)used * (size_t)natom * 3, sizeof(long double));
+    if (!Fthr) {
+        free(Facc);
+        free(gstart);
+        return -4;
+    }
+#ifdef _OPENMP
 #pragma omp parallel for schedule(dynamic, 1)
 #endif
     for (int64_t g = 0; g < ngroup; g++) {
+        int me = 0;
+#ifdef _OPENMP
+        me = omp_get_thread_num();
+#endif
+        long double *Fme = Fthr + (size_t)me * (size_t)natom * 3;
         const int I = bi[gstart[g]];
         const orc_species *sI = &sp[atom_species[I]];
         const double *tI = pos + 3 * (size_t)I;
@@ -680,20 +695,16 @@ int orc_fvl(const double *lattice, const int *ngrid, int nspecies, const double 
                                 }
                             }
                         for (int c = 0; c < 3; c++) {
-                            long double aI = (long double)(v * fI[c]), aJ = (long double)(v * fJ[c]);
-#ifdef _OPENMP
-#pragma omp atomic
-#endif
-                            Facc[3 * (size_t)I + c] += aI;
-#ifdef _OPENMP
-#pragma omp atomic
-#endif
-                            Facc[3 * (size_t)J + c] += aJ;
+                            Fme[3 * (size_t)I + c] += (long double)(v * fI[c]);
+                            Fme[3 * (size_t)J + c] += (long double)(v * fJ[c]);
                         }
                     }
                 }
     }
+    for (int t = 0; t < used; t++)
+        for (int i = 0; i < 3 * natom; i++) Facc[i] += Fthr[(size_t)t * (size_t)natom * 3 + i];
     for (int i = 0; i < 3 * natom; i++) F[i] = (double)(Facc[i] * (long double)dV);
+    free(Fthr);
     free(Facc);
     free(gstart);
     return used;
