@@ -68,6 +68,14 @@ __device__ __forceinline__ bool group_stage_active(const FvlPlan& F, const Regio
     return *reinterpret_cast<const unsigned long long*>(gm) != 0ull;
 }
 
+// 16 bits: nibble j = fragments of row group g with an in-sphere point in k-pair j (8 points) of the stage
+__device__ __forceinline__ uint32_t kpair_masks(const FvlPlan& F, const Region* reg, int g, int stage) {
+    const uint8_t* gm = F.gmask + __ldg(&reg->gmask_off) + (size_t)g * F.nks_pad + (size_t)stage * kStageKsteps;
+    const uint2 w = __ldg(reinterpret_cast<const uint2*>(gm));   // 8 k-steps, one byte each (low nibble)
+    const uint32_t a = (w.x | (w.x >> 8)) & 0x000F000Fu, b = (w.y | (w.y >> 8)) & 0x000F000Fu;
+    return (a & 0xFu) | ((a >> 12) & 0xF0u) | ((b & 0xFu) << 8) | ((b >> 4) & 0xF000u);
+}
+
 }  // namespace
 
 // ---- E = D + D^T of every region, A-fragment order -------------------------------------------------------
@@ -152,23 +160,57 @@ gint_tgemm_kernel(const __grid_constant__ DevicePlan P, const __grid_constant__ 
     const int q = lane >> 2, r = lane & 3;
     // B operand of (kc, j): Phi[row 4 kc + r of gb][point 8 j + q]; point 8 j + q is point q % 4 of k-step 2 j + q / 4
     const int boff = (q >> 2) * 128 + (r >> 1) * 8 + (q & 3) * 2 + (r & 1);
+    const uint32_t rp = mine ? kpair_masks(F, reg, ga, stage) : 0u;   // row fragments of ga active per k-pair
+    // bit j: some row fragment of ga is active in k-pair j
+    const uint32_t rj_any = ((rp & 0xFu) ? 1u : 0u) | ((rp & 0xF0u) ? 2u : 0u) | ((rp & 0xF00u) ? 4u : 0u) | ((rp & 0xF000u) ? 8u : 0u);
     for (int gb = 0; gb < ngroup; gb++) {
         if (tid == 0 && gb + 1 < ngroup) issue(gb + 1);   // the other buffer was released by the barrier below
         bar_wait(smem_addr(bars + (gb & 1)), (uint32_t)(gb >> 1) & 1u);
-        if (mine && group_stage_active(F, reg, gb, stage)) {
+        const uint32_t cp = mine ? kpair_masks(F, reg, gb, stage) : 0u;   // column fragments of gb active per k-pair
+        if (cp) {
             const double* bufE = reinterpret_cast<const double*>(smem + (gb & 1) * kTgBufBytes + (warp >> 2) * kChunkBytes) + lane;
             const double* bufP = reinterpret_cast<const double*>(smem + (gb & 1) * kTgBufBytes + (4 + (warp & 3)) * kChunkBytes) + boff;
+            if ((rp & cp) == 0xFFFFu) {   // every fragment active in every k-pair: dense
 #pragma unroll 2
-            for (int kc = 0; kc < 8; kc++) {
-                double a[4], b[4];
+                for (int kc = 0; kc < 8; kc++) {
+                    double a[4], b[4];
 #pragma unroll
-                for (int i = 0; i < 4; i++) a[i] = bufE[(kc * 4 + i) * 32];
+                    for (int i = 0; i < 4; i++) a[i] = bufE[(kc * 4 + i) * 32];
 #pragma unroll
-                for (int j = 0; j < 4; j++) b[j] = bufP[j * 256 + kc * 16];
+                    for (int j = 0; j < 4; j++) b[j] = bufP[j * 256 + kc * 16];
 #pragma unroll
-                for (int i = 0; i < 4; i++)
+                    for (int i = 0; i < 4; i++)
 #pragma unroll
-                    for (int j = 0; j < 4; j++) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                        for (int j = 0; j < 4; j++) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                }
+            } else {
+                // blocks of 8 DMMAs (column fragment f = columns 8 f .. 8 f + 7, k-pair j = 8 points, all four row
+                // fragments) only where the column fragment holds an in-sphere point in the k-pair and some row of the
+                // group does too.  Real, warp-uniform branches (a predicated-off DMMA still costs its pipe cycles, hence
+                // the never-taken back edges); 8 DMMAs on 4 accumulators keep the pipe busy by themselves.
+#pragma unroll
+                for (int f = 0; f < 4; f++) {
+                    const uint32_t jm = ((cp >> f) & 1u) | (((cp >> (4 + f)) & 1u) << 1) | (((cp >> (8 + f)) & 1u) << 2) | (((cp >> (12 + f)) & 1u) << 3);
+                    if ((jm & rj_any) == 0u) continue;
+                    double a0[4], a1[4];
+#pragma unroll
+                    for (int i = 0; i < 4; i++) {
+                        a0[i] = bufE[(8 * f + i) * 32];
+                        a1[i] = bufE[(8 * f + 4 + i) * 32];
+                    }
+#pragma unroll
+                    for (int j = 0; j < 4; j++) {
+                        if ((jm & rj_any) & (1u << j)) {
+                            do {
+                                const double b0 = bufP[j * 256 + (2 * f) * 16], b1 = bufP[j * 256 + (2 * f + 1) * 16];
+#pragma unroll
+                                for (int i = 0; i < 4; i++) dmma(acc[i][j][0], acc[i][j][1], a0[i], b0);
+#pragma unroll
+                                for (int i = 0; i < 4; i++) dmma(acc[i][j][0], acc[i][j][1], a1[i], b1);
+                            } while (P.never);
+                        }
+                    }
+                }
             }
         }
         __syncthreads();
