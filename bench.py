@@ -307,7 +307,7 @@ def main():
         fold_ms = f0.elapsed_time(f1) / 10
         fold_bytes = 8.0 * ctx.h_len + 16.0 * ntot * ntot
         fold = {"ms_per_call": fold_ms, "algorithmic_bytes": fold_bytes, "achieved_gbs": fold_bytes / (fold_ms * 1e-3) * 1e-9,
-                "norb_tot": ntot, "note": "gint_fold_k: H blocks read once, dense complex H(k) written once (memset + kernel)"}
+                "norb_tot": ntot, "note": "gint_fold_k: H blocks read once, dense complex H(k) written once (single pass, zeros included)"}
         del Hk
         # charge density (Eq. 44), first cut
         Dm = torch.randn(ctx.h_len, dtype=torch.float64, device=dev)
@@ -332,8 +332,8 @@ def main():
         torch.cuda.synchronize()
         fvl_ms = f0.elapsed_time(f1) / 2
         fvl_info = {"ms_per_call": fvl_ms, "useful_flops": F_pt, "achieved_tflops": F_pt / (fvl_ms * 1e-3) * 1e-12,
-                    "note": "gint_fvl (Eq. 46): psi kernel + E = D + D^T gather + T = E Phi (DMMA, dense inside active "
-                            "(row group, stage) pairs) + force kernel; T needs every (row, column) pair, so F_pt accounting"}
+                    "note": "gint_fvl (Eq. 46): psi kernel + E = D + D^T gather + T = E Phi (DMMA) + force kernel; T needs every "
+                            "(row, column) pair, so F_pt accounting"}
         del Dm, rho, Fv
 
     if rank != 0:

@@ -88,6 +88,8 @@ typedef struct {
  *   cuda_device       >= 0: device ordinal; < 0: host-only context (no CUDA call is
  *                     made; block table and statistics can be queried, gint_vlocal
  *                     returns GINT_ENODEVICE)
+ * The host plan is built with std::thread workers (hardware_concurrency, at most 32; the environment variable
+ * GINT_SETUP_THREADS overrides the count; the result does not depend on it).
  * On failure *out is NULL. */
 int gint_setup(gint_ctx **out, const double *lattice, const int32_t *ngrid, int32_t nspecies,
                const gint_species *species, int32_t natom, const int32_t *atom_species, const double *atom_pos,

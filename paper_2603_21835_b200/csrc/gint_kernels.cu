@@ -404,11 +404,6 @@ __device__ __forceinline__ uint32_t nonzero_nibbles(uint32_t m) { return (m | (m
     if (cond) {                        \
         do { body } while (never);     \
     }
-#define RHO_ROW(i)                                                           \
-    RHO_GUARD(ra & (1u << i), {                                              \
-        dmma8x8x4(C[i][0], C[i][1], A[i][2 * j], b0);                        \
-        dmma8x8x4(C[i][0], C[i][1], A[i][2 * j + 1], b1);                    \
-    })
 __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* __restrict__ D, double* __restrict__ rho,
                                              uint64_t* s_full, uint64_t* s_empty, uint64_t* s_dfull, uint64_t* s_dempty,
                                              const ItemDesc* s_desc, const unsigned char* s_ring, int nring, int never,
@@ -495,10 +490,15 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
                     } else {
 #pragma unroll
                         for (int j = 0; j < 4; j++) {
+                            // blocks of 8 DMMAs on 4 accumulators (all four row fragments: guarding single row
+                            // fragments costs more in lost instruction-level parallelism than the skipped DMMAs save)
                             RHO_GUARD(ca & (1u << j), {
                                 const double b0 = bsrc[j * 32];
                                 const double b1 = bsrc[j * 32 + 16];
-                                RHO_ROW(0) RHO_ROW(1) RHO_ROW(2) RHO_ROW(3)
+#pragma unroll
+                                for (int i = 0; i < 4; i++) dmma8x8x4(C[i][0], C[i][1], A[i][2 * j], b0);
+#pragma unroll
+                                for (int i = 0; i < 4; i++) dmma8x8x4(C[i][0], C[i][1], A[i][2 * j + 1], b1);
                             })
                         }
                     }
@@ -537,7 +537,6 @@ __device__ __forceinline__ void rho_consumer(const DevicePlan& P, const double* 
         if (lane == 0) mbar_arrive(smem_u32(s_dempty + ds));
     }
 }
-#undef RHO_ROW
 #undef RHO_GUARD
 
 // MODE 0: gint_vlocal (H -/+= psi psi^T, Eq. 45 with the one-signed potential).  MODE 1: gint_rho (Eq. 44): the same items, stages and

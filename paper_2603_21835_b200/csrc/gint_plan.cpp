@@ -875,7 +875,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[4] = 512.0 * exec_dmma;
     P.stats[5] = flush_elems;
     P.stats[6] = (double)P.smem_bytes;
-    P.stats[7] = 3;
+    P.stats[7] = 5;   // gint_vrange_kernel, gint_hinit_kernel, gint_psi_kernel, gint_contract_kernel<0>, gint_mirror_kernel
     P.stats[8] = fpt;
     P.stats[9] = fsym;
     P.stats[10] = n_insphere;
