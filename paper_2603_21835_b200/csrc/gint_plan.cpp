@@ -379,59 +379,57 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         std::vector<Tmp>().swap(tmp_thread[t]);
     }
     auto rkey = [](const Entry& e) { return (uint32_t)(e.Rpack & 0xFFFFFF); };
-    // query lists: per region sorted by (atom, R)
+    // bucket the entries by region (counting sort), then per region, in parallel: the query list sorted by (atom, R),
+    // and the kernel order -- entries that cover the whole region first (most active k-steps first, then (atom, R)),
+    // and among the partially covering entries a greedy chain of similar coverage (Jaccard index of the k-step masks):
+    // rows of consecutive entries share 8-row fragments and 32-row groups, whose activity is the OR of their entries'
+    // masks, so neighbours that cover the same part of the region execute fewer wasted DMMAs (executed / useful
+    // 1.32 -> 1.28 at si512_dzp)
     {
-        std::vector<size_t> idx(tmp.size());
-        std::iota(idx.begin(), idx.end(), size_t(0));
-        std::sort(idx.begin(), idx.end(), [&](size_t a, size_t b) {
-            if (tmp[a].cell != tmp[b].cell) return tmp[a].cell < tmp[b].cell;
-            if (tmp[a].e.atom != tmp[b].e.atom) return tmp[a].e.atom < tmp[b].e.atom;
-            return rkey(tmp[a].e) < rkey(tmp[b].e);
-        });
         P.cell_start.assign((size_t)ncells + 1, 0);
         for (auto& t : tmp) P.cell_start[(size_t)t.cell + 1]++;
         for (int64_t c = 0; c < ncells; c++) P.cell_start[(size_t)c + 1] += P.cell_start[(size_t)c];
+        std::vector<Tmp> byc(tmp.size());
+        {
+            std::vector<int64_t> fill(P.cell_start.begin(), P.cell_start.end() - 1);
+            for (auto& t : tmp) byc[(size_t)fill[(size_t)t.cell]++] = t;
+        }
+        tmp.swap(byc);
+        std::vector<Tmp>().swap(byc);
         P.cell_atom.resize(tmp.size());
         P.cell_R.resize(3 * tmp.size());
-        for (size_t i = 0; i < idx.size(); i++) {
-            const Entry& e = tmp[idx[i]].e;
-            P.cell_atom[i] = e.atom;
-            P.cell_R[3 * i] = ((e.Rpack >> 16) & 0xFF) - 128;
-            P.cell_R[3 * i + 1] = ((e.Rpack >> 8) & 0xFF) - 128;
-            P.cell_R[3 * i + 2] = (e.Rpack & 0xFF) - 128;
-        }
-    }
-    // kernel order: per region densest entries first (most active k-steps), then (atom, R)
-    std::sort(tmp.begin(), tmp.end(), [&](const Tmp& a, const Tmp& b) {
-        if (a.cell != b.cell) return a.cell < b.cell;
-        if (a.npop != b.npop) return a.npop > b.npop;
-        if (a.e.atom != b.e.atom) return a.e.atom < b.e.atom;
-        return rkey(a.e) < rkey(b.e);
-    });
-    // ... and among the partially covering entries a greedy chain of similar coverage (Jaccard index of the k-step
-    // masks): rows of consecutive entries share 8-row fragments and 32-row groups, whose activity is the OR of
-    // their entries' masks, so neighbours that cover the same part of the region execute fewer wasted DMMAs
-    // (executed / useful 1.32 -> 1.28 at si512_dzp)
-    for (size_t a = 0; a < tmp.size();) {
-        size_t b = a;
-        while (b < tmp.size() && tmp[b].cell == tmp[a].cell) b++;
-        size_t f = a;
-        while (f < b && tmp[f].npop >= P.nks) f++;   // fully covering entries stay first
-        for (size_t i = (f > a ? f - 1 : a); i + 1 < b; i++) {
-            size_t best = i + 1;
-            double best_score = -1;
-            for (size_t j = i + 1; j < b; j++) {
-                int in = 0, un = 0;
-                for (int k = 0; k < 4; k++) {
-                    in += __builtin_popcount(tmp[i].e.kmask[k] & tmp[j].e.kmask[k]);
-                    un += __builtin_popcount(tmp[i].e.kmask[k] | tmp[j].e.kmask[k]);
-                }
-                const double score = (double)in / (double)un;
-                if (score > best_score) { best_score = score; best = j; }
+        parallel_for((size_t)ncells, 16, [&](size_t c, unsigned) {
+            const size_t a = (size_t)P.cell_start[c], b = (size_t)P.cell_start[c + 1];
+            if (a == b) return;
+            std::sort(tmp.begin() + (ptrdiff_t)a, tmp.begin() + (ptrdiff_t)b, [&](const Tmp& x, const Tmp& y) {
+                if (x.e.atom != y.e.atom) return x.e.atom < y.e.atom;
+                return rkey(x.e) < rkey(y.e);
+            });
+            for (size_t i = a; i < b; i++) {
+                const Entry& e = tmp[i].e;
+                P.cell_atom[i] = e.atom;
+                P.cell_R[3 * i] = ((e.Rpack >> 16) & 0xFF) - 128;
+                P.cell_R[3 * i + 1] = ((e.Rpack >> 8) & 0xFF) - 128;
+                P.cell_R[3 * i + 2] = (e.Rpack & 0xFF) - 128;
             }
-            std::swap(tmp[i + 1], tmp[best]);
-        }
-        a = b;
+            std::stable_sort(tmp.begin() + (ptrdiff_t)a, tmp.begin() + (ptrdiff_t)b, [](const Tmp& x, const Tmp& y) { return x.npop > y.npop; });
+            size_t f = a;
+            while (f < b && tmp[f].npop >= P.nks) f++;   // fully covering entries stay first
+            for (size_t i = (f > a ? f - 1 : a); i + 1 < b; i++) {
+                size_t best = i + 1;
+                double best_score = -1;
+                for (size_t j = i + 1; j < b; j++) {
+                    int in = 0, un = 0;
+                    for (int k = 0; k < 4; k++) {
+                        in += __builtin_popcount(tmp[i].e.kmask[k] & tmp[j].e.kmask[k]);
+                        un += __builtin_popcount(tmp[i].e.kmask[k] | tmp[j].e.kmask[k]);
+                    }
+                    const double score = (double)in / (double)un;
+                    if (score > best_score) { best_score = score; best = j; }
+                }
+                std::swap(tmp[i + 1], tmp[best]);
+            }
+        });
     }
     P.entries.resize(tmp.size());
     for (size_t i = 0; i < tmp.size(); i++) P.entries[i] = tmp[i].e;
