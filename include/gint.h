@@ -78,6 +78,9 @@ typedef struct {
                          divides N (8 otherwise).  Need not divide N; clamped to N; product <= 512, edge <= 255. */
     int32_t rank;     /* this process' share of the big cells: cells with                                   */
     int32_t nranks;   /*   (cell index along a1) % nranks == rank are integrated; 0/1 -> all (single GPU)  */
+    int64_t scratch_max_bytes; /* upper bound for the psi scratch buffer (0 -> 16 GiB).  When all regions do not fit,
+                         consecutive batches of regions reuse the buffer (each call then runs its psi and contraction
+                         kernels once per batch; results are the same); never smaller than one region needs.      */
 } gint_options;
 
 /* Build the context: validate, enumerate (I,J,R) blocks, partition the mesh into

@@ -24,7 +24,7 @@ EXPORTED = ("gint_setup", "gint_update_positions", "gint_num_blocks", "gint_get_
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
               "regions", "ksteps_full", "ksteps_partial", "dmma_in_partial_ksteps", "stage_visits", "dmma_max_sched_item", "dmma_max_sched_stage", "dmma_max_warp_stage", "bcell1", "bcell2", "bcell3",
-              "dmma_diag_runs", "dmma_rect_runs", "dmma_other_runs", "runs", "s30", "s31")
+              "dmma_diag_runs", "dmma_rect_runs", "dmma_other_runs", "runs", "batches", "s31")
 
 
 class GintError(RuntimeError):
@@ -39,7 +39,8 @@ class _Species(ctypes.Structure):
 
 
 class _Options(ctypes.Structure):
-    _fields_ = [("bcell", ctypes.c_int32 * 3), ("rank", ctypes.c_int32), ("nranks", ctypes.c_int32)]
+    _fields_ = [("bcell", ctypes.c_int32 * 3), ("rank", ctypes.c_int32), ("nranks", ctypes.c_int32),
+                ("pad", ctypes.c_int32), ("scratch_max_bytes", ctypes.c_int64)]
 
 
 def _load() -> ctypes.CDLL:
@@ -257,7 +258,7 @@ class GintContext:
 
 
 def gint_setup(lattice, ngrid, species: Sequence, atom_species, atom_pos, cuda_device: int = 0,
-               bcell=(0, 0, 0), rank: int = 0, nranks: int = 1) -> GintContext:
+               bcell=(0, 0, 0), rank: int = 0, nranks: int = 1, scratch_max_bytes: int = 0) -> GintContext:
     """species: objects with .rcut .dr .l[nrad] .table[nrad][ntab].  cuda_device < 0: host-only context."""
     lattice = np.ascontiguousarray(lattice, dtype=np.float64).reshape(9)
     ng = np.ascontiguousarray(ngrid, dtype=np.int32).reshape(3)
@@ -280,6 +281,7 @@ def gint_setup(lattice, ngrid, species: Sequence, atom_species, atom_pos, cuda_d
     for d in range(3):
         opt.bcell[d] = int(bcell[d])
     opt.rank, opt.nranks = int(rank), int(nranks)
+    opt.scratch_max_bytes = int(scratch_max_bytes)
     h = ctypes.c_void_p()
     _check(_lib.gint_setup(ctypes.byref(h), _ptr(lattice, ctypes.c_double), _ptr(ng, ctypes.c_int32), len(species),
                            arr, int(pos.shape[0]), _ptr(asp, ctypes.c_int32), _ptr(pos, ctypes.c_double),

@@ -25,6 +25,8 @@ struct gint_ctx {
     bool profiling = false;
     bool have_events = false;
     cudaEvent_t ev[5];
+    std::vector<gint::BatchRange> batches;   // regions that share the psi scratch, one after the other
+    std::vector<int32_t> tg0;                // gint_fvl: first T-kernel task of each batch (+ end)
     gint::FvlPlan fvl{};           // built at the first gint_fvl call
     bool have_fvl = false;
     size_t force_smem = 0;
@@ -111,6 +113,7 @@ int device_init(gint_ctx* ctx) {
     UP(P.etasks, &D.etasks)
     UP(P.pair, &D.pair)
     UP(P.pair_direct, &D.pair_direct)
+    UP(P.gmask, &D.gmask)
     UP(P.slot_xyz, &D.slot_xyz)
     UP(P.mirror, &D.mirror)
     UP(P.tab_packed, &D.tab)
@@ -173,6 +176,9 @@ int device_init(gint_ctx* ctx) {
     D.nstage = P.nstage;
     D.nregions = (int32_t)P.regions.size();
     D.nring = P.nring;
+    D.multibatch = P.batches.size() > 1 ? 1 : 0;
+    ctx->batches.clear();
+    for (const gint::Plan::Batch& B : P.batches) ctx->batches.push_back(gint::BatchRange{B.item0, B.nitems, B.wr0, B.nwr});
     D.never = 0;
     D.nitems = (int32_t)P.descs.size();
     D.nmirror = (int32_t)P.mirror.size();
@@ -193,8 +199,9 @@ int device_init(gint_ctx* ctx) {
         std::vector<double> one(nV, 1.0);
         e = cudaMemcpy(ones, one.data(), nV * sizeof(double), cudaMemcpyHostToDevice);
         if (e == cudaSuccess)
-            e = gint::launch_vlocal(D, ctx->psi_smem, ctx->contract_smem, P.tables_in_smem, ctx->nsm, nH,
-                                    reinterpret_cast<const double*>(ones), reinterpret_cast<double*>(Sd), true, nullptr, nullptr);
+            e = gint::launch_vlocal(D, ctx->psi_smem, ctx->contract_smem, P.tables_in_smem, ctx->nsm, ctx->batches.data(),
+                                    (int)ctx->batches.size(), nH, reinterpret_cast<const double*>(ones),
+                                    reinterpret_cast<double*>(Sd), true, nullptr, nullptr);
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
         cudaFree(ones);
         if (e != cudaSuccess) { return fail_cuda(e, "grid overlap S"); }
@@ -244,7 +251,7 @@ int gint_setup(gint_ctx** out, const double* lattice, const int32_t* ngrid, int3
         std::string err;
         const int32_t* bc = opt ? opt->bcell : nullptr;
         const int rc = gint::build_plan(ctx->plan, lattice, ngrid, nspecies, sp.data(), natom, atom_species, atom_pos,
-                                        bc, opt ? opt->rank : 0, opt ? opt->nranks : 1, err);
+                                        bc, opt ? opt->rank : 0, opt ? opt->nranks : 1, opt ? opt->scratch_max_bytes : 0, err);
         if (rc != GINT_OK) {
             delete ctx;
             return fail(rc, err);
@@ -284,7 +291,7 @@ int gint_update_positions(gint_ctx* ctx, const double* atom_pos) {
         const int32_t ng[3] = {old.ngrid[0], old.ngrid[1], old.ngrid[2]};
         const int32_t bc[3] = {old.bcell[0], old.bcell[1], old.bcell[2]};
         const int rc = gint::build_plan(fresh->plan, old.lattice, ng, (int)old.species.size(), old.species.data(), natom,
-                                        asp.data(), atom_pos, bc, old.rank, old.nranks, err);
+                                        asp.data(), atom_pos, bc, old.rank, old.nranks, old.scratch_max_bytes, err);
         if (rc != GINT_OK) {
             delete fresh;
             return fail(rc, err);   // the context is unchanged
@@ -329,7 +336,8 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* stream)
     DeviceGuard guard(ctx->device);
     if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaError_t e = gint::launch_vlocal(ctx->dev, ctx->psi_smem, ctx->contract_smem, ctx->plan.tables_in_smem, ctx->nsm,
-                                        (size_t)ctx->plan.blk_off.back(), V_dev, H_dev, false,
+                                        ctx->batches.data(), (int)ctx->batches.size(), (size_t)ctx->plan.blk_off.back(),
+                                        V_dev, H_dev, false,
                                         reinterpret_cast<cudaStream_t>(stream), ctx->profiling ? ctx->ev : nullptr);
     if (e != cudaSuccess) return fail_cuda(e, "gint_vlocal launch");
     return GINT_OK;
@@ -341,9 +349,8 @@ int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* stream) 
     DeviceGuard guard(ctx->device);
     if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    cudaError_t e = gint::launch_psi(ctx->dev, ctx->psi_smem, ctx->plan.tables_in_smem, ctx->nsm, nullptr, st);
-    if (e != cudaSuccess) return fail_cuda(e, "gint_rho psi launch");
-    e = gint::launch_rho_dmma(ctx->dev, ctx->contract_smem, ctx->nsm, D_dev, rho_dev, st);
+    cudaError_t e = gint::launch_rho(ctx->dev, ctx->psi_smem, ctx->contract_smem, ctx->plan.tables_in_smem, ctx->nsm,
+                                     ctx->batches.data(), (int)ctx->batches.size(), D_dev, rho_dev, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_rho launch");
     return GINT_OK;
 }
@@ -355,17 +362,24 @@ static int fvl_init(gint_ctx* ctx) {
     gint::FvlPlan& F = ctx->fvl;
     std::vector<int64_t> e0(P.regions.size(), 0);
     std::vector<int4> tasks;
-    int64_t echunks = 0;
+    int64_t echunks = 0, ecur = 0;   // E scratch: as large as its largest batch needs
+    ctx->tg0.assign(1, 0);
     for (size_t r = 0; r < P.regions.size(); r++) {
         const gint::Region& R = P.regions[r];
+        if (r > 0 && P.region_batch[r] != P.region_batch[r - 1]) {
+            ecur = 0;
+            ctx->tg0.push_back((int32_t)tasks.size());
+        }
         if (R.ntile <= 0) continue;
-        e0[r] = echunks;
-        echunks += (int64_t)R.ngroup * R.ngroup;
+        e0[r] = ecur;
+        ecur += (int64_t)R.ngroup * R.ngroup;
+        echunks = std::max(echunks, ecur);
         for (int rq = 0; rq * 4 < R.ngroup; rq++)
             for (int sq = 0; sq * 4 < P.nstage; sq++) tasks.push_back(make_int4((int)r, rq, sq, 0));
     }
+    while (ctx->tg0.size() < P.batches.size() + 1) ctx->tg0.push_back((int32_t)tasks.size());
     cudaError_t e;
-    if ((e = upload(ctx, P.gmask, &F.gmask)) != cudaSuccess) return fail_cuda(e, "upload gmask");
+    F.gmask = ctx->dev.gmask;
     if ((e = upload(ctx, P.rowinfo, &F.rowinfo)) != cudaSuccess) return fail_cuda(e, "upload rowinfo");
     if ((e = upload(ctx, e0, &F.e_chunk0)) != cudaSuccess) return fail_cuda(e, "upload e_chunk0");
     if ((e = upload(ctx, tasks, &F.tg_tasks)) != cudaSuccess) return fail_cuda(e, "upload tgemm tasks");
@@ -394,10 +408,9 @@ int gint_fvl(gint_ctx* ctx, const double* V_dev, const double* D_dev, double* F_
         if (rc != GINT_OK) return rc;
     }
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    cudaError_t e = gint::launch_psi(ctx->dev, ctx->psi_smem, ctx->plan.tables_in_smem, ctx->nsm, nullptr, st);
-    if (e != cudaSuccess) return fail_cuda(e, "gint_fvl psi launch");
-    e = gint::launch_fvl(ctx->dev, ctx->fvl, ctx->force_smem, ctx->plan.tables_in_smem, ctx->nsm, (int)ctx->plan.atom_species.size(),
-                         V_dev, D_dev, F_dev, st, nullptr);
+    cudaError_t e = gint::launch_fvl(ctx->dev, ctx->fvl, ctx->psi_smem, ctx->force_smem, ctx->plan.tables_in_smem, ctx->nsm,
+                                     (int)ctx->plan.atom_species.size(), ctx->batches.data(), ctx->tg0.data(),
+                                     (int)ctx->batches.size(), V_dev, D_dev, F_dev, st);
     if (e != cudaSuccess) return fail_cuda(e, "gint_fvl launch");
     return GINT_OK;
 }

@@ -37,6 +37,7 @@ struct DevicePlan {
     double* psi;              // scratch: psi_chunks x 1024 doubles, zero-filled once at setup
     unsigned int* counter;    // work-queue head, reset before every launch
     const int32_t* work_regions;   // indices of the regions that own work items
+    const uint8_t* gmask;     // per region [ngroup][nks_pad]: fragment activity nibble per k-step (Region::gmask_off)
     double estep[9];          // mesh step vectors a_d / N_d (rows)
     double dV;
     int32_t ngrid[3];
@@ -45,6 +46,7 @@ struct DevicePlan {
     int32_t tab_doubles;
     int32_t nspecies;
     int32_t nring;
+    int32_t multibatch;       // several batches of regions reuse the psi scratch: the psi kernel zero-fills what it skips
     int32_t never;            // always 0: a branch condition the compiler cannot fold (see KROW in gint_kernels.cu)
 };
 
@@ -71,22 +73,29 @@ struct FvlPlan {
     double* tscratch;          // T = E Phi, psi chunk layout (same chunk indices as the psi scratch)
     int32_t ntg, nks_pad;
 };
+// The launchers walk the plan's batches (regions that share the psi scratch one after the other): nbatch entries of
+// (first item, items, first work region, work regions).
+struct BatchRange { int32_t item0, nitems, wr0, nwr; };
 size_t force_kernel_smem(size_t table_bytes, int nspecies);
 cudaError_t configure_fvl(size_t force_smem, bool tab_smem);
-cudaError_t launch_fvl(const DevicePlan& P, const FvlPlan& F, size_t force_smem, bool tab_smem, int nsm, int natom,
-                       const double* V, const double* D, double* Fout, cudaStream_t stream, cudaEvent_t* ev);
+cudaError_t launch_fvl(const DevicePlan& P, const FvlPlan& F, size_t psi_smem, size_t force_smem, bool tab_smem, int nsm,
+                       int natom, const BatchRange* batches, const int32_t* tg0, int nbatch, const double* V, const double* D,
+                       double* Fout, cudaStream_t stream);
+DevicePlan batch_plan(const DevicePlan& P, const BatchRange& B);
 cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream);
-cudaError_t launch_rho_dmma(const DevicePlan& P, size_t contract_smem_bytes, int nsm, const double* D, double* rho,
-                            cudaStream_t stream);
+cudaError_t launch_rho(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
+                       const BatchRange* batches, int nbatch, const double* D, double* rho, cudaStream_t stream);
 cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac, double* Hk, cudaStream_t stream);
 
 size_t psi_kernel_smem(size_t table_bytes, int nspecies);
 size_t contract_kernel_smem(int nring);
 cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool tab_smem);
-// ev: nullptr, or 5 events recorded at call start / before psi / before contraction / after it / after mirror
+// ev: nullptr, or 5 events recorded at call start / before psi / before contraction / after it / after mirror (with
+// several batches: before the first psi kernel / -- / after the last contraction)
 // raw: integrate a non-negative V without the shift (builds S at setup)
 cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
-                          size_t h_len, const double* V, double* H, bool raw, cudaStream_t stream, cudaEvent_t* ev);
+                          const BatchRange* batches, int nbatch, size_t h_len, const double* V, double* H, bool raw,
+                          cudaStream_t stream, cudaEvent_t* ev);
 cudaError_t measure_dmma_peak(double seconds, int nsm, double* tflops);
 
 }  // namespace gint

@@ -409,21 +409,27 @@ cudaError_t configure_fvl(size_t force_smem, bool tab_smem) {
                     : cudaFuncSetAttribute(gint_force_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)force_smem);
 }
 
-// Phi must be in the psi scratch (gint_psi_kernel with unit weights).  ev: nullptr or 4 events (start, after E, after T, end).
-cudaError_t launch_fvl(const DevicePlan& P, const FvlPlan& F, size_t force_smem, bool tab_smem, int nsm, int natom,
-                       const double* V, const double* D, double* Fout, cudaStream_t stream, cudaEvent_t* ev) {
+// F <- 0; per batch of regions: Phi (psi kernel with unit weights), E gather, T = E Phi, force kernel
+cudaError_t launch_fvl(const DevicePlan& P, const FvlPlan& F, size_t psi_smem, size_t force_smem, bool tab_smem, int nsm,
+                       int natom, const BatchRange* batches, const int32_t* tg0, int nbatch, const double* V, const double* D,
+                       double* Fout, cudaStream_t stream) {
     cudaError_t e = cudaMemsetAsync(Fout, 0, (size_t)natom * 3 * sizeof(double), stream);
-    if (e != cudaSuccess || P.nwork_regions <= 0) return e;
-    if (ev) cudaEventRecord(ev[0], stream);
-    gint_egather_kernel<<<P.nwork_regions, 256, 0, stream>>>(P, F, D);
-    if (ev) cudaEventRecord(ev[1], stream);
-    if (F.ntg > 0) gint_tgemm_kernel<<<F.ntg, kTgThreads, kTgSmem, stream>>>(P, F);
-    if (ev) cudaEventRecord(ev[2], stream);
-    const int grid = P.nwork_regions < 2 * nsm ? P.nwork_regions : 2 * nsm;
-    if (tab_smem) gint_force_kernel<true><<<grid, kFvThreads, force_smem, stream>>>(P, F, V, Fout);
-    else gint_force_kernel<false><<<grid, kFvThreads, force_smem, stream>>>(P, F, V, Fout);
-    if (ev) cudaEventRecord(ev[3], stream);
-    return cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    for (int b = 0; b < nbatch; b++) {
+        const DevicePlan Q = batch_plan(P, batches[b]);
+        if (Q.nwork_regions <= 0 || Q.nitems <= 0) continue;
+        if ((e = launch_psi(Q, psi_smem, tab_smem, nsm, nullptr, stream)) != cudaSuccess) return e;
+        gint_egather_kernel<<<Q.nwork_regions, 256, 0, stream>>>(Q, F, D);
+        FvlPlan G = F;
+        G.tg_tasks = F.tg_tasks + tg0[b];
+        G.ntg = tg0[b + 1] - tg0[b];
+        if (G.ntg > 0) gint_tgemm_kernel<<<G.ntg, kTgThreads, kTgSmem, stream>>>(Q, G);
+        const int grid = Q.nwork_regions < 2 * nsm ? Q.nwork_regions : 2 * nsm;
+        if (tab_smem) gint_force_kernel<true><<<grid, kFvThreads, force_smem, stream>>>(Q, F, V, Fout);
+        else gint_force_kernel<false><<<grid, kFvThreads, force_smem, stream>>>(Q, F, V, Fout);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 }  // namespace gint

@@ -343,13 +343,13 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
         const int gstride = P.nstage * kChunkDoubles;
         // the entry of a task (position, species, first row, activity of the run's 8 stages: byte s of the 64 k-step
         // bits starting at stage s0) is fetched one task ahead: two dependent global loads hidden behind an evaluation
-        struct TaskRegs { double relx, rely, relz; int rp, row0, s0; uint2 km; };
+        struct TaskRegs { double relx, rely, relz; int rp, row0, s0, norb; uint2 km; };
         auto fetch_task = [&](int t, TaskRegs& tr) {
             const uint32_t tk = __ldg(tasks + t);
             const Entry* en = entries + (tk & 0xFFFFu);
             tr.s0 = (int)(tk >> 16) * 8;
             tr.relx = __ldg(&en->rel[0]); tr.rely = __ldg(&en->rel[1]); tr.relz = __ldg(&en->rel[2]);
-            tr.rp = __ldg(&en->Rpack); tr.row0 = __ldg(&en->row0);
+            tr.rp = __ldg(&en->Rpack); tr.row0 = __ldg(&en->row0); tr.norb = __ldg(&en->norb);
             tr.km = __ldg(reinterpret_cast<const uint2*>(&en->kmask[tr.s0 >> 2]));
         };
         TaskRegs nxt;
@@ -362,8 +362,21 @@ gint_psi_kernel(const __grid_constant__ DevicePlan P, const double* __restrict__
             const uint2 km = cur.km;
             const SpeciesDev& sp = s_spec[spi];
             for (int q = 0; q < 8 && s0 + q < P.nstage; q++) {
-                if ((((q < 4 ? km.x : km.y) >> (8 * (q & 3))) & 0xFFu) == 0u) continue;
                 const int stage = s0 + q;
+                if ((((q < 4 ? km.x : km.y) >> (8 * (q & 3))) & 0xFFu) == 0u) {
+                    // No point of the stage inside the sphere.  With one batch the rows stay zero from the memset at
+                    // setup; when batches share the scratch they hold another region's values and are zeroed here,
+                    // in the chunks that will be read (row group active in the stage).
+                    if (P.multibatch) {
+                        const uint8_t* gm = P.gmask + __ldg(&reg->gmask_off) + (size_t)stage * kStageKsteps;
+                        double* out = psi_region + (size_t)stage * kChunkDoubles + (lane >> 2) * kKstepDoubles + (lane & 3) * 2;
+                        for (int R = row0; R < row0 + cur.norb; R++) {
+                            if (*reinterpret_cast<const unsigned long long*>(gm + (size_t)(R >> 5) * P.nks_pad) != 0ull)
+                                out[(R >> 5) * gstride + ((R & 31) >> 1) * 8 + (R & 1)] = 0.0;
+                        }
+                    }
+                    continue;
+                }
                 eval_task(sp, tab, relx, rely, relz, row0, gstride, stage, lane, s_off, s_sqrtw,
                           psi_region + (size_t)stage * kChunkDoubles);
             }
@@ -865,6 +878,16 @@ cudaError_t configure_kernels(size_t psi_smem, size_t contract_smem_bytes, bool 
     return cudaFuncSetAttribute(gint_contract_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)contract_smem_bytes);
 }
 
+// the parameter block of one batch: its slice of the work-region list and of the item queue
+DevicePlan batch_plan(const DevicePlan& P, const BatchRange& B) {
+    DevicePlan Q = P;
+    Q.descs = P.descs + B.item0;
+    Q.nitems = B.nitems;
+    Q.work_regions = P.work_regions + B.wr0;
+    Q.nwork_regions = B.nwr;
+    return Q;
+}
+
 cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int nsm, const double* V, cudaStream_t stream) {
     if (P.nitems <= 0) return cudaSuccess;
     const int pgrid = P.nwork_regions < kEvalCtasPerSm * nsm ? P.nwork_regions : kEvalCtasPerSm * nsm;
@@ -877,10 +900,10 @@ cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int 
 
 // raw = true: no shift (c = 0, H <- sum_g phi V phi dV for a non-negative V): used once at setup to build S.
 cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
-                          size_t h_len, const double* V, double* H, bool raw, cudaStream_t stream, cudaEvent_t* ev) {
+                          const BatchRange* batches, int nbatch, size_t h_len, const double* V, double* H, bool raw,
+                          cudaStream_t stream, cudaEvent_t* ev) {
     if (ev) cudaEventRecord(ev[0], stream);
-    cudaError_t e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 4, stream);   // work-queue head
-    if (e != cudaSuccess) return e;
+    cudaError_t e;
     if (raw) {
         if ((e = cudaMemsetAsync(P.shift, 0, sizeof(ShiftDev), stream)) != cudaSuccess) return e;
         if ((e = cudaMemsetAsync(H, 0, h_len * sizeof(double), stream)) != cudaSuccess) return e;
@@ -891,16 +914,19 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[1], stream);
-    e = launch_psi(P, psi_smem, tab_smem, nsm, V, stream);
-    if (e != cudaSuccess) return e;
-    if (ev) cudaEventRecord(ev[2], stream);
-    if (P.nitems > 0) {
-        const int grid = P.nitems < nsm ? P.nitems : nsm;
-        gint_contract_kernel<0><<<grid, kThreads, contract_smem_bytes, stream>>>(P, nullptr, H);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
+    for (int b = 0; b < nbatch; b++) {
+        const DevicePlan Q = batch_plan(P, batches[b]);
+        if (Q.nitems <= 0) continue;
+        if ((e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 4, stream)) != cudaSuccess) return e;   // work-queue head
+        if ((e = launch_psi(Q, psi_smem, tab_smem, nsm, V, stream)) != cudaSuccess) return e;
+        if (ev && b == nbatch - 1) cudaEventRecord(ev[2], stream);
+        const int grid = Q.nitems < nsm ? Q.nitems : nsm;
+        gint_contract_kernel<0><<<grid, kThreads, contract_smem_bytes, stream>>>(Q, nullptr, H);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
+    if (ev && (nbatch == 0 || batches[nbatch - 1].nitems <= 0)) cudaEventRecord(ev[2], stream);
     if (ev) cudaEventRecord(ev[3], stream);
+    e = cudaSuccess;
     if (P.nmirror > 0) {
         const int wpb = 256 / 32;
         gint_mirror_kernel<<<(P.nmirror + wpb - 1) / wpb, 256, 0, stream>>>(P.mirror, P.nmirror, H);
@@ -910,17 +936,23 @@ cudaError_t launch_vlocal(const DevicePlan& P, size_t psi_smem, size_t contract_
     return e;
 }
 
-// gint_rho on the tensor pipe: rho <- 0, queue head <- 0, contraction kernel in MODE 1 (phi must be in the scratch)
-cudaError_t launch_rho_dmma(const DevicePlan& P, size_t contract_smem_bytes, int nsm, const double* D, double* rho,
-                            cudaStream_t stream) {
+// gint_rho on the tensor pipe: rho <- 0; per batch: phi (psi kernel with unit weights), queue head <- 0, contraction
+// kernel in MODE 1
+cudaError_t launch_rho(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
+                       const BatchRange* batches, int nbatch, const double* D, double* rho, cudaStream_t stream) {
     const size_t npts = (size_t)P.ngrid[0] * P.ngrid[1] * P.ngrid[2];
     cudaError_t e = cudaMemsetAsync(rho, 0, npts * sizeof(double), stream);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 4, stream);
-    if (e != cudaSuccess || P.nitems <= 0) return e;
-    const int grid = P.nitems < nsm ? P.nitems : nsm;
-    gint_contract_kernel<1><<<grid, kThreads, contract_smem_bytes, stream>>>(P, D, rho);
-    return cudaGetLastError();
+    for (int b = 0; b < nbatch; b++) {
+        const DevicePlan Q = batch_plan(P, batches[b]);
+        if (Q.nitems <= 0) continue;
+        if ((e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int) * 4, stream)) != cudaSuccess) return e;
+        if ((e = launch_psi(Q, psi_smem, tab_smem, nsm, nullptr, stream)) != cudaSuccess) return e;
+        const int grid = Q.nitems < nsm ? Q.nitems : nsm;
+        gint_contract_kernel<1><<<grid, kThreads, contract_smem_bytes, stream>>>(Q, D, rho);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 // ---- FP64 tensor peak: register-resident DMMA.8x8x4 loop --------------------------------

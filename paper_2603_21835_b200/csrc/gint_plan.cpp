@@ -69,7 +69,7 @@ constexpr unsigned kMaxThreads = 32;
 
 int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecies, const SpeciesHost* species,
                int natom, const int32_t* atom_species, const double* atom_pos, const int32_t bcell[3], int rank,
-               int nranks, std::string& err) {
+               int nranks, int64_t scratch_max_bytes, std::string& err) {
     // ---- validation -------------------------------------------------------
     if (!lattice || !ngrid || !species || !atom_species || !atom_pos) { err = "null argument"; return GINT_EINVAL; }
     if (nspecies <= 0 || nspecies > 127 || natom <= 0 || natom >= (1 << 20)) { err = "nspecies/natom out of range"; return GINT_EINVAL; }
@@ -86,6 +86,8 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     std::memcpy(P.lattice, lattice, sizeof(P.lattice));
     P.rank = rank;
     P.nranks = nranks;
+    if (scratch_max_bytes < 0) { err = "scratch_max_bytes negative"; return GINT_EINVAL; }
+    P.scratch_max_bytes = scratch_max_bytes;
     P.species.assign(species, species + nspecies);
     double rc_max = 0;
     for (int s = 0; s < nspecies; s++) {
@@ -459,6 +461,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     // prepass (serial, cheap): region boundaries in the entry list, rows, offsets into the shared tables
     struct Span { size_t pos, end; };
     std::vector<Span> spans;
+    int64_t total_chunks = 0;
     {
         const int task_runs = (nslice + 7) / 8;
         size_t gm_off = 0, ri_off = 0, pr_off = 0, tk_off = 0;
@@ -504,11 +507,16 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         }
         P.gmask.assign(gm_off, 0);
         P.rowinfo.assign(ri_off, kNoBlock);
+        for (const Region& R : P.regions) total_chunks += (int64_t)R.ngroup * nstage;
         P.pair.assign(pr_off, PairWord{kNoBlock, 0, 0});
         P.pair_direct.assign(pr_off, kNoBlock);
         P.etasks.assign(tk_off, 0u);
     }
     const size_t nreg = P.regions.size();
+    const int64_t max_chunks = std::max<int64_t>(1, (scratch_max_bytes > 0 ? scratch_max_bytes : kDefaultScratchBytes) / kChunkBytes);
+    // several batches share the scratch: rows that no task of a region writes must then be zeroed by the psi kernel
+    // (they hold another region's values), so every (entry, run of stages) becomes a task
+    const bool multibatch = total_chunks > max_chunks;
     std::vector<std::vector<Proto>> region_protos(nreg);
     std::vector<int> region_active(nreg, 0);
     region_cost.assign(nreg, 0.0);
@@ -525,7 +533,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 int na = 0;
                 for (int s = h * 8; s < std::min(nslice, h * 8 + 8); s++)
                     if ((e.kmask[(s * kSliceKsteps) >> 5] >> ((s * kSliceKsteps) & 31)) & 0xFFu) na++;
-                if (na) P.etasks[(size_t)R.task_off + (size_t)(R.ntask++)] = pack_etask(i, h);
+                if (na || multibatch) P.etasks[(size_t)R.task_off + (size_t)(R.ntask++)] = pack_etask(i, h);
                 nactive += na;
             }
         }
@@ -628,14 +636,34 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
         region_cost[rix] = rcost;
         region_protos[rix] = std::move(protos);
     });
-    for (size_t rix = 0; rix < nreg; rix++) {   // psi scratch chunks in region order; proto-items in region order
-        Region& R = P.regions[rix];
-        R.psi_chunk0 = P.psi_chunks;
-        if (R.ntile > 0) {
-            P.psi_chunks += (int64_t)R.ngroup * nstage;
-            n_etask += region_active[rix];
+    // psi scratch chunks in region order, starting over with every batch; proto-items in region order
+    P.region_batch.assign(nreg, 0);
+    {
+        int batch = 0;
+        int64_t used = 0;
+        for (size_t rix = 0; rix < nreg; rix++) {
+            Region& R = P.regions[rix];
+            const int64_t need = R.ntile > 0 ? (int64_t)R.ngroup * nstage : 0;
+            if (used > 0 && used + need > max_chunks) {
+                batch++;
+                used = 0;
+            }
+            P.region_batch[rix] = batch;
+            R.psi_chunk0 = used;
+            used += need;
+            P.psi_chunks = std::max(P.psi_chunks, used);
+            if (R.ntile > 0) n_etask += region_active[rix];
+            for (Proto& p : region_protos[rix]) all_protos.push_back(std::move(p));
         }
-        for (Proto& p : region_protos[rix]) all_protos.push_back(std::move(p));
+        P.batches.assign((size_t)batch + 1, Plan::Batch{0, 0, 0, 0});
+        int wr = 0;
+        for (size_t rix = 0; rix < nreg; rix++)
+            if (P.regions[rix].ntile > 0) {
+                Plan::Batch& B = P.batches[(size_t)P.region_batch[rix]];
+                if (B.nwr == 0) B.wr0 = wr;
+                B.nwr++;
+                wr++;
+            }
     }
     tmp.clear();
     tmp.shrink_to_fit();
@@ -644,6 +672,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     // queue order: heaviest regions first, the proto-items of a region consecutive (their CTAs share its psi in L2)
     std::stable_sort(all_protos.begin(), all_protos.end(), [&](const Proto& a, const Proto& b) {
         const int ra = a.tiles[0].region, rb = b.tiles[0].region;
+        if (P.region_batch[(size_t)ra] != P.region_batch[(size_t)rb]) return P.region_batch[(size_t)ra] < P.region_batch[(size_t)rb];
         if (region_cost[(size_t)ra] != region_cost[(size_t)rb]) return region_cost[(size_t)ra] > region_cost[(size_t)rb];
         return ra < rb;
     });
@@ -660,6 +689,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 for (size_t b = a + 1; b < std::min(all_protos.size(), a + 1 + window); b++) {
                     if (dead[b]) continue;
                     const Proto& pb = all_protos[b];
+                    if (P.region_batch[(size_t)pb.tiles[0].region] != P.region_batch[(size_t)pa.tiles[0].region]) break;
                     if (pa.tiles.size() + pb.tiles.size() > (size_t)kTilesPerItem) continue;
                     size_t nu = pa.slots.size();
                     for (auto g : pb.slots)
@@ -681,6 +711,11 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
                 w++;
             }
         all_protos.resize(w);
+    }
+    for (size_t it = 0; it < all_protos.size(); it++) {   // item ranges of the batches (the queue is batch-major)
+        Plan::Batch& B = P.batches[(size_t)P.region_batch[(size_t)all_protos[it].tiles[0].region]];
+        if (B.nitems == 0) B.item0 = (int32_t)it;
+        B.nitems++;
     }
     // descriptors: everything the contraction kernel needs for an item, contiguous (one bulk copy)
     double exec_dmma = 0, flush_elems = 0, chunk_loads = 0;
@@ -890,6 +925,7 @@ int build_plan(Plan& P, const double* lattice, const int32_t* ngrid, int nspecie
     P.stats[21] = bal_stage;   // same if the warps moved through the stages in lockstep
     P.stats[22] = bal_warp;    // sum over (item, stage) of the heaviest single warp's DMMAs
     for (int d = 0; d < 3; d++) P.stats[23 + d] = (double)P.bcell[d];
+    P.stats[30] = (double)P.batches.size();   // batches sharing the psi scratch
     P.stats[26] = dmma_diag;   // DMMAs in diagonal-tile runs / all-row rectangular runs / other patterns (k-step by k-step)
     P.stats[27] = dmma_rect;
     P.stats[28] = dmma_slow;

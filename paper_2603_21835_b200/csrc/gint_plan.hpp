@@ -193,7 +193,13 @@ struct Plan {
     std::vector<uint32_t> rowinfo;
     std::vector<PairWord> pair;                 // [nentry][nentry] per region, a <= b filled
     std::vector<uint32_t> pair_direct;          // same indexing: offset of block (I_a, I_b, R_b - R_a) itself, any order (gint_rho)
-    std::vector<ItemDesc> descs;                // one per work item, queue order
+    // Batches: the psi scratch is reused by consecutive batches of regions when one buffer for all regions would exceed
+    // scratch_max_bytes (one batch otherwise).  A batch owns consecutive regions, work-region indices and work items.
+    struct Batch { int32_t item0, nitems, wr0, nwr; };
+    std::vector<Batch> batches;
+    std::vector<int32_t> region_batch;          // [regions]
+    int64_t scratch_max_bytes = 0;              // as given (0 = default)
+    std::vector<ItemDesc> descs;                // one per work item, queue order (batch-major)
     std::vector<uint32_t> etasks;               // evaluation tasks, region-major
     int64_t psi_chunks = 0;                     // 8 KB chunks of the psi scratch buffer
     // packed radial tables for the device: per species [ntab+4][nradp] (node-major, nradp = nrad rounded up
@@ -225,6 +231,7 @@ inline uint64_t hash_mix(uint64_t k) {
 // Returns 0 or a negative GINT_* code; err receives a message.
 int build_plan(Plan& plan, const double* lattice, const int32_t* ngrid, int nspecies, const SpeciesHost* species,
                int natom, const int32_t* atom_species, const double* atom_pos, const int32_t bcell[3], int rank,
-               int nranks, std::string& err);
+               int nranks, int64_t scratch_max_bytes, std::string& err);
+constexpr int64_t kDefaultScratchBytes = int64_t(16) << 30;   // psi scratch limit when the caller gives none
 
 }  // namespace gint

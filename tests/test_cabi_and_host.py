@@ -232,3 +232,21 @@ def test_update_positions_equals_fresh_setup(cfg1):
     with pytest.raises(Exception):
         ctx.gint_update_positions(bad)
     assert ctx.gint_get_stats() == ref.gint_get_stats()
+
+
+def test_scratch_limit_makes_batches(cfg1):
+    """scratch_max_bytes (host logic): the plan cuts the regions into batches that fit, keeps work and block table, and
+    never goes below what the largest region needs."""
+    from paper_2603_21835_b200 import gint_setup
+    full = gint_setup(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cuda_device=-1)
+    s0 = full.gint_get_stats()
+    assert s0["batches"] == 1
+    for limit in (1, 1 << 16, 1 << 18):
+        ctx = gint_setup(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cuda_device=-1,
+                         scratch_max_bytes=limit)
+        s = ctx.gint_get_stats()
+        assert s["batches"] > 1 and s["psi_scratch_bytes"] < s0["psi_scratch_bytes"]
+        assert s["psi_scratch_bytes"] <= max(limit, 8192 * 40 * 16)       # one region at most: 40 groups x 16 stages
+        assert s["F_sym"] == s0["F_sym"] and s["executed_flops"] == s0["executed_flops"] and ctx.nblocks == full.nblocks
+    with pytest.raises(Exception):
+        gint_setup(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cuda_device=-1, scratch_max_bytes=-5)

@@ -528,3 +528,31 @@ def test_update_positions_on_device(cfg1):
     assert_force_parity(ctx.gint_fvl(Vd, Dd).cpu().numpy(), Fr, "moved atoms")
     ctx.gint_update_positions(w.atom_pos)
     assert np.abs(ctx.gint_vlocal(Vd).cpu().numpy() - H0).max() <= 1e-13 * np.abs(H0).max()
+
+
+@pytest.mark.parametrize("name,limit", [("si8_sz", 1 << 16), ("si64_dzp", 48 << 20), ("cluster60", 8 << 20)])
+def test_scratch_limit_batches(name, limit):
+    """gint_options.scratch_max_bytes: when the psi scratch may not hold all regions, consecutive batches of regions
+    reuse it (the psi kernel then zero-fills what it skips).  All three calls against the oracle with many batches,
+    and the context really uses the small buffer."""
+    torch = _torch()
+    import oracle
+    from paper_2603_21835_b200 import gint_setup, workloads as wl
+    w = wl.make(name)
+    Hr, blocks = oracle_H(w)
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, scratch_max_bytes=limit)
+    st = ctx.gint_get_stats()
+    full = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1).gint_get_stats()
+    assert st["batches"] >= 4 and st["psi_scratch_bytes"] < full["psi_scratch_bytes"] / 3
+    assert st["F_sym"] == full["F_sym"] and st["executed_flops"] == full["executed_flops"]
+    Vd = torch.from_numpy(w.V).cuda()
+    rng = np.random.default_rng(71)
+    D = rng.normal(size=Hr.shape)
+    Dd = torch.from_numpy(D).cuda()
+    rho_ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blocks)
+    F_ref = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blocks)
+    for rep in range(2):   # second round: the scratch holds the last batch's values of the previous call
+        assert_parity(ctx.gint_vlocal(Vd).cpu().numpy(), Hr, "%s batched, round %d" % (name, rep))
+        got = ctx.gint_rho(Dd).cpu().numpy()
+        assert np.abs(got - rho_ref).max() <= TOL * np.abs(rho_ref).max()
+        assert_force_parity(ctx.gint_fvl(Vd, Dd).cpu().numpy(), F_ref, "%s batched" % name)
