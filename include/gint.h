@@ -121,7 +121,7 @@ int gint_get_blocks(const gint_ctx *ctx, int32_t *iat, int32_t *jat, int32_t *R,
  * Asynchronous: enqueues two memsets, the psi kernel, the contraction kernel and the
  * mirror kernel on `stream`; no host synchronisation, no allocation, no host<->device
  * copy.  The context owns a device scratch buffer for psi (stats[12] bytes; 8.5 GB for
- * the 512-atom Si-like workload).
+ * the 512-atom Si-like workload; bounded by gint_options.scratch_max_bytes, stats[30] batches).
  * With nranks > 1 H holds this rank's partial sum (sum over ranks = full H).
  * Kernel faults surface at the caller's next synchronisation. */
 int gint_vlocal(gint_ctx *ctx, const double *V_dev, double *H_dev, void *stream);
@@ -180,7 +180,8 @@ int gint_fold_k(gint_ctx *ctx, const double *H_dev, const double *kfrac, double 
  * gint_get_kernel_ms synchronises on the last call's events and returns durations in
  * milliseconds: ms[0] contraction kernel, ms[1] mirror kernel, ms[2] whole call incl. the
  * memsets, ms[3] psi (orbital evaluation) kernel.  Used by bench.py for the roofline's
- * per-launch duration. */
+ * per-launch duration.  With several batches (stats[30] > 1) ms[0] is the last batch's contraction and ms[3]
+ * everything between the first psi kernel and it; ms[2] is always the whole call. */
 int gint_set_profiling(gint_ctx *ctx, int32_t on);
 int gint_get_kernel_ms(gint_ctx *ctx, double *ms /* [4] */);
 
@@ -198,6 +199,7 @@ int gint_get_kernel_ms(gint_ctx *ctx, double *ms /* [4] */);
  * stats[14] 8 KB chunk buffers of the shared-memory ring    stats[15] non-empty regions
  * stats[16..22] k-step / balance statistics of the plan, stats[23..25] big-cell edge actually used,
  * stats[26..29] DMMAs by code path of the contraction kernel (diagonal runs, all-row runs, other) and number of runs
+ * stats[30] batches of regions that share the psi scratch (1 unless scratch_max_bytes forces more)
  * Returns the number of entries written (<= n, at most 32). */
 int gint_get_stats(const gint_ctx *ctx, double *stats, int32_t n);
 
