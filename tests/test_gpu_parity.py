@@ -556,3 +556,28 @@ def test_scratch_limit_batches(name, limit):
         got = ctx.gint_rho(Dd).cpu().numpy()
         assert np.abs(got - rho_ref).max() <= TOL * np.abs(rho_ref).max()
         assert_force_parity(ctx.gint_fvl(Vd, Dd).cpu().numpy(), F_ref, "%s batched" % name)
+
+
+def test_large_tables_stay_in_global_memory():
+    """Radial tables too large for shared memory (fine dr: 2 species x 4 padded functions x 3004 nodes = 192 KB > 56 KB)
+    take the kernels' global-memory table path (psi and force kernels instantiated with TAB_SMEM = false): all three
+    calls against the oracle on a triclinic cell with two species."""
+    torch = _torch()
+    import oracle
+    from paper_2603_21835_b200 import gint_setup, workloads as wl
+    w = wl.tiny(seed=17, natom=4, ngrid=(11, 10, 12))
+    fine = [wl.make_species("fine-a", 3.0, [(0, 0.6), (1, 0.5), (2, 0.7)], dr=0.001),
+            wl.make_species("fine-b", 3.0, [(0, 0.9), (1, 0.8), (3, 0.6)], dr=0.001)]
+    w.species = fine
+    w.atom_species = np.array([0, 1, 0, 1], dtype=np.int32)
+    Hr, blocks = oracle_H(w)
+    ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos)
+    Vd = torch.from_numpy(w.V).cuda()
+    assert_parity(ctx.gint_vlocal(Vd).cpu().numpy(), Hr, "tables in global memory")
+    rng = np.random.default_rng(81)
+    D = rng.normal(size=Hr.shape)
+    Dd = torch.from_numpy(D).cuda()
+    ref = oracle.rho(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, D, blocks)
+    assert np.abs(ctx.gint_rho(Dd).cpu().numpy() - ref).max() <= TOL * np.abs(ref).max()
+    Fr = oracle.fvl(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, w.V, D, blocks)
+    assert_force_parity(ctx.gint_fvl(Vd, Dd).cpu().numpy(), Fr, "tables in global memory")
