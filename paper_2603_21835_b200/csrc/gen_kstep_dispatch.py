@@ -52,53 +52,56 @@ def diag():
 
 
 def run_block(name, tblname, key, a_frags, b_frags, pairs, diag):
-    """One pattern of a RUN of consecutive k-steps (1 KB apart in the chunks): software-pipelined loop over two
-    register sets (ping-pong, no copies) -- the operands of the next k-step are loaded (predicated on there being
-    one) before the DMMAs of the current one are issued, so a single warp can keep the FP64 tensor pipe busy by
-    itself, with the fewest instructions around the DMMAs.  Operands: %0..%31 accumulators, %32 / %33 shared-memory
-    byte addresses of the lane's A / B element of the first k-step, %34 number of k-steps, %35 pattern."""
+    """One pattern of a RUN of consecutive k-steps (1 KB apart in the chunks).  The DMMAs of a k-step go row fragment by
+    row fragment; as soon as the DMMAs of row fragment i are issued, its A operand register is reloaded for the next
+    k-step (rolling reload: no second A set), and the B operands alternate between two register sets (the B fragments
+    are read by every row).  A single warp still keeps the FP64 tensor pipe busy by itself, with 24 operand registers
+    instead of 32.  Diagonal tiles (B = A) need no second set at all: a_i is dead once row i is done (rows r <= i
+    are the only readers of a_i as a B operand).
+    Operands: %0..%31 accumulators, %32 / %33 shared-memory byte addresses of the lane's A / B element of the first
+    k-step, %34 number of k-steps, %35 pattern."""
     L = name + str(key)
     o = ['"%s:\\n\\t"' % L]
 
-    def lds(pred, dst_prefix, off):
+    def ld_a(pred, i, off):
+        return '"%sld.shared.f64 a%d, [pa+%d];\\n\\t"' % (pred, i, 256 * i + off)
+
+    def ld_b(pred, prefix, off):
+        return ['"%sld.shared.f64 %sb%d, [pb+%d];\\n\\t"' % (pred, prefix, j, 256 * j + off) for j in b_frags]
+
+    def step(bprefix, next_off):
         out = []
         for i in a_frags:
-            out.append('"%sld.shared.f64 %sa%d, [pa+%d];\\n\\t"' % (pred, dst_prefix, i, 256 * i + off))
-        for j in b_frags:
-            out.append('"%sld.shared.f64 %sb%d, [pb+%d];\\n\\t"' % (pred, dst_prefix, j, 256 * j + off))
+            for (pi, j) in pairs:
+                if pi != i:
+                    continue
+                c0, c1 = (4 * i + j) * 2, (4 * i + j) * 2 + 1
+                bop = ("a%d" % j) if diag else ("%sb%d" % (bprefix, j))
+                out.append('"mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%%%d,%%%d}, {a%d}, {%s}, {%%%d,%%%d};\\n\\t"' % (c0, c1, i, bop, c0, c1))
+            out.append(ld_a("@p ", i, next_off))
         return out
 
-    def mmas(prefix):
-        out = []
-        for (i, j) in pairs:
-            c0, c1 = (4 * i + j) * 2, (4 * i + j) * 2 + 1
-            bop = ("%sa%d" % (prefix, j)) if diag else ("%sb%d" % (prefix, j))
-            out.append('"mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%%%d,%%%d}, {%sa%d}, {%s}, {%%%d,%%%d};\\n\\t"' % (c0, c1, prefix, i, bop, c0, c1))
-        return out
-
-    def advance(nbytes):
-        out = ['"add.u32 pa, pa, %d;\\n\\t"' % nbytes]
-        if b_frags:
-            out.append('"add.u32 pb, pb, %d;\\n\\t"' % nbytes)
-        return out
-
-    o += lds("", "", 0)
+    for i in a_frags:
+        o.append(ld_a("", i, 0))
+    o += ld_b("", "", 0)
     o.append('"%sL:\\n\\t"' % L)
     o.append('"setp.gt.u32 p, n, 1;\\n\\t"')
-    o += lds("@p ", "n", 1024)
-    o += mmas("")
+    o += ld_b("@p ", "n", 1024)
+    o += step("", 1024)
     o.append('"@!p bra.uni %sDONE;\\n\\t"' % name)
     o.append('"setp.gt.u32 p, n, 2;\\n\\t"')
-    o += lds("@p ", "", 2048)
-    o += mmas("n")
-    o += advance(2048)
+    o += ld_b("@p ", "", 2048)
+    o += step("n", 2048)
+    o.append('"add.u32 pa, pa, 2048;\\n\\t"')
+    if b_frags:
+        o.append('"add.u32 pb, pb, 2048;\\n\\t"')
     o.append('"sub.u32 n, n, 2;\\n\\t"')
     o.append('"@p bra.uni %sL;\\n\\t"' % L)
     o.append('"bra.uni %sDONE;\\n\\t"' % name)
     return o
 
 
-RUN_HEAD = ['"{\\n\\t"', '".reg .f64 a<4>, b<4>, na<4>, nb<4>;\\n\\t"', '".reg .pred p;\\n\\t"', '".reg .u32 pa, pb, n;\\n\\t"',
+RUN_HEAD = ['"{\\n\\t"', '".reg .f64 a<4>, b<4>, nb<4>;\\n\\t"', '".reg .pred p;\\n\\t"', '".reg .u32 pa, pb, n;\\n\\t"',
             '"mov.u32 pa, %32;\\n\\t"', '"mov.u32 pb, %33;\\n\\t"', '"mov.u32 n, %34;\\n\\t"']
 
 
