@@ -15,8 +15,8 @@
 // Three kernels after gint_psi_kernel (unit weights, Phi in the psi scratch):
 //   gint_egather_kernel  E of every region, dense, in DMMA A-fragment order (32 x 32 sub-blocks of 8 KB)
 //   gint_tgemm_kernel    T = E Phi per region on the FP64 tensor pipe (DMMA.8x8x4): CTA tile 128 rows x 128 points,
-//                        16 warps x (32 rows x 32 points), K = the region's row groups streamed through a 2-deep
-//                        shared-memory ring with cp.async.bulk + mbarrier; (row group, stage) pairs without an
+//                        16 warps x (32 rows x 32 points), K = the region's row groups streamed through a 3-deep
+//                        shared-memory ring with cp.async.bulk + full / empty mbarriers; (row group, stage) pairs without an
 //                        in-sphere point are skipped; T is written in the psi chunk layout
 //   gint_force_kernel    per (entry, 32-point stage): V dV, grad phi (analytic angular part, interpolant derivative),
 //                        dot with T, warp reduction, three atomics per task into F
@@ -111,12 +111,13 @@ __global__ void __launch_bounds__(256) gint_egather_kernel(const __grid_constant
 // ---- T = E Phi ----------------------------------------------------------------------------------------------
 constexpr int kTgThreads = 512;
 constexpr int kTgBufBytes = 8 * kChunkBytes;          // 4 E sub-blocks + 4 psi chunks
-constexpr int kTgSmem = 2 * kTgBufBytes + 64;
+constexpr int kTgRing = 3;                            // K steps in flight
+constexpr int kTgSmem = kTgRing * kTgBufBytes + 64;
 
 __global__ void __launch_bounds__(kTgThreads, 1)
 gint_tgemm_kernel(const __grid_constant__ DevicePlan P, const __grid_constant__ FvlPlan F) {
     extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + 2 * kTgBufBytes);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kTgRing * kTgBufBytes);   // full[3], empty[3]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int4 task = __ldg(F.tg_tasks + blockIdx.x);   // region, row quad, stage quad
     const Region* reg = P.regions + task.x;
@@ -126,15 +127,17 @@ gint_tgemm_kernel(const __grid_constant__ DevicePlan P, const __grid_constant__ 
     const double* Ebase = F.escratch + (size_t)__ldg(F.e_chunk0 + task.x) * kChunkDoubles;
     const double* psi_region = P.psi + (size_t)__ldg(&reg->psi_chunk0) * kChunkDoubles;
     if (tid == 0) {
-        bar_init(smem_addr(bars), 1);
-        bar_init(smem_addr(bars + 1), 1);
+        for (int i = 0; i < kTgRing; i++) {
+            bar_init(smem_addr(bars + i), 1);
+            bar_init(smem_addr(bars + kTgRing + i), kTgThreads / 32);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     asm volatile("fence.proxy.async;" ::: "memory");
     __syncthreads();
     // thread 0 streams, per column group gb: E(4 rq + i, gb) and Phi(gb, 4 sq + j), i, j = 0..3
     auto issue = [&](int gb) {
-        const uint32_t buf = smem_addr(smem) + (gb & 1) * kTgBufBytes, bar = smem_addr(bars + (gb & 1));
+        const uint32_t buf = smem_addr(smem) + (gb % kTgRing) * kTgBufBytes, bar = smem_addr(bars + gb % kTgRing);
         uint32_t n = 0;
         bool e_on[4], p_on[4];
         for (int i = 0; i < 4; i++) {
@@ -151,7 +154,10 @@ gint_tgemm_kernel(const __grid_constant__ DevicePlan P, const __grid_constant__ 
                 bulk_copy(buf + (4 + i) * kChunkBytes, psi_region + ((size_t)gb * nstage + 4 * task.z + i) * kChunkDoubles, kChunkBytes, bar);
         }
     };
-    if (tid == 0) issue(0);
+    if (tid == 0) {
+        issue(0);
+        if (ngroup > 1) issue(1);
+    }
     double acc[4][4][2];
 #pragma unroll
     for (int i = 0; i < 4; i++)
@@ -164,12 +170,20 @@ gint_tgemm_kernel(const __grid_constant__ DevicePlan P, const __grid_constant__ 
     // bit j: some row fragment of ga is active in k-pair j
     const uint32_t rj_any = ((rp & 0xFu) ? 1u : 0u) | ((rp & 0xF0u) ? 2u : 0u) | ((rp & 0xF00u) ? 4u : 0u) | ((rp & 0xF000u) ? 8u : 0u);
     for (int gb = 0; gb < ngroup; gb++) {
-        if (tid == 0 && gb + 1 < ngroup) issue(gb + 1);   // the other buffer was released by the barrier below
-        bar_wait(smem_addr(bars + (gb & 1)), (uint32_t)(gb >> 1) & 1u);
+        // K step gb + 2 goes into the buffer of K step gb - 1 once all 16 warps have released it; the warps take turns at
+        // waiting for that (no block-wide barrier: a warp whose tile is sparse runs ahead by up to two K steps)
+        if (warp == (gb & 15) && gb + 2 < ngroup) {
+            if (lane == 0) {
+                if (gb >= 1) bar_wait(smem_addr(bars + kTgRing + (gb + 2) % kTgRing), (uint32_t)((gb + 2) / kTgRing - 1) & 1u);
+                issue(gb + 2);
+            }
+            __syncwarp();
+        }
+        bar_wait(smem_addr(bars + gb % kTgRing), (uint32_t)(gb / kTgRing) & 1u);
         const uint32_t cp = mine ? kpair_masks(F, reg, gb, stage) : 0u;   // column fragments of gb active per k-pair
         if (cp) {
-            const double* bufE = reinterpret_cast<const double*>(smem + (gb & 1) * kTgBufBytes + (warp >> 2) * kChunkBytes) + lane;
-            const double* bufP = reinterpret_cast<const double*>(smem + (gb & 1) * kTgBufBytes + (4 + (warp & 3)) * kChunkBytes) + boff;
+            const double* bufE = reinterpret_cast<const double*>(smem + (gb % kTgRing) * kTgBufBytes + (warp >> 2) * kChunkBytes) + lane;
+            const double* bufP = reinterpret_cast<const double*>(smem + (gb % kTgRing) * kTgBufBytes + (4 + (warp & 3)) * kChunkBytes) + boff;
             if ((rp & cp) == 0xFFFFu) {   // every fragment active in every k-pair: dense
 #pragma unroll 2
                 for (int kc = 0; kc < 8; kc++) {
@@ -213,7 +227,8 @@ gint_tgemm_kernel(const __grid_constant__ DevicePlan P, const __grid_constant__ 
                 }
             }
         }
-        __syncthreads();
+        __syncwarp();
+        if (lane == 0) bar_arrive(smem_addr(bars + kTgRing + gb % kTgRing));   // this warp is done with the buffer
     }
     if (mine) {   // T tile -> scratch, psi chunk layout: (row R, point 4 ks + k) at ks * 128 + (R / 2) * 8 + k * 2 + R % 2
         double* Tc = F.tscratch + ((size_t)__ldg(&reg->psi_chunk0) + (size_t)ga * nstage + stage) * kChunkDoubles;
