@@ -41,22 +41,17 @@ UNIT = "TFLOP/s"
 
 def ncu_traffic(workload):
     """DRAM traffic of the contraction kernel per launch (dram__bytes_read.sum + dram__bytes_write.sum of the latest
-    ncu --set full capture), read from profiles/ncu_traffic.json at run time; None if no capture is recorded."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    ncu --set full capture), read from profiles/ncu_traffic.csv at run time; None if no capture is recorded."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     try:
         with open(p) as f:
-            rec = json.load(f).get(workload)
-        return None if rec is None else float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"])
-    except (OSError, ValueError, KeyError):
-        return None
-
-
-def measured_peaks():
-    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(p):
-        with open(p) as f:
-            return json.load(f), "measured"
-    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+            for line in f.read().splitlines()[1:]:
+                cols = line.split(",")
+                if cols[0] == workload:
+                    return float(cols[2]) + float(cols[3])
+    except (OSError, ValueError, IndexError):
+        pass
+    return None
 
 
 class ClockSampler:
