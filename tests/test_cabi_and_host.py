@@ -250,3 +250,18 @@ def test_scratch_limit_makes_batches(cfg1):
         assert s["F_sym"] == s0["F_sym"] and s["executed_flops"] == s0["executed_flops"] and ctx.nblocks == full.nblocks
     with pytest.raises(Exception):
         gint_setup(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cuda_device=-1, scratch_max_bytes=-5)
+
+
+def test_bench_helpers_run_without_a_gpu():
+    """bench.py's host-side helpers: the peaks file (or its fallback) and the ncu traffic record under profiles/."""
+    import importlib.util
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    peaks, src = bench.measured_peaks()
+    assert peaks["hbm_gbs"] > 1000 and peaks["bf16_tflops"] > 100 and src in ("measured", "fallback")
+    t = bench.ncu_traffic("si512_dzp")
+    assert t is not None and 1e9 < t < 1e11
+    assert bench.ncu_traffic("no_such_workload") is None
