@@ -2,7 +2,7 @@
 //
 //   H_mu,nu(R) = sum_g phi_mu(r_g - tau_I) V(r_g) phi_nu(r_g - tau_J - R) dV   (Eq. 45)
 //
-// Two kernels per call, both behind gint_vlocal (plus a tiny mirror kernel):
+// Five kernels per gint_vlocal call (per batch of regions for the two in the middle, see launch_vlocal):
 //
 //   gint_vrange_kernel / gint_hinit_kernel   range of V, then H <- c S with S the grid overlap (Eq. 45 with
 //       V = 1, computed once at setup) and c = max V (or min V, whichever is smaller in magnitude): the rest of
@@ -16,15 +16,16 @@
 //   gint_contract_kernel<0>  (gint_vlocal) output-stationary contraction (the paper's per-BigGrid dense
 //       contraction).  One persistent CTA per SM pulls work items from a global
 //       queue; a work item is a set of up to 15 32x32 tiles (one per consumer warp) of the upper
-//       triangle of a region's C (small left-over tile sets of several regions share an item).  A producer warp stages the item descriptor and streams the row
-//       groups the tiles need through a ring of shared-memory stages (32 points each) with
-//       cp.async.bulk + mbarrier, running ahead across item boundaries; the 15 consumer warps keep
-//       their tile in registers and issue mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has no FP64
-//       kind).  (fragment, k-step) pairs that hold no in-sphere point are skipped by warp-uniform
-//       branches on host-built activity nibbles (a predicated-off DMMA still costs its 16 pipe
-//       cycles) -- one indexed jump per k-step into straight-line code for its fragment pattern.
-//       After the last stage the warp adds its tile into
-//       the canonical H blocks with red.global.add.f64 (once per item, not once per BigGrid).
+//       triangle of a region's C (small left-over tile sets of several regions share an item).  A producer warp
+//       stages the item descriptor and streams the row groups the tiles need through a ring of 8 KB chunk buffers in
+//       shared memory (a 32-point stage takes one buffer per active row group) with cp.async.bulk + mbarrier, running
+//       ahead across item boundaries; the 15 consumer warps keep their tile in registers and issue
+//       mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4; tcgen05 has no FP64 kind).  (fragment, k-step) pairs that hold no
+//       in-sphere point are skipped by warp-uniform control flow decided on the host (a predicated-off DMMA still
+//       costs its 16 pipe cycles): per (warp, stage) a program of runs of k-steps with one fragment pattern, one
+//       indexed jump per run into a software-pipelined loop for the pattern (gint_kstep_dispatch.inc).  After the
+//       last stage the warp adds its tile into the canonical H blocks with red.global.add.f64 (once per item, not
+//       once per BigGrid).
 //   gint_contract_kernel<1>  (gint_rho, Eq. 44): same items, stages and producer;
 //       see rho_consumer.
 //   gint_mirror_kernel  writes every non-canonical block as the transpose of its partner,
