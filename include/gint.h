@@ -170,10 +170,26 @@ int gint_fvl(gint_ctx *ctx, const double *V_dev, const double *D_dev, double *F_
  *   kfrac    HOST pointer, 3 doubles
  *   Hk_dev   device pointer, [norb_tot][norb_tot] complex numbers as interleaved (re, im) doubles, row-major;
  *            rows: orbitals of atom I (atoms in input order), columns: orbitals of atom J; OVERWRITTEN
- * Asynchronous on `stream` (one memset, one kernel).  gint_num_orbitals returns norb_tot and, if `first` is not
- * NULL, first[natom+1] = the first row/column of every atom (first[natom] = norb_tot). */
+ * Asynchronous on `stream` (two kernels: the phases exp(i k.R) of all blocks into a scratch array the context
+ * owns, then one pass that writes every element of H(k) once).  gint_num_orbitals returns norb_tot and, if `first`
+ * is not NULL, first[natom+1] = the first row/column of every atom (first[natom] = norb_tot). */
 int gint_num_orbitals(const gint_ctx *ctx, int64_t *norb_tot, int64_t *first);
 int gint_fold_k(gint_ctx *ctx, const double *H_dev, const double *kfrac, double *Hk_dev, void *stream);
+
+/* gint_fold_k for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same result (Eq. 5), same two kernels, but the phase scratch is
+ * a fixed array inside the library -- a file-scope `static __device__` array of gint_fold_k_static_max_blocks() =
+ * 262144 entries x 16 bytes = 4 MiB that every GPU loading the library holds until the process exits -- instead of
+ * memory the context allocated.  Its device address is resolved once per device at gint_setup
+ * (cudaGetSymbolAddress); the call itself runs no cudaMalloc, cudaFree or allocating library routine.
+ *   - a context with more blocks than the maximum: GINT_EUNSUPPORTED, nothing launched (use gint_fold_k);
+ *   - nothing in the array has to start at zero: the first kernel rewrites entries 0 .. nblk-1, the second reads only
+ *     those, on the same stream;
+ *   - ALL contexts of a device share the array and it keeps the last call's contents: calls that can overlap on the
+ *     GPU (different streams, or different contexts on one device) race on it -- keep them on one stream or order
+ *     them with events.  gint_fold_k has no such restriction between contexts. */
+int64_t gint_fold_k_static_max_blocks(void);
+int gint_fold_k_static(gint_ctx *ctx, const double *H_dev, const double *kfrac, double *Hk_dev, void *stream);
 
 /* Per-kernel timing on the launch stream.  After gint_set_profiling(ctx, 1) every
  * gint_vlocal call records CUDA events around its kernels on `stream`;

@@ -13,7 +13,7 @@ from . import workloads  # noqa: F401
 
 
 def __getattr__(name):
-    if name in ("gint_setup", "gint_measure_fp64_peak", "GintContext", "GintError", "binding"):
+    if name in ("gint_setup", "gint_measure_fp64_peak", "gint_fold_k_static_max_blocks", "GintContext", "GintError", "binding"):
         import importlib
         binding = importlib.import_module(__name__ + ".binding")
         return binding if name == "binding" else getattr(binding, name)

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgint_b200.so")
 GINT_OK, GINT_EINVAL, GINT_EUNSUPPORTED, GINT_ENOMEM, GINT_ECUDA, GINT_ENODEVICE = 0, -1, -2, -3, -4, -5
 
 EXPORTED = ("gint_setup", "gint_update_positions", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
-            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_rho", "gint_fvl", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
+            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_fold_k_static", "gint_fold_k_static_max_blocks", "gint_rho", "gint_fvl", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
@@ -66,6 +66,10 @@ def _load() -> ctypes.CDLL:
     lib.gint_num_orbitals.argtypes = [vp, P(i64), P(i64)]
     lib.gint_fold_k.restype = ctypes.c_int
     lib.gint_fold_k.argtypes = [vp, vp, P(dbl), vp, vp]
+    lib.gint_fold_k_static.restype = ctypes.c_int
+    lib.gint_fold_k_static.argtypes = [vp, vp, P(dbl), vp, vp]
+    lib.gint_fold_k_static_max_blocks.restype = ctypes.c_int64
+    lib.gint_fold_k_static_max_blocks.argtypes = []
     lib.gint_rho.restype = ctypes.c_int
     lib.gint_rho.argtypes = [vp, vp, vp, vp]
     lib.gint_fvl.restype = ctypes.c_int
@@ -234,6 +238,21 @@ class GintContext:
                                 ctypes.c_void_p(Hk_dev.data_ptr()), ctypes.c_void_p(s)), "gint_fold_k")
         return Hk_dev
 
+    def gint_fold_k_static(self, H_dev, kfrac, Hk_dev, stream=None):
+        """gint_fold_k with the phase scratch in the library's fixed device array (no allocation: the caller passes
+        Hk_dev); GintError(GINT_EUNSUPPORTED) beyond gint_fold_k_static_max_blocks() blocks."""
+        import torch
+        n = self.gint_num_orbitals()[0]
+        if not (H_dev.is_cuda and H_dev.dtype == torch.float64 and H_dev.is_contiguous() and H_dev.numel() == self.h_len):
+            raise ValueError("H_dev must be a contiguous CUDA float64 tensor of h_len elements")
+        if not (Hk_dev.is_cuda and Hk_dev.dtype == torch.complex128 and Hk_dev.is_contiguous() and tuple(Hk_dev.shape) == (n, n)):
+            raise ValueError("Hk_dev must be a contiguous CUDA complex128 tensor [norb_tot][norb_tot]")
+        k = np.ascontiguousarray(kfrac, dtype=np.float64).reshape(3)
+        s = torch.cuda.current_stream(H_dev.device).cuda_stream if stream is None else int(stream)
+        _check(_lib.gint_fold_k_static(self._h, ctypes.c_void_p(H_dev.data_ptr()), _ptr(k, ctypes.c_double),
+                                       ctypes.c_void_p(Hk_dev.data_ptr()), ctypes.c_void_p(s)), "gint_fold_k_static")
+        return Hk_dev
+
     def gint_vlocal_host(self, V_host: np.ndarray, H_host: Optional[np.ndarray] = None) -> np.ndarray:
         """End-to-end call with HOST buffers (H2D of V, kernels, D2H of H, synchronise)."""
         V_host = np.ascontiguousarray(V_host, dtype=np.float64)
@@ -287,6 +306,10 @@ def gint_setup(lattice, ngrid, species: Sequence, atom_species, atom_pos, cuda_d
                            arr, int(pos.shape[0]), _ptr(asp, ctypes.c_int32), _ptr(pos, ctypes.c_double),
                            int(cuda_device), ctypes.byref(opt)), "gint_setup")
     return GintContext(h.value, ng, pos.shape[0])
+
+
+def gint_fold_k_static_max_blocks() -> int:
+    return int(_lib.gint_fold_k_static_max_blocks())
 
 
 def gint_measure_fp64_peak(cuda_device: int = 0, seconds: float = 0.5) -> float:

@@ -20,6 +20,7 @@ struct gint_ctx {
     int nsm = 0;
     std::vector<void*> allocs;
     gint::FoldPlan fold{};
+    double2* fold_static_phase = nullptr;   // gint_fold_k_static: device address of the library's fixed phase array
     std::vector<int64_t> first_orb;   // [natom+1]
     size_t psi_smem = 0, contract_smem = 0;
     bool profiling = false;
@@ -146,6 +147,8 @@ int device_init(gint_ctx* ctx) {
         ctx->fold.phase = reinterpret_cast<double2*>(ph);
         ctx->fold.nblk = (int32_t)P.blk_i.size();
         ctx->fold.natom = natom;
+        if ((e = gint::fold_static_scratch(ctx->device, &ctx->fold_static_phase)) != cudaSuccess)
+            return fail_cuda(e, "cudaGetSymbolAddress fold phases");
     }
 #undef UP
     void* ctr = nullptr;   // work-queue head, shift of the potential, partial (min, max) of V
@@ -429,6 +432,23 @@ int gint_fold_k(gint_ctx* ctx, const double* H_dev, const double* kfrac, double*
     if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
     cudaError_t e = gint::launch_fold(ctx->fold, H_dev, kfrac, Hk_dev, reinterpret_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, "gint_fold_k launch");
+    return GINT_OK;
+}
+
+int64_t gint_fold_k_static_max_blocks(void) { return gint::kFoldStaticMaxBlocks; }
+
+int gint_fold_k_static(gint_ctx* ctx, const double* H_dev, const double* kfrac, double* Hk_dev, void* stream) {
+    if (!ctx || !H_dev || !kfrac || !Hk_dev) return fail(GINT_EINVAL, "null argument");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    if (ctx->fold.nblk > gint::kFoldStaticMaxBlocks)
+        return fail(GINT_EUNSUPPORTED, "gint_fold_k_static: " + std::to_string(ctx->fold.nblk) + " blocks exceed the fixed scratch of " +
+                                           std::to_string(gint::kFoldStaticMaxBlocks) + " blocks; use gint_fold_k");
+    if (!ctx->fold_static_phase) return fail(GINT_ECUDA, "gint_fold_k_static: the fixed scratch was not resolved at set-up");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
+    cudaError_t e = gint::launch_fold_static(ctx->fold, ctx->fold_static_phase, H_dev, kfrac, Hk_dev,
+                                             reinterpret_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "gint_fold_k_static launch");
     return GINT_OK;
 }
 

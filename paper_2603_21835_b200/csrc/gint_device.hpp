@@ -86,6 +86,11 @@ cudaError_t launch_psi(const DevicePlan& P, size_t psi_smem, bool tab_smem, int 
 cudaError_t launch_rho(const DevicePlan& P, size_t psi_smem, size_t contract_smem_bytes, bool tab_smem, int nsm,
                        const BatchRange* batches, int nbatch, const double* D, double* rho, cudaStream_t stream);
 cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac, double* Hk, cudaStream_t stream);
+// gint_fold_k_static: phases in a file-scope device array of kFoldStaticMaxBlocks entries (gint_fold.cu)
+constexpr int kFoldStaticMaxBlocks = 1 << 18;
+cudaError_t fold_static_scratch(int device, double2** out);   // `device` must be current; address cached per device
+cudaError_t launch_fold_static(const FoldPlan& F, double2* static_phase, const double* H, const double* kfrac, double* Hk,
+                               cudaStream_t stream);
 
 size_t psi_kernel_smem(size_t table_bytes, int nspecies);
 size_t contract_kernel_smem(int nring);

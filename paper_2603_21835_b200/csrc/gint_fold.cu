@@ -11,6 +11,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <mutex>
 
 #include "gint_device.hpp"
 
@@ -83,6 +84,44 @@ cudaError_t launch_fold(const FoldPlan& F, const double* H, const double* kfrac,
     const dim3 grid((unsigned)((F.norb_tot + kFoldCols * 256 - 1) / (kFoldCols * 256)), (unsigned)F.natom);
     gint_fold_kernel<<<grid, 256, 0, stream>>>(F, H, reinterpret_cast<double2*>(Hk));
     return cudaGetLastError();
+}
+
+// ---- gint_fold_k_static: the same two kernels with the phase scratch in a file-scope array ---------------------
+// For callers that may not allocate (CUDA graph capture, serving loops): the phases exp(2 pi i kfrac . R) go to a fixed
+// array that every GPU loading the library holds until exit (kFoldStaticMaxBlocks x 16 bytes = 4 MiB) instead of the
+// context's own buffer.  In host code the array's name is only a stand-in; its device address comes from
+// cudaGetSymbolAddress, once per device with that device current (fold_static_scratch, called by the set-up), and is
+// handed to the kernels in FoldPlan::phase.  Nothing has to start at zero: gint_fold_phase_kernel rewrites entries
+// 0 .. nblk-1 before gint_fold_kernel reads them on the same stream.  All contexts of a device share the array, so
+// calls that overlap on the GPU (two streams, two contexts) race on it.
+static __device__ __align__(256) double2 g_fold_static_phase[kFoldStaticMaxBlocks];
+
+cudaError_t fold_static_scratch(int device, double2** out) {
+    constexpr int kMaxDevices = 64;
+    static std::mutex mu;
+    static double2* addr[kMaxDevices] = {};
+    *out = nullptr;
+    int current = -1;
+    cudaError_t e = cudaGetDevice(&current);
+    if (e != cudaSuccess) return e;
+    if (device < 0 || device >= kMaxDevices || current != device) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[device]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_fold_static_phase);
+        if (e != cudaSuccess) return e;
+        addr[device] = reinterpret_cast<double2*>(p);
+    }
+    *out = addr[device];
+    return cudaSuccess;
+}
+
+cudaError_t launch_fold_static(const FoldPlan& F, double2* static_phase, const double* H, const double* kfrac, double* Hk,
+                               cudaStream_t stream) {
+    if (!static_phase || F.nblk > kFoldStaticMaxBlocks) return cudaErrorInvalidValue;
+    FoldPlan G = F;
+    G.phase = static_phase;
+    return launch_fold(G, H, kfrac, Hk, stream);
 }
 
 }  // namespace gint
