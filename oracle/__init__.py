@@ -1,4 +1,4 @@
-"""CPU oracle for gint_vlocal / gint_rho / gint_fvl / gint_fold_k -- TEST INFRASTRUCTURE ONLY.
+"""CPU oracle for gint_vlocal / gint_rho / gint_fvl / gint_fold_k / gint_snap_psibeta -- TEST INFRASTRUCTURE ONLY.
 
 Thin ctypes binding of oracle/gint_oracle.c (which holds all the arithmetic and
 cites the paper).  Only tests/, __graft_entry__.smoke() and bench.py's
@@ -232,3 +232,80 @@ def fvl(lattice, ngrid, species, atom_species, atom_pos, V, D_flat, blocks, nthr
     if rc < 0:
         raise RuntimeError("orc_fvl failed: %d" % rc)
     return F
+
+
+# ---- spherical-grid integration of the velocity-gauge nonlocal overlaps (Sec. 3.3.2, Eq. 47) ------
+def enumerate_snap_pairs(lattice, species, proj, atom_species, atom_pos):
+    """Every (I, J, R): projectors of atom I (cutoff rb_I) against orbitals of the image of atom J at tau_J + R
+    (cutoff rc_J) with |tau_J + R - tau_I| < rb_I + rc_J (strict), sorted by (I, J, R1, R2, R3); species without
+    projectors (no radial function) host none.  Brute force over a box of images.  Returns (iat, jat, R[n][3],
+    offset[n+1]); block b holds n_J x m_I complex numbers, n_J orbitals of J (rows), m_I projector components of I."""
+    lat = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
+    pos = np.asarray(atom_pos, dtype=np.float64).reshape(-1, 3)
+    asp = np.asarray(atom_species).reshape(-1)
+    rmax = max(float(p.rcut) for p in proj) + max(float(s.rcut) for s in species)
+    inv = np.linalg.inv(lat)
+    heights = 1.0 / np.linalg.norm(inv, axis=0)          # distance between lattice planes along each axis
+    frac = pos @ inv
+    span = frac.max(axis=0) - frac.min(axis=0)
+    nmax = [int(np.ceil(rmax / heights[k] + span[k])) + 1 for k in range(3)]
+    out = []
+    for I in range(pos.shape[0]):
+        if np.asarray(proj[asp[I]].l).shape[0] == 0:
+            continue
+        for J in range(pos.shape[0]):
+            cut = float(proj[asp[I]].rcut) + float(species[asp[J]].rcut)
+            for r1 in range(-nmax[0], nmax[0] + 1):
+                for r2 in range(-nmax[1], nmax[1] + 1):
+                    for r3 in range(-nmax[2], nmax[2] + 1):
+                        d = pos[J] + r1 * lat[0] + r2 * lat[1] + r3 * lat[2] - pos[I]
+                        if float(d @ d) < cut * cut:
+                            out.append((I, J, r1, r2, r3))
+    out.sort()
+    arr = np.array(out, dtype=np.int64).reshape(-1, 5)
+    norb = np.array([int(np.sum(2 * np.asarray(s.l) + 1)) for s in species], dtype=np.int64)
+    mproj = np.array([int(np.sum(2 * np.asarray(p.l) + 1)) for p in proj], dtype=np.int64)
+    sizes = norb[asp[arr[:, 1]]] * mproj[asp[arr[:, 0]]] if len(out) else np.zeros(0, dtype=np.int64)
+    off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    return (arr[:, 0].astype(np.int32), arr[:, 1].astype(np.int32), np.ascontiguousarray(arr[:, 2:5].astype(np.int32)), off)
+
+
+def snap_psibeta(lattice, species, proj, atom_species, atom_pos, A, rad_x, rad_w, ang_n, ang_w, pairs=None):
+    """S(I, J, R)[mu][b] = < phi_mu(r - tau_J - R) | exp(-i A.r) | beta_b(r - tau_I) >     (Eq. 47)
+
+    by quadrature on a grid centred on the projector's atom, as the paper states it: radial nodes
+    r_i = rad_x[i] * rb_I with weights rad_w[i] * rb_I (Gauss-Legendre on [0, rb_I]), angular nodes ang_n[a] with
+    weights ang_w[a] (Lebedev-Laikov, sum 4 pi):
+
+        S = sum_i sum_a  rad_w_i rb r_i^2  ang_w_a  phi_mu(tau_I + r_i n_a - tau_J - R)
+                         exp(-i A . (tau_I + r_i n_a))  beta_b(r_i n_a)
+
+    phi real (so the bra needs no conjugate), r the absolute Cartesian position with the atoms where the caller put
+    them, beta_{l m zeta}(r) = b_{l zeta}(|r|) Y_lm(r/|r|) with the same table interpolation and real Y_lm as the
+    orbitals (orc_phi evaluates both).  Straight nested sums, one pair at a time; complex128.
+    Returns (S_flat complex128[offset[-1]], pairs)."""
+    lat = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
+    pos = np.asarray(atom_pos, dtype=np.float64).reshape(-1, 3)
+    asp = np.asarray(atom_species).reshape(-1)
+    A = np.asarray(A, dtype=np.float64).reshape(3)
+    rad_x = np.asarray(rad_x, dtype=np.float64)
+    rad_w = np.asarray(rad_w, dtype=np.float64)
+    ang_n = np.asarray(ang_n, dtype=np.float64).reshape(-1, 3)
+    ang_w = np.asarray(ang_w, dtype=np.float64)
+    if pairs is None:
+        pairs = enumerate_snap_pairs(lat, species, proj, asp, pos)
+    iat, jat, R, off = pairs
+    S = np.zeros(int(off[-1]), dtype=np.complex128)
+    for b in range(len(iat)):
+        I, J = int(iat[b]), int(jat[b])
+        rb = float(proj[asp[I]].rcut)
+        r = rad_x * rb                                                   # [nr]
+        pts = (r[:, None, None] * ang_n[None, :, :]).reshape(-1, 3)      # [nr * na][3], relative to tau_I
+        wq = ((rad_w * rb * r * r)[:, None] * ang_w[None, :]).reshape(-1)
+        beta = phi(proj, int(asp[I]), pts)                               # [npts][m_I]
+        centre = pos[J] + R[b, 0] * lat[0] + R[b, 1] * lat[1] + R[b, 2] * lat[2]
+        ph = phi(species, int(asp[J]), pts + (pos[I] - centre))          # [npts][n_J]
+        phase = np.exp(-1j * ((pts + pos[I]) @ A))
+        blk = ph.T @ ((wq * phase)[:, None] * beta)                      # [n_J][m_I]
+        S[off[b]:off[b + 1]] = blk.reshape(-1)
+    return S, pairs

@@ -148,6 +148,34 @@ def species_2s1p(name: str, rcut: float, a1: float, a2: float) -> Species:
 
 
 # ----------------------------------------------------------------------------
+# nonlocal projectors and atom-centred quadrature tables (gint_snap_psibeta)
+# ----------------------------------------------------------------------------
+def projector_species(name: str = "Si-beta", rcut: float = 3.0) -> Species:
+    """Projector functions beta_{l zeta} of a norm-conserving pseudopotential, tabulated like the orbitals: two s and
+    two p projectors (8 components), localised within `rcut` of the nucleus (the paper's projectors are "extremely
+    localised around atomic cores").  No real pseudopotential file is available offline; the shapes stand in."""
+    return make_species(name, rcut, [(0, 1.2), (0, 2.5), (1, 1.0), (1, 2.0)])
+
+
+def radial_quadrature(n: int = 140):
+    """n-point Gauss-Legendre rule mapped to the unit interval: nodes x in (0, 1) and weights with sum 1 (the paper's
+    140-point radial grid; the caller scales by the projector cutoff).  Library routine, no arithmetic
+    of the method."""
+    x, w = np.polynomial.legendre.leggauss(int(n))
+    return np.ascontiguousarray(0.5 * (x + 1.0)), np.ascontiguousarray(0.5 * w)
+
+
+def angular_quadrature(npts: int = 110):
+    """Lebedev-Laikov rule on the unit sphere: unit vectors [npts][3] and weights with sum 4 pi (110 points = order 17,
+    PAPER.md:424).  Taken from scipy's table."""
+    from scipy.integrate import lebedev_rule
+    order = {6: 3, 14: 5, 26: 7, 38: 9, 50: 11, 74: 13, 86: 15, 110: 17, 146: 19, 170: 21, 194: 23, 230: 25, 266: 27,
+             302: 29, 350: 31, 434: 35, 590: 41}[int(npts)]
+    x, w = lebedev_rule(order)
+    return np.ascontiguousarray(x.T), np.ascontiguousarray(w)
+
+
+# ----------------------------------------------------------------------------
 # potentials (orthorhombic cells only -- all BASELINE configs are cubic)
 # ----------------------------------------------------------------------------
 def _periodic_gauss_1d(n: int, length: float, centre: np.ndarray, sigma2: float, reach: float) -> np.ndarray:
