@@ -191,6 +191,41 @@ int gint_fold_k(gint_ctx *ctx, const double *H_dev, const double *kfrac, double 
 int64_t gint_fold_k_static_max_blocks(void);
 int gint_fold_k_static(gint_ctx *ctx, const double *H_dev, const double *kfrac, double *Hk_dev, void *stream);
 
+/* Spherical-grid integration of the velocity-gauge nonlocal overlaps (the paper's snap_psibeta, independent of the
+ * uniform mesh) -- PAPER.md:415-426 (Sec. 3.3.2, Eq. 47):
+ *
+ *   S(I, J, R)[mu][b] = < phi_mu(r - tau_J - R) | exp(-i A.r) | beta_b(r - tau_I) >
+ *     = sum_i sum_a  rad_w[i] rb r_i^2  ang_w[a]  phi_mu(tau_I + r_i n_a - tau_J - R)
+ *                    exp(-i A.(tau_I + r_i n_a))  beta_b(r_i n_a),       r_i = rad_x[i] rb,  n_a = ang_xyz[a]
+ *
+ * for every atom I whose species has projectors and every orbital-carrying image (J, R) with
+ * |tau_J + R - tau_I| < rb_I + rc_J (strict).  Readings of the paper: r is the absolute Cartesian position with the
+ * atoms where the caller put them (never wrapped); phi is real, so the bra needs no conjugate; a projector
+ * beta_{l m zeta}(r) = b_{l zeta}(|r|) Y_lm(r/|r|) is tabulated and interpolated exactly like an orbital (same
+ * stencil, cutoff rule, r -> 0 rule and real Y_lm as above); the quadrature is centred on atom I, radial nodes from a
+ * rule on (0, 1) scaled by the projector cutoff rb of I's species (the paper: 140-point Gauss-Legendre), angular
+ * nodes on the unit sphere with weights summing to 4 pi (the paper: 110-point Lebedev-Laikov).  The tables are the
+ * caller's: the library does not generate quadrature rules.
+ *
+ * gint_snap_setup   proj[nspecies]: the projectors of each species in the gint_species layout (nrad = 0: the species
+ *                   hosts none; nrad <= 8, l <= 3, at most 16 components per species; at most 32 orbitals per atom on
+ *                   the orbital side: GINT_EUNSUPPORTED beyond); rad_x[nrad_pts], rad_w[nrad_pts], ang_xyz[nang][3],
+ *                   ang_w[nang]: HOST arrays, copied.  Builds the pair list for the context's current positions and
+ *                   uploads the tables; may be called again (new projectors or rules).  gint_update_positions
+ *                   discards the pair list: call gint_snap_setup again afterwards.
+ * gint_snap_num_pairs / gint_snap_get_pairs   the pairs sorted by (I, J, R1, R2, R3): iat[n], jat[n], R[n][3],
+ *                   offset[n+1] in COMPLEX elements; block b is [n_J][m_I] row-major (rows: orbitals of J in block
+ *                   order, columns: projector components of I, radial functions in the order given, m = -l..l).
+ * gint_snap_psibeta A: HOST pointer, 3 doubles (bohr^-1); S_dev: device pointer, 2 s_len doubles, interleaved
+ *                   (re, im); OVERWRITTEN, every element written once.  Asynchronous on `stream`, one kernel (one
+ *                   CTA per pair, the sum over points on the FP64 tensor pipe), no atomics: results are bit-wise
+ *                   reproducible.  Allocates nothing. */
+int gint_snap_setup(gint_ctx *ctx, const gint_species *proj, int32_t nrad_pts, const double *rad_x, const double *rad_w,
+                    int32_t nang, const double *ang_xyz, const double *ang_w);
+int gint_snap_num_pairs(const gint_ctx *ctx, int64_t *npair, int64_t *s_len);
+int gint_snap_get_pairs(const gint_ctx *ctx, int32_t *iat, int32_t *jat, int32_t *R, int64_t *offset);
+int gint_snap_psibeta(gint_ctx *ctx, const double *A, double *S_dev, void *stream);
+
 /* Per-kernel timing on the launch stream.  After gint_set_profiling(ctx, 1) every
  * gint_vlocal call records CUDA events around its kernels on `stream`;
  * gint_get_kernel_ms synchronises on the last call's events and returns durations in

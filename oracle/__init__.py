@@ -258,7 +258,8 @@ def enumerate_snap_pairs(lattice, species, proj, atom_species, atom_pos):
             for r1 in range(-nmax[0], nmax[0] + 1):
                 for r2 in range(-nmax[1], nmax[1] + 1):
                     for r3 in range(-nmax[2], nmax[2] + 1):
-                        d = pos[J] + r1 * lat[0] + r2 * lat[1] + r3 * lat[2] - pos[I]
+                        # (tau_J - tau_I) first: a self image sits at exactly |R|, so a tie with the cutoff stays a tie
+                        d = (pos[J] - pos[I]) + (r1 * lat[0] + r2 * lat[1] + r3 * lat[2])
                         if float(d @ d) < cut * cut:
                             out.append((I, J, r1, r2, r3))
     out.sort()

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgint_b200.so")
 GINT_OK, GINT_EINVAL, GINT_EUNSUPPORTED, GINT_ENOMEM, GINT_ECUDA, GINT_ENODEVICE = 0, -1, -2, -3, -4, -5
 
 EXPORTED = ("gint_setup", "gint_update_positions", "gint_num_blocks", "gint_get_blocks", "gint_vlocal", "gint_vlocal_host", "gint_get_stats",
-            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_fold_k_static", "gint_fold_k_static_max_blocks", "gint_rho", "gint_fvl", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
+            "gint_set_profiling", "gint_get_kernel_ms", "gint_num_orbitals", "gint_fold_k", "gint_fold_k_static", "gint_fold_k_static_max_blocks", "gint_snap_setup", "gint_snap_num_pairs", "gint_snap_get_pairs", "gint_snap_psibeta", "gint_rho", "gint_fvl", "gint_get_cell_lists", "gint_measure_fp64_peak", "gint_destroy", "gint_strerror", "gint_last_error")
 
 STAT_NAMES = ("cells", "items", "entries", "max_rows", "executed_flops", "flush_elems", "smem_bytes", "kernels_per_call",
               "F_pt", "F_sym", "insphere_pairs", "evaluated_pairs", "psi_scratch_bytes", "psi_load_bytes", "ring_stages",
@@ -70,6 +70,14 @@ def _load() -> ctypes.CDLL:
     lib.gint_fold_k_static.argtypes = [vp, vp, P(dbl), vp, vp]
     lib.gint_fold_k_static_max_blocks.restype = ctypes.c_int64
     lib.gint_fold_k_static_max_blocks.argtypes = []
+    lib.gint_snap_setup.restype = ctypes.c_int
+    lib.gint_snap_setup.argtypes = [vp, P(_Species), i32, P(dbl), P(dbl), i32, P(dbl), P(dbl)]
+    lib.gint_snap_num_pairs.restype = ctypes.c_int
+    lib.gint_snap_num_pairs.argtypes = [vp, P(i64), P(i64)]
+    lib.gint_snap_get_pairs.restype = ctypes.c_int
+    lib.gint_snap_get_pairs.argtypes = [vp, P(i32), P(i32), P(i32), P(i64)]
+    lib.gint_snap_psibeta.restype = ctypes.c_int
+    lib.gint_snap_psibeta.argtypes = [vp, P(dbl), vp, vp]
     lib.gint_rho.restype = ctypes.c_int
     lib.gint_rho.argtypes = [vp, vp, vp, vp]
     lib.gint_fvl.restype = ctypes.c_int
@@ -253,6 +261,45 @@ class GintContext:
                                        ctypes.c_void_p(Hk_dev.data_ptr()), ctypes.c_void_p(s)), "gint_fold_k_static")
         return Hk_dev
 
+    def gint_snap_setup(self, proj: Sequence, rad_x, rad_w, ang_xyz, ang_w):
+        """Projector tables (objects like the species; nrad = 0 allowed) and the quadrature tables of gint_snap_psibeta."""
+        arr, keep = _species_array(proj)
+        rx = np.ascontiguousarray(rad_x, dtype=np.float64).reshape(-1)
+        rw = np.ascontiguousarray(rad_w, dtype=np.float64).reshape(-1)
+        an = np.ascontiguousarray(ang_xyz, dtype=np.float64).reshape(-1, 3)
+        aw = np.ascontiguousarray(ang_w, dtype=np.float64).reshape(-1)
+        if rx.shape != rw.shape or an.shape[0] != aw.shape[0]:
+            raise ValueError("quadrature nodes and weights disagree in length")
+        _check(_lib.gint_snap_setup(self._h, arr, int(rx.shape[0]), _ptr(rx, ctypes.c_double), _ptr(rw, ctypes.c_double),
+                                    int(aw.shape[0]), _ptr(an, ctypes.c_double), _ptr(aw, ctypes.c_double)), "gint_snap_setup")
+        del keep
+
+    def gint_snap_get_pairs(self):
+        """(iat[n], jat[n], R[n][3], offset[n+1]) of the (I, J, R) pairs; offsets in complex elements."""
+        n, slen = ctypes.c_int64(), ctypes.c_int64()
+        _check(_lib.gint_snap_num_pairs(self._h, ctypes.byref(n), ctypes.byref(slen)), "gint_snap_num_pairs")
+        n = int(n.value)
+        iat = np.zeros(n, dtype=np.int32); jat = np.zeros(n, dtype=np.int32)
+        R = np.zeros((n, 3), dtype=np.int32); off = np.zeros(n + 1, dtype=np.int64)
+        _check(_lib.gint_snap_get_pairs(self._h, _ptr(iat, ctypes.c_int32), _ptr(jat, ctypes.c_int32), _ptr(R, ctypes.c_int32),
+                                        _ptr(off, ctypes.c_int64)), "gint_snap_get_pairs")
+        return iat, jat, R, off
+
+    def gint_snap_psibeta(self, A, S_dev=None, stream=None):
+        """S = <phi| exp(-i A.r) |beta> of every pair (Eq. 47); returns a CUDA complex128 tensor of s_len elements."""
+        import torch
+        slen = ctypes.c_int64()
+        _check(_lib.gint_snap_num_pairs(self._h, None, ctypes.byref(slen)), "gint_snap_num_pairs")
+        if S_dev is None:
+            S_dev = torch.empty(int(slen.value), dtype=torch.complex128, device="cuda")
+        if not (S_dev.is_cuda and S_dev.dtype == torch.complex128 and S_dev.is_contiguous() and S_dev.numel() == int(slen.value)):
+            raise ValueError("S_dev must be a contiguous CUDA complex128 tensor of s_len elements")
+        a = np.ascontiguousarray(A, dtype=np.float64).reshape(3)
+        s = torch.cuda.current_stream(S_dev.device).cuda_stream if stream is None else int(stream)
+        _check(_lib.gint_snap_psibeta(self._h, _ptr(a, ctypes.c_double), ctypes.c_void_p(S_dev.data_ptr()), ctypes.c_void_p(s)),
+               "gint_snap_psibeta")
+        return S_dev
+
     def gint_vlocal_host(self, V_host: np.ndarray, H_host: Optional[np.ndarray] = None) -> np.ndarray:
         """End-to-end call with HOST buffers (H2D of V, kernels, D2H of H, synchronise)."""
         V_host = np.ascontiguousarray(V_host, dtype=np.float64)
@@ -276,15 +323,8 @@ class GintContext:
             pass
 
 
-def gint_setup(lattice, ngrid, species: Sequence, atom_species, atom_pos, cuda_device: int = 0,
-               bcell=(0, 0, 0), rank: int = 0, nranks: int = 1, scratch_max_bytes: int = 0) -> GintContext:
-    """species: objects with .rcut .dr .l[nrad] .table[nrad][ntab].  cuda_device < 0: host-only context."""
-    lattice = np.ascontiguousarray(lattice, dtype=np.float64).reshape(9)
-    ng = np.ascontiguousarray(ngrid, dtype=np.int32).reshape(3)
-    pos = np.ascontiguousarray(atom_pos, dtype=np.float64).reshape(-1, 3)
-    asp = np.ascontiguousarray(atom_species, dtype=np.int32).reshape(-1)
-    if asp.shape[0] != pos.shape[0]:
-        raise ValueError("atom_species and atom_pos disagree on natom")
+def _species_array(species: Sequence):
+    """ctypes array of gint_species for objects with .rcut .dr .l[nrad] .table[nrad][ntab] (+ the arrays to keep alive)."""
     keep = []
     arr = (_Species * len(species))()
     for i, s in enumerate(species):
@@ -296,6 +336,19 @@ def gint_setup(lattice, ngrid, species: Sequence, atom_species, atom_pos, cuda_d
         arr[i].rcut, arr[i].dr = float(s.rcut), float(s.dr)
         arr[i].ntab, arr[i].nrad = int(tab.shape[1]), int(l.shape[0])
         arr[i].l, arr[i].table = _ptr(l, ctypes.c_int32), _ptr(tab, ctypes.c_double)
+    return arr, keep
+
+
+def gint_setup(lattice, ngrid, species: Sequence, atom_species, atom_pos, cuda_device: int = 0,
+               bcell=(0, 0, 0), rank: int = 0, nranks: int = 1, scratch_max_bytes: int = 0) -> GintContext:
+    """species: objects with .rcut .dr .l[nrad] .table[nrad][ntab].  cuda_device < 0: host-only context."""
+    lattice = np.ascontiguousarray(lattice, dtype=np.float64).reshape(9)
+    ng = np.ascontiguousarray(ngrid, dtype=np.int32).reshape(3)
+    pos = np.ascontiguousarray(atom_pos, dtype=np.float64).reshape(-1, 3)
+    asp = np.ascontiguousarray(atom_species, dtype=np.int32).reshape(-1)
+    if asp.shape[0] != pos.shape[0]:
+        raise ValueError("atom_species and atom_pos disagree on natom")
+    arr, keep = _species_array(species)
     opt = _Options()
     for d in range(3):
         opt.bcell[d] = int(bcell[d])

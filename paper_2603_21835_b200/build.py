@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgint_b200.so")
-SOURCES = ["gint_api.cu", "gint_kernels.cu", "gint_fold.cu", "gint_fvl.cu", "gint_plan.cpp"]
+SOURCES = ["gint_api.cu", "gint_kernels.cu", "gint_fold.cu", "gint_fvl.cu", "gint_snap.cu", "gint_plan.cpp"]
 HEADERS = ["gint_device.hpp", "gint_plan.hpp", "gint_kstep_dispatch.inc", os.path.join("..", "..", "include", "gint.h")]
 
 

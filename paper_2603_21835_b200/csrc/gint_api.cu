@@ -1,6 +1,8 @@
 // gint_api.cu -- extern "C" boundary of libgint_b200.so (declared in include/gint.h).
 #include <cuda_runtime.h>
 
+#include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -31,6 +33,12 @@ struct gint_ctx {
     gint::FvlPlan fvl{};           // built at the first gint_fvl call
     bool have_fvl = false;
     size_t force_smem = 0;
+    gint::SnapPlan snap{};         // gint_snap_setup
+    bool have_snap = false;
+    int snap_fr = 2, snap_fc = 2;
+    std::vector<void*> snap_allocs;
+    std::vector<int32_t> snap_iat, snap_jat, snap_R;
+    std::vector<int64_t> snap_off;
     double* V_scratch = nullptr;   // gint_vlocal_host only
     double* H_scratch = nullptr;
 };
@@ -79,6 +87,7 @@ void release(gint_ctx* ctx) {
     if (ctx->device >= 0) {
         DeviceGuard guard(ctx->device);
         for (void* p : ctx->allocs) cudaFree(p);
+        for (void* p : ctx->snap_allocs) cudaFree(p);
         if (ctx->have_events)
             for (int i = 0; i < 5; i++) cudaEventDestroy(ctx->ev[i]);
         if (ctx->V_scratch) cudaFree(ctx->V_scratch);
@@ -224,6 +233,29 @@ void device_release_arrays(gint_ctx* ctx) {
     if (ctx->H_scratch) { cudaFree(ctx->H_scratch); ctx->H_scratch = nullptr; }
 }
 
+void snap_release(gint_ctx* ctx) {
+    if (ctx->device >= 0 && !ctx->snap_allocs.empty()) {
+        DeviceGuard guard(ctx->device);
+        for (void* p : ctx->snap_allocs) cudaFree(p);
+    }
+    ctx->snap_allocs.clear();
+    ctx->snap = gint::SnapPlan{};
+    ctx->have_snap = false;
+    ctx->snap_iat.clear(); ctx->snap_jat.clear(); ctx->snap_R.clear(); ctx->snap_off.clear();
+}
+
+template <typename T>
+cudaError_t snap_upload(gint_ctx* ctx, const std::vector<T>& host, const T** dev_out) {
+    void* p = nullptr;
+    const size_t bytes = host.size() * sizeof(T);
+    cudaError_t e = cudaMalloc(&p, bytes ? bytes : 16);
+    if (e != cudaSuccess) return e;
+    ctx->snap_allocs.push_back(p);
+    if (bytes) e = cudaMemcpy(p, host.data(), bytes, cudaMemcpyHostToDevice);
+    *dev_out = reinterpret_cast<const T*>(p);
+    return e;
+}
+
 }  // namespace
 
 extern "C" {
@@ -312,6 +344,7 @@ int gint_update_positions(gint_ctx* ctx, const double* atom_pos) {
         cudaDeviceSynchronize();   // calls in flight still read the old tables
     }
     device_release_arrays(ctx);
+    snap_release(ctx);   // pair list of the old geometry: gint_snap_setup has to be called again
     return device_init(ctx);
 }
 
@@ -449,6 +482,147 @@ int gint_fold_k_static(gint_ctx* ctx, const double* H_dev, const double* kfrac, 
     cudaError_t e = gint::launch_fold_static(ctx->fold, ctx->fold_static_phase, H_dev, kfrac, Hk_dev,
                                              reinterpret_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, "gint_fold_k_static launch");
+    return GINT_OK;
+}
+
+int gint_snap_setup(gint_ctx* ctx, const gint_species* proj, int32_t nrad_pts, const double* rad_x, const double* rad_w,
+                    int32_t nang, const double* ang_xyz, const double* ang_w) {
+    if (!ctx || !proj || !rad_x || !rad_w || !ang_xyz || !ang_w) return fail(GINT_EINVAL, "null argument");
+    if (nrad_pts <= 0 || nang <= 0) return fail(GINT_EINVAL, "empty quadrature table");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    const gint::Plan& P = ctx->plan;
+    const int nsp = (int)P.species.size(), natom = (int)P.atom_species.size();
+    try {
+        std::vector<gint::SnapSpecies> orb((size_t)nsp), prj((size_t)nsp);
+        std::vector<double> tab;
+        int max_n = 0, max_m = 0;
+        for (int s = 0; s < nsp; s++) {
+            const gint::SpeciesHost& h = P.species[(size_t)s];
+            gint::SnapSpecies& o = orb[(size_t)s];
+            std::memset(&o, 0, sizeof(o));
+            o.tab_off = (int32_t)tab.size(); o.ntab = h.ntab; o.nrad = h.nrad; o.ncomp = h.norb;
+            for (int f = 0; f < h.nrad; f++) o.l[f] = h.l[(size_t)f];
+            o.rcut = h.rcut; o.inv_dr = 1.0 / h.dr;
+            tab.insert(tab.end(), h.table.begin(), h.table.end());
+            max_n = std::max(max_n, h.norb);
+            const gint_species& q = proj[s];
+            gint::SnapSpecies& b = prj[(size_t)s];
+            std::memset(&b, 0, sizeof(b));
+            if (q.nrad < 0 || q.nrad > 8) return fail(GINT_EUNSUPPORTED, "more than 8 projector radial functions per species");
+            if (q.nrad == 0) continue;   // this species hosts no projectors
+            if (!q.l || !q.table || !(q.rcut > 0) || !(q.dr > 0)) return fail(GINT_EINVAL, "bad projector species");
+            if ((double)q.ntab * q.dr < q.rcut + 3.0 * q.dr - 1e-9) return fail(GINT_EINVAL, "projector table too short for rcut + 3 dr");
+            b.tab_off = (int32_t)tab.size(); b.ntab = q.ntab; b.nrad = q.nrad;
+            for (int f = 0; f < q.nrad; f++) {
+                if (q.l[f] < 0 || q.l[f] > 3) return fail(GINT_EUNSUPPORTED, "projector l > 3");
+                b.l[f] = q.l[f];
+                b.ncomp += 2 * q.l[f] + 1;
+            }
+            b.rcut = q.rcut; b.inv_dr = 1.0 / q.dr;
+            tab.insert(tab.end(), q.table, q.table + (size_t)q.nrad * q.ntab);
+            max_m = std::max(max_m, b.ncomp);
+        }
+        if (max_n > 32) return fail(GINT_EUNSUPPORTED, "gint_snap: more than 32 orbitals per atom");
+        if (max_m > 16) return fail(GINT_EUNSUPPORTED, "gint_snap: more than 16 projector components per atom");
+        // pair list: every (I, J, R) with |tau_J + R - tau_I| < rb_I + rc_J, in (I, J, R1, R2, R3) order
+        const double* a = P.lattice;
+        const double c0[3] = {a[4] * a[8] - a[5] * a[7], a[5] * a[6] - a[3] * a[8], a[3] * a[7] - a[4] * a[6]};   // a2 x a3
+        const double c1[3] = {a[7] * a[2] - a[8] * a[1], a[8] * a[0] - a[6] * a[2], a[6] * a[1] - a[7] * a[0]};   // a3 x a1
+        const double c2[3] = {a[1] * a[5] - a[2] * a[4], a[2] * a[3] - a[0] * a[5], a[0] * a[4] - a[1] * a[3]};   // a1 x a2
+        const double vol = a[0] * c0[0] + a[1] * c0[1] + a[2] * c0[2];
+        const double* cr[3] = {c0, c1, c2};
+        double height[3];
+        for (int k = 0; k < 3; k++) height[k] = std::fabs(vol) / std::sqrt(cr[k][0] * cr[k][0] + cr[k][1] * cr[k][1] + cr[k][2] * cr[k][2]);
+        std::vector<gint::SnapPair> pairs;
+        snap_release(ctx);
+        int64_t off = 0;
+        for (int I = 0; I < natom; I++) {
+            const gint::SnapSpecies& b = prj[(size_t)P.atom_species[(size_t)I]];
+            if (b.nrad == 0) continue;
+            const double* tI = &P.atom_pos[3 * (size_t)I];
+            for (int J = 0; J < natom; J++) {
+                const gint::SnapSpecies& o = orb[(size_t)P.atom_species[(size_t)J]];
+                const double* tJ = &P.atom_pos[3 * (size_t)J];
+                const double cut = b.rcut + o.rcut;
+                const double dx = tJ[0] - tI[0], dy = tJ[1] - tI[1], dz = tJ[2] - tI[2];
+                int lo[3], hi[3];
+                for (int k = 0; k < 3; k++) {   // fractional coordinate of tau_J - tau_I along a_k, plus the reach of the cutoff
+                    const double f = (dx * cr[k][0] + dy * cr[k][1] + dz * cr[k][2]) / vol;
+                    lo[k] = (int)std::floor(-f - cut / height[k]) - 1;
+                    hi[k] = (int)std::ceil(-f + cut / height[k]) + 1;
+                }
+                for (int r1 = lo[0]; r1 <= hi[0]; r1++)
+                    for (int r2 = lo[1]; r2 <= hi[1]; r2++)
+                        for (int r3 = lo[2]; r3 <= hi[2]; r3++) {
+                            const double ex = dx + r1 * a[0] + r2 * a[3] + r3 * a[6];
+                            const double ey = dy + r1 * a[1] + r2 * a[4] + r3 * a[7];
+                            const double ez = dz + r1 * a[2] + r2 * a[5] + r3 * a[8];
+                            if (!(ex * ex + ey * ey + ez * ez < cut * cut)) continue;
+                            gint::SnapPair pr;
+                            pr.d[0] = -ex; pr.d[1] = -ey; pr.d[2] = -ez;
+                            pr.tauI[0] = tI[0]; pr.tauI[1] = tI[1]; pr.tauI[2] = tI[2];
+                            pr.off = off;
+                            pr.spI = P.atom_species[(size_t)I]; pr.spJ = P.atom_species[(size_t)J];
+                            pairs.push_back(pr);
+                            ctx->snap_iat.push_back(I); ctx->snap_jat.push_back(J);
+                            ctx->snap_R.push_back(r1); ctx->snap_R.push_back(r2); ctx->snap_R.push_back(r3);
+                            ctx->snap_off.push_back(off);
+                            off += (int64_t)o.ncomp * b.ncomp;
+                        }
+            }
+        }
+        ctx->snap_off.push_back(off);
+        if (pairs.size() > 0x7FFFFFFFull) return fail(GINT_EUNSUPPORTED, "gint_snap: too many pairs");
+        DeviceGuard guard(ctx->device);
+        if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
+        cudaError_t e;
+        gint::SnapPlan& S = ctx->snap;
+        const std::vector<double> rx(rad_x, rad_x + nrad_pts), rw(rad_w, rad_w + nrad_pts), an(ang_xyz, ang_xyz + 3 * (size_t)nang),
+            aw(ang_w, ang_w + nang);
+        if ((e = snap_upload(ctx, orb, &S.orb)) != cudaSuccess || (e = snap_upload(ctx, prj, &S.proj)) != cudaSuccess ||
+            (e = snap_upload(ctx, tab, &S.tab)) != cudaSuccess || (e = snap_upload(ctx, pairs, &S.pairs)) != cudaSuccess ||
+            (e = snap_upload(ctx, rx, &S.rad_x)) != cudaSuccess || (e = snap_upload(ctx, rw, &S.rad_w)) != cudaSuccess ||
+            (e = snap_upload(ctx, an, &S.ang_xyz)) != cudaSuccess || (e = snap_upload(ctx, aw, &S.ang_w)) != cudaSuccess) {
+            snap_release(ctx);
+            return fail_cuda(e, "gint_snap_setup upload");
+        }
+        S.npair = (int32_t)pairs.size(); S.nrad = nrad_pts; S.nang = nang;
+        ctx->snap_fr = (max_n + 7) / 8; ctx->snap_fc = (2 * max_m + 7) / 8;
+        ctx->have_snap = true;
+    } catch (const std::bad_alloc&) {
+        snap_release(ctx);
+        return fail(GINT_ENOMEM, "host allocation failed");
+    }
+    return GINT_OK;
+}
+
+int gint_snap_num_pairs(const gint_ctx* ctx, int64_t* npair, int64_t* s_len) {
+    if (!ctx) return fail(GINT_EINVAL, "ctx is null");
+    if (!ctx->have_snap) return fail(GINT_EINVAL, "gint_snap_setup has not been called (or the positions changed since)");
+    if (npair) *npair = (int64_t)ctx->snap_iat.size();
+    if (s_len) *s_len = ctx->snap_off.back();
+    return GINT_OK;
+}
+
+int gint_snap_get_pairs(const gint_ctx* ctx, int32_t* iat, int32_t* jat, int32_t* R, int64_t* offset) {
+    if (!ctx) return fail(GINT_EINVAL, "ctx is null");
+    if (!ctx->have_snap) return fail(GINT_EINVAL, "gint_snap_setup has not been called (or the positions changed since)");
+    const size_t n = ctx->snap_iat.size();
+    if (iat && n) std::memcpy(iat, ctx->snap_iat.data(), n * sizeof(int32_t));
+    if (jat && n) std::memcpy(jat, ctx->snap_jat.data(), n * sizeof(int32_t));
+    if (R && n) std::memcpy(R, ctx->snap_R.data(), 3 * n * sizeof(int32_t));
+    if (offset) std::memcpy(offset, ctx->snap_off.data(), (n + 1) * sizeof(int64_t));
+    return GINT_OK;
+}
+
+int gint_snap_psibeta(gint_ctx* ctx, const double* A, double* S_dev, void* stream) {
+    if (!ctx || !A || !S_dev) return fail(GINT_EINVAL, "null argument");
+    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
+    if (!ctx->have_snap) return fail(GINT_EINVAL, "gint_snap_setup has not been called (or the positions changed since)");
+    DeviceGuard guard(ctx->device);
+    if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
+    cudaError_t e = gint::launch_snap(ctx->snap, ctx->snap_fr, ctx->snap_fc, A, S_dev, reinterpret_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "gint_snap_psibeta launch");
     return GINT_OK;
 }
 

@@ -73,6 +73,31 @@ struct FvlPlan {
     double* tscratch;          // T = E Phi, psi chunk layout (same chunk indices as the psi scratch)
     int32_t ntg, nks_pad;
 };
+// spherical-grid overlaps < phi | exp(-i A.r) | beta > (gint_snap.cu)
+struct SnapSpecies {           // orbitals of a species, or its projectors: plain tables [nrad][ntab] at tab + tab_off
+    int32_t tab_off, ntab, nrad, ncomp;
+    int32_t l[8];
+    double rcut, inv_dr;
+};
+struct SnapPair {              // projectors of atom I against the orbitals of the image of atom J at tau_J + R
+    double d[3];               // tau_I - (tau_J + R)
+    double tauI[3];
+    int64_t off;               // first complex element of the block [n_J][m_I] in S
+    int32_t spI, spJ;
+};
+struct SnapPlan {
+    const SnapSpecies* orb;    // [nspecies]
+    const SnapSpecies* proj;   // [nspecies]
+    const double* tab;
+    const SnapPair* pairs;
+    const double* rad_x;       // [nrad] nodes on (0, 1)
+    const double* rad_w;       // [nrad] weights, sum 1
+    const double* ang_xyz;     // [nang][3] unit vectors
+    const double* ang_w;       // [nang] weights, sum 4 pi
+    int32_t npair, nrad, nang, pad;
+};
+cudaError_t launch_snap(const SnapPlan& P, int fr, int fc, const double* A, double* S, cudaStream_t stream);
+
 // The launchers walk the plan's batches (regions that share the psi scratch one after the other): nbatch entries of
 // (first item, items, first work region, work regions).
 struct BatchRange { int32_t item0, nitems, wr0, nwr; };

@@ -1,0 +1,204 @@
+// gint_snap.cu -- spherical-grid integration of the velocity-gauge nonlocal overlaps (the paper's snap_psibeta),
+// PAPER.md:415-426 (Sec. 3.3.2, Eq. 47):
+//
+//   S(I, J, R)[mu][b] = < phi_mu(r - tau_J - R) | exp(-i A.r) | beta_b(r - tau_I) >
+//                     = sum_i sum_a  w_i rb r_i^2  w_a  phi_mu(tau_I + r_i n_a - tau_J - R)
+//                                    exp(-i A.(tau_I + r_i n_a))  beta_b(r_i n_a),
+//
+// quadrature centred on the projector's atom: radial nodes r_i = x_i rb_I (Gauss-Legendre, 140 in the paper), angular
+// nodes n_a (Lebedev-Laikov, 110 in the paper), both tables given by the caller.  beta_{l m zeta} = b(|r|) Y_lm like an
+// orbital.  One CTA per (I, J, R) pair (the paper batches all neighbours of a central atom into one launch; here all
+// pairs of all atoms are one launch).  The 128 threads walk the nr x na quadrature points; a thread evaluates the n_J
+// orbitals and the m_I weighted, phase-modulated projector components of its point into its warp's staging tile in
+// shared memory, and the warp contracts 32 points at a time on the FP64 tensor pipe:
+//   C[mu][c] += sum_p Phi[p][mu] G[p][c],   G[p][2b] = Re, G[p][2b+1] = Im of  w_p beta_b(p) exp(-i A.r_p)
+// (DMMA.8x8x4, K = points).  No atomics: the four warps' partial C are added through shared memory in a fixed order
+// and every element of S is written once (the paper's kernel reduces with shuffles and shared memory for the same
+// reason).
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "gint_device.hpp"
+
+namespace gint {
+
+namespace {
+
+__device__ __forceinline__ void dmma_s(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// values of all components of a species (orbitals or projectors) at displacement (dx, dy, dz) from its centre, written
+// to out[0 .. ncomp-1]: cubic Lagrange interpolation on the forward stencil k .. k+3, k = floor(r / dr); zero for
+// r >= rcut; real Y_lm as in include/gint.h (l <= 3); for r < 1e-12 the direction is (0, 0, 0).
+__device__ __forceinline__ void snap_eval(const SnapSpecies& sp, const double* __restrict__ tab, double dx, double dy, double dz,
+                                          double scale, double* __restrict__ out) {
+    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    if (!(r2 < sp.rcut * sp.rcut)) {
+        for (int c = 0; c < sp.ncomp; c++) out[c] = 0.0;
+        return;
+    }
+    const double r = sqrt(r2);
+    double x = 0.0, y = 0.0, z = 0.0, nz = 0.0;
+    if (r >= 1e-12) {
+        const double ri = 1.0 / r;
+        x = dx * ri; y = dy * ri; z = dz * ri;
+        nz = 1.0;
+    }
+    const double s = r * sp.inv_dr;
+    const int k = (int)floor(s);
+    const double t = s - (double)k;
+    const double L0 = (1.0 - t) * (2.0 - t) * (3.0 - t) * (1.0 / 6.0);
+    const double L1 = t * (2.0 - t) * (3.0 - t) * 0.5;
+    const double L2 = -t * (1.0 - t) * (3.0 - t) * 0.5;
+    const double L3 = t * (1.0 - t) * (2.0 - t) * (1.0 / 6.0);
+    int c = 0;
+    for (int f = 0; f < sp.nrad; f++) {
+        const double* T = tab + sp.tab_off + (size_t)f * sp.ntab + k;
+        const double fv = scale * fma(T[0], L0, fma(T[1], L1, fma(T[2], L2, T[3] * L3)));
+        const int l = sp.l[f];
+        if (l == 0) {
+            out[c++] = 0.28209479177387814 * fv;
+        } else if (l == 1) {
+            const double g = 0.48860251190291992 * fv;
+            out[c++] = g * y; out[c++] = g * z; out[c++] = g * x;
+        } else if (l == 2) {
+            const double g = 1.0925484305920792 * fv;
+            out[c++] = g * (x * y);
+            out[c++] = g * (y * z);
+            out[c++] = 0.31539156525252005 * fv * fma(3.0 * z, z, -nz);
+            out[c++] = g * (x * z);
+            out[c++] = 0.54627421529603959 * fv * fma(x, x, -(y * y));
+        } else {
+            const double x2 = x * x, y2 = y * y, q = fma(5.0 * z, z, -nz);
+            out[c++] = 0.59004358992664352 * fv * y * fma(3.0, x2, -y2);
+            out[c++] = 2.8906114426405538 * fv * (x * y * z);
+            out[c++] = 0.45704579946446577 * fv * y * q;
+            out[c++] = 0.37317633259011540 * fv * z * fma(5.0 * z, z, -3.0 * nz);
+            out[c++] = 0.45704579946446577 * fv * x * q;
+            out[c++] = 1.4453057213202769 * fv * z * (x2 - y2);
+            out[c++] = 0.59004358992664352 * fv * x * fma(-3.0, y2, x2);
+        }
+    }
+}
+
+constexpr int kSnapThreads = 128;
+constexpr int kSnapStride = 33;   // doubles per staged point: 32 values + 1 (bank spread for the per-lane row writes)
+
+}  // namespace
+
+// FR x FC accumulator fragments of 8 x 8: rows = orbitals of J (n_J <= 8 FR), columns = (Re, Im) of the projector
+// components of I (2 m_I <= 8 FC)
+template <int FR, int FC>
+__global__ void __launch_bounds__(kSnapThreads) gint_snap_kernel(const SnapPlan P, double ax, double ay, double az, double* __restrict__ S) {
+    extern __shared__ __align__(16) double snap_smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double* sPhi = snap_smem + (size_t)warp * 2 * 32 * kSnapStride;   // [32 points][33]
+    double* sG = sPhi + 32 * kSnapStride;                            // [32 points][33]
+    const SnapPair pr = P.pairs[blockIdx.x];
+    const SnapSpecies& so = P.orb[pr.spJ];
+    const SnapSpecies& sb = P.proj[pr.spI];
+    const int nJ = so.ncomp, mI = sb.ncomp;
+    const double rb = sb.rcut;
+    const int npts = P.nrad * P.nang;
+    double acc[FR][FC][2];
+#pragma unroll
+    for (int i = 0; i < FR; i++)
+#pragma unroll
+        for (int j = 0; j < FC; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+    // zero the staging tiles once: columns beyond n_J and 2 m_I stay zero for good
+    for (int e = lane; e < 2 * 32 * kSnapStride; e += 32) sPhi[e] = 0.0;
+    __syncwarp();
+    const int frow = lane >> 2, fk = lane & 3;
+    for (int p0 = warp * 32; p0 < npts; p0 += kSnapThreads) {
+        const int p = p0 + lane;
+        double* myPhi = sPhi + lane * kSnapStride;
+        double* myG = sG + lane * kSnapStride;
+        if (p < npts) {
+            const int ir = p / P.nang, ia = p - ir * P.nang;
+            const double r = P.rad_x[ir] * rb;
+            const double ux = r * P.ang_xyz[3 * ia], uy = r * P.ang_xyz[3 * ia + 1], uz = r * P.ang_xyz[3 * ia + 2];
+            const double w = P.rad_w[ir] * rb * r * r * P.ang_w[ia];
+            // weighted real projector values through the Phi row of this point, then G = beta (cos - i sin)(A.r)
+            snap_eval(sb, P.tab, ux, uy, uz, w, myPhi);
+            double sn, cs;
+            sincos(ax * (pr.tauI[0] + ux) + ay * (pr.tauI[1] + uy) + az * (pr.tauI[2] + uz), &sn, &cs);
+            for (int b = 0; b < mI; b++) {
+                const double bv = myPhi[b];
+                myG[2 * b] = bv * cs;
+                myG[2 * b + 1] = -(bv * sn);
+            }
+            for (int c = nJ; c < mI; c++) myPhi[c] = 0.0;
+            snap_eval(so, P.tab, ux + pr.d[0], uy + pr.d[1], uz + pr.d[2], 1.0, myPhi);
+        } else {
+            for (int c = 0; c < nJ; c++) myPhi[c] = 0.0;
+            for (int c = 0; c < 2 * mI; c++) myG[c] = 0.0;
+        }
+        __syncwarp();
+        // 32 points = 8 k-steps of 4 points: A[row mu = 8 i + lane / 4][k = lane % 4], B[k = lane % 4][col = 8 j + lane / 4]
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            double a[FR], b[FC];
+#pragma unroll
+            for (int i = 0; i < FR; i++) a[i] = sPhi[(4 * q + fk) * kSnapStride + 8 * i + frow];
+#pragma unroll
+            for (int j = 0; j < FC; j++) b[j] = sG[(4 * q + fk) * kSnapStride + 8 * j + frow];
+#pragma unroll
+            for (int i = 0; i < FR; i++)
+#pragma unroll
+                for (int j = 0; j < FC; j++) dmma_s(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+        __syncwarp();
+    }
+    // cross-warp sum in a fixed order: warp w writes its fragments, then thread e adds the four copies of element e
+    __syncthreads();
+    double* red = snap_smem;   // [4 warps][FR * 8][FC * 8]
+    constexpr int kCols = FC * 8;
+#pragma unroll
+    for (int i = 0; i < FR; i++)
+#pragma unroll
+        for (int j = 0; j < FC; j++) {
+            // C fragment: lane holds (row lane / 4, columns 2 (lane % 4), 2 (lane % 4) + 1)
+            double* dst = red + ((size_t)warp * FR * 8 + 8 * i + frow) * kCols + 8 * j + 2 * fk;
+            dst[0] = acc[i][j][0];
+            dst[1] = acc[i][j][1];
+        }
+    __syncthreads();
+    double* out = S + 2 * pr.off;   // block [n_J][m_I] complex = [n_J][2 m_I] doubles
+    for (int e = tid; e < nJ * 2 * mI; e += kSnapThreads) {
+        const int mu = e / (2 * mI), c = e - mu * 2 * mI;
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < kSnapThreads / 32; w++) v += red[((size_t)w * FR * 8 + mu) * kCols + c];
+        out[e] = v;
+    }
+}
+
+size_t snap_kernel_smem(int fr, int fc) {
+    const size_t stage = (size_t)(kSnapThreads / 32) * 2 * 32 * kSnapStride * sizeof(double);
+    const size_t red = (size_t)(kSnapThreads / 32) * fr * 8 * fc * 8 * sizeof(double);
+    return std::max(stage, red);
+}
+
+cudaError_t launch_snap(const SnapPlan& P, int fr, int fc, const double* A, double* S, cudaStream_t stream) {
+    if (P.npair <= 0) return cudaSuccess;
+    const size_t smem = snap_kernel_smem(fr <= 2 ? 2 : 4, fc <= 2 ? 2 : 4);
+    cudaError_t e;
+    if (fr <= 2 && fc <= 2) {
+        if ((e = cudaFuncSetAttribute(gint_snap_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        gint_snap_kernel<2, 2><<<P.npair, kSnapThreads, smem, stream>>>(P, A[0], A[1], A[2], S);
+    } else {
+        if ((e = cudaFuncSetAttribute(gint_snap_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        gint_snap_kernel<4, 4><<<P.npair, kSnapThreads, smem, stream>>>(P, A[0], A[1], A[2], S);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace gint

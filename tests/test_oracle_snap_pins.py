@@ -148,3 +148,16 @@ def test_pair_list_against_a_replicated_supercell():
             count += sum(1 for k in near if k % 4 == J and np.linalg.norm(images[k] - w.atom_pos[I]) < cut)
     assert count == len(keys)
     assert off[-1] == sum(int(species[asp[j]].norb) * 1 for j in jat)
+
+
+def test_pair_cutoff_is_strict_for_a_self_image_exactly_at_the_cutoff():
+    """|a1| = rb + rc exactly: the self images (0, 0, +-1, 0, 0) sit ON the cutoff and are not pairs (strict
+    inequality, and the displacement is formed as (tau_J - tau_I) + R so that rounding cannot turn the tie)."""
+    sp = wl.make_species("A", 3.0, [(0, 0.6)])
+    pj = wl.make_species("beta", 2.0, [(0, 1.5)])
+    lat = np.array([[5.0, 0.0, 0.0], [0.0, 9.0, 0.0], [0.0, 0.0, 9.0]])
+    iat, jat, R, off = oracle.enumerate_snap_pairs(lat, [sp], [pj], [0], np.array([[0.123456789, 1.1, 2.2]]))
+    assert [tuple(r) for r in R.tolist()] == [(0, 0, 0)]
+    lat[0, 0] = 5.0 - 1e-9
+    iat, jat, R, off = oracle.enumerate_snap_pairs(lat, [sp], [pj], [0], np.array([[0.123456789, 1.1, 2.2]]))
+    assert [tuple(r) for r in R.tolist()] == [(-1, 0, 0), (0, 0, 0), (1, 0, 0)]
