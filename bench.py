@@ -294,7 +294,7 @@ def main():
     e2e_val = F_sym / (e2e_ms * 1e-3) * 1e-12
 
     # ---- next step of the workflow, outside the headline: H(k) = sum_R exp(i k.R) H(R) (Eq. 5) -------------
-    fold = rho_info = fvl_info = None
+    fold = rho_info = fvl_info = snap_info = None
     if world == 1:
         ntot = ctx.gint_num_orbitals()[0]
         Hk = torch.empty((ntot, ntot), dtype=torch.complex128, device=dev)
@@ -338,6 +338,32 @@ def main():
                     "note": "gint_fvl (Eq. 46): psi kernel + E = D + D^T gather + T = E Phi (DMMA) + force kernel; T needs every "
                             "(row, column) pair, so F_pt accounting"}
         del Dm, rho, Fv
+        # velocity-gauge nonlocal overlaps on the atom-centred quadrature grid (Eq. 47)
+        proj = [workloads.projector_species() for _ in w.species]
+        rx, rw = workloads.radial_quadrature(140)
+        an, aw = workloads.angular_quadrature(110)
+        t1 = time.perf_counter()
+        ctx.gint_snap_setup(proj, rx, rw, an, aw)
+        snap_setup_s = time.perf_counter() - t1
+        sp_iat, sp_jat, _, sp_off = ctx.gint_snap_get_pairs()
+        Sv = ctx.gint_snap_psibeta((0.08, -0.11, 0.05))
+        torch.cuda.synchronize()
+        f0.record()
+        for _ in range(3):
+            ctx.gint_snap_psibeta((0.08, -0.11, 0.05), Sv)
+        f1.record()
+        torch.cuda.synchronize()
+        snap_ms = f0.elapsed_time(f1) / 3
+        npts = len(rx) * len(aw)
+        snap_flops = 4.0 * float(sp_off[-1]) * npts      # one complex += real x complex per (orbital, projector, point)
+        snap_info = {"ms_per_call": snap_ms, "pairs": int(len(sp_iat)), "points_per_pair": int(npts),
+                     "point_evaluations_per_s": len(sp_iat) * npts / (snap_ms * 1e-3),
+                     "contraction_flops": snap_flops, "contraction_tflops": snap_flops / (snap_ms * 1e-3) * 1e-12,
+                     "setup_s": snap_setup_s,
+                     "note": "gint_snap_psibeta (Eq. 47): 140 x 110 quadrature points around every projector atom, all "
+                             "(I, J, R) pairs in one launch; bound by the per-point evaluation of orbitals and projectors "
+                             "(FP64 ALU), the sum over points runs on the tensor pipe"}
+        del Sv
 
     if rank != 0:
         if world > 1:
@@ -401,6 +427,7 @@ def main():
         fvl_info["peak_tflops"] = peak
         fvl_info["frac"] = fvl_info["achieved_tflops"] / peak
         out["fvl"] = fvl_info
+        out["snap_psibeta"] = snap_info
     if not args.no_cpu_baseline and world == 1:
         na = min(w.natom, args.ref_atoms or 256)
         dt, used, nblk, ntot = oracle_sample(w, na)

@@ -587,7 +587,8 @@ int gint_snap_setup(gint_ctx* ctx, const gint_species* proj, int32_t nrad_pts, c
             return fail_cuda(e, "gint_snap_setup upload");
         }
         S.npair = (int32_t)pairs.size(); S.nrad = nrad_pts; S.nang = nang;
-        ctx->snap_fr = (max_n + 7) / 8; ctx->snap_fc = (2 * max_m + 7) / 8;
+        // projector values pass through the orbital columns of the staging tile: at least max_m of them
+        ctx->snap_fr = std::max(1, (std::max(max_n, max_m) + 7) / 8); ctx->snap_fc = std::max(1, (2 * max_m + 7) / 8);
         ctx->have_snap = true;
     } catch (const std::bad_alloc&) {
         snap_release(ctx);

@@ -36,13 +36,13 @@ __device__ __forceinline__ void dmma_s(double& c0, double& c1, double a, double 
 }
 
 // values of all components of a species (orbitals or projectors) at displacement (dx, dy, dz) from its centre, written
-// to out[0 .. ncomp-1]: cubic Lagrange interpolation on the forward stencil k .. k+3, k = floor(r / dr); zero for
+// to out[0], out[os], .. out[(ncomp-1) os]: cubic Lagrange interpolation on the forward stencil k .. k+3, k = floor(r / dr); zero for
 // r >= rcut; real Y_lm as in include/gint.h (l <= 3); for r < 1e-12 the direction is (0, 0, 0).
 __device__ __forceinline__ void snap_eval(const SnapSpecies& sp, const double* __restrict__ tab, double dx, double dy, double dz,
-                                          double scale, double* __restrict__ out) {
+                                          double scale, double* __restrict__ out, int os) {
     const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
     if (!(r2 < sp.rcut * sp.rcut)) {
-        for (int c = 0; c < sp.ncomp; c++) out[c] = 0.0;
+        for (int c = 0; c < sp.ncomp; c++) out[c * os] = 0.0;
         return;
     }
     const double r = sqrt(r2);
@@ -65,43 +65,44 @@ __device__ __forceinline__ void snap_eval(const SnapSpecies& sp, const double* _
         const double fv = scale * fma(T[0], L0, fma(T[1], L1, fma(T[2], L2, T[3] * L3)));
         const int l = sp.l[f];
         if (l == 0) {
-            out[c++] = 0.28209479177387814 * fv;
+            out[os * c++] = 0.28209479177387814 * fv;
         } else if (l == 1) {
             const double g = 0.48860251190291992 * fv;
-            out[c++] = g * y; out[c++] = g * z; out[c++] = g * x;
+            out[os * c++] = g * y; out[os * c++] = g * z; out[os * c++] = g * x;
         } else if (l == 2) {
             const double g = 1.0925484305920792 * fv;
-            out[c++] = g * (x * y);
-            out[c++] = g * (y * z);
-            out[c++] = 0.31539156525252005 * fv * fma(3.0 * z, z, -nz);
-            out[c++] = g * (x * z);
-            out[c++] = 0.54627421529603959 * fv * fma(x, x, -(y * y));
+            out[os * c++] = g * (x * y);
+            out[os * c++] = g * (y * z);
+            out[os * c++] = 0.31539156525252005 * fv * fma(3.0 * z, z, -nz);
+            out[os * c++] = g * (x * z);
+            out[os * c++] = 0.54627421529603959 * fv * fma(x, x, -(y * y));
         } else {
             const double x2 = x * x, y2 = y * y, q = fma(5.0 * z, z, -nz);
-            out[c++] = 0.59004358992664352 * fv * y * fma(3.0, x2, -y2);
-            out[c++] = 2.8906114426405538 * fv * (x * y * z);
-            out[c++] = 0.45704579946446577 * fv * y * q;
-            out[c++] = 0.37317633259011540 * fv * z * fma(5.0 * z, z, -3.0 * nz);
-            out[c++] = 0.45704579946446577 * fv * x * q;
-            out[c++] = 1.4453057213202769 * fv * z * (x2 - y2);
-            out[c++] = 0.59004358992664352 * fv * x * fma(-3.0, y2, x2);
+            out[os * c++] = 0.59004358992664352 * fv * y * fma(3.0, x2, -y2);
+            out[os * c++] = 2.8906114426405538 * fv * (x * y * z);
+            out[os * c++] = 0.45704579946446577 * fv * y * q;
+            out[os * c++] = 0.37317633259011540 * fv * z * fma(5.0 * z, z, -3.0 * nz);
+            out[os * c++] = 0.45704579946446577 * fv * x * q;
+            out[os * c++] = 1.4453057213202769 * fv * z * (x2 - y2);
+            out[os * c++] = 0.59004358992664352 * fv * x * fma(-3.0, y2, x2);
         }
     }
 }
 
 constexpr int kSnapThreads = 128;
-constexpr int kSnapStride = 33;   // doubles per staged point: 32 values + 1 (bank spread for the per-lane row writes)
+constexpr int kSnapStride = 36;   // staging tiles are [column][point]: 32 points + 4, so that the lanes' writes (one column,
+                                  // 32 points) and the fragment reads (4 points x 8 columns) are both free of bank conflicts
 
 }  // namespace
 
 // FR x FC accumulator fragments of 8 x 8: rows = orbitals of J (n_J <= 8 FR), columns = (Re, Im) of the projector
 // components of I (2 m_I <= 8 FC)
 template <int FR, int FC>
-__global__ void __launch_bounds__(kSnapThreads) gint_snap_kernel(const SnapPlan P, double ax, double ay, double az, double* __restrict__ S) {
+__global__ void __launch_bounds__(kSnapThreads, 4) gint_snap_kernel(const SnapPlan P, double ax, double ay, double az, double* __restrict__ S) {
     extern __shared__ __align__(16) double snap_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    double* sPhi = snap_smem + (size_t)warp * 2 * 32 * kSnapStride;   // [32 points][33]
-    double* sG = sPhi + 32 * kSnapStride;                            // [32 points][33]
+    double* sPhi = snap_smem + (size_t)warp * (FR + FC) * 8 * kSnapStride;   // [8 FR columns: orbitals][36]
+    double* sG = sPhi + FR * 8 * kSnapStride;                                // [8 FC columns: Re, Im of the projectors][36]
     const SnapPair pr = P.pairs[blockIdx.x];
     const SnapSpecies& so = P.orb[pr.spJ];
     const SnapSpecies& sb = P.proj[pr.spI];
@@ -114,32 +115,32 @@ __global__ void __launch_bounds__(kSnapThreads) gint_snap_kernel(const SnapPlan 
 #pragma unroll
         for (int j = 0; j < FC; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
     // zero the staging tiles once: columns beyond n_J and 2 m_I stay zero for good
-    for (int e = lane; e < 2 * 32 * kSnapStride; e += 32) sPhi[e] = 0.0;
+    for (int e = lane; e < (FR + FC) * 8 * kSnapStride; e += 32) sPhi[e] = 0.0;
     __syncwarp();
     const int frow = lane >> 2, fk = lane & 3;
     for (int p0 = warp * 32; p0 < npts; p0 += kSnapThreads) {
         const int p = p0 + lane;
-        double* myPhi = sPhi + lane * kSnapStride;
-        double* myG = sG + lane * kSnapStride;
+        double* myPhi = sPhi + lane;   // column c of this lane's point: myPhi[c * kSnapStride]
+        double* myG = sG + lane;
         if (p < npts) {
             const int ir = p / P.nang, ia = p - ir * P.nang;
             const double r = P.rad_x[ir] * rb;
             const double ux = r * P.ang_xyz[3 * ia], uy = r * P.ang_xyz[3 * ia + 1], uz = r * P.ang_xyz[3 * ia + 2];
             const double w = P.rad_w[ir] * rb * r * r * P.ang_w[ia];
-            // weighted real projector values through the Phi row of this point, then G = beta (cos - i sin)(A.r)
-            snap_eval(sb, P.tab, ux, uy, uz, w, myPhi);
+            // weighted real projector values through the Phi columns of this point, then G = beta (cos - i sin)(A.r)
+            snap_eval(sb, P.tab, ux, uy, uz, w, myPhi, kSnapStride);
             double sn, cs;
             sincos(ax * (pr.tauI[0] + ux) + ay * (pr.tauI[1] + uy) + az * (pr.tauI[2] + uz), &sn, &cs);
             for (int b = 0; b < mI; b++) {
-                const double bv = myPhi[b];
-                myG[2 * b] = bv * cs;
-                myG[2 * b + 1] = -(bv * sn);
+                const double bv = myPhi[b * kSnapStride];
+                myG[(2 * b) * kSnapStride] = bv * cs;
+                myG[(2 * b + 1) * kSnapStride] = -(bv * sn);
             }
-            for (int c = nJ; c < mI; c++) myPhi[c] = 0.0;
-            snap_eval(so, P.tab, ux + pr.d[0], uy + pr.d[1], uz + pr.d[2], 1.0, myPhi);
+            for (int c = nJ; c < mI; c++) myPhi[c * kSnapStride] = 0.0;
+            snap_eval(so, P.tab, ux + pr.d[0], uy + pr.d[1], uz + pr.d[2], 1.0, myPhi, kSnapStride);
         } else {
-            for (int c = 0; c < nJ; c++) myPhi[c] = 0.0;
-            for (int c = 0; c < 2 * mI; c++) myG[c] = 0.0;
+            for (int c = 0; c < nJ; c++) myPhi[c * kSnapStride] = 0.0;
+            for (int c = 0; c < 2 * mI; c++) myG[c * kSnapStride] = 0.0;
         }
         __syncwarp();
         // 32 points = 8 k-steps of 4 points: A[row mu = 8 i + lane / 4][k = lane % 4], B[k = lane % 4][col = 8 j + lane / 4]
@@ -147,9 +148,9 @@ __global__ void __launch_bounds__(kSnapThreads) gint_snap_kernel(const SnapPlan 
         for (int q = 0; q < 8; q++) {
             double a[FR], b[FC];
 #pragma unroll
-            for (int i = 0; i < FR; i++) a[i] = sPhi[(4 * q + fk) * kSnapStride + 8 * i + frow];
+            for (int i = 0; i < FR; i++) a[i] = sPhi[(8 * i + frow) * kSnapStride + 4 * q + fk];
 #pragma unroll
-            for (int j = 0; j < FC; j++) b[j] = sG[(4 * q + fk) * kSnapStride + 8 * j + frow];
+            for (int j = 0; j < FC; j++) b[j] = sG[(8 * j + frow) * kSnapStride + 4 * q + fk];
 #pragma unroll
             for (int i = 0; i < FR; i++)
 #pragma unroll
@@ -182,23 +183,33 @@ __global__ void __launch_bounds__(kSnapThreads) gint_snap_kernel(const SnapPlan 
 }
 
 size_t snap_kernel_smem(int fr, int fc) {
-    const size_t stage = (size_t)(kSnapThreads / 32) * 2 * 32 * kSnapStride * sizeof(double);
+    const size_t stage = (size_t)(kSnapThreads / 32) * (fr + fc) * 8 * kSnapStride * sizeof(double);
     const size_t red = (size_t)(kSnapThreads / 32) * fr * 8 * fc * 8 * sizeof(double);
     return std::max(stage, red);
 }
 
+template <int FR, int FC>
+static cudaError_t launch_snap_t(const SnapPlan& P, const double* A, double* S, cudaStream_t stream) {
+    const size_t smem = snap_kernel_smem(FR, FC);
+    cudaError_t e = cudaFuncSetAttribute(gint_snap_kernel<FR, FC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    gint_snap_kernel<FR, FC><<<P.npair, kSnapThreads, smem, stream>>>(P, A[0], A[1], A[2], S);
+    return cudaGetLastError();
+}
+
+// fr = ceil(max orbitals per atom / 8) <= 4, fc = ceil(2 max projector components / 8) <= 4
 cudaError_t launch_snap(const SnapPlan& P, int fr, int fc, const double* A, double* S, cudaStream_t stream) {
     if (P.npair <= 0) return cudaSuccess;
-    const size_t smem = snap_kernel_smem(fr <= 2 ? 2 : 4, fc <= 2 ? 2 : 4);
-    cudaError_t e;
-    if (fr <= 2 && fc <= 2) {
-        if ((e = cudaFuncSetAttribute(gint_snap_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        gint_snap_kernel<2, 2><<<P.npair, kSnapThreads, smem, stream>>>(P, A[0], A[1], A[2], S);
-    } else {
-        if ((e = cudaFuncSetAttribute(gint_snap_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        gint_snap_kernel<4, 4><<<P.npair, kSnapThreads, smem, stream>>>(P, A[0], A[1], A[2], S);
+    if (fr < 1 || fr > 4 || fc < 1 || fc > 4) return cudaErrorInvalidValue;
+#define SNAP_CASE(R, C) case (R) * 4 + (C): return launch_snap_t<R, C>(P, A, S, stream);
+    switch (fr * 4 + fc) {
+        SNAP_CASE(1, 1) SNAP_CASE(1, 2) SNAP_CASE(1, 3) SNAP_CASE(1, 4)
+        SNAP_CASE(2, 1) SNAP_CASE(2, 2) SNAP_CASE(2, 3) SNAP_CASE(2, 4)
+        SNAP_CASE(3, 1) SNAP_CASE(3, 2) SNAP_CASE(3, 3) SNAP_CASE(3, 4)
+        SNAP_CASE(4, 1) SNAP_CASE(4, 2) SNAP_CASE(4, 3) SNAP_CASE(4, 4)
     }
-    return cudaGetLastError();
+#undef SNAP_CASE
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace gint
