@@ -35,34 +35,25 @@ __device__ __forceinline__ void dmma_s(double& c0, double& c1, double a, double 
                  : "d"(a), "d"(b));
 }
 
-// values of all components of a species (orbitals or projectors) at displacement (dx, dy, dz) from its centre, written
-// to out[0], out[os], .. out[(ncomp-1) os]: cubic Lagrange interpolation on the forward stencil k .. k+3, k = floor(r / dr); zero for
-// r >= rcut; real Y_lm as in include/gint.h (l <= 3); for r < 1e-12 the direction is (0, 0, 0).
-__device__ __forceinline__ void snap_eval(const SnapSpecies& sp, const double* __restrict__ tab, double dx, double dy, double dz,
-                                          double scale, double* __restrict__ out, int os) {
-    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-    if (!(r2 < sp.rcut * sp.rcut)) {
-        for (int c = 0; c < sp.ncomp; c++) out[c * os] = 0.0;
-        return;
-    }
-    const double r = sqrt(r2);
-    double x = 0.0, y = 0.0, z = 0.0, nz = 0.0;
-    if (r >= 1e-12) {
-        const double ri = 1.0 / r;
-        x = dx * ri; y = dy * ri; z = dz * ri;
-        nz = 1.0;
-    }
+// Values of all components of a species (orbitals or projectors) at distance r (< rcut) and direction (x, y, z) from
+// its centre, times `scale`, written to out[0], out[os], .. out[(ncomp-1) os]: cubic Lagrange interpolation on the
+// forward stencil k .. k+3, k = floor(r / dr); real Y_lm as in include/gint.h (l <= 3); nz = 0 marks r < 1e-12, where
+// the direction is (0, 0, 0).
+__device__ __forceinline__ void snap_eval_core(const SnapSpecies& sp, const double* __restrict__ tab, double r, double x, double y, double z,
+                                               double nz, double scale, double* __restrict__ out, int os) {
     const double s = r * sp.inv_dr;
-    const int k = (int)floor(s);
+    const int k = __double2int_rd(s);
     const double t = s - (double)k;
-    const double L0 = (1.0 - t) * (2.0 - t) * (3.0 - t) * (1.0 / 6.0);
-    const double L1 = t * (2.0 - t) * (3.0 - t) * 0.5;
-    const double L2 = -t * (1.0 - t) * (3.0 - t) * 0.5;
-    const double L3 = t * (1.0 - t) * (2.0 - t) * (1.0 / 6.0);
+    const double t1 = 1.0 - t, t2 = 2.0 - t, t3 = 3.0 - t;
+    const double a23 = t2 * t3, b01 = t * t1;
+    const double L0 = (t1 * a23) * (scale * (1.0 / 6.0));
+    const double L1 = (t * a23) * (scale * 0.5);
+    const double L2 = (b01 * t3) * (scale * -0.5);
+    const double L3 = (b01 * t2) * (scale * (1.0 / 6.0));
     int c = 0;
     for (int f = 0; f < sp.nrad; f++) {
         const double* T = tab + sp.tab_off + (size_t)f * sp.ntab + k;
-        const double fv = scale * fma(T[0], L0, fma(T[1], L1, fma(T[2], L2, T[3] * L3)));
+        const double fv = fma(T[0], L0, fma(T[1], L1, fma(T[2], L2, T[3] * L3)));
         const int l = sp.l[f];
         if (l == 0) {
             out[os * c++] = 0.28209479177387814 * fv;
@@ -73,20 +64,40 @@ __device__ __forceinline__ void snap_eval(const SnapSpecies& sp, const double* _
             const double g = 1.0925484305920792 * fv;
             out[os * c++] = g * (x * y);
             out[os * c++] = g * (y * z);
-            out[os * c++] = 0.31539156525252005 * fv * fma(3.0 * z, z, -nz);
+            out[os * c++] = (0.31539156525252005 * fv) * fma(3.0 * z, z, -nz);
             out[os * c++] = g * (x * z);
-            out[os * c++] = 0.54627421529603959 * fv * fma(x, x, -(y * y));
+            out[os * c++] = (0.54627421529603959 * fv) * fma(x, x, -(y * y));
         } else {
             const double x2 = x * x, y2 = y * y, q = fma(5.0 * z, z, -nz);
-            out[os * c++] = 0.59004358992664352 * fv * y * fma(3.0, x2, -y2);
-            out[os * c++] = 2.8906114426405538 * fv * (x * y * z);
-            out[os * c++] = 0.45704579946446577 * fv * y * q;
-            out[os * c++] = 0.37317633259011540 * fv * z * fma(5.0 * z, z, -3.0 * nz);
-            out[os * c++] = 0.45704579946446577 * fv * x * q;
-            out[os * c++] = 1.4453057213202769 * fv * z * (x2 - y2);
-            out[os * c++] = 0.59004358992664352 * fv * x * fma(-3.0, y2, x2);
+            const double g3 = 0.59004358992664352 * fv, g1 = 0.45704579946446577 * fv;
+            out[os * c++] = (g3 * y) * fma(3.0, x2, -y2);
+            out[os * c++] = (2.8906114426405538 * fv) * (x * y * z);
+            out[os * c++] = (g1 * y) * q;
+            out[os * c++] = (0.37317633259011540 * fv * z) * fma(5.0 * z, z, -3.0 * nz);
+            out[os * c++] = (g1 * x) * q;
+            out[os * c++] = (1.4453057213202769 * fv * z) * (x2 - y2);
+            out[os * c++] = (g3 * x) * fma(-3.0, y2, x2);
         }
     }
+}
+
+// orbitals at displacement (dx, dy, dz): zero for r >= rcut; 1/r from the hardware seed and one cubic correction
+__device__ __forceinline__ void snap_eval(const SnapSpecies& sp, const double* __restrict__ tab, double dx, double dy, double dz,
+                                          double* __restrict__ out, int os) {
+    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    if (!(r2 < sp.rcut * sp.rcut)) {
+        for (int c = 0; c < sp.ncomp; c++) out[c * os] = 0.0;
+        return;
+    }
+    double rinv = 0.0, nz = 0.0;
+    if (r2 >= 1e-24) {
+        double y0;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));   // relative error ~2^-22
+        const double e = fma(-(r2 * y0), y0, 1.0);                   // 1 - r2 y0^2
+        rinv = fma(e * y0, fma(0.375, e, 0.5), y0);                  // y0 (1 + e/2 + 3 e^2/8): error ~e^3
+        nz = 1.0;
+    }
+    snap_eval_core(sp, tab, r2 * rinv, dx * rinv, dy * rinv, dz * rinv, nz, 1.0, out, os);
 }
 
 constexpr int kSnapThreads = 128;
@@ -125,10 +136,12 @@ __global__ void __launch_bounds__(kSnapThreads, 4) gint_snap_kernel(const SnapPl
         if (p < npts) {
             const int ir = p / P.nang, ia = p - ir * P.nang;
             const double r = P.rad_x[ir] * rb;
-            const double ux = r * P.ang_xyz[3 * ia], uy = r * P.ang_xyz[3 * ia + 1], uz = r * P.ang_xyz[3 * ia + 2];
+            const double nx = P.ang_xyz[3 * ia], ny = P.ang_xyz[3 * ia + 1], nz_ = P.ang_xyz[3 * ia + 2];
+            const double ux = r * nx, uy = r * ny, uz = r * nz_;
             const double w = P.rad_w[ir] * rb * r * r * P.ang_w[ia];
             // weighted real projector values through the Phi columns of this point, then G = beta (cos - i sin)(A.r)
-            snap_eval(sb, P.tab, ux, uy, uz, w, myPhi, kSnapStride);
+            // (the quadrature point sits at distance r < rb in direction n_a by construction: no square root)
+            snap_eval_core(sb, P.tab, r, nx, ny, nz_, 1.0, w, myPhi, kSnapStride);
             double sn, cs;
             sincos(ax * (pr.tauI[0] + ux) + ay * (pr.tauI[1] + uy) + az * (pr.tauI[2] + uz), &sn, &cs);
             for (int b = 0; b < mI; b++) {
@@ -137,7 +150,7 @@ __global__ void __launch_bounds__(kSnapThreads, 4) gint_snap_kernel(const SnapPl
                 myG[(2 * b + 1) * kSnapStride] = -(bv * sn);
             }
             for (int c = nJ; c < mI; c++) myPhi[c * kSnapStride] = 0.0;
-            snap_eval(so, P.tab, ux + pr.d[0], uy + pr.d[1], uz + pr.d[2], 1.0, myPhi, kSnapStride);
+            snap_eval(so, P.tab, ux + pr.d[0], uy + pr.d[1], uz + pr.d[2], myPhi, kSnapStride);
         } else {
             for (int c = 0; c < nJ; c++) myPhi[c * kSnapStride] = 0.0;
             for (int c = 0; c < 2 * mI; c++) myG[c * kSnapStride] = 0.0;
