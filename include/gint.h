@@ -212,7 +212,8 @@ int gint_fold_k_static(gint_ctx *ctx, const double *H_dev, const double *kfrac, 
  *                   the orbital side: GINT_EUNSUPPORTED beyond); rad_x[nrad_pts], rad_w[nrad_pts], ang_xyz[nang][3],
  *                   ang_w[nang]: HOST arrays, copied.  Builds the pair list for the context's current positions and
  *                   uploads the tables; may be called again (new projectors or rules).  gint_update_positions
- *                   discards the pair list: call gint_snap_setup again afterwards.
+ *                   discards the pair list: call gint_snap_setup again afterwards.  Works on a host-only context
+ *                   too (pair list only; gint_snap_psibeta then returns GINT_ENODEVICE).
  * gint_snap_num_pairs / gint_snap_get_pairs   the pairs sorted by (I, J, R1, R2, R3): iat[n], jat[n], R[n][3],
  *                   offset[n+1] in COMPLEX elements; block b is [n_J][m_I] row-major (rows: orbitals of J in block
  *                   order, columns: projector components of I, radial functions in the order given, m = -l..l).

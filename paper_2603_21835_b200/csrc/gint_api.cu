@@ -489,7 +489,6 @@ int gint_snap_setup(gint_ctx* ctx, const gint_species* proj, int32_t nrad_pts, c
                     int32_t nang, const double* ang_xyz, const double* ang_w) {
     if (!ctx || !proj || !rad_x || !rad_w || !ang_xyz || !ang_w) return fail(GINT_EINVAL, "null argument");
     if (nrad_pts <= 0 || nang <= 0) return fail(GINT_EINVAL, "empty quadrature table");
-    if (ctx->device < 0) return fail(GINT_ENODEVICE, "host-only context");
     const gint::Plan& P = ctx->plan;
     const int nsp = (int)P.species.size(), natom = (int)P.atom_species.size();
     try {
@@ -573,6 +572,12 @@ int gint_snap_setup(gint_ctx* ctx, const gint_species* proj, int32_t nrad_pts, c
         }
         ctx->snap_off.push_back(off);
         if (pairs.size() > 0x7FFFFFFFull) return fail(GINT_EUNSUPPORTED, "gint_snap: too many pairs");
+        ctx->snap_fr = std::max(1, (std::max(max_n, max_m) + 7) / 8);   // projector values pass through the orbital columns
+        ctx->snap_fc = std::max(1, (2 * max_m + 7) / 8);
+        if (ctx->device < 0) {   // host-only context: the pair list can be queried, gint_snap_psibeta returns GINT_ENODEVICE
+            ctx->have_snap = true;
+            return GINT_OK;
+        }
         DeviceGuard guard(ctx->device);
         if (guard.err != cudaSuccess) return fail_cuda(guard.err, "cudaSetDevice");
         cudaError_t e;
@@ -587,8 +592,6 @@ int gint_snap_setup(gint_ctx* ctx, const gint_species* proj, int32_t nrad_pts, c
             return fail_cuda(e, "gint_snap_setup upload");
         }
         S.npair = (int32_t)pairs.size(); S.nrad = nrad_pts; S.nang = nang;
-        // projector values pass through the orbital columns of the staging tile: at least max_m of them
-        ctx->snap_fr = std::max(1, (std::max(max_n, max_m) + 7) / 8); ctx->snap_fc = std::max(1, (2 * max_m + 7) / 8);
         ctx->have_snap = true;
     } catch (const std::bad_alloc&) {
         snap_release(ctx);

@@ -265,3 +265,33 @@ def test_bench_helpers_run_without_a_gpu():
     t = bench.ncu_traffic("si512_dzp")
     assert t is not None and 1e9 < t < 1e11
     assert bench.ncu_traffic("no_such_workload") is None
+
+
+def test_snap_pair_list_equals_the_oracles_enumeration():
+    """gint_snap_setup on host-only contexts: the (I, J, R) list and the block offsets of Eq. 47
+    against oracle.enumerate_snap_pairs -- cubic cfg1 with image pairs, a triclinic cell with a species that has no
+    projectors, and a self image exactly at the cutoff (strict inequality)."""
+    import oracle
+    from paper_2603_21835_b200 import gint_setup
+    from paper_2603_21835_b200.binding import GintError
+    rx, rw = wl.radial_quadrature(8)
+    an, aw = wl.angular_quadrature(6)
+    none = wl.Species(name="none", rcut=0.0, dr=0.01, l=np.zeros(0, np.int32), table=np.zeros((0, 8)))
+    w1 = wl.make("si8_sz")
+    w2 = wl.tiny(seed=9, natom=5, ngrid=(12, 12, 12), rcut=3.0)
+    sp2 = [wl.make_species("A", 3.0, [(0, 0.6), (1, 0.5)]), wl.make_species("B", 2.4, [(0, 0.9)])]
+    asp2 = np.array([0, 1, 0, 1, 0], dtype=np.int32)
+    cases = [(w1.lattice, w1.ngrid, w1.species, w1.atom_species, w1.atom_pos, [wl.projector_species()]),
+             (w2.lattice, w2.ngrid, sp2, asp2, w2.atom_pos, [wl.make_species("beta", 2.0, [(0, 1.5), (1, 1.8)]), none]),
+             (np.diag([5.0, 9.0, 9.0]), (10, 18, 18), [wl.make_species("A", 3.0, [(0, 0.6)])], np.zeros(1, np.int32),
+              np.array([[0.123456789, 1.1, 2.2]]), [wl.make_species("beta", 2.0, [(0, 1.5)])])]
+    for lat, ng, species, asp, pos, proj in cases:
+        ctx = gint_setup(lat, ng, species, asp, pos, cuda_device=-1)
+        with pytest.raises(GintError):
+            ctx.gint_snap_get_pairs()                       # not set up yet
+        ctx.gint_snap_setup(proj, rx, rw, an, aw)
+        got = ctx.gint_snap_get_pairs()
+        ref = oracle.enumerate_snap_pairs(lat, species, proj, asp, pos)
+        assert all(np.array_equal(a, b) for a, b in zip(got, ref))
+        assert len(got[0]) > 0
+    assert [tuple(r) for r in got[2].tolist()] == [(0, 0, 0)]   # the tie case: no (+-1, 0, 0) self image
