@@ -591,6 +591,19 @@ int gint_snap_setup(gint_ctx* ctx, const gint_species* proj, int32_t nrad_pts, c
             snap_release(ctx);
             return fail_cuda(e, "gint_snap_setup upload");
         }
+        std::vector<int32_t> groups;   // consecutive pairs of one projector atom share a CTA
+        for (size_t b0 = 0; b0 < pairs.size();) {
+            size_t n = 1;
+            while (n < (size_t)gint::kSnapGroupPairs && b0 + n < pairs.size() && ctx->snap_iat[b0 + n] == ctx->snap_iat[b0]) n++;
+            groups.push_back((int32_t)b0);
+            groups.push_back((int32_t)n);
+            b0 += n;
+        }
+        if ((e = snap_upload(ctx, groups, &S.groups)) != cudaSuccess) {
+            snap_release(ctx);
+            return fail_cuda(e, "gint_snap_setup upload");
+        }
+        S.ngroup = (int32_t)(groups.size() / 2);
         S.npair = (int32_t)pairs.size(); S.nrad = nrad_pts; S.nang = nang;
         ctx->have_snap = true;
     } catch (const std::bad_alloc&) {

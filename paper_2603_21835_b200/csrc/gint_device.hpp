@@ -94,8 +94,10 @@ struct SnapPlan {
     const double* rad_w;       // [nrad] weights, sum 1
     const double* ang_xyz;     // [nang][3] unit vectors
     const double* ang_w;       // [nang] weights, sum 4 pi
-    int32_t npair, nrad, nang, pad;
+    const int32_t* groups;     // [ngroup][2]: first pair and number of pairs (<= kSnapGroupPairs, same atom I) of a CTA
+    int32_t npair, nrad, nang, ngroup;
 };
+constexpr int kSnapGroupPairs = 2;   // 4: 200+ registers, 2 CTAs per SM, slower (measured)
 cudaError_t launch_snap(const SnapPlan& P, int fr, int fc, const double* A, double* S, cudaStream_t stream);
 
 // The launchers walk the plan's batches (regions that share the psi scratch one after the other): nbatch entries of

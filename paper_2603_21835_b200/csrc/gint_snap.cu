@@ -7,8 +7,8 @@
 //
 // quadrature centred on the projector's atom: radial nodes r_i = x_i rb_I (Gauss-Legendre, 140 in the paper), angular
 // nodes n_a (Lebedev-Laikov, 110 in the paper), both tables given by the caller.  beta_{l m zeta} = b(|r|) Y_lm like an
-// orbital.  One CTA per (I, J, R) pair (the paper batches all neighbours of a central atom into one launch; here all
-// pairs of all atoms are one launch).  The 128 threads walk the nr x na quadrature points; a thread evaluates the n_J
+// orbital.  One CTA per two consecutive (I, J, R) pairs of an atom I (the paper batches all neighbours of a central atom
+// into one launch; here all pairs of all atoms are one launch).  The 128 threads walk the nr x na quadrature points; a thread evaluates the n_J
 // orbitals and the m_I weighted, phase-modulated projector components of its point into its warp's staging tile in
 // shared memory, and the warp contracts 32 points at a time on the FP64 tensor pipe:
 //   C[mu][c] += sum_p Phi[p][mu] G[p][c],   G[p][2b] = Re, G[p][2b+1] = Im of  w_p beta_b(p) exp(-i A.r_p)
@@ -109,23 +109,35 @@ constexpr int kSnapStride = 36;   // staging tiles are [column][point]: 32 point
 // FR x FC accumulator fragments of 8 x 8: rows = orbitals of J (n_J <= 8 FR), columns = (Re, Im) of the projector
 // components of I (2 m_I <= 8 FC)
 template <int FR, int FC>
-__global__ void __launch_bounds__(kSnapThreads, 4) gint_snap_kernel(const SnapPlan P, double ax, double ay, double az, double* __restrict__ S) {
+__global__ void __launch_bounds__(kSnapThreads, kSnapGroupPairs <= 2 ? 3 : 2) gint_snap_kernel(const SnapPlan P, double ax, double ay, double az, double* __restrict__ S) {
     extern __shared__ __align__(16) double snap_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     double* sPhi = snap_smem + (size_t)warp * (FR + FC) * 8 * kSnapStride;   // [8 FR columns: orbitals][36]
     double* sG = sPhi + FR * 8 * kSnapStride;                                // [8 FC columns: Re, Im of the projectors][36]
-    const SnapPair pr = P.pairs[blockIdx.x];
-    const SnapSpecies& so = P.orb[pr.spJ];
+    // a CTA takes up to kSnapGroupPairs consecutive pairs of ONE projector atom: the projector side of a point (beta,
+    // weight, phase) is evaluated once and contracted with the orbitals of each of them
+    const int g0 = P.groups[2 * blockIdx.x], gn = P.groups[2 * blockIdx.x + 1];
+    const SnapPair pr = P.pairs[g0];
     const SnapSpecies& sb = P.proj[pr.spI];
-    const int nJ = so.ncomp, mI = sb.ncomp;
+    const int mI = sb.ncomp;
     const double rb = sb.rcut;
     const int npts = P.nrad * P.nang;
-    double acc[FR][FC][2];
+    double dq[kSnapGroupPairs][3];
+    int spq[kSnapGroupPairs];
 #pragma unroll
-    for (int i = 0; i < FR; i++)
+    for (int nb = 0; nb < kSnapGroupPairs; nb++) {
+        const SnapPair& q = P.pairs[g0 + (nb < gn ? nb : 0)];
+        dq[nb][0] = q.d[0]; dq[nb][1] = q.d[1]; dq[nb][2] = q.d[2];
+        spq[nb] = q.spJ;
+    }
+    double acc[kSnapGroupPairs][FR][FC][2];
 #pragma unroll
-        for (int j = 0; j < FC; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
-    // zero the staging tiles once: columns beyond n_J and 2 m_I stay zero for good
+    for (int nb = 0; nb < kSnapGroupPairs; nb++)
+#pragma unroll
+        for (int i = 0; i < FR; i++)
+#pragma unroll
+            for (int j = 0; j < FC; j++) acc[nb][i][j][0] = acc[nb][i][j][1] = 0.0;
+    // zero the staging tiles once: columns that are never written stay zero
     for (int e = lane; e < (FR + FC) * 8 * kSnapStride; e += 32) sPhi[e] = 0.0;
     __syncwarp();
     const int frow = lane >> 2, fk = lane & 3;
@@ -133,11 +145,12 @@ __global__ void __launch_bounds__(kSnapThreads, 4) gint_snap_kernel(const SnapPl
         const int p = p0 + lane;
         double* myPhi = sPhi + lane;   // column c of this lane's point: myPhi[c * kSnapStride]
         double* myG = sG + lane;
+        double ux = 0.0, uy = 0.0, uz = 0.0;
         if (p < npts) {
             const int ir = p / P.nang, ia = p - ir * P.nang;
             const double r = P.rad_x[ir] * rb;
             const double nx = P.ang_xyz[3 * ia], ny = P.ang_xyz[3 * ia + 1], nz_ = P.ang_xyz[3 * ia + 2];
-            const double ux = r * nx, uy = r * ny, uz = r * nz_;
+            ux = r * nx; uy = r * ny; uz = r * nz_;
             const double w = P.rad_w[ir] * rb * r * r * P.ang_w[ia];
             // weighted real projector values through the Phi columns of this point, then G = beta (cos - i sin)(A.r)
             // (the quadrature point sits at distance r < rb in direction n_a by construction: no square root)
@@ -149,49 +162,65 @@ __global__ void __launch_bounds__(kSnapThreads, 4) gint_snap_kernel(const SnapPl
                 myG[(2 * b) * kSnapStride] = bv * cs;
                 myG[(2 * b + 1) * kSnapStride] = -(bv * sn);
             }
-            for (int c = nJ; c < mI; c++) myPhi[c * kSnapStride] = 0.0;
-            snap_eval(so, P.tab, ux + pr.d[0], uy + pr.d[1], uz + pr.d[2], myPhi, kSnapStride);
         } else {
-            for (int c = 0; c < nJ; c++) myPhi[c * kSnapStride] = 0.0;
             for (int c = 0; c < 2 * mI; c++) myG[c * kSnapStride] = 0.0;
         }
-        __syncwarp();
-        // 32 points = 8 k-steps of 4 points: A[row mu = 8 i + lane / 4][k = lane % 4], B[k = lane % 4][col = 8 j + lane / 4]
 #pragma unroll
-        for (int q = 0; q < 8; q++) {
-            double a[FR], b[FC];
+        for (int nb = 0; nb < kSnapGroupPairs; nb++) {
+            if (nb < gn) {
+                const SnapSpecies& so = P.orb[spq[nb]];
+                if (p < npts) {
+                    // rows beyond n_J keep what the step before left there (projector values or another neighbour's
+                    // orbitals): they only reach accumulator rows that are never written out
+                    snap_eval(so, P.tab, ux + dq[nb][0], uy + dq[nb][1], uz + dq[nb][2], myPhi, kSnapStride);
+                } else {
+                    for (int c = 0; c < FR * 8; c++) myPhi[c * kSnapStride] = 0.0;
+                }
+                __syncwarp();
+                // 32 points = 8 k-steps of 4 points: A[row mu = 8 i + lane / 4][k = lane % 4], B[k = lane % 4][col = 8 j + lane / 4]
 #pragma unroll
-            for (int i = 0; i < FR; i++) a[i] = sPhi[(8 * i + frow) * kSnapStride + 4 * q + fk];
+                for (int q = 0; q < 8; q++) {
+                    double a[FR], b[FC];
 #pragma unroll
-            for (int j = 0; j < FC; j++) b[j] = sG[(8 * j + frow) * kSnapStride + 4 * q + fk];
+                    for (int i = 0; i < FR; i++) a[i] = sPhi[(8 * i + frow) * kSnapStride + 4 * q + fk];
 #pragma unroll
-            for (int i = 0; i < FR; i++)
+                    for (int j = 0; j < FC; j++) b[j] = sG[(8 * j + frow) * kSnapStride + 4 * q + fk];
 #pragma unroll
-                for (int j = 0; j < FC; j++) dmma_s(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                    for (int i = 0; i < FR; i++)
+#pragma unroll
+                        for (int j = 0; j < FC; j++) dmma_s(acc[nb][i][j][0], acc[nb][i][j][1], a[i], b[j]);
+                }
+                __syncwarp();
+            }
         }
-        __syncwarp();
     }
     // cross-warp sum in a fixed order: warp w writes its fragments, then thread e adds the four copies of element e
-    __syncthreads();
     double* red = snap_smem;   // [4 warps][FR * 8][FC * 8]
     constexpr int kCols = FC * 8;
 #pragma unroll
-    for (int i = 0; i < FR; i++)
+    for (int nb = 0; nb < kSnapGroupPairs; nb++) {
+        if (nb < gn) {
+            __syncthreads();
 #pragma unroll
-        for (int j = 0; j < FC; j++) {
-            // C fragment: lane holds (row lane / 4, columns 2 (lane % 4), 2 (lane % 4) + 1)
-            double* dst = red + ((size_t)warp * FR * 8 + 8 * i + frow) * kCols + 8 * j + 2 * fk;
-            dst[0] = acc[i][j][0];
-            dst[1] = acc[i][j][1];
+            for (int i = 0; i < FR; i++)
+#pragma unroll
+                for (int j = 0; j < FC; j++) {
+                    // C fragment: lane holds (row lane / 4, columns 2 (lane % 4), 2 (lane % 4) + 1)
+                    double* dst = red + ((size_t)warp * FR * 8 + 8 * i + frow) * kCols + 8 * j + 2 * fk;
+                    dst[0] = acc[nb][i][j][0];
+                    dst[1] = acc[nb][i][j][1];
+                }
+            __syncthreads();
+            const int nJ = P.orb[spq[nb]].ncomp;
+            double* out = S + 2 * P.pairs[g0 + nb].off;   // block [n_J][m_I] complex = [n_J][2 m_I] doubles
+            for (int e = tid; e < nJ * 2 * mI; e += kSnapThreads) {
+                const int mu = e / (2 * mI), c = e - mu * 2 * mI;
+                double v = 0.0;
+#pragma unroll
+                for (int w = 0; w < kSnapThreads / 32; w++) v += red[((size_t)w * FR * 8 + mu) * kCols + c];
+                out[e] = v;
+            }
         }
-    __syncthreads();
-    double* out = S + 2 * pr.off;   // block [n_J][m_I] complex = [n_J][2 m_I] doubles
-    for (int e = tid; e < nJ * 2 * mI; e += kSnapThreads) {
-        const int mu = e / (2 * mI), c = e - mu * 2 * mI;
-        double v = 0.0;
-#pragma unroll
-        for (int w = 0; w < kSnapThreads / 32; w++) v += red[((size_t)w * FR * 8 + mu) * kCols + c];
-        out[e] = v;
     }
 }
 
@@ -206,7 +235,7 @@ static cudaError_t launch_snap_t(const SnapPlan& P, const double* A, double* S, 
     const size_t smem = snap_kernel_smem(FR, FC);
     cudaError_t e = cudaFuncSetAttribute(gint_snap_kernel<FR, FC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    gint_snap_kernel<FR, FC><<<P.npair, kSnapThreads, smem, stream>>>(P, A[0], A[1], A[2], S);
+    gint_snap_kernel<FR, FC><<<P.ngroup, kSnapThreads, smem, stream>>>(P, A[0], A[1], A[2], S);
     return cudaGetLastError();
 }
 
