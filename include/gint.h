@@ -220,8 +220,10 @@ int gint_fold_k_static(gint_ctx *ctx, const double *H_dev, const double *kfrac, 
  * gint_snap_psibeta A: HOST pointer, 3 doubles (bohr^-1); S_dev: device pointer, 2 s_len doubles, interleaved
  *                   (re, im); OVERWRITTEN, every element written once.  Asynchronous on `stream`, one kernel (one
  *                   CTA per two pairs of an atom I, the sum over points on the FP64 tensor pipe), no atomics: results
- *                   are bit-wise reproducible.  Allocates nothing.  Independent of the mesh, hence of
- *                   gint_options.rank / nranks: every rank of a sharded run computes all pairs. */
+ *                   are bit-wise reproducible.  Allocates nothing.
+ * With gint_options.nranks > 1 the pairs are independent problems dealt out by projector atom: a context keeps the
+ * pairs of the atoms I with I % nranks == rank (its pair list and S cover those only; no collective is involved, the
+ * caller gathers the blocks if it needs them in one place). */
 int gint_snap_setup(gint_ctx *ctx, const gint_species *proj, int32_t nrad_pts, const double *rad_x, const double *rad_w,
                     int32_t nang, const double *ang_xyz, const double *ang_w);
 int gint_snap_num_pairs(const gint_ctx *ctx, int64_t *npair, int64_t *s_len);

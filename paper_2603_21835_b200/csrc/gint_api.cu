@@ -538,6 +538,7 @@ int gint_snap_setup(gint_ctx* ctx, const gint_species* proj, int32_t nrad_pts, c
         for (int I = 0; I < natom; I++) {
             const gint::SnapSpecies& b = prj[(size_t)P.atom_species[(size_t)I]];
             if (b.nrad == 0) continue;
+            if (P.nranks > 1 && I % P.nranks != P.rank) continue;   // sharded context: projector atoms dealt out by index
             const double* tI = &P.atom_pos[3 * (size_t)I];
             for (int J = 0; J < natom; J++) {
                 const gint::SnapSpecies& o = orb[(size_t)P.atom_species[(size_t)J]];

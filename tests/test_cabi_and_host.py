@@ -295,3 +295,24 @@ def test_snap_pair_list_equals_the_oracles_enumeration():
         assert all(np.array_equal(a, b) for a, b in zip(got, ref))
         assert len(got[0]) > 0
     assert [tuple(r) for r in got[2].tolist()] == [(0, 0, 0)]   # the tie case: no (+-1, 0, 0) self image
+
+
+def test_snap_pairs_are_dealt_out_by_projector_atom():
+    """nranks = 3: the ranks' pair lists are disjoint, cover the full list, and rank r holds exactly the pairs of the
+    atoms I with I % 3 == r (host-only contexts)."""
+    from paper_2603_21835_b200 import gint_setup
+    w = wl.make("si8_sz")
+    proj = [wl.projector_species()]
+    rx, rw = wl.radial_quadrature(8)
+    an, aw = wl.angular_quadrature(6)
+    def pairs(rank, nranks):
+        ctx = gint_setup(w.lattice, w.ngrid, w.species, w.atom_species, w.atom_pos, cuda_device=-1, rank=rank, nranks=nranks)
+        ctx.gint_snap_setup(proj, rx, rw, an, aw)
+        iat, jat, R, off = ctx.gint_snap_get_pairs()
+        assert off[0] == 0 and np.all(np.diff(off) > 0)
+        return [tuple(x) for x in np.column_stack([iat, jat, R]).tolist()]
+    full = pairs(0, 1)
+    parts = [pairs(r, 3) for r in range(3)]
+    for r, p in enumerate(parts):
+        assert p and all(k[0] % 3 == r for k in p)
+    assert sorted(sum(parts, [])) == full

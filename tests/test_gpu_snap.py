@@ -149,3 +149,29 @@ def test_headline_size_sampled_pairs():
     for q, b in enumerate(pick):
         d = np.abs(got[off[b]:off[b + 1]] - ref[sub_off[q]:sub_off[q + 1]]).max()
         assert d <= TOL * scale, (int(b), d / scale)
+
+
+def test_sharded_contexts_cover_all_pairs(cfg1):
+    """nranks = 2 on one GPU: every rank computes the pairs of its projector atoms; together they reproduce the
+    unsharded result block by block (no collective on this path)."""
+    torch = _torch()
+    from paper_2603_21835_b200 import gint_setup, workloads as wl
+    proj = [wl.projector_species()]
+    A = (0.1, -0.05, 0.2)
+    full_ctx = _context(cfg1, proj)
+    full = full_ctx.gint_snap_psibeta(A).cpu().numpy()
+    fi, fj, fR, foff = full_ctx.gint_snap_get_pairs()
+    index = {(int(fi[b]), int(fj[b])) + tuple(int(x) for x in fR[b]): b for b in range(len(fi))}
+    seen = 0
+    for rank in range(2):
+        ctx = gint_setup(cfg1.lattice, cfg1.ngrid, cfg1.species, cfg1.atom_species, cfg1.atom_pos, cuda_device=0,
+                         rank=rank, nranks=2)
+        ctx.gint_snap_setup(proj, *_quad())
+        S = ctx.gint_snap_psibeta(A).cpu().numpy()
+        iat, jat, R, off = ctx.gint_snap_get_pairs()
+        assert np.all(iat % 2 == rank)
+        for b in range(len(iat)):
+            g = index[(int(iat[b]), int(jat[b])) + tuple(int(x) for x in R[b])]
+            assert np.array_equal(S[off[b]:off[b + 1]], full[foff[g]:foff[g + 1]])   # same kernel, same order: bit-wise
+        seen += len(iat)
+    assert seen == len(fi)
