@@ -236,6 +236,7 @@ void device_release_arrays(gint_ctx* ctx) {
 void snap_release(gint_ctx* ctx) {
     if (ctx->device >= 0 && !ctx->snap_allocs.empty()) {
         DeviceGuard guard(ctx->device);
+        cudaDeviceSynchronize();   // a gint_snap_psibeta in flight still reads these tables
         for (void* p : ctx->snap_allocs) cudaFree(p);
     }
     ctx->snap_allocs.clear();
