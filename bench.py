@@ -345,7 +345,7 @@ def main():
         t1 = time.perf_counter()
         ctx.gint_snap_setup(proj, rx, rw, an, aw)
         snap_setup_s = time.perf_counter() - t1
-        sp_iat, sp_jat, _, sp_off = ctx.gint_snap_get_pairs()
+        sp_iat, sp_jat, sp_R, sp_off = ctx.gint_snap_get_pairs()
         Sv = ctx.gint_snap_psibeta((0.08, -0.11, 0.05))
         torch.cuda.synchronize()
         f0.record()
@@ -437,6 +437,17 @@ def main():
             "sample": "all %d blocks of the first %d of %d row atoms, %.1f s; flops = F_pt*%d/%d (oracle computes both "
                       "(I,J,R) and (J,I,-R))" % (nblk, na, w.natom, dt, na, w.natom),
             "ms_per_call_extrapolated": dt * 1e3 * w.natom / na}
+        if snap_info is not None:
+            # the same oracle-beside-it for gint_snap_psibeta: the first 256 pairs, one at a time (NumPy, one core)
+            import oracle
+            nsamp = min(256, len(sp_iat))
+            sub_n = (sp_off[1:] - sp_off[:-1])[:nsamp]
+            sub = (sp_iat[:nsamp], sp_jat[:nsamp], sp_R[:nsamp], np.concatenate([[0], np.cumsum(sub_n)]).astype(np.int64))
+            t1 = time.perf_counter()
+            oracle.snap_psibeta(w.lattice, w.species, proj, w.atom_species, w.atom_pos, (0.08, -0.11, 0.05), rx, rw, an, aw, pairs=sub)
+            dts = time.perf_counter() - t1
+            snap_info["cpu_oracle"] = {"pairs": int(nsamp), "seconds": dts, "cores": 1, "kind": "oracle",
+                                       "ms_per_call_extrapolated": dts * 1e3 * len(sp_iat) / nsamp}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
