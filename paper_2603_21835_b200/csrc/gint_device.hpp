@@ -97,7 +97,7 @@ struct SnapPlan {
     const int32_t* groups;     // [ngroup][2]: first pair and number of pairs (<= kSnapGroupPairs, same atom I) of a CTA
     int32_t npair, nrad, nang, ngroup;
 };
-constexpr int kSnapGroupPairs = 2;   // 4: 200+ registers, 2 CTAs per SM, slower (measured)
+constexpr int kSnapGroupPairs = 2;   // 3: spills at 128 registers (si512_tzdp slower), 4: worse still (measured)
 cudaError_t launch_snap(const SnapPlan& P, int fr, int fc, const double* A, double* S, cudaStream_t stream);
 
 // The launchers walk the plan's batches (regions that share the psi scratch one after the other): nbatch entries of

@@ -109,7 +109,7 @@ constexpr int kSnapStride = 36;   // staging tiles are [column][point]: 32 point
 // FR x FC accumulator fragments of 8 x 8: rows = orbitals of J (n_J <= 8 FR), columns = (Re, Im) of the projector
 // components of I (2 m_I <= 8 FC)
 template <int FR, int FC>
-__global__ void __launch_bounds__(kSnapThreads, kSnapGroupPairs <= 2 ? 3 : 2) gint_snap_kernel(const SnapPlan P, double ax, double ay, double az, double* __restrict__ S) {
+__global__ void __launch_bounds__(kSnapThreads, 4) gint_snap_kernel(const SnapPlan P, double ax, double ay, double az, double* __restrict__ S) {
     extern __shared__ __align__(16) double snap_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     double* sPhi = snap_smem + (size_t)warp * (FR + FC) * 8 * kSnapStride;   // [8 FR columns: orbitals][36]
