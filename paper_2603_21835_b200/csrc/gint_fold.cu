@@ -5,7 +5,7 @@
 // with k = kfrac . (b1, b2, b3), a_i . b_j = 2 pi delta_ij, so k.R = 2 pi kfrac . (R1, R2, R3).  The block table is
 // sorted by (I, J, R), so the blocks of an atom pair are consecutive (a "run").  Single pass, every element of the
 // dense matrix written exactly once, zeros included (no memset): one CTA per row atom I sweeps the n_I rows of the
-// dense matrix, consecutive threads on consecutive columns (coalesced 16-byte stores); a column's atom J comes from a
+// dense matrix, consecutive threads on consecutive columns (coalesced 16-byte stores, one column per thread); a column's atom J comes from a
 // table, the run (I, J) from a binary search in the row's run list (shared memory), the phases exp(2 pi i kfrac . R)
 // of all blocks from a small kernel run first.  HBM-bound: H read once, H(k) written once.
 #include <cuda_runtime.h>
@@ -27,7 +27,8 @@ __global__ void __launch_bounds__(256) gint_fold_phase_kernel(const FoldPlan F, 
 }
 
 constexpr int kFoldRunsSmem = 4096;   // run list of a row atom kept in shared memory up to this length
-constexpr int kFoldCols = 4;          // columns per thread: a CTA covers 1024 consecutive columns of one row atom
+constexpr int kFoldCols = 1;          // columns per thread: a CTA covers 256 consecutive columns of one row atom (1 beats 2 and 4: the kernel
+                                      // lives on threads in flight for its dependent block-offset -> H loads)
 
 __global__ void __launch_bounds__(256) gint_fold_kernel(const FoldPlan F, const double* __restrict__ H, double2* __restrict__ Hk) {
     __shared__ int32_t s_runJ[kFoldRunsSmem];
